@@ -1,0 +1,152 @@
+"""CPU oracle for the Henon Monte Carlo orbit step (arXiv 1206.5878).
+
+TEST INFRASTRUCTURE ONLY.  Nothing under ``paper_1206_5878_b200/`` may import
+this package; only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s
+``cpu_baseline`` / ``--impl reference`` legs do.  The arithmetic lives in
+``hmc_oracle.c`` (plain C, one translation unit, written from the paper); this
+file only compiles it with gcc and marshals numpy arrays through ctypes.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "hmc_oracle.c")
+_LIB = os.path.join(_HERE, "libhmc_oracle.so")
+# -ffp-contract=off: no FMA contraction; see the header of hmc_oracle.c.
+CFLAGS = ["-O2", "-ffp-contract=off", "-fPIC", "-shared", "-std=gnu11", "-Wall"]
+
+ST_UNBOUND, ST_RADIAL, ST_DEGENERATE, ST_CIRCULAR, ST_MAXTRIES, ST_CLIPPED = 1, 2, 4, 8, 16, 32
+T_MAX = 4096
+C_F = 1.2
+
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile hmc_oracle.c -> libhmc_oracle.so (in-tree) if missing or stale."""
+    stale = (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC)
+    if force or stale:
+        tmp = _LIB + ".tmp.%d" % os.getpid()
+        subprocess.run(["gcc", *CFLAGS, _SRC, "-o", tmp, "-lm"], check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def lib() -> ctypes.CDLL:
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _f64(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a
+
+
+def philox4x32_10(ctr, key):
+    c = np.asarray(ctr, dtype=np.uint32).copy()
+    k = np.asarray(key, dtype=np.uint32).copy()
+    out = np.zeros(4, dtype=np.uint32)
+    lib().hmc_ref_philox4x32_10(_p(c), _p(k), _p(out))
+    return out
+
+
+def sort_by_radius(r_in, cols=(), ids=None):
+    """-> (r_sorted, perm, [cols_sorted...], ids_sorted or None)"""
+    r_in = _f64(r_in)
+    n = r_in.shape[0]
+    r_sorted = np.empty(n, np.float64)
+    perm = np.empty(n, np.uint32)
+    cols = [_f64(c) for c in cols]
+    outs = [np.empty(n, np.float64) for _ in cols]
+    PtrArr = ctypes.c_void_p * max(len(cols), 1)
+    cin = PtrArr(*[c.ctypes.data for c in cols]) if cols else PtrArr()
+    cout = PtrArr(*[c.ctypes.data for c in outs]) if cols else PtrArr()
+    id_out = None
+    if ids is not None:
+        ids = np.ascontiguousarray(ids, dtype=np.uint32)
+        id_out = np.empty(n, np.uint32)
+    rc = lib().hmc_ref_sort_by_radius(ctypes.c_uint64(n), _p(r_in), _p(r_sorted), _p(perm),
+                                      ctypes.c_int(len(cols)), cin, cout, _p(ids), _p(id_out))
+    assert rc == 0
+    return r_sorted, perm, outs, id_out
+
+
+def potential(r, m, G=1.0):
+    """-> (phi, m_cum) on the radius-sorted arrays r, m."""
+    r, m = _f64(r), _f64(m)
+    n = r.shape[0]
+    phi = np.empty(n, np.float64)
+    mc = np.empty(n, np.float64)
+    rc = lib().hmc_ref_potential(ctypes.c_uint64(n), ctypes.c_double(G), _p(r), _p(m), _p(phi), _p(mc))
+    assert rc == 0
+    return phi, mc
+
+
+def orbit_turning_points(r, v_r, v_t, phi, m_cum, G=1.0, first=0, stride=1, count=None):
+    """-> dict(E, J, r_min, r_max, k_min, k_max, status), compact over the selected stars."""
+    r, v_r, v_t, phi, m_cum = map(_f64, (r, v_r, v_t, phi, m_cum))
+    n = r.shape[0]
+    if count is None:
+        count = 0 if n <= first else (n - first + stride - 1) // stride
+    o = dict(E=np.empty(count), J=np.empty(count), r_min=np.empty(count), r_max=np.empty(count),
+             k_min=np.empty(count, np.uint32), k_max=np.empty(count, np.uint32),
+             status=np.empty(count, np.uint8))
+    rc = lib().hmc_ref_orbit_turning_points(
+        ctypes.c_uint64(n), ctypes.c_double(G), _p(r), _p(v_r), _p(v_t), _p(phi), _p(m_cum),
+        ctypes.c_uint64(first), ctypes.c_uint64(stride), ctypes.c_uint64(count),
+        _p(o["E"]), _p(o["J"]), _p(o["r_min"]), _p(o["r_max"]), _p(o["k_min"]), _p(o["k_max"]),
+        _p(o["status"]))
+    assert rc == 0
+    return o
+
+
+def sample_new_radius(r, phi, m_cum, r_self, v_r_self, v_t_self, E, J, r_min, r_max, k_min, k_max,
+                      ids, status, seed, step, G=1.0):
+    """Tables r, phi, m_cum have length n; every other array is compact over the selected stars.
+    -> dict(r_new, v_r_new, v_t_new, n_try, status, trials)"""
+    r, phi, m_cum = map(_f64, (r, phi, m_cum))
+    r_self, v_r_self, v_t_self, E, J, r_min, r_max = map(_f64, (r_self, v_r_self, v_t_self, E, J, r_min, r_max))
+    k_min = np.ascontiguousarray(k_min, np.uint32)
+    k_max = np.ascontiguousarray(k_max, np.uint32)
+    ids = np.ascontiguousarray(ids, np.uint32)
+    status = np.ascontiguousarray(status, np.uint8)
+    n, count = r.shape[0], E.shape[0]
+    o = dict(r_new=np.empty(count), v_r_new=np.empty(count), v_t_new=np.empty(count),
+             n_try=np.empty(count, np.uint16), status=np.empty(count, np.uint8))
+    counters = np.zeros(1, np.uint64)
+    rc = lib().hmc_ref_sample_new_radius(
+        ctypes.c_uint64(n), ctypes.c_double(G), ctypes.c_uint64(seed), ctypes.c_uint32(step),
+        _p(r), _p(phi), _p(m_cum), ctypes.c_uint64(count),
+        _p(r_self), _p(v_r_self), _p(v_t_self), _p(E), _p(J), _p(r_min), _p(r_max),
+        _p(k_min), _p(k_max), _p(ids), _p(status),
+        _p(o["r_new"]), _p(o["v_r_new"]), _p(o["v_t_new"]), _p(o["n_try"]), _p(o["status"]), _p(counters))
+    assert rc == 0
+    o["trials"] = int(counters[0])
+    return o
+
+
+def orbit_step(r, v_r, v_t, m, ids, seed, step, G=1.0, sample=None):
+    """One pass of the whole path: sort -> potential -> turning points -> new radius.
+
+    ``sample=(first, stride)`` restricts S3/S4 to every stride-th star of the sorted order
+    (S1, S2 always run on all stars).  Returns a dict with every intermediate.
+    """
+    rs, perm, (vrs, vts, ms), ids_s = sort_by_radius(r, (v_r, v_t, m), ids)
+    phi, mc = potential(rs, ms, G)
+    first, stride = sample if sample is not None else (0, 1)
+    tp = orbit_turning_points(rs, vrs, vts, phi, mc, G, first, stride)
+    sl = slice(first, None, stride)
+    sm = sample_new_radius(rs, phi, mc, rs[sl], vrs[sl], vts[sl], tp["E"], tp["J"], tp["r_min"], tp["r_max"],
+                           tp["k_min"], tp["k_max"], ids_s[sl], tp["status"], seed, step, G)
+    return dict(r=rs, perm=perm, v_r=vrs, v_t=vts, m=ms, id=ids_s, phi=phi, m_cum=mc, tp=tp, sample=sm)

@@ -1,0 +1,357 @@
+/*
+ * hmc_oracle.c -- CPU ORACLE for the orbit step of the Henon Monte Carlo method
+ * (arXiv 1206.5878, Pattabiraman et al.; cited below as PAPER.md:LINE).
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  It is a plain, slow,
+ * single-threaded restatement of what the hot path computes, written from the
+ * paper, so that the CUDA library can be checked against it star by star.
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may load it.  It shares no code, header, table or
+ * constant generator with paper_1206_5878_b200/csrc/.
+ *
+ * Build:  gcc -O2 -ffp-contract=off -fPIC -shared hmc_oracle.c -o libhmc_oracle.so -lm
+ * (-ffp-contract=off: no fused multiply-add, every +,-,*,/,sqrt below is one
+ *  correctly rounded IEEE-754 binary64 operation, evaluated in the order the
+ *  parentheses state -- DESIGN.md "Readings" R2.)
+ *
+ * Numbering.  The paper numbers the radius-sorted stars 1..N.
+ * Arrays here are 0-based: array element a holds node j = a+1.  Sentinel nodes
+ * (R4): node 0 at r = 0 and node N+1 at r = +inf with Phi_{N+1} = 0
+ * (Eq. 2).  "Shell j" is the interval [r_j, r_{j+1}], j = 0..N.
+ *
+ * Pins (tests/test_oracle_*.py, run with -m "not gpu"):
+ *   philox      : Random123 known-answer vectors (tests/golden/philox4x32_10_kat.txt)
+ *   sort        : numpy stable argsort / lexsort; adversarial keys
+ *   potential   : O(N^2) shell-theorem brute force in exact rational arithmetic,
+ *                 Eq. 2-5 recursion, hand cases, Plummer closed form (statistical)
+ *   turning pts : linear-scan brute force, Q(root)=0 with Phi from brute force,
+ *                 Kepler closed form, circular orbit
+ *   sampling    : energy identity, KS vs Kepler time-weighted CDF, closed-form
+ *                 acceptance rate, order independence
+ * No function in this file is "parity unpinned".
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+/* per-star status bits (same numeric values as include/hmc.h, restated) */
+#define ST_UNBOUND    1u   /* E >= 0 (or not a number): no turning points, no draw   */
+#define ST_RADIAL     2u   /* J^2 == 0: pericentre is r = 0, no draw                 */
+#define ST_DEGENERATE 4u   /* closed-form root not defined (C >= 0 in outer shell)   */
+#define ST_CIRCULAR   8u   /* r_max - r_min <= 0 or end slopes of wrong sign         */
+#define ST_MAXTRIES   16u  /* rejection loop hit T_MAX                               */
+#define ST_CLIPPED    32u  /* some trial had g > F (density clipped; informational)  */
+
+#define T_MAX 4096u        /* DESIGN.md R7 */
+#define C_F   1.2          /* DESIGN.md R7 */
+
+/* ------------------------------------------------------------------------ */
+/* Philox4x32-10 (Salmon et al. 2011, "Parallel random numbers: as easy as  */
+/* 1, 2, 3").  Replaces the paper's per-thread Tausworthe streams           */
+/* so that a star's draws depend only on           */
+/* (seed, step, star id) -- DESIGN.md R9; the paper's own reproducibility   */
+/* test needed the same stream->star mapping on both sides.  */
+/* ------------------------------------------------------------------------ */
+void hmc_ref_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        uint32_t n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        uint32_t n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* ------------------------------------------------------------------------ */
+/* S1.  Sort stars by radial distance (step 6).               */
+/* The paper uses Quicksort and does not say how ties are ordered; the      */
+/* reading (R1) is the unique order by the pair (r_i, i).         */
+/* perm[k] = original index of the k-th smallest radius.                    */
+/* ------------------------------------------------------------------------ */
+typedef struct { double r; uint32_t i; } key_index;
+
+static int cmp_key_index(const void *pa, const void *pb)
+{
+    const key_index *a = (const key_index *)pa, *b = (const key_index *)pb;
+    if (a->r < b->r) return -1;
+    if (a->r > b->r) return 1;
+    if (a->i < b->i) return -1;
+    if (a->i > b->i) return 1;
+    return 0;
+}
+
+int hmc_ref_sort_by_radius(uint64_t n, const double *r_in, double *r_sorted, uint32_t *perm,
+                           int ncols, const double *const *cols_in, double *const *cols_out,
+                           const uint32_t *id_in, uint32_t *id_out)
+{
+    if (n == 0) return 0;
+    key_index *a = (key_index *)malloc(n * sizeof(key_index));
+    if (!a) return -1;
+    for (uint64_t i = 0; i < n; ++i) { a[i].r = r_in[i]; a[i].i = (uint32_t)i; }
+    qsort(a, n, sizeof(key_index), cmp_key_index);   /* Quicksort */
+    for (uint64_t k = 0; k < n; ++k) {
+        perm[k] = a[k].i;
+        r_sorted[k] = a[k].r;
+    }
+    for (int c = 0; c < ncols; ++c)
+        for (uint64_t k = 0; k < n; ++k) cols_out[c][k] = cols_in[c][perm[k]];
+    if (id_in && id_out)
+        for (uint64_t k = 0; k < n; ++k) id_out[k] = id_in[perm[k]];
+    free(a);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------ */
+/* S2.  Potential at the star positions (Eq. 1 at r = r_k): */
+/*   Phi_k = -G ( M_k / r_k  +  S_k ),                                      */
+/*   M_k = sum_{i<=k} m_i ,   S_k = sum_{i>k} m_i / r_i .                   */
+/* Eq. 2-5 is the same quantity as a recursion; tests check both.           */
+/* Precision (R1p): the paper says only "double precision"        */
+/* (PAPER.md:326).  M_k and S_k are defined here as the EXACT sums of the   */
+/* binary64 terms m_i and fl(m_i / r_i), rounded once to binary64; the      */
+/* running sums are therefore carried in binary128 (113-bit significand,    */
+/* error ~N*2^-113, far below half an ulp of binary64 except with           */
+/* probability ~N*2^-33 per run).  Phi_k is then three binary64 operations. */
+/* ------------------------------------------------------------------------ */
+int hmc_ref_potential(uint64_t n, double G, const double *r, const double *m,
+                      double *phi, double *m_cum)
+{
+    __float128 acc = 0;
+    for (uint64_t a = 0; a < n; ++a) {            /* Eq. 3 taken prefix by prefix */
+        acc += (__float128)m[a];
+        m_cum[a] = (double)acc;
+    }
+    acc = 0;                                      /* S_N = 0 <=> Phi_{N+1} = 0, Eq. 2 */
+    for (uint64_t a = n; a-- > 0;) {
+        double S = (double)acc;
+        phi[a] = -(G * (m_cum[a] / r[a] + S));    /* Eq. 1 at r = r_k */
+        double t = m[a] / r[a];
+        acc += (__float128)t;
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------ */
+/* Table access with sentinels, paper numbering j = 0..N+1.                 */
+/* ------------------------------------------------------------------------ */
+typedef struct {
+    uint64_t n;
+    double G;
+    const double *r, *phi, *mc;   /* 0-based arrays of length n */
+} table;
+
+/* Sign test of Q(r_j) = 2E - 2Phi_j - J^2/r_j^2 (Eq. 12) at a
+ * table node: returns 1 when Q_j < 0.  Written division-free by multiplying
+ * with r_j^2 > 0 (R2): Q_j < 0  <=>  2 (E - Phi_j) r_j^2 < J^2.
+ * Node 0 (r = 0): Q = -inf for J > 0.  Node N+1 (r = inf, Phi = 0): Q = 2E < 0
+ * for a bound star.  Both sentinels therefore answer "negative". */
+static int q_negative(const table *T, uint64_t j, double E, double J2)
+{
+    if (j == 0 || j == T->n + 1) return 1;
+    double rj = T->r[j - 1];
+    return 2.0 * ((E - T->phi[j - 1]) * (rj * rj)) < J2;
+}
+
+/* Coefficients of Q inside shell j, as a function of u = 1/r:
+ *   Phi(u) = Phi_j - G M_j (u - u_j)  (Eq. 1 == Eq. 6 anchored at node j, R3)
+ *   Q(u)   = 2 C + 2 B u - J^2 u^2,  B = G M_j,  C = (E - Phi_j) - B u_j.
+ * Shell 0 (inside the innermost star): Phi == Phi_1, so B = 0, C = E - Phi_1. */
+static void shell_coeff(const table *T, uint64_t j, double E, double *B, double *C)
+{
+    if (j == 0) {
+        *B = 0.0;
+        *C = E - T->phi[0];
+    } else {
+        double b = T->G * T->mc[j - 1];
+        *B = b;
+        *C = (E - T->phi[j - 1]) - b * (1.0 / T->r[j - 1]);
+    }
+}
+
+/* ------------------------------------------------------------------------ */
+/* S3.  Pericentre and apocentre.                        */
+/* For star k (node k): E = Phi_k + (v_r^2 + v_t^2)/2  (Eq. 16,             */
+/* PAPER.md:202), J = r_k v_t.  "We need to determine k such that           */
+/* Q(r_k) < 0 < Q(r_k+1).  We use the bisection method":     */
+/*   k_min = the node j in [0, k-1]  with Q_j < 0 <= Q_{j+1}  (pericentre)  */
+/*   k_max = the node j in [k, N]    with Q_j >= 0 > Q_{j+1}  (apocentre)   */
+/* The star's own node is taken as Q >= 0 without being evaluated           */
+/* (Q(r_k) = v_r^2, R5).  Then "Phi, and thus Q, can be computed  */
+/* analytically in that interval, and so can r_min and r_max"               */
+/* (PAPER.md:124): the roots of the quadratic in u of shell_coeff().        */
+/* Stars are selected as array index first + i*stride, i < count; outputs   */
+/* are compact arrays of length count.                                      */
+/* ------------------------------------------------------------------------ */
+int hmc_ref_orbit_turning_points(uint64_t n, double G,
+        const double *r, const double *v_r, const double *v_t,
+        const double *phi, const double *m_cum,
+        uint64_t first, uint64_t stride, uint64_t count,
+        double *E_out, double *J_out, double *r_min_out, double *r_max_out,
+        uint32_t *k_min_out, uint32_t *k_max_out, uint8_t *status_out)
+{
+    table T = { n, G, r, phi, m_cum };
+    for (uint64_t i = 0; i < count; ++i) {
+        uint64_t a = first + i * stride;        /* array index           */
+        uint64_t k = a + 1;                     /* node number, 1..N     */
+        double E = phi[a] + 0.5 * (v_r[a] * v_r[a] + v_t[a] * v_t[a]);   /* Eq. 16 */
+        double J = r[a] * v_t[a];
+        double J2 = J * J;
+        E_out[i] = E; J_out[i] = J;
+        unsigned st = 0;
+        if (!(E < 0.0)) st |= ST_UNBOUND;
+        if (J2 == 0.0) st |= ST_RADIAL;
+        if (st) {
+            r_min_out[i] = (st & ST_RADIAL) ? 0.0 : r[a];
+            r_max_out[i] = (st & ST_UNBOUND) ? INFINITY : r[a];
+            k_min_out[i] = (uint32_t)(k - 1); k_max_out[i] = (uint32_t)k;
+            status_out[i] = (uint8_t)st;
+            continue;
+        }
+        /* bisection for the pericentre bracket: Q_lo < 0, Q_hi >= 0 */
+        uint64_t lo = 0, hi = k;
+        while (hi - lo > 1) {
+            uint64_t mid = lo + (hi - lo) / 2;
+            if (q_negative(&T, mid, E, J2)) lo = mid; else hi = mid;
+        }
+        uint64_t kmin = lo;
+        /* bisection for the apocentre bracket: Q_lo >= 0, Q_hi < 0 */
+        lo = k; hi = n + 1;
+        while (hi - lo > 1) {
+            uint64_t mid = lo + (hi - lo) / 2;
+            if (q_negative(&T, mid, E, J2)) hi = mid; else lo = mid;
+        }
+        uint64_t kmax = lo;
+
+        double B, C, D;
+        shell_coeff(&T, kmin, E, &B, &C);
+        D = B * B + 2.0 * (J2 * C);
+        if (D < 0.0) D = 0.0;
+        double rmin = J2 / (B + sqrt(D));                 /* larger-u root  */
+        shell_coeff(&T, kmax, E, &B, &C);
+        D = B * B + 2.0 * (J2 * C);
+        if (D < 0.0) D = 0.0;
+        double rmax;
+        if (C < 0.0) rmax = (B + sqrt(D)) / (-2.0 * C);   /* smaller-u root, via the product of roots */
+        else { rmax = INFINITY; st |= ST_DEGENERATE; }
+        r_min_out[i] = rmin; r_max_out[i] = rmax;
+        k_min_out[i] = (uint32_t)kmin; k_max_out[i] = (uint32_t)kmax;
+        status_out[i] = (uint8_t)st;
+    }
+    return 0;
+}
+
+/* "To get the potential Phi(r) at any other radius, one first finds k such
+ * that r_k <= r <= r_{k+1}": j = #{ i : r_i <= x } by bisection,
+ * restricted to the orbit's own bracket [k_min, k_max]. */
+static uint64_t shell_of(const table *T, double x, uint64_t kmin, uint64_t kmax)
+{
+    uint64_t lo = kmin, hi = kmax + 1;   /* answer in [kmin, kmax]; invariant r_lo <= x < r_hi (by clamping) */
+    while (hi - lo > 1) {
+        uint64_t mid = lo + (hi - lo) / 2;          /* node mid, 1..N */
+        if (T->r[mid - 1] <= x) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+/* Eq. 6 in the anchored form of DESIGN.md R3. */
+static double phi_in_shell(const table *T, uint64_t j, double x)
+{
+    if (j == 0) return T->phi[0];
+    return T->phi[j - 1] - (T->G * T->mc[j - 1]) * (1.0 / x - 1.0 / T->r[j - 1]);
+}
+
+/* ------------------------------------------------------------------------ */
+/* S4.  New radial position: von Neumann rejection with  */
+/* density f(r) ~ 1/|v_r|, v_r = sqrt(Q(r)) (Eq. 13).  The paper's Eq. 14-15 */
+/* draw r_0 uniformly and compare F X' with f(r_0); "a slightly modified    */
+/* version of the method is used, since f(r) = 1/|v_r| becomes infinite at  */
+/* both ends", details deferred to Joshi et al. (2000).      */
+/* Reading DESIGN.md R7 (Henon's change of variable):                       */
+/*   s = 2X - 1,  r_0 = (r_min+r_max)/2 + (Delta/4)(3s - s^3)               */
+/*   g(s) = f(r_0) dr/ds = (3/4) Delta (1 - s^2) / sqrt(Q(r_0))  (bounded)  */
+/*   F = C_F max( sqrt(3 Delta / Q'(r_min)), sqrt(-3 Delta / Q'(r_max)) )   */
+/*   accept iff Q(r_0) > 0 and F X' < g.                                    */
+/* Random numbers: trial t of star `id` at step `step` uses                 */
+/* Philox4x32-10(counter = (id, 0, step, t), key = (seed_lo, seed_hi)):     */
+/* X from words 0,1 and X' from words 2,3 (53 bits each); the sign of the   */
+/* new v_r from bit 0 of word 3 (R8, R9).                         */
+/* All per-star arrays are compact, length count.                           */
+/* counters[0] += total trials (if counters != NULL).                       */
+/* ------------------------------------------------------------------------ */
+int hmc_ref_sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step,
+        const double *r, const double *phi, const double *m_cum,
+        uint64_t count,
+        const double *r_self, const double *v_r_self, const double *v_t_self,
+        const double *E_in, const double *J_in, const double *r_min_in, const double *r_max_in,
+        const uint32_t *k_min_in, const uint32_t *k_max_in, const uint32_t *id,
+        const uint8_t *status_in,
+        double *r_new, double *v_r_new, double *v_t_new, uint16_t *n_try, uint8_t *status_out,
+        uint64_t *counters)
+{
+    table T = { n, G, r, phi, m_cum };
+    const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    const double two_m53 = 1.0 / 9007199254740992.0;
+    uint64_t total_trials = 0;
+    for (uint64_t i = 0; i < count; ++i) {
+        unsigned st = status_in[i];
+        r_new[i] = r_self[i]; v_r_new[i] = v_r_self[i]; v_t_new[i] = v_t_self[i];
+        if (n_try) n_try[i] = 0;
+        if (st & (ST_UNBOUND | ST_RADIAL | ST_DEGENERATE)) { status_out[i] = (uint8_t)st; continue; }
+        double E = E_in[i], J = J_in[i], J2 = J * J;
+        double rmin = r_min_in[i], rmax = r_max_in[i];
+        uint64_t kmin = k_min_in[i], kmax = k_max_in[i];
+        double delta = rmax - rmin;
+        if (!(delta > 0.0)) { status_out[i] = (uint8_t)(st | ST_CIRCULAR); continue; }
+        /* end slopes Q'(r) = 2 J^2 / r^3 - 2 G M_j / r^2 inside the bracketing shells */
+        double Bmin = (kmin == 0) ? 0.0 : G * m_cum[kmin - 1];
+        double Bmax = (kmax == 0) ? 0.0 : G * m_cum[kmax - 1];
+        double q1 = (2.0 * (J2 / rmin - Bmin)) / (rmin * rmin);
+        double q2 = (2.0 * (J2 / rmax - Bmax)) / (rmax * rmax);
+        if (!(q1 > 0.0) || !(q2 < 0.0)) { status_out[i] = (uint8_t)(st | ST_CIRCULAR); continue; }
+        double F = C_F * fmax(sqrt((3.0 * delta) / q1), sqrt((3.0 * delta) / (-q2)));
+        double mid = 0.5 * (rmin + rmax);
+        double quarter = 0.25 * delta, three_q = 0.75 * delta;
+        int accepted = 0, have_good = 0;
+        double good_r = 0, good_Q = 0; uint32_t good_w3 = 0;
+        uint32_t t;
+        for (t = 0; t < T_MAX; ++t) {
+            uint32_t ctr[4] = { id[i], 0u, step, t }, w[4];
+            hmc_ref_philox4x32_10(ctr, key, w);
+            double X  = (double)((((uint64_t)w[0] << 32) | w[1]) >> 11) * two_m53;
+            double Xp = (double)((((uint64_t)w[2] << 32) | w[3]) >> 11) * two_m53;
+            double s = 2.0 * X - 1.0;
+            double r0 = mid + quarter * (3.0 * s - (s * s) * s);       /* replaces Eq. 14 */
+            uint64_t j = shell_of(&T, r0, kmin, kmax);
+            double phi0 = phi_in_shell(&T, j, r0);                      /* Eq. 6 */
+            double Q0 = 2.0 * (E - phi0) - J2 / (r0 * r0);              /* Eq. 12 */
+            if (Q0 > 0.0) {
+                double g = (three_q * (1.0 - s * s)) / sqrt(Q0);
+                have_good = 1; good_r = r0; good_Q = Q0; good_w3 = w[3];
+                if (g > F) st |= ST_CLIPPED;
+                if (F * Xp < g) { accepted = 1; break; }                /* Eq. 15 with f -> g */
+            }
+        }
+        uint32_t used = accepted ? t + 1 : T_MAX;
+        total_trials += used;
+        if (!accepted) st |= ST_MAXTRIES;
+        if (have_good) {
+            r_new[i] = good_r;
+            v_t_new[i] = J / good_r;
+            double vr = sqrt(good_Q);                                   /* v_r = Q^(1/2) */
+            v_r_new[i] = (good_w3 & 1u) ? -vr : vr;
+        }
+        if (n_try) n_try[i] = (uint16_t)used;
+        status_out[i] = (uint8_t)st;
+    }
+    if (counters) counters[0] += total_trials;
+    return 0;
+}
