@@ -1,0 +1,184 @@
+/*
+ * hmc.h -- C ABI of libhmc: the per-timestep orbit computation of the Henon Monte Carlo
+ * method (arXiv 1206.5878, Pattabiraman et al.; cited as PAPER.md:LINE) on one NVIDIA B200.
+ *
+ * One "orbit step" over N spherically symmetric stars is four calls, in this order:
+ *
+ *   hmc_sort_by_radius        PAPER.md:139  (step 6, "Sort stars by radial distance")
+ *   hmc_potential             PAPER.md:67-79 (step 1, Eq. 1-5)
+ *   hmc_orbit_turning_points  PAPER.md:117-124 (step 5, Eq. 12, bracket + analytic roots)
+ *   hmc_sample_new_radius     PAPER.md:126-137 (step 5, Eq. 13-15, rejection sampling)
+ *
+ * Conventions common to all calls
+ * -------------------------------
+ *  - Unless a parameter says "host", every array pointer is a DEVICE pointer owned by the
+ *    caller.  The library never allocates, frees or keeps device memory between calls; scratch
+ *    space is the caller's `workspace` of at least hmc_workspace_bytes(n) bytes, 256-byte aligned.
+ *  - Every call is asynchronous on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
+ *    legacy default stream) and never synchronises the host.
+ *  - Inputs are never modified; outputs must not alias inputs or each other.
+ *  - fp64 arrays must be 8-byte aligned, uint32 arrays 4-byte aligned.
+ *  - Arrays are 0-based; element a of a radius-sorted array is the paper's star k = a + 1.
+ *    Shell indices k_min / k_max use the paper's numbering: shell j is [r_j, r_{j+1}],
+ *    j = 0 (inside the innermost star) ... N (beyond the outermost star).
+ *  - n == 0 is a no-op returning HMC_OK.  n > HMC_MAX_N returns HMC_ERR_SIZE.
+ *  - Return value: HMC_OK or a negative call-level error; nothing is thrown.  A launch failure
+ *    returns HMC_ERR_CUDA and leaves the CUDA error readable through cudaGetLastError().
+ *  - Per-star data problems never fail a call: they set bits in `star_status` and the star is
+ *    left where it is (r_new = r, velocities unchanged).
+ *  - Arithmetic is IEEE-754 binary64 throughout, without fused multiply-add contraction; the
+ *    operation order of every formula is fixed in DESIGN.md ("Readings", R1p-R9) so that results
+ *    can be compared bit for bit with a CPU evaluation of the same formulas.
+ *  - Thread safety: calls are re-entrant when they use distinct workspaces.
+ */
+#ifndef HMC_H
+#define HMC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef int32_t hmc_status;
+
+#if defined(__GNUC__)
+#define HMC_API __attribute__((visibility("default")))
+#else
+#define HMC_API
+#endif
+
+#define HMC_OK              0
+#define HMC_ERR_NULL       (-1)  /* a required pointer is NULL                              */
+#define HMC_ERR_SIZE       (-2)  /* n > HMC_MAX_N, or ncols out of range                    */
+#define HMC_ERR_WORKSPACE  (-3)  /* workspace NULL, misaligned or smaller than required     */
+#define HMC_ERR_ALIGN      (-4)  /* an array pointer is not aligned to its element size     */
+#define HMC_ERR_CUDA       (-5)  /* a CUDA runtime call or kernel launch failed             */
+
+#define HMC_MAX_N      (1ull << 30)   /* stars per call                                     */
+#define HMC_MAX_COLS   8              /* fp64 record columns carried by the sort            */
+
+/* star_status bits */
+#define HMC_STAR_UNBOUND     1u   /* E >= 0 (or NaN): no apocentre; r_max = +inf, no draw           */
+#define HMC_STAR_RADIAL      2u   /* J^2 == 0: pericentre at r = 0; no draw                         */
+#define HMC_STAR_DEGENERATE  4u   /* outer quadratic has C >= 0 (cannot happen for a genuine bracket)*/
+#define HMC_STAR_CIRCULAR    8u   /* r_max - r_min <= 0 or end slopes of the wrong sign; no draw    */
+#define HMC_STAR_MAXTRIES   16u   /* rejection loop reached HMC_T_MAX trials                        */
+#define HMC_STAR_CLIPPED    32u   /* some trial had g > F (density clipped there); draw still valid */
+
+#define HMC_T_MAX   4096u         /* cap on rejection trials per star (R7)        */
+
+/* device counters accumulated (atomically) by the orbit calls; the caller zeroes them */
+enum {
+    HMC_CNT_UNBOUND = 0, HMC_CNT_RADIAL, HMC_CNT_DEGENERATE, HMC_CNT_CIRCULAR,
+    HMC_CNT_MAXTRIES, HMC_CNT_CLIPPED, HMC_CNT_TRIALS, HMC_CNT_RESERVED,
+    HMC_NCOUNTERS
+};
+
+/* Bytes of scratch any of the calls below may need for n stars (the maximum over the calls). */
+HMC_API size_t hmc_workspace_bytes(uint64_t n);
+
+/* Static string for a status code. */
+HMC_API const char* hmc_status_string(hmc_status s);
+
+/* Library version as major*10000 + minor*100 + patch. */
+HMC_API int32_t hmc_version(void);
+
+/*
+ * S1  "Sort stars by radial distance".
+ * Produces the unique ascending order by the pair (r_i, i): a stable sort, ties kept in
+ * input order (the paper's Quicksort leaves tie order open; R1).
+ *   r_in[n]        radii, finite and > 0 (their bit patterns are sorted as unsigned integers)
+ *   r_sorted[n]    out: radii ascending
+ *   perm[n]        out: perm[k] = index into r_in of the k-th smallest radius
+ *   ncols          0..HMC_MAX_COLS record columns to carry along
+ *   cols_in/out    HOST arrays of ncols DEVICE pointers: cols_out[c][k] = cols_in[c][perm[k]]
+ *   id_in/id_out   optional (both or neither NULL) persistent star-id column, gathered likewise
+ * Method: least-significant-digit radix sort of (key, index) pairs, 8-bit digits, one
+ * decoupled-look-back sweep per digit, then one gather of the record columns by perm.
+ */
+HMC_API hmc_status hmc_sort_by_radius(uint64_t n,
+        const double* r_in, double* r_sorted, uint32_t* perm,
+        int32_t ncols, const double* const* cols_in, double* const* cols_out,
+        const uint32_t* id_in, uint32_t* id_out,
+        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * S2  "Potential calculation".  On radius-sorted r, m:
+ *   m_cum[k] = M_k   = sum_{i<=k} m_i                       (Eq. 3, 5)
+ *   phi[k]   = Phi_k = -G ( M_k / r_k + sum_{i>k} m_i / r_i )   (Eq. 1 at r = r_k; == Eq. 2-5)
+ * Both sums are accumulated in double-double and rounded once (R1p).
+ * Preconditions: r ascending, finite, > 0; m >= 0.
+ */
+HMC_API hmc_status hmc_potential(uint64_t n, double G,
+        const double* r_sorted, const double* m_sorted,
+        double* phi, double* m_cum,
+        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * S3  Pericentre and apocentre of every star's orbit.
+ * For star k:  E = Phi_k + (v_r^2 + v_t^2)/2  (Eq. 16),  J = r_k v_t,
+ *   Q(r) = 2E - 2Phi(r) - J^2/r^2  (Eq. 12);
+ *   k_min = largest  j <= k-1 with Q(r_j) < 0   (node 0, r = 0, counts as negative)
+ *   k_max = (smallest j >= k+1 with Q(r_j) < 0) - 1   (node N+1, r = inf, counts as negative)
+ *   r_min / r_max = root of Q inside shell k_min / k_max, where Phi = Phi_j - G M_j (1/r - 1/r_j)
+ *   makes Q quadratic in 1/r (closed form; R3, R5).
+ * Outputs are [n] in the same (sorted) order.  star_status gets UNBOUND / RADIAL / DEGENERATE.
+ * counters: device uint64[HMC_NCOUNTERS], accumulated; may be NULL.
+ */
+HMC_API hmc_status hmc_orbit_turning_points(uint64_t n, double G,
+        const double* r_sorted, const double* v_r, const double* v_t,
+        const double* phi, const double* m_cum,
+        double* E, double* J, double* r_min, double* r_max,
+        uint32_t* k_min, uint32_t* k_max, uint8_t* star_status,
+        uint64_t* counters,
+        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * S4  New radial position on the orbit: von Neumann rejection with density
+ * proportional to 1/|v_r|, v_r = sqrt(Q(r)) (Eq. 13-15), in the variable s of DESIGN.md R7 that
+ * removes the end-point singularities the paper mentions.
+ * Trial t of the star with persistent id `id[k]` at step `step` uses
+ * Philox4x32-10(counter = (id, 0, step, t), key = (seed low word, seed high word)); a star's
+ * draw therefore does not depend on its position in the arrays (R9).
+ *   tables   r_sorted, phi, m_cum [n]
+ *   per star E, J, r_min, r_max, k_min, k_max, star_status_in (outputs of S3), id,
+ *            v_r, v_t (copied through for stars that are not drawn)
+ *   outputs  r_new, v_r_new, v_t_new [n]; n_try[n] (trials used, may be NULL);
+ *            star_status_out[n] (input bits plus CIRCULAR / MAXTRIES / CLIPPED)
+ * v_t_new = J / r_new, v_r_new = +-sqrt(Q(r_new)) with the sign from a spare random bit.
+ */
+HMC_API hmc_status hmc_sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step,
+        const double* r_sorted, const double* phi, const double* m_cum,
+        const double* v_r, const double* v_t,
+        const double* E, const double* J, const double* r_min, const double* r_max,
+        const uint32_t* k_min, const uint32_t* k_max, const uint32_t* id,
+        const uint8_t* star_status_in,
+        double* r_new, double* v_r_new, double* v_t_new, uint16_t* n_try,
+        uint8_t* star_status_out, uint64_t* counters,
+        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * Host-buffer variant of one whole orbit step (the four calls above, in order), for callers
+ * whose star data lives in HOST memory.  r, v_r, v_t, m, id are HOST arrays [n] (unsorted);
+ * r_new, v_r_new, v_t_new, m_out, id_out are HOST arrays [n] receiving the stars in radius-sorted
+ * order of the INPUT radii.  Host buffers should be page-locked for the copies to be asynchronous.
+ * `device_arena` is a DEVICE buffer of at least hmc_step_host_arena_bytes(n) bytes (256-byte
+ * aligned) holding the staged columns, every intermediate and the workspace.
+ * The call enqueues H2D copies, the four stages and D2H copies on `cuda_stream`; the host arrays
+ * are valid after the caller synchronises the stream.  counters_host (HOST uint64[HMC_NCOUNTERS],
+ * may be NULL) receives the step's counters.
+ */
+HMC_API size_t hmc_step_host_arena_bytes(uint64_t n);
+
+HMC_API hmc_status hmc_step_host(uint64_t n, double G, uint64_t seed, uint32_t step,
+        const double* r, const double* v_r, const double* v_t, const double* m, const uint32_t* id,
+        double* r_new, double* v_r_new, double* v_t_new, double* m_out, uint32_t* id_out,
+        uint64_t* counters_host,
+        void* device_arena, size_t arena_bytes, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HMC_H */

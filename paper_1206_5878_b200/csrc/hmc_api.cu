@@ -1,0 +1,217 @@
+// hmc_api.cu -- extern "C" boundary of libhmc (include/hmc.h): argument checks, workspace
+// carve-up, stream plumbing.  No arithmetic of the method lives here.
+#include "hmc_common.cuh"
+
+namespace hmc {
+
+int sm_count()
+{
+    static int cached = 0;
+    if (cached == 0) {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+            cached = sms;
+        else
+            cached = HMC_SM_COUNT_FALLBACK;
+    }
+    return cached;
+}
+
+static hmc_status check_ws(const void* ws, size_t bytes, uint64_t n)
+{
+    if (!ws) return HMC_ERR_WORKSPACE;
+    if (misaligned(ws, 256)) return HMC_ERR_WORKSPACE;
+    if (bytes < carve(nullptr, n).total) return HMC_ERR_WORKSPACE;
+    return HMC_OK;
+}
+
+// arena of the host-buffer step: every device array the four stages touch
+struct Arena {
+    double *r, *vr, *vt, *m;             // staged inputs (unsorted)
+    uint32_t* id;
+    double *rs, *vrs, *vts, *ms;         // sorted
+    uint32_t *ids, *perm;
+    double *phi, *mcum, *E, *J, *rmin, *rmax;
+    uint32_t *kmin, *kmax;
+    uint8_t *st0, *st1;
+    double *rn, *vrn, *vtn;
+    uint64_t* counters;
+    void* ws;
+    size_t ws_bytes;
+    size_t total;
+};
+
+static Arena carve_arena(void* base, uint64_t n)
+{
+    Arena a;
+    char* p = static_cast<char*>(base);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { char* q = p ? p + off : nullptr; off += align_up(bytes, 256); return q; };
+    auto f64 = [&]() { return reinterpret_cast<double*>(take(n * 8)); };
+    auto u32 = [&]() { return reinterpret_cast<uint32_t*>(take(n * 4)); };
+    auto u8 = [&]() { return reinterpret_cast<uint8_t*>(take(n)); };
+    a.r = f64(); a.vr = f64(); a.vt = f64(); a.m = f64(); a.id = u32();
+    a.rs = f64(); a.vrs = f64(); a.vts = f64(); a.ms = f64(); a.ids = u32(); a.perm = u32();
+    a.phi = f64(); a.mcum = f64(); a.E = f64(); a.J = f64(); a.rmin = f64(); a.rmax = f64();
+    a.kmin = u32(); a.kmax = u32(); a.st0 = u8(); a.st1 = u8();
+    a.rn = f64(); a.vrn = f64(); a.vtn = f64();
+    a.counters = reinterpret_cast<uint64_t*>(take(HMC_NCOUNTERS * 8));
+    a.ws_bytes = carve(nullptr, n).total;
+    a.ws = take(a.ws_bytes);
+    a.total = off;
+    return a;
+}
+
+}  // namespace hmc
+
+using namespace hmc;
+
+#define REQUIRE_PTR(p)  do { if (!(p)) return HMC_ERR_NULL; } while (0)
+#define REQUIRE_ALIGN(p, a) do { if (misaligned((p), (a))) return HMC_ERR_ALIGN; } while (0)
+
+extern "C" {
+
+size_t hmc_workspace_bytes(uint64_t n) { return carve(nullptr, n).total; }
+
+int32_t hmc_version(void) { return 100; }
+
+const char* hmc_status_string(hmc_status s)
+{
+    switch (s) {
+        case HMC_OK: return "HMC_OK";
+        case HMC_ERR_NULL: return "HMC_ERR_NULL: a required pointer is NULL";
+        case HMC_ERR_SIZE: return "HMC_ERR_SIZE: n or ncols out of range";
+        case HMC_ERR_WORKSPACE: return "HMC_ERR_WORKSPACE: workspace NULL, misaligned or too small";
+        case HMC_ERR_ALIGN: return "HMC_ERR_ALIGN: array pointer not aligned to its element size";
+        case HMC_ERR_CUDA: return "HMC_ERR_CUDA: CUDA runtime call or kernel launch failed";
+        default: return "HMC: unknown status";
+    }
+}
+
+hmc_status hmc_sort_by_radius(uint64_t n, const double* r_in, double* r_sorted, uint32_t* perm, int32_t ncols,
+                              const double* const* cols_in, double* const* cols_out, const uint32_t* id_in,
+                              uint32_t* id_out, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (n > HMC_MAX_N || ncols < 0 || ncols > HMC_MAX_COLS) return HMC_ERR_SIZE;
+    if (n == 0) return HMC_OK;
+    REQUIRE_PTR(r_in); REQUIRE_PTR(r_sorted); REQUIRE_PTR(perm);
+    if (ncols > 0) { REQUIRE_PTR(cols_in); REQUIRE_PTR(cols_out); }
+    for (int c = 0; c < ncols; ++c) {
+        REQUIRE_PTR(cols_in[c]); REQUIRE_PTR(cols_out[c]);
+        REQUIRE_ALIGN(cols_in[c], 8); REQUIRE_ALIGN(cols_out[c], 8);
+    }
+    if ((id_in == nullptr) != (id_out == nullptr)) return HMC_ERR_NULL;
+    REQUIRE_ALIGN(r_in, 8); REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(perm, 4);
+    if (id_in) { REQUIRE_ALIGN(id_in, 4); REQUIRE_ALIGN(id_out, 4); }
+    hmc_status s = check_ws(workspace, workspace_bytes, n);
+    if (s != HMC_OK) return s;
+    return sort_by_radius(n, r_in, r_sorted, perm, ncols, cols_in, cols_out, id_in, id_out, carve(workspace, n),
+                          static_cast<cudaStream_t>(cuda_stream));
+}
+
+hmc_status hmc_potential(uint64_t n, double G, const double* r_sorted, const double* m_sorted, double* phi,
+                         double* m_cum, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (n > HMC_MAX_N) return HMC_ERR_SIZE;
+    if (n == 0) return HMC_OK;
+    REQUIRE_PTR(r_sorted); REQUIRE_PTR(m_sorted); REQUIRE_PTR(phi); REQUIRE_PTR(m_cum);
+    REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(m_sorted, 8); REQUIRE_ALIGN(phi, 8); REQUIRE_ALIGN(m_cum, 8);
+    hmc_status s = check_ws(workspace, workspace_bytes, n);
+    if (s != HMC_OK) return s;
+    return potential(n, G, r_sorted, m_sorted, phi, m_cum, carve(workspace, n), static_cast<cudaStream_t>(cuda_stream));
+}
+
+hmc_status hmc_orbit_turning_points(uint64_t n, double G, const double* r_sorted, const double* v_r,
+                                    const double* v_t, const double* phi, const double* m_cum, double* E, double* J,
+                                    double* r_min, double* r_max, uint32_t* k_min, uint32_t* k_max,
+                                    uint8_t* star_status, uint64_t* counters, void* workspace,
+                                    size_t workspace_bytes, void* cuda_stream)
+{
+    if (n > HMC_MAX_N) return HMC_ERR_SIZE;
+    if (n == 0) return HMC_OK;
+    REQUIRE_PTR(r_sorted); REQUIRE_PTR(v_r); REQUIRE_PTR(v_t); REQUIRE_PTR(phi); REQUIRE_PTR(m_cum);
+    REQUIRE_PTR(E); REQUIRE_PTR(J); REQUIRE_PTR(r_min); REQUIRE_PTR(r_max); REQUIRE_PTR(k_min); REQUIRE_PTR(k_max);
+    REQUIRE_PTR(star_status);
+    REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(v_r, 8); REQUIRE_ALIGN(v_t, 8); REQUIRE_ALIGN(phi, 8);
+    REQUIRE_ALIGN(m_cum, 8); REQUIRE_ALIGN(E, 8); REQUIRE_ALIGN(J, 8); REQUIRE_ALIGN(r_min, 8);
+    REQUIRE_ALIGN(r_max, 8); REQUIRE_ALIGN(k_min, 4); REQUIRE_ALIGN(k_max, 4);
+    if (counters) REQUIRE_ALIGN(counters, 8);
+    hmc_status s = check_ws(workspace, workspace_bytes, n);
+    if (s != HMC_OK) return s;
+    return turning_points(n, G, r_sorted, v_r, v_t, phi, m_cum, E, J, r_min, r_max, k_min, k_max, star_status,
+                          counters, carve(workspace, n), static_cast<cudaStream_t>(cuda_stream));
+}
+
+hmc_status hmc_sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step, const double* r_sorted,
+                                 const double* phi, const double* m_cum, const double* v_r, const double* v_t,
+                                 const double* E, const double* J, const double* r_min, const double* r_max,
+                                 const uint32_t* k_min, const uint32_t* k_max, const uint32_t* id,
+                                 const uint8_t* star_status_in, double* r_new, double* v_r_new, double* v_t_new,
+                                 uint16_t* n_try, uint8_t* star_status_out, uint64_t* counters, void* workspace,
+                                 size_t workspace_bytes, void* cuda_stream)
+{
+    if (n > HMC_MAX_N) return HMC_ERR_SIZE;
+    if (n == 0) return HMC_OK;
+    REQUIRE_PTR(r_sorted); REQUIRE_PTR(phi); REQUIRE_PTR(m_cum); REQUIRE_PTR(v_r); REQUIRE_PTR(v_t);
+    REQUIRE_PTR(E); REQUIRE_PTR(J); REQUIRE_PTR(r_min); REQUIRE_PTR(r_max); REQUIRE_PTR(k_min); REQUIRE_PTR(k_max);
+    REQUIRE_PTR(id); REQUIRE_PTR(star_status_in); REQUIRE_PTR(r_new); REQUIRE_PTR(v_r_new); REQUIRE_PTR(v_t_new);
+    REQUIRE_PTR(star_status_out);
+    REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(phi, 8); REQUIRE_ALIGN(m_cum, 8); REQUIRE_ALIGN(v_r, 8);
+    REQUIRE_ALIGN(v_t, 8); REQUIRE_ALIGN(E, 8); REQUIRE_ALIGN(J, 8); REQUIRE_ALIGN(r_min, 8); REQUIRE_ALIGN(r_max, 8);
+    REQUIRE_ALIGN(k_min, 4); REQUIRE_ALIGN(k_max, 4); REQUIRE_ALIGN(id, 4); REQUIRE_ALIGN(r_new, 8);
+    REQUIRE_ALIGN(v_r_new, 8); REQUIRE_ALIGN(v_t_new, 8);
+    if (n_try) REQUIRE_ALIGN(n_try, 2);
+    if (counters) REQUIRE_ALIGN(counters, 8);
+    hmc_status s = check_ws(workspace, workspace_bytes, n);
+    if (s != HMC_OK) return s;
+    return sample_new_radius(n, G, seed, step, r_sorted, phi, m_cum, v_r, v_t, E, J, r_min, r_max, k_min, k_max, id,
+                             star_status_in, r_new, v_r_new, v_t_new, n_try, star_status_out, counters,
+                             carve(workspace, n), static_cast<cudaStream_t>(cuda_stream));
+}
+
+size_t hmc_step_host_arena_bytes(uint64_t n) { return carve_arena(nullptr, n).total; }
+
+hmc_status hmc_step_host(uint64_t n, double G, uint64_t seed, uint32_t step, const double* r, const double* v_r,
+                         const double* v_t, const double* m, const uint32_t* id, double* r_new, double* v_r_new,
+                         double* v_t_new, double* m_out, uint32_t* id_out, uint64_t* counters_host,
+                         void* device_arena, size_t arena_bytes, void* cuda_stream)
+{
+    if (n > HMC_MAX_N) return HMC_ERR_SIZE;
+    if (n == 0) return HMC_OK;
+    REQUIRE_PTR(r); REQUIRE_PTR(v_r); REQUIRE_PTR(v_t); REQUIRE_PTR(m); REQUIRE_PTR(id);
+    REQUIRE_PTR(r_new); REQUIRE_PTR(v_r_new); REQUIRE_PTR(v_t_new); REQUIRE_PTR(m_out); REQUIRE_PTR(id_out);
+    if (!device_arena || misaligned(device_arena, 256)) return HMC_ERR_WORKSPACE;
+    Arena a = carve_arena(device_arena, n);
+    if (arena_bytes < a.total) return HMC_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    HMC_CUDA_TRY(cudaMemcpyAsync(a.r, r, n * 8, cudaMemcpyHostToDevice, st));
+    HMC_CUDA_TRY(cudaMemcpyAsync(a.vr, v_r, n * 8, cudaMemcpyHostToDevice, st));
+    HMC_CUDA_TRY(cudaMemcpyAsync(a.vt, v_t, n * 8, cudaMemcpyHostToDevice, st));
+    HMC_CUDA_TRY(cudaMemcpyAsync(a.m, m, n * 8, cudaMemcpyHostToDevice, st));
+    HMC_CUDA_TRY(cudaMemcpyAsync(a.id, id, n * 4, cudaMemcpyHostToDevice, st));
+    HMC_CUDA_TRY(cudaMemsetAsync(a.counters, 0, HMC_NCOUNTERS * 8, st));
+    Workspace ws = carve(a.ws, n);
+    const double* cin[3] = { a.vr, a.vt, a.m };
+    double* cout[3] = { a.vrs, a.vts, a.ms };
+    hmc_status s = sort_by_radius(n, a.r, a.rs, a.perm, 3, cin, cout, a.id, a.ids, ws, st);
+    if (s != HMC_OK) return s;
+    s = potential(n, G, a.rs, a.ms, a.phi, a.mcum, ws, st);
+    if (s != HMC_OK) return s;
+    s = turning_points(n, G, a.rs, a.vrs, a.vts, a.phi, a.mcum, a.E, a.J, a.rmin, a.rmax, a.kmin, a.kmax, a.st0,
+                       a.counters, ws, st);
+    if (s != HMC_OK) return s;
+    s = sample_new_radius(n, G, seed, step, a.rs, a.phi, a.mcum, a.vrs, a.vts, a.E, a.J, a.rmin, a.rmax, a.kmin,
+                          a.kmax, a.ids, a.st0, a.rn, a.vrn, a.vtn, nullptr, a.st1, a.counters, ws, st);
+    if (s != HMC_OK) return s;
+    HMC_CUDA_TRY(cudaMemcpyAsync(r_new, a.rn, n * 8, cudaMemcpyDeviceToHost, st));
+    HMC_CUDA_TRY(cudaMemcpyAsync(v_r_new, a.vrn, n * 8, cudaMemcpyDeviceToHost, st));
+    HMC_CUDA_TRY(cudaMemcpyAsync(v_t_new, a.vtn, n * 8, cudaMemcpyDeviceToHost, st));
+    HMC_CUDA_TRY(cudaMemcpyAsync(m_out, a.ms, n * 8, cudaMemcpyDeviceToHost, st));
+    HMC_CUDA_TRY(cudaMemcpyAsync(id_out, a.ids, n * 4, cudaMemcpyDeviceToHost, st));
+    if (counters_host)
+        HMC_CUDA_TRY(cudaMemcpyAsync(counters_host, a.counters, HMC_NCOUNTERS * 8, cudaMemcpyDeviceToHost, st));
+    return HMC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,164 @@
+// hmc_common.cuh -- shared by the kernels of libhmc (sm_100a only).
+// Compiled with -fmad=false: every fp64 +,-,*,/,sqrt below is one IEEE-754 operation in the
+// order written (R2).  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "hmc.h"
+
+#define HMC_SM_COUNT_FALLBACK 148
+
+namespace hmc {
+
+// ---- host-side checks ---------------------------------------------------------------------
+static inline bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) != 0; }
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+static inline uint64_t umin64(uint64_t a, uint64_t b) { return a < b ? a : b; }
+
+static inline hmc_status cuda_ok(cudaError_t e) { return e == cudaSuccess ? HMC_OK : HMC_ERR_CUDA; }
+
+#define HMC_CUDA_TRY(expr)                                   \
+    do {                                                     \
+        cudaError_t _e = (expr);                             \
+        if (_e != cudaSuccess) return HMC_ERR_CUDA;          \
+    } while (0)
+
+#define HMC_LAUNCH_CHECK()                                   \
+    do {                                                     \
+        if (cudaPeekAtLastError() != cudaSuccess) return HMC_ERR_CUDA; \
+    } while (0)
+
+int sm_count();   // cached multiprocessor count of the current device
+
+// ---- workspace layout (one carve-up used by every call) -------------------------------------
+// All offsets are multiples of 256 bytes.
+struct Workspace {
+    // sort
+    uint64_t* keys_alt;      // [n]
+    uint32_t* vals_alt;      // [n]
+    uint32_t* digit_hist;    // [8][256] global digit counts -> exclusive bin offsets
+    uint32_t* lookback;      // [8][sort_tiles][256] tile status words
+    uint32_t* tickets;       // [32]: sort tile tickets 0..7, sort pass_live 8..15, scan tickets 16..17
+    // potential
+    double*   scan_status;   // [2][scan_tiles][8] (flag, agg_hi, agg_lo, inc_hi, inc_lo, pad)
+    // orbit
+    double2*  rphi;          // [n] interleaved (r_j, Phi_j) search table
+    size_t    total;
+};
+
+static constexpr int SORT_TILE = 4096;     // keys per sort tile
+static constexpr int SCAN_TILE = 2048;     // elements per scan tile
+
+static inline Workspace carve(void* base, uint64_t n)
+{
+    Workspace w;
+    char* p = static_cast<char*>(base);
+    size_t off = 0;
+    const uint64_t sort_tiles = (n + SORT_TILE - 1) / SORT_TILE;
+    const uint64_t scan_tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
+    auto take = [&](size_t bytes) { char* q = p ? p + off : nullptr; off += align_up(bytes, 256); return q; };
+    w.keys_alt    = reinterpret_cast<uint64_t*>(take(n * 8));
+    w.vals_alt    = reinterpret_cast<uint32_t*>(take(n * 4));
+    w.digit_hist  = reinterpret_cast<uint32_t*>(take(8 * 256 * 4));
+    w.lookback    = reinterpret_cast<uint32_t*>(take(8 * sort_tiles * 256 * 4));
+    w.tickets     = reinterpret_cast<uint32_t*>(take(32 * 4));
+    w.scan_status = reinterpret_cast<double*>(take(2 * scan_tiles * 8 * 8));
+    w.rphi        = reinterpret_cast<double2*>(take(n * 16));
+    w.total = off;
+    return w;
+}
+
+#ifdef __CUDACC__
+// ---- double-double arithmetic (error-free transformations; needs -fmad=false) ---------------
+struct dd { double hi, lo; };
+
+__device__ __forceinline__ dd two_sum(double a, double b)
+{
+    double s = a + b;
+    double bb = s - a;
+    double e = (a - (s - bb)) + (b - bb);
+    return dd{ s, e };
+}
+
+__device__ __forceinline__ dd quick_two_sum(double a, double b)   // requires |a| >= |b|
+{
+    double s = a + b;
+    double e = b - (s - a);
+    return dd{ s, e };
+}
+
+// accurate double-double addition (both components through two_sum), result normalised:
+// |lo| <= ulp(hi)/2, so hi is the double-double value rounded to nearest binary64.
+__device__ __forceinline__ dd dd_add(dd a, dd b)
+{
+    dd s = two_sum(a.hi, b.hi);
+    dd t = two_sum(a.lo, b.lo);
+    s.lo += t.hi;
+    s = quick_two_sum(s.hi, s.lo);
+    s.lo += t.lo;
+    return quick_two_sum(s.hi, s.lo);
+}
+
+__device__ __forceinline__ dd dd_add_d(dd a, double b)
+{
+    dd s = two_sum(a.hi, b);
+    s.lo += a.lo;
+    return quick_two_sum(s.hi, s.lo);
+}
+
+__device__ __forceinline__ dd dd_shfl_up(dd v, int delta)
+{
+    return dd{ __shfl_up_sync(0xffffffffu, v.hi, delta), __shfl_up_sync(0xffffffffu, v.lo, delta) };
+}
+
+// ---- memory helpers -------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t* p)
+{
+    uint32_t v;
+    asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ double ld_volatile_f64(const double* p)
+{
+    double v;
+    asm volatile("ld.volatile.global.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void st_volatile_f64(double* p, double v)
+{
+    asm volatile("st.volatile.global.f64 [%0], %1;" ::"l"(p), "d"(v));
+}
+__device__ __forceinline__ void st_volatile_u32(uint32_t* p, uint32_t v)
+{
+    asm volatile("st.volatile.global.u32 [%0], %1;" ::"l"(p), "r"(v));
+}
+
+__device__ __forceinline__ unsigned lanemask_lt()
+{
+    unsigned m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+#endif  // __CUDACC__
+
+// stage entry points implemented in the .cu files (same signatures as hmc.h, Workspace carved)
+hmc_status sort_by_radius(uint64_t n, const double* r_in, double* r_sorted, uint32_t* perm, int ncols,
+                          const double* const* cols_in, double* const* cols_out, const uint32_t* id_in,
+                          uint32_t* id_out, const Workspace& ws, cudaStream_t st);
+hmc_status potential(uint64_t n, double G, const double* r, const double* m, double* phi, double* m_cum,
+                     const Workspace& ws, cudaStream_t st);
+hmc_status turning_points(uint64_t n, double G, const double* r, const double* v_r, const double* v_t,
+                          const double* phi, const double* m_cum, double* E, double* J, double* r_min,
+                          double* r_max, uint32_t* k_min, uint32_t* k_max, uint8_t* status, uint64_t* counters,
+                          const Workspace& ws, cudaStream_t st);
+hmc_status sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step, const double* r,
+                             const double* phi, const double* m_cum, const double* v_r, const double* v_t,
+                             const double* E, const double* J, const double* r_min, const double* r_max,
+                             const uint32_t* k_min, const uint32_t* k_max, const uint32_t* id,
+                             const uint8_t* status_in, double* r_new, double* v_r_new, double* v_t_new,
+                             uint16_t* n_try, uint8_t* status_out, uint64_t* counters, const Workspace& ws,
+                             cudaStream_t st);
+
+}  // namespace hmc

@@ -1,0 +1,268 @@
+"""Thin binding over libhmc.so (C ABI declared in include/hmc.h).
+
+Argument marshalling only: every step of the path runs in the CUDA kernels of the library.
+torch is used for device memory and the current stream, nothing else.  There is no CPU
+fallback: if the library cannot be loaded, or a tensor is not a contiguous CUDA tensor of the
+right dtype, the call raises.
+
+The function names are those of the C ABI.  Outputs may be passed in (``out=...`` style keyword
+arguments) to avoid allocation inside a timed loop; otherwise they are allocated with
+``torch.empty`` on the inputs' device.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libhmc.so")
+
+ST_UNBOUND, ST_RADIAL, ST_DEGENERATE, ST_CIRCULAR, ST_MAXTRIES, ST_CLIPPED = 1, 2, 4, 8, 16, 32
+COUNTER_NAMES = ("unbound", "radial", "degenerate", "circular", "maxtries", "clipped", "trials", "reserved")
+NCOUNTERS = 8
+MAX_N = 1 << 30
+
+_lib = None
+
+
+class HmcError(RuntimeError):
+    pass
+
+
+def lib() -> ctypes.CDLL:
+    """Load libhmc.so (built in-tree by paper_1206_5878_b200.build).  Raises if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise HmcError("libhmc.so not found at %s; run `python -m paper_1206_5878_b200.build` "
+                           "(there is no CPU fallback)" % LIB_PATH)
+        L = ctypes.CDLL(LIB_PATH)
+        L.hmc_workspace_bytes.restype = ctypes.c_size_t
+        L.hmc_workspace_bytes.argtypes = [ctypes.c_uint64]
+        L.hmc_step_host_arena_bytes.restype = ctypes.c_size_t
+        L.hmc_step_host_arena_bytes.argtypes = [ctypes.c_uint64]
+        L.hmc_status_string.restype = ctypes.c_char_p
+        L.hmc_status_string.argtypes = [ctypes.c_int32]
+        L.hmc_version.restype = ctypes.c_int32
+        for name in ("hmc_sort_by_radius", "hmc_potential", "hmc_orbit_turning_points", "hmc_sample_new_radius",
+                     "hmc_step_host"):
+            getattr(L, name).restype = ctypes.c_int32
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise HmcError("%s failed: %s" % (what, lib().hmc_status_string(rc).decode()))
+
+
+def _dev(t: Optional[torch.Tensor], dtype, n: int, name: str):
+    if t is None:
+        return ctypes.c_void_p(0)
+    if not t.is_cuda:
+        raise HmcError("%s must be a CUDA tensor (no CPU path)" % name)
+    if t.dtype != dtype or not t.is_contiguous() or t.numel() != n:
+        raise HmcError("%s must be contiguous %s[%d], got %s%s" % (name, dtype, n, t.dtype, tuple(t.shape)))
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def workspace_bytes(n: int) -> int:
+    return int(lib().hmc_workspace_bytes(ctypes.c_uint64(n)))
+
+
+def alloc_workspace(n: int, device="cuda") -> torch.Tensor:
+    return torch.empty(max(workspace_bytes(n), 256), dtype=torch.uint8, device=device)
+
+
+def alloc_counters(device="cuda") -> torch.Tensor:
+    return torch.zeros(NCOUNTERS, dtype=torch.int64, device=device)
+
+
+def _ws(workspace, n, device):
+    if workspace is None:
+        workspace = alloc_workspace(n, device)
+    return workspace, ctypes.c_void_p(workspace.data_ptr()), ctypes.c_size_t(workspace.numel())
+
+
+def hmc_sort_by_radius(r_in: torch.Tensor, cols: Sequence[torch.Tensor] = (), ids: Optional[torch.Tensor] = None, *,
+                       r_sorted=None, perm=None, cols_out=None, ids_out=None, workspace=None):
+    """S1.  -> (r_sorted, perm, [cols_sorted...], ids_sorted or None)"""
+    n = r_in.numel()
+    dev = r_in.device
+    r_sorted = torch.empty(n, dtype=torch.float64, device=dev) if r_sorted is None else r_sorted
+    perm = torch.empty(n, dtype=torch.int32, device=dev) if perm is None else perm
+    cols = list(cols)
+    cols_out = [torch.empty(n, dtype=torch.float64, device=dev) for _ in cols] if cols_out is None else list(cols_out)
+    if ids is not None and ids_out is None:
+        ids_out = torch.empty(n, dtype=torch.int32, device=dev)
+    nc = len(cols)
+    Arr = ctypes.c_void_p * max(nc, 1)
+    cin = Arr(*[_dev(c, torch.float64, n, "cols[%d]" % i).value or 0 for i, c in enumerate(cols)])
+    cout = Arr(*[_dev(c, torch.float64, n, "cols_out[%d]" % i).value or 0 for i, c in enumerate(cols_out)])
+    workspace, wp, wb = _ws(workspace, n, dev)
+    rc = lib().hmc_sort_by_radius(ctypes.c_uint64(n), _dev(r_in, torch.float64, n, "r_in"),
+                                  _dev(r_sorted, torch.float64, n, "r_sorted"), _dev(perm, torch.int32, n, "perm"),
+                                  ctypes.c_int32(nc), cin, cout, _dev(ids, torch.int32, n, "ids"),
+                                  _dev(ids_out, torch.int32, n, "ids_out"), wp, wb, _stream())
+    _check(rc, "hmc_sort_by_radius")
+    return r_sorted, perm, cols_out, ids_out
+
+
+def hmc_potential(r_sorted: torch.Tensor, m_sorted: torch.Tensor, G: float = 1.0, *, phi=None, m_cum=None,
+                  workspace=None):
+    """S2.  -> (phi, m_cum)"""
+    n = r_sorted.numel()
+    dev = r_sorted.device
+    phi = torch.empty(n, dtype=torch.float64, device=dev) if phi is None else phi
+    m_cum = torch.empty(n, dtype=torch.float64, device=dev) if m_cum is None else m_cum
+    workspace, wp, wb = _ws(workspace, n, dev)
+    rc = lib().hmc_potential(ctypes.c_uint64(n), ctypes.c_double(G), _dev(r_sorted, torch.float64, n, "r_sorted"),
+                             _dev(m_sorted, torch.float64, n, "m_sorted"), _dev(phi, torch.float64, n, "phi"),
+                             _dev(m_cum, torch.float64, n, "m_cum"), wp, wb, _stream())
+    _check(rc, "hmc_potential")
+    return phi, m_cum
+
+
+def hmc_orbit_turning_points(r_sorted, v_r, v_t, phi, m_cum, G: float = 1.0, *, out=None, counters=None,
+                             workspace=None):
+    """S3.  -> dict(E, J, r_min, r_max, k_min, k_max, status)"""
+    n = r_sorted.numel()
+    dev = r_sorted.device
+    if out is None:
+        out = alloc_turning_points(n, dev)
+    workspace, wp, wb = _ws(workspace, n, dev)
+    f = torch.float64
+    rc = lib().hmc_orbit_turning_points(
+        ctypes.c_uint64(n), ctypes.c_double(G), _dev(r_sorted, f, n, "r_sorted"), _dev(v_r, f, n, "v_r"),
+        _dev(v_t, f, n, "v_t"), _dev(phi, f, n, "phi"), _dev(m_cum, f, n, "m_cum"), _dev(out["E"], f, n, "E"),
+        _dev(out["J"], f, n, "J"), _dev(out["r_min"], f, n, "r_min"), _dev(out["r_max"], f, n, "r_max"),
+        _dev(out["k_min"], torch.int32, n, "k_min"), _dev(out["k_max"], torch.int32, n, "k_max"),
+        _dev(out["status"], torch.uint8, n, "status"), _dev(counters, torch.int64, NCOUNTERS, "counters"), wp, wb,
+        _stream())
+    _check(rc, "hmc_orbit_turning_points")
+    return out
+
+
+def alloc_turning_points(n: int, device="cuda"):
+    f = dict(dtype=torch.float64, device=device)
+    i = dict(dtype=torch.int32, device=device)
+    return dict(E=torch.empty(n, **f), J=torch.empty(n, **f), r_min=torch.empty(n, **f), r_max=torch.empty(n, **f),
+                k_min=torch.empty(n, **i), k_max=torch.empty(n, **i),
+                status=torch.empty(n, dtype=torch.uint8, device=device))
+
+
+def alloc_sample(n: int, device="cuda", with_n_try: bool = True):
+    f = dict(dtype=torch.float64, device=device)
+    return dict(r_new=torch.empty(n, **f), v_r_new=torch.empty(n, **f), v_t_new=torch.empty(n, **f),
+                n_try=torch.empty(n, dtype=torch.int16, device=device) if with_n_try else None,
+                status=torch.empty(n, dtype=torch.uint8, device=device))
+
+
+def hmc_sample_new_radius(r_sorted, phi, m_cum, v_r, v_t, tp, ids, seed: int, step: int, G: float = 1.0, *,
+                          out=None, counters=None, workspace=None):
+    """S4.  ``tp`` is the dict returned by hmc_orbit_turning_points.
+    -> dict(r_new, v_r_new, v_t_new, n_try, status)"""
+    n = r_sorted.numel()
+    dev = r_sorted.device
+    if out is None:
+        out = alloc_sample(n, dev)
+    workspace, wp, wb = _ws(workspace, n, dev)
+    f = torch.float64
+    rc = lib().hmc_sample_new_radius(
+        ctypes.c_uint64(n), ctypes.c_double(G), ctypes.c_uint64(seed), ctypes.c_uint32(step),
+        _dev(r_sorted, f, n, "r_sorted"), _dev(phi, f, n, "phi"), _dev(m_cum, f, n, "m_cum"), _dev(v_r, f, n, "v_r"),
+        _dev(v_t, f, n, "v_t"), _dev(tp["E"], f, n, "E"), _dev(tp["J"], f, n, "J"), _dev(tp["r_min"], f, n, "r_min"),
+        _dev(tp["r_max"], f, n, "r_max"), _dev(tp["k_min"], torch.int32, n, "k_min"),
+        _dev(tp["k_max"], torch.int32, n, "k_max"), _dev(ids, torch.int32, n, "ids"),
+        _dev(tp["status"], torch.uint8, n, "status_in"), _dev(out["r_new"], f, n, "r_new"),
+        _dev(out["v_r_new"], f, n, "v_r_new"), _dev(out["v_t_new"], f, n, "v_t_new"),
+        _dev(out.get("n_try"), torch.int16, n, "n_try"), _dev(out["status"], torch.uint8, n, "status_out"),
+        _dev(counters, torch.int64, NCOUNTERS, "counters"), wp, wb, _stream())
+    _check(rc, "hmc_sample_new_radius")
+    return out
+
+
+class OrbitStepper:
+    """Pre-allocated device state for repeated orbit steps (sort -> potential -> turning points ->
+    new radius), the loop of BASELINE.json's multi-step configs.  Holds the carried state
+    (r, v_r, v_t, m, id) and every intermediate; ``step()`` makes the four C-ABI calls on the
+    current stream and swaps (r, v_r, v_t) <- (r_new, v_r', v_t'); m and id follow the sort."""
+
+    KERNELS_PER_STEP = 2 + 8 + 1 + 1 + 2 + 2 + 1   # hist, scan, 8 passes, iota, gather, 2 scans, table, S3, S4
+
+    def __init__(self, r, v_r, v_t, m, ids, seed: int, G: float = 1.0, with_n_try: bool = True):
+        self.n = n = r.numel()
+        dev = r.device
+        self.G, self.seed, self.step_index = G, seed, 0
+        self.state = dict(r=r.clone(), v_r=v_r.clone(), v_t=v_t.clone(), m=m.clone(), id=ids.clone())
+        f = dict(dtype=torch.float64, device=dev)
+        self.sorted = dict(r=torch.empty(n, **f), v_r=torch.empty(n, **f), v_t=torch.empty(n, **f),
+                           m=torch.empty(n, **f), id=torch.empty(n, dtype=torch.int32, device=dev),
+                           perm=torch.empty(n, dtype=torch.int32, device=dev))
+        self.phi = torch.empty(n, **f)
+        self.m_cum = torch.empty(n, **f)
+        self.tp = alloc_turning_points(n, dev)
+        self.sample = alloc_sample(n, dev, with_n_try)
+        self.counters = alloc_counters(dev)
+        self.workspace = alloc_workspace(n, dev)
+
+    def step(self):
+        s, so = self.state, self.sorted
+        hmc_sort_by_radius(s["r"], (s["v_r"], s["v_t"], s["m"]), s["id"], r_sorted=so["r"], perm=so["perm"],
+                           cols_out=(so["v_r"], so["v_t"], so["m"]), ids_out=so["id"], workspace=self.workspace)
+        hmc_potential(so["r"], so["m"], self.G, phi=self.phi, m_cum=self.m_cum, workspace=self.workspace)
+        hmc_orbit_turning_points(so["r"], so["v_r"], so["v_t"], self.phi, self.m_cum, self.G, out=self.tp,
+                                 counters=self.counters, workspace=self.workspace)
+        hmc_sample_new_radius(so["r"], self.phi, self.m_cum, so["v_r"], so["v_t"], self.tp, so["id"], self.seed,
+                              self.step_index, self.G, out=self.sample, counters=self.counters,
+                              workspace=self.workspace)
+        # carried state for the next step: new phase-space coordinates, masses and ids in sorted order
+        sm = self.sample
+        s["r"], sm["r_new"] = sm["r_new"], s["r"]
+        s["v_r"], sm["v_r_new"] = sm["v_r_new"], s["v_r"]
+        s["v_t"], sm["v_t_new"] = sm["v_t_new"], s["v_t"]
+        s["m"], so["m"] = so["m"], s["m"]
+        s["id"], so["id"] = so["id"], s["id"]
+        self.step_index += 1
+
+
+def step_host_arena_bytes(n: int) -> int:
+    return int(lib().hmc_step_host_arena_bytes(ctypes.c_uint64(n)))
+
+
+def hmc_step_host(r, v_r, v_t, m, ids, out, seed: int, step: int, G: float = 1.0, *, arena: torch.Tensor,
+                  counters_host: Optional[torch.Tensor] = None):
+    """Host-buffer variant of one whole step.  r, v_r, v_t, m (float64) and ids (int32) are HOST
+    tensors (pinned for asynchronous copies); ``out`` is a dict of HOST tensors r_new, v_r_new,
+    v_t_new, m, id; ``arena`` a CUDA uint8 tensor of step_host_arena_bytes(n).  Enqueues the copies
+    and kernels on the current stream; synchronise before reading ``out``."""
+    n = r.numel()
+
+    def host(t, dtype, name):
+        if t.is_cuda or t.dtype != dtype or not t.is_contiguous() or t.numel() != n:
+            raise HmcError("%s must be a contiguous host %s[%d]" % (name, dtype, n))
+        return ctypes.c_void_p(t.data_ptr())
+
+    f = torch.float64
+    cp = ctypes.c_void_p(0)
+    if counters_host is not None:
+        if counters_host.is_cuda or counters_host.dtype != torch.int64 or counters_host.numel() != NCOUNTERS:
+            raise HmcError("counters_host must be a host int64[%d]" % NCOUNTERS)
+        cp = ctypes.c_void_p(counters_host.data_ptr())
+    if not arena.is_cuda or arena.dtype != torch.uint8:
+        raise HmcError("arena must be a CUDA uint8 tensor")
+    rc = lib().hmc_step_host(
+        ctypes.c_uint64(n), ctypes.c_double(G), ctypes.c_uint64(seed), ctypes.c_uint32(step), host(r, f, "r"),
+        host(v_r, f, "v_r"), host(v_t, f, "v_t"), host(m, f, "m"), host(ids, torch.int32, "ids"),
+        host(out["r_new"], f, "r_new"), host(out["v_r_new"], f, "v_r_new"), host(out["v_t_new"], f, "v_t_new"),
+        host(out["m"], f, "m_out"), host(out["id"], torch.int32, "id_out"), cp, ctypes.c_void_p(arena.data_ptr()),
+        ctypes.c_size_t(arena.numel()), _stream())
+    _check(rc, "hmc_step_host")
+    return out

@@ -1,0 +1,263 @@
+"""Parity of the CUDA path (through the C ABI, via the thin binding) with the CPU oracle.
+
+Bars (BASELINE.json north_star):
+  * sort permutation and bracket indices k_min / k_max: bit-exact
+  * Phi, r_min, r_max: <= 1e-12 relative
+  * new radii: <= 1e-10 relative for >= 99.999 % of the stars; rejection-branch flips
+    (different trial count than the oracle) counted and reported
+Because both sides evaluate the same binary64 expressions without FMA (R2) the
+observed differences are normally exactly zero; the tests print the counts.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_1206_5878_b200 import hmc, inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL_PHI = 1e-12
+TOL_ROOT = 1e-12
+TOL_RNEW = 1e-10
+FRAC_RNEW = 0.99999
+
+
+def dev(a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.to(dtype)
+    elif t.dtype == torch.uint32:
+        t = t.view(torch.int32)
+    return t.cuda()
+
+
+def host(t, dtype=None):
+    a = t.cpu().numpy()
+    if dtype is not None:
+        a = a.view(dtype)
+    return a
+
+
+def rel(a, b):
+    with np.errstate(divide="ignore", invalid="ignore"):
+        d = np.abs(a - b) / np.maximum(np.abs(b), 1e-300)
+    d[(a == b)] = 0.0           # also covers inf == inf
+    return d
+
+
+def gpu_sort(c):
+    ids = dev(c["id"].view(np.int32))
+    rs, perm, cols, ids_s = hmc.hmc_sort_by_radius(dev(c["r"]), (dev(c["v_r"]), dev(c["v_t"]), dev(c["m"])), ids)
+    return rs, perm, cols, ids_s
+
+
+# ----------------------------------------------------------------------------- S1
+@pytest.mark.parametrize("n", [1, 2, 31, 4095, 4096, 4097, 100_000, 1_000_003])
+def test_sort_matches_oracle(oracle, n):
+    c = inputs.plummer(n, 100 + n % 97)
+    rs, perm, cols, ids_s = gpu_sort(c)
+    o_rs, o_perm, o_cols, o_ids = oracle.sort_by_radius(c["r"], (c["v_r"], c["v_t"], c["m"]), c["id"])
+    assert np.array_equal(host(perm, np.uint32), o_perm)
+    assert np.array_equal(host(rs), o_rs)
+    for g, o in zip(cols, o_cols):
+        assert np.array_equal(host(g), o)
+    assert np.array_equal(host(ids_s, np.uint32), o_ids)
+
+
+@pytest.mark.parametrize("kind", ["ties", "all_equal", "sorted", "reversed", "extreme", "two_values"])
+def test_sort_adversarial_keys(oracle, kind):
+    g = np.random.default_rng(5)
+    n = 50_001
+    r = dict(
+        ties=np.floor(g.random(n) * 40) + 1.0,
+        all_equal=np.full(n, 0.75),
+        sorted=np.sort(g.random(n) + 0.5),
+        reversed=np.sort(g.random(n) + 0.5)[::-1].copy(),
+        extreme=10.0 ** g.uniform(-300, 300, n),
+        two_values=np.where(g.random(n) < 0.5, 1.0, 2.0),
+    )[kind]
+    rs, perm, _, _ = hmc.hmc_sort_by_radius(dev(r))
+    o_rs, o_perm, _, _ = oracle.sort_by_radius(r)
+    assert np.array_equal(host(perm, np.uint32), o_perm)
+    assert np.array_equal(host(rs), o_rs)
+
+
+def test_sort_empty_and_errors():
+    e = torch.empty(0, dtype=torch.float64, device="cuda")
+    rs, perm, _, _ = hmc.hmc_sort_by_radius(e)
+    assert rs.numel() == 0
+    r = torch.ones(8, dtype=torch.float64, device="cuda")
+    with pytest.raises(hmc.HmcError):
+        hmc.hmc_sort_by_radius(r, workspace=torch.empty(256, dtype=torch.uint8, device="cuda"))   # too small
+    with pytest.raises(hmc.HmcError):
+        hmc.hmc_sort_by_radius(r.float())
+
+
+# ----------------------------------------------------------------------------- S2
+@pytest.mark.parametrize("n,masses", [(1, "equal"), (2047, "equal"), (2048, "equal"), (2049, "salpeter"),
+                                      (100_000, "equal"), (1_000_003, "salpeter")])
+def test_potential_matches_oracle(oracle, n, masses):
+    c = inputs.plummer(n, 200 + n % 89, masses)
+    o = np.argsort(c["r"], kind="stable")
+    r, m = c["r"][o], c["m"][o]
+    phi, mc = hmc.hmc_potential(dev(r), dev(m), 1.0)
+    o_phi, o_mc = oracle.potential(r, m, 1.0)
+    phi, mc = host(phi), host(mc)
+    assert rel(phi, o_phi).max() <= TOL_PHI
+    assert rel(mc, o_mc).max() <= TOL_PHI
+    nbit = int((phi != o_phi).sum() + (mc != o_mc).sum())
+    print("potential n=%d: %d of %d values not bit-identical" % (n, nbit, 2 * n))
+    assert nbit <= max(2, n // 100_000)        # both sides round the exact sums once (R1p)
+
+
+def test_potential_with_ties_and_G(oracle):
+    r = np.sort(np.floor(np.random.default_rng(1).random(5000) * 100) + 1.0)
+    m = np.random.default_rng(2).random(5000)
+    phi, mc = hmc.hmc_potential(dev(r), dev(m), 2.5)
+    o_phi, o_mc = oracle.potential(r, m, 2.5)
+    assert np.array_equal(host(phi), o_phi) and np.array_equal(host(mc), o_mc)
+
+
+# ----------------------------------------------------------------------------- S3 + S4
+def oracle_chain(oracle, c, seed, step, sample=None):
+    return oracle.orbit_step(c["r"], c["v_r"], c["v_t"], c["m"], c["id"], seed, step, sample=sample)
+
+
+def check_orbit_against(oracle, o, tp, sm, sl=slice(None), report=""):
+    otp, osm = o["tp"], o["sample"]
+    kmin, kmax = host(tp["k_min"], np.uint32)[sl], host(tp["k_max"], np.uint32)[sl]
+    assert np.array_equal(kmin, otp["k_min"]) and np.array_equal(kmax, otp["k_max"])
+    assert np.array_equal(host(tp["status"])[sl], otp["status"])
+    for key in ("E", "J", "r_min", "r_max"):
+        assert rel(host(tp[key])[sl], otp[key]).max() <= TOL_ROOT, key
+    assert np.array_equal(host(sm["status"])[sl], osm["status"])
+    d = rel(host(sm["r_new"])[sl], osm["r_new"])
+    flips = int((host(sm["n_try"], np.uint16)[sl] != osm["n_try"]).sum())
+    frac = float((d <= TOL_RNEW).mean())
+    nbit = int((host(sm["r_new"])[sl] != osm["r_new"]).sum())
+    print("%s stars=%d  r_new within 1e-10: %.6f%%  not bit-identical: %d  rejection flips: %d"
+          % (report, d.size, 100 * frac, nbit, flips))
+    assert frac >= FRAC_RNEW
+    assert flips <= max(1, d.size // 100_000)
+    ok = d <= TOL_RNEW
+    assert rel(host(sm["v_t_new"])[sl][ok], osm["v_t_new"][ok]).max() <= 1e-9
+    assert rel(np.abs(host(sm["v_r_new"])[sl][ok]), np.abs(osm["v_r_new"][ok])).max() <= 1e-6
+    return flips
+
+
+@pytest.mark.parametrize("n,masses,seed", [(1, "equal", 3), (2, "equal", 4), (1000, "equal", 5), (100_000, "equal", 1),
+                                           (250_007, "salpeter", 9)])
+def test_orbit_stage_isolation_on_oracle_tables(oracle, n, masses, seed):
+    """S3 and S4 fed the ORACLE's sorted arrays and potential (stage isolation)."""
+    c = inputs.plummer(n, seed, masses)
+    o = oracle_chain(oracle, c, seed, 2)
+    rs, vrs, vts, phi, mc = (dev(o[k]) for k in ("r", "v_r", "v_t", "phi", "m_cum"))
+    counters = hmc.alloc_counters()
+    tp = hmc.hmc_orbit_turning_points(rs, vrs, vts, phi, mc, 1.0, counters=counters)
+    sm = hmc.hmc_sample_new_radius(rs, phi, mc, vrs, vts, tp, dev(o["id"].view(np.int32)), seed, 2, 1.0,
+                                   counters=counters)
+    check_orbit_against(oracle, o, tp, sm, report="isolated n=%d" % n)
+    cnt = host(counters)
+    assert cnt[hmc.COUNTER_NAMES.index("trials")] == o["sample"]["trials"]
+
+
+def test_config1_whole_step_chained(oracle):
+    """BASELINE.json configs[0]: Plummer N = 1e5, seed 1, one orbit step -- all four GPU stages chained."""
+    cfg = inputs.config(0)
+    c = {k: cfg[k] for k in ("r", "v_r", "v_t", "m", "id")}
+    o = oracle_chain(oracle, c, cfg["seed"], 0)
+    st = hmc.OrbitStepper(dev(c["r"]), dev(c["v_r"]), dev(c["v_t"]), dev(c["m"]), dev(c["id"].view(np.int32)),
+                          cfg["seed"])
+    st.step()
+    assert np.array_equal(host(st.sorted["perm"], np.uint32), o["perm"])
+    assert rel(host(st.phi), o["phi"]).max() <= TOL_PHI
+    # after the step the carried state holds r_new etc.; the sample dict holds the swapped-out buffers
+    sm = dict(st.sample)
+    sm["r_new"], sm["v_r_new"], sm["v_t_new"] = st.state["r"], st.state["v_r"], st.state["v_t"]
+    check_orbit_against(oracle, o, st.tp, sm, report="config1")
+    assert np.array_equal(host(st.state["id"], np.uint32), o["id"])
+    assert np.array_equal(host(st.state["m"]), o["m"])
+
+
+def test_config2_eleven_chained_steps(oracle):
+    """BASELINE.json configs[1] at reduced N (same recipe, seed 2): 1 + 10 steps re-sorting each step.
+    The oracle is fed its own previous output; the GPU its own.  Any divergence would compound."""
+    cfg = inputs.config(1, n_override=60_000)
+    c = {k: cfg[k] for k in ("r", "v_r", "v_t", "m", "id")}
+    st = hmc.OrbitStepper(dev(c["r"]), dev(c["v_r"]), dev(c["v_t"]), dev(c["m"]), dev(c["id"].view(np.int32)),
+                          cfg["seed"])
+    r, vr, vt, m, ids = c["r"], c["v_r"], c["v_t"], c["m"], c["id"]
+    total_flips = 0
+    for step in range(11):
+        o = oracle.orbit_step(r, vr, vt, m, ids, cfg["seed"], step)
+        st.step()
+        sm = dict(st.sample)
+        sm["r_new"], sm["v_r_new"], sm["v_t_new"] = st.state["r"], st.state["v_r"], st.state["v_t"]
+        assert np.array_equal(host(st.sorted["perm"], np.uint32), o["perm"])
+        total_flips += check_orbit_against(oracle, o, st.tp, sm, report="config2 step %d" % step)
+        s = o["sample"]
+        r, vr, vt, m, ids = s["r_new"], s["v_r_new"], s["v_t_new"], o["m"], o["id"]
+    assert total_flips == 0
+    cnt = host(st.counters)
+    assert cnt[:5].sum() == 0                     # no unbound / radial / degenerate / circular / maxtries
+
+
+def test_order_independence_of_the_draw(oracle):
+    """Permuting the stars of S4's per-star inputs permutes its outputs exactly (Philox keyed by id)."""
+    c = inputs.plummer(30_000, 77)
+    o = oracle_chain(oracle, c, 77, 0)
+    rs, vrs, vts, phi, mc = (dev(o[k]) for k in ("r", "v_r", "v_t", "phi", "m_cum"))
+    ids = dev(o["id"].view(np.int32))
+    tp = hmc.hmc_orbit_turning_points(rs, vrs, vts, phi, mc)
+    a = hmc.hmc_sample_new_radius(rs, phi, mc, vrs, vts, tp, ids, 77, 0)
+    p = torch.randperm(30_000, device="cuda", generator=torch.Generator("cuda").manual_seed(0))
+    tpp = {k: v[p].contiguous() for k, v in tp.items()}
+    # tables stay in sorted order; only the per-star arrays are permuted.  v_r / v_t pass-through columns too.
+    b = hmc.hmc_sample_new_radius(rs, phi, mc, vrs[p].contiguous(), vts[p].contiguous(), tpp, ids[p].contiguous(), 77, 0)
+    # r pass-through uses r_sorted[a] for flagged stars only; none are flagged here
+    assert int(a["status"].sum()) == 0
+    for key in ("r_new", "v_r_new", "v_t_new", "n_try"):
+        assert torch.equal(b[key], a[key][p])
+
+
+def test_flagged_stars(oracle):
+    r = np.array([1.0, 2.0, 3.0, 4.0])
+    m = np.array([0.25, 0.25, 0.25, 0.25])
+    vr = np.array([0.1, 5.0, 0.1, 0.0])
+    vt = np.array([0.3, 0.1, 0.0, 0.3])
+    phi, mc = oracle.potential(r, m)
+    otp = oracle.orbit_turning_points(r, vr, vt, phi, mc)
+    ids = np.arange(4, dtype=np.uint32)
+    osm = oracle.sample_new_radius(r, phi, mc, r, vr, vt, otp["E"], otp["J"], otp["r_min"], otp["r_max"],
+                                   otp["k_min"], otp["k_max"], ids, otp["status"], 1, 0)
+    counters = hmc.alloc_counters()
+    tp = hmc.hmc_orbit_turning_points(dev(r), dev(vr), dev(vt), dev(phi), dev(mc), counters=counters)
+    sm = hmc.hmc_sample_new_radius(dev(r), dev(phi), dev(mc), dev(vr), dev(vt), tp, dev(ids.view(np.int32)), 1, 0,
+                                   counters=counters)
+    assert np.array_equal(host(tp["status"]), otp["status"])
+    assert np.array_equal(host(sm["status"]), osm["status"])
+    for key in ("r_new", "v_r_new", "v_t_new"):
+        assert np.array_equal(host(sm[key]), osm[key])
+    assert np.array_equal(host(tp["r_max"]), otp["r_max"]) and np.array_equal(host(tp["r_min"]), otp["r_min"])
+    cnt = host(counters)
+    assert cnt[0] == 1 and cnt[1] == 1
+
+
+def test_host_buffer_step_matches_device_step(oracle):
+    n = 50_000
+    c = inputs.plummer(n, 55)
+    o = oracle_chain(oracle, c, 55, 7)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    out = dict(r_new=torch.empty(n, dtype=torch.float64).pin_memory(), v_r_new=torch.empty(n, dtype=torch.float64).pin_memory(),
+               v_t_new=torch.empty(n, dtype=torch.float64).pin_memory(), m=torch.empty(n, dtype=torch.float64).pin_memory(),
+               id=torch.empty(n, dtype=torch.int32).pin_memory())
+    arena = torch.empty(hmc.step_host_arena_bytes(n), dtype=torch.uint8, device="cuda")
+    cnt = torch.zeros(hmc.NCOUNTERS, dtype=torch.int64).pin_memory()
+    hmc.hmc_step_host(pin(c["r"]), pin(c["v_r"]), pin(c["v_t"]), pin(c["m"]), pin(c["id"].view(np.int32)), out, 55, 7,
+                      arena=arena, counters_host=cnt)
+    torch.cuda.synchronize()
+    assert np.array_equal(out["id"].numpy().view(np.uint32), o["id"])
+    assert np.array_equal(out["m"].numpy(), o["m"])
+    d = rel(out["r_new"].numpy(), o["sample"]["r_new"])
+    assert (d <= TOL_RNEW).mean() >= FRAC_RNEW
+    assert int(cnt[hmc.COUNTER_NAMES.index("trials")]) == o["sample"]["trials"]
