@@ -1,0 +1,411 @@
+#!/usr/bin/env python
+"""bench.py -- stars/s per orbit step (sort + potential + turning points + sampling), fp64.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl reference]
+
+A "step" is one pass of the whole hot path over one synthetic Plummer cluster; steps are chained
+(the output of a step is the input of the next, re-sorting each step), as in BASELINE.json's
+multi-step configs.  The default workload is the configuration the metric is quoted on:
+configs[2], N = 1e7 equal-mass stars, seed 3.
+
+Timing: W untimed warm-up steps, then exactly K steps between barrier + torch.cuda.synchronize()
+on both sides, CUDA events on the launching stream, MAX over ranks.  The star arrays (440 MB of
+state and intermediates per step at N = 1e7) are several times the 126 MB L2, so no explicit L2
+flush is needed between steps; `config.l2` says so.
+
+N > 1 ranks run independent replicas (one cluster per GPU, seed + rank): the path does not shard
+in this round, there is no data-path collective, scaling is "weak".
+
+Prints ONE JSON line on rank 0.  `--impl reference` times the CPU oracle instead (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "stars/sec per orbit step (sort+potential+turning points+sampling), fp64, N=1e7"
+UNIT = "stars/s"
+STAGES = ("sort", "potential", "turning_points", "sampling")
+KERNELS_PER_STEP = 17   # sort: histogram, bin scan, 8 digit passes, identity guard, gather; potential: 2 scans;
+                        # turning points: table build + search; sampling: 1
+
+
+# --------------------------------------------------------------------------- roofline model
+def algorithmic_bytes_per_star(n: int) -> dict:
+    """bytes the method itself must move per star (each streamed array once,
+    one table entry per probe of the paper's bisection: 16 B for an (r, Phi) probe, 8 B for an
+    r-only probe)."""
+    lg = math.log2(n)
+    return dict(
+        sort=8 + 8 * (12 + 12) + (4 + 28 + 28),
+        potential=16 + 16,
+        turning_points=40 + 41 + 16 * (2 * lg - 2.9) + 16,
+        sampling=45 + 24 + 16 + 1.9 * (8 * (lg - 1.5) + 16),
+    )
+
+
+def measured_peak_gbs():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
+
+
+def ncu_traffic_bytes(kernel: str, n: int):
+    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture, if any."""
+    p = os.path.join(ROOT, "profiles", "dram_traffic.json")
+    try:
+        rec = json.load(open(p))
+        return rec.get(str(n), {}).get(kernel)
+    except Exception:
+        return None
+
+
+# --------------------------------------------------------------------------- clocks
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period: float = 0.002):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.sm_max = [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            "hw_slowdown": nv.nvmlClocksEventReasonHwSlowdown if hasattr(nv, "nvmlClocksEventReasonHwSlowdown") else 0x8,
+            "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4, "hw_power_brake": 0x80,
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if mask & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join(timeout=2)
+        s = sorted(self.samples)
+        return dict(sm_mhz=(s[len(s) // 2] if s else None), sm_max_mhz=self.sm_max, reasons=sorted(self.reasons),
+                    samples=len(s))
+
+
+# --------------------------------------------------------------------------- distributed plumbing
+def dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def dist_init(backend: str):
+    """Initialise torch.distributed from the torchrun environment (no-op for world size 1)."""
+    import torch.distributed as dist
+    rank, local_rank, world = dist_env()
+    if world > 1 and not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group(backend=backend, rank=rank, world_size=world)
+    return rank, local_rank, world
+
+
+def dist_barrier():
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized():
+        dist.barrier()
+
+
+def dist_max(x: float, device="cpu") -> float:
+    """MAX over ranks of a host float (device-timed milliseconds)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return float(x)
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def dist_sum(x: float, device="cpu") -> float:
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return float(x)
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def aggregate_throughput(stars_this_rank: float, ms_this_rank: float, device="cpu"):
+    """Whole-job stars/s: stars processed by all ranks / max-over-ranks time."""
+    ms = dist_max(ms_this_rank, device)
+    stars = dist_sum(stars_this_rank, device)
+    return stars / (ms * 1e-3), ms
+
+
+# --------------------------------------------------------------------------- CPU oracle legs
+def oracle_sampled_step(cluster, seed, step, stride):
+    """Time the oracle as it stands on a bounded sample of one step: S1 and S2 on all stars, S3 and
+    S4 on every `stride`-th star of the sorted order; returns (estimated seconds for the full step,
+    per-stage seconds measured, result of the step)."""
+    import oracle
+    t0 = time.perf_counter()
+    rs, perm, (vrs, vts, ms), ids = oracle.sort_by_radius(cluster["r"], (cluster["v_r"], cluster["v_t"], cluster["m"]),
+                                                          cluster["id"])
+    t1 = time.perf_counter()
+    phi, mc = oracle.potential(rs, ms)
+    t2 = time.perf_counter()
+    tp = oracle.orbit_turning_points(rs, vrs, vts, phi, mc, 1.0, 0, stride)
+    t3 = time.perf_counter()
+    sl = slice(0, None, stride)
+    sm = oracle.sample_new_radius(rs, phi, mc, rs[sl], vrs[sl], vts[sl], tp["E"], tp["J"], tp["r_min"], tp["r_max"],
+                                  tp["k_min"], tp["k_max"], ids[sl], tp["status"], seed, step)
+    t4 = time.perf_counter()
+    n = len(rs)
+    scale = n / max(len(tp["E"]), 1)
+    meas = dict(sort=t1 - t0, potential=t2 - t1, turning_points=t3 - t2, sampling=t4 - t3)
+    est = meas["sort"] + meas["potential"] + scale * (meas["turning_points"] + meas["sampling"])
+    return est, meas, scale
+
+
+def cpu_baseline_leg(cluster, seed, stride=64):
+    est, meas, scale = oracle_sampled_step(cluster, seed, 0, stride)
+    n = len(cluster["r"])
+    return dict(value=n / est, unit=UNIT, cores=1, kind="oracle",
+                sample="one step at N=%d: sort and potential on all stars, turning points and sampling on every "
+                       "%d-th star of the sorted order (%.1f s measured), orbit stages scaled x%.0f"
+                       % (n, stride, sum(meas.values()), scale),
+                seconds_measured=round(sum(meas.values()), 2), est_seconds_per_step=round(est, 2),
+                stage_seconds_measured={k: round(v, 3) for k, v in meas.items()})
+
+
+def run_reference(args, cfg):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    from paper_1206_5878_b200 import inputs
+    import oracle
+    oracle.build()
+    c = inputs.config(args.config, args.n)
+    cluster = {k: c[k] for k in ("r", "v_r", "v_t", "m", "id")}
+    n = c["n"]
+    stride = args.ref_stride
+    ests = []
+    for i in range(args.warmup + args.steps):
+        est, meas, scale = oracle_sampled_step(cluster, c["seed"], i, stride)
+        if i >= args.warmup:
+            ests.append(est)
+    ms = 1e3 * sum(ests) / len(ests)
+    value = n / (ms * 1e-3)
+    line = dict(impl="reference", metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
+                warmup=args.warmup, ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="f64", data="synthetic", config=cfg,
+                cpu_baseline=dict(value=value, unit=UNIT, cores=1, kind="oracle",
+                                  sample="each step: sort and potential on all %d stars, turning points and sampling "
+                                         "on every %d-th star of the sorted order, orbit stages scaled x%d" % (n, stride, stride)),
+                e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line))
+    return 0
+
+
+# --------------------------------------------------------------------------- GPU arm
+def run_gpu(args, cfg):
+    import numpy as np
+    import torch
+    from paper_1206_5878_b200 import hmc, inputs
+
+    rank, local_rank, world = dist_init("nccl")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    devs = "cuda:%d" % local_rank
+    hmc.lib()
+
+    c = inputs.config(args.config, args.n)
+    n = c["n"]
+    if world > 1:   # independent replica per rank
+        c.update(inputs.plummer(n, c["seed"] + 1000 * rank, c["masses"]))
+    cluster = {k: c[k] for k in ("r", "v_r", "v_t", "m", "id")}
+    seed = c["seed"] + 1000 * rank
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(devs)
+    stepper = hmc.OrbitStepper(d(cluster["r"]), d(cluster["v_r"]), d(cluster["v_t"]), d(cluster["m"]),
+                               d(cluster["id"].view(np.int32)), seed, with_n_try=False)
+    stream = torch.cuda.current_stream()
+
+    def staged_step(ev):
+        """One step with an event after every stage (events are recorded on the launching stream)."""
+        s, so = stepper.state, stepper.sorted
+        ev[0].record(stream)
+        hmc.hmc_sort_by_radius(s["r"], (s["v_r"], s["v_t"], s["m"]), s["id"], r_sorted=so["r"], perm=so["perm"],
+                               cols_out=(so["v_r"], so["v_t"], so["m"]), ids_out=so["id"], workspace=stepper.workspace)
+        ev[1].record(stream)
+        hmc.hmc_potential(so["r"], so["m"], stepper.G, phi=stepper.phi, m_cum=stepper.m_cum, workspace=stepper.workspace)
+        ev[2].record(stream)
+        hmc.hmc_orbit_turning_points(so["r"], so["v_r"], so["v_t"], stepper.phi, stepper.m_cum, stepper.G,
+                                     out=stepper.tp, counters=stepper.counters, workspace=stepper.workspace)
+        ev[3].record(stream)
+        hmc.hmc_sample_new_radius(so["r"], stepper.phi, stepper.m_cum, so["v_r"], so["v_t"], stepper.tp, so["id"],
+                                  stepper.seed, stepper.step_index, stepper.G, out=stepper.sample,
+                                  counters=stepper.counters, workspace=stepper.workspace)
+        ev[4].record(stream)
+        sm = stepper.sample
+        s["r"], sm["r_new"] = sm["r_new"], s["r"]
+        s["v_r"], sm["v_r_new"] = sm["v_r_new"], s["v_r"]
+        s["v_t"], sm["v_t_new"] = sm["v_t_new"], s["v_t"]
+        s["m"], so["m"] = so["m"], s["m"]
+        s["id"], so["id"] = so["id"], s["id"]
+        stepper.step_index += 1
+
+    mk = lambda: [torch.cuda.Event(enable_timing=True) for _ in range(5)]
+    for _ in range(args.warmup):
+        staged_step(mk())
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    dist_barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    evs = [mk() for _ in range(args.steps)]
+    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_start.record(stream)
+    for i in range(args.steps):
+        staged_step(evs[i])
+    t_end.record(stream)
+    torch.cuda.synchronize()
+    dist_barrier()
+    clocks = sampler.stop()
+    ms_total = t_start.elapsed_time(t_end)
+    value, ms_max = aggregate_throughput(float(n) * args.steps, ms_total, devs)
+    stage_ms = {name: sum(e[i].elapsed_time(e[i + 1]) for e in evs) / args.steps for i, name in enumerate(STAGES)}
+    counters = {k: int(v) for k, v in zip(hmc.COUNTER_NAMES, stepper.counters.cpu().tolist())}
+
+    # ---- end to end through the host-buffer C-ABI call: pinned host inputs in, results out, every step
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        hin = dict(r=pin(cluster["r"]), v_r=pin(cluster["v_r"]), v_t=pin(cluster["v_t"]), m=pin(cluster["m"]),
+                   id=pin(cluster["id"].view(np.int32)))
+        hout = dict(r_new=torch.empty(n, dtype=torch.float64).pin_memory(), v_r_new=torch.empty(n, dtype=torch.float64).pin_memory(),
+                    v_t_new=torch.empty(n, dtype=torch.float64).pin_memory(), m=torch.empty(n, dtype=torch.float64).pin_memory(),
+                    id=torch.empty(n, dtype=torch.int32).pin_memory())
+        del stepper
+        torch.cuda.empty_cache()
+        arena = torch.empty(hmc.step_host_arena_bytes(n), dtype=torch.uint8, device=devs)
+
+        def host_step(i):
+            nonlocal hin, hout
+            hmc.hmc_step_host(hin["r"], hin["v_r"], hin["v_t"], hin["m"], hin["id"], hout, seed, i, arena=arena)
+            nxt = dict(r=hout["r_new"], v_r=hout["v_r_new"], v_t=hout["v_t_new"], m=hout["m"], id=hout["id"])
+            hout = dict(r_new=hin["r"], v_r_new=hin["v_r"], v_t_new=hin["v_t"], m=hin["m"], id=hin["id"])
+            hin = nxt
+
+        e2e_steps = max(1, min(args.steps, args.e2e_steps))
+        for i in range(2):
+            host_step(i)
+        torch.cuda.synchronize()
+        dist_barrier()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for i in range(e2e_steps):
+            host_step(2 + i)
+        b.record(stream)
+        torch.cuda.synchronize()
+        dist_barrier()
+        e2e_value, _ = aggregate_throughput(float(n) * e2e_steps, a.elapsed_time(b), devs)
+        e2e = dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=n * (4 * 8 + 4), d2h_bytes_per_step=n * (4 * 8 + 4),
+                   steps=e2e_steps, api="hmc_step_host (pinned host buffers; H2D, 4 stages, D2H per step)")
+
+    if rank != 0:
+        return 0
+
+    # ---- roofline of the dominant stage's kernel
+    model = algorithmic_bytes_per_star(n)
+    peak, peak_src = measured_peak_gbs()
+    dom = max(STAGES, key=lambda s: stage_ms[s])
+    dom_kernel = dict(sort="sort_onesweep_kernel (8 launches) + histogram + gather", potential="potential_scan_kernel (2 launches)",
+                      turning_points="turning_points_kernel (+ build_rphi_kernel)", sampling="sample_new_radius_kernel")[dom]
+    achieved = model[dom] * n / (stage_ms[dom] * 1e-3) / 1e9
+    roofline = dict(bound="hbm", kernel=dom_kernel, stage=dom, achieved=achieved, peak=peak, unit="GB/s",
+                    frac=achieved / peak, traffic=ncu_traffic_bytes(dom, n), peak_source=peak_src,
+                    algorithmic_bytes_per_star=model[dom], stars_per_launch=n)
+    orbit_ms = stage_ms["potential"] + stage_ms["turning_points"] + stage_ms["sampling"]
+    orbit_bytes = model["potential"] + model["turning_points"] + model["sampling"]
+    stages = {s: dict(ms=stage_ms[s], stars_per_s=n / (stage_ms[s] * 1e-3), algorithmic_bytes_per_star=model[s],
+                      achieved_gbs=model[s] * n / (stage_ms[s] * 1e-3) / 1e9,
+                      frac_of_peak=model[s] * n / (stage_ms[s] * 1e-3) / 1e9 / peak) for s in STAGES}
+    potential_plus_orbit = dict(ms=orbit_ms, stars_per_s=n / (orbit_ms * 1e-3),
+                                achieved_gbs=orbit_bytes * n / (orbit_ms * 1e-3) / 1e9,
+                                frac_of_measured_peak=orbit_bytes * n / (orbit_ms * 1e-3) / 1e9 / peak,
+                                frac_of_8TBs=orbit_bytes * n / (orbit_ms * 1e-3) / 1e9 / 8000.0)
+
+    cpu = None
+    if world == 1 or rank == 0:
+        if not args.no_cpu_baseline:
+            import oracle
+            oracle.build()
+            cpu = cpu_baseline_leg(cluster, c["seed"], args.ref_stride)
+
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+                ms_per_step=ms_max / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
+                data="synthetic", config=cfg, clocks=clocks, e2e=e2e, gpu_launches=KERNELS_PER_STEP * args.steps,
+                roofline=roofline, cpu_baseline=cpu, stages=stages, potential_plus_orbit=potential_plus_orbit,
+                counters=counters)
+    print(json.dumps(line))
+    return 0
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (default 2: N=1e7, the metric's)")
+    ap.add_argument("--n", type=int, default=None, help="override N (same recipe and seed); not a bench line")
+    ap.add_argument("--ref-stride", type=int, default=64, help="oracle legs: orbit stages on every k-th star")
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args(argv)
+    from paper_1206_5878_b200 import inputs
+    base = inputs.CONFIGS[args.config]
+    n = args.n or base["n"]
+    cfg = dict(workload="BASELINE.json configs[%d]: %s, N=%d, %s masses, seed %d, chained orbit steps"
+                        % (args.config, base["name"], n, base["masses"], base["seed"]),
+               n_stars=n, masses=base["masses"], seed=base["seed"], parallelism="replicas x%d" % max(args.gpus, 1),
+               l2="working set per step (>= 44 B/star state + 97 B/star intermediates) exceeds the 126 MB L2 at "
+                  "N=1e7; no explicit flush")
+    if args.impl == "reference":
+        return run_reference(args, cfg)
+    return run_gpu(args, cfg)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

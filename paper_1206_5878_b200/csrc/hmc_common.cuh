@@ -45,6 +45,8 @@ struct Workspace {
     double*   scan_status;   // [2][scan_tiles][8] (flag, agg_hi, agg_lo, inc_hi, inc_lo, pad)
     // orbit
     double2*  rphi;          // [n] interleaved (r_j, Phi_j) search table
+    double2*  rphi_mid;      // [n/8 + 1] every 8th node of rphi
+    double*   r_mid;         // [n/8 + 1] every 8th node of r
     size_t    total;
 };
 
@@ -66,6 +68,8 @@ static inline Workspace carve(void* base, uint64_t n)
     w.tickets     = reinterpret_cast<uint32_t*>(take(32 * 4));
     w.scan_status = reinterpret_cast<double*>(take(2 * scan_tiles * 8 * 8));
     w.rphi        = reinterpret_cast<double2*>(take(n * 16));
+    w.rphi_mid    = reinterpret_cast<double2*>(take((n / 8 + 1) * 16));
+    w.r_mid       = reinterpret_cast<double*>(take((n / 8 + 1) * 8));
     w.total = off;
     return w;
 }

@@ -25,29 +25,45 @@ static constexpr uint32_t FLAG_INC = 2u << 30;
 static constexpr uint32_t FLAG_MASK = 3u << 30;
 
 // ---- digit histograms of all 8 digits in one read -------------------------------------------
-__global__ void __launch_bounds__(512) sort_histogram_kernel(const uint64_t* __restrict__ keys, uint64_t n,
-                                                             uint32_t* __restrict__ hist /*[8][256]*/)
+// Low digits of a radius are uniformly distributed: plain shared-memory atomics on one of
+// HIST_COPIES replicated histograms hardly ever collide.  The two top digits (sign, exponent, top
+// mantissa bits) take only a handful of values, so those are first aggregated across the warp.
+static constexpr int HIST_THREADS = 512;
+static constexpr int HIST_COPIES = 4;
+static constexpr int HIST_SKEWED_FROM = 6;      // digits >= this are warp-aggregated
+
+__global__ void __launch_bounds__(HIST_THREADS) sort_histogram_kernel(const uint64_t* __restrict__ keys, uint64_t n,
+                                                                      uint32_t* __restrict__ hist /*[8][256]*/)
 {
-    __shared__ uint32_t sh[NPASS * RADIX];
-    for (int i = threadIdx.x; i < NPASS * RADIX; i += blockDim.x) sh[i] = 0;
+    __shared__ uint32_t sh[HIST_COPIES][NPASS * RADIX];
+    for (int i = threadIdx.x; i < HIST_COPIES * NPASS * RADIX; i += HIST_THREADS) (&sh[0][0])[i] = 0;
     __syncthreads();
-    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    uint32_t* mine = sh[(threadIdx.x >> 5) % HIST_COPIES];
+    const uint64_t stride = (uint64_t)gridDim.x * HIST_THREADS;
     const uint64_t iters = (n + stride - 1) / stride;           // same trip count for every thread
-    uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    uint64_t i = (uint64_t)blockIdx.x * HIST_THREADS + threadIdx.x;
     for (uint64_t it = 0; it < iters; ++it, i += stride) {
         const bool ok = i < n;
-        uint64_t k = ok ? keys[i] : 0ull;
+        uint64_t k = ok ? __ldg(keys + i) : 0ull;
+        if (ok) {
 #pragma unroll
-        for (int p = 0; p < NPASS; ++p) {
+            for (int p = 0; p < HIST_SKEWED_FROM; ++p)
+                atomicAdd(&mine[p * RADIX + ((uint32_t)(k >> (p * RADIX_BITS)) & (RADIX - 1))], 1u);
+        }
+#pragma unroll
+        for (int p = HIST_SKEWED_FROM; p < NPASS; ++p) {
             uint32_t d = ok ? ((uint32_t)(k >> (p * RADIX_BITS)) & (RADIX - 1)) : (uint32_t)RADIX;
-            // warp-aggregate: the high digits of radii take only a handful of values
             unsigned peers = __match_any_sync(0xffffffffu, d);
-            if (ok && (peers & lanemask_lt()) == 0) atomicAdd(&sh[p * RADIX + d], __popc(peers));
+            if (ok && (peers & lanemask_lt()) == 0) atomicAdd(&mine[p * RADIX + d], __popc(peers));
         }
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < NPASS * RADIX; i += blockDim.x)
-        if (sh[i]) atomicAdd(&hist[i], sh[i]);
+    for (int b = threadIdx.x; b < NPASS * RADIX; b += HIST_THREADS) {
+        uint32_t c = 0;
+#pragma unroll
+        for (int q = 0; q < HIST_COPIES; ++q) c += sh[q][b];
+        if (c) atomicAdd(&hist[b], c);
+    }
 }
 
 // exclusive scan of each digit's 256 counts; pass_live[p] = 0 when one bin holds every key
@@ -261,8 +277,8 @@ hmc_status sort_by_radius(uint64_t n, const double* r_in, double* r_sorted, uint
     const int sms = sm_count();
     const uint64_t* keys0 = reinterpret_cast<const uint64_t*>(r_in);
     {
-        int blocks = (int)umin64((n + 511) / 512, (uint64_t)sms * 4);
-        sort_histogram_kernel<<<blocks, 512, 0, st>>>(keys0, n, ws.digit_hist);
+        int blocks = (int)umin64((n + HIST_THREADS - 1) / HIST_THREADS, (uint64_t)sms * 3);
+        sort_histogram_kernel<<<blocks, HIST_THREADS, 0, st>>>(keys0, n, ws.digit_hist);
         HMC_LAUNCH_CHECK();
         sort_scan_hist_kernel<<<NPASS, RADIX, 0, st>>>(ws.digit_hist, n, pass_live);
         HMC_LAUNCH_CHECK();
