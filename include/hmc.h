@@ -56,7 +56,7 @@ typedef int32_t hmc_status;
 #define HMC_ERR_ALIGN      (-4)  /* an array pointer is not aligned to its element size     */
 #define HMC_ERR_CUDA       (-5)  /* a CUDA runtime call or kernel launch failed             */
 
-#define HMC_MAX_N      (1ull << 30)   /* stars per call                                     */
+#define HMC_MAX_N      (1ull << 28)   /* stars per call                                     */
 #define HMC_MAX_COLS   8              /* fp64 record columns carried by the sort            */
 
 /* star_status bits */

@@ -10,6 +10,11 @@
 
 namespace hmc {
 
+// One entry of the node table the orbit kernels search: node j (paper numbering, 0..N+1) holds
+// r_j, Phi_j, B_j = G M_j and u_j = 1/r_j -- everything Eq. 6 and the in-shell quadratic need, in
+// one 32-byte sector.  Sentinels: node 0 = (0, Phi_1, 0, 0), node N+1 = (+inf, 0, G M_N, 0).
+struct __align__(32) Node { double r, phi, B, u; };
+
 // ---- host-side checks ---------------------------------------------------------------------
 static inline bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) != 0; }
 
@@ -44,11 +49,28 @@ struct Workspace {
     // potential
     double*   scan_status;   // [2][scan_tiles][8] (flag, agg_hi, agg_lo, inc_hi, inc_lo, pad)
     // orbit
-    double2*  rphi;          // [n] interleaved (r_j, Phi_j) search table
-    double2*  rphi_mid;      // [n/8 + 1] every 8th node of rphi
-    double*   r_mid;         // [n/8 + 1] every 8th node of r
+    Node*     nodes;         // [n + 2] node table with sentinels (hmc_orbit.cu)
+    uint16_t* dir;           // radius directory, dir_entries(n) entries (hmc_orbit.cu)
     size_t    total;
 };
+
+// ---- orbit tables: sizes shared by carve() and hmc_orbit.cu ---------------------------------
+static constexpr uint32_t COARSE_CAP = 13824;        // (r, Phi) pairs of the shared-memory coarse table: 216 KB
+
+// coarse nodes are the multiples of 2^shift; smallest shift with (n >> shift) + 2 <= COARSE_CAP
+static inline int coarse_shift(uint64_t n)
+{
+    int t = 0;
+    while ((n >> t) + 2 > COARSE_CAP) ++t;
+    return t;
+}
+
+// the directory holds, for each of the (n >> shift) + 1 coarse intervals, 2^shift + 1 offsets
+static inline uint64_t dir_entries(uint64_t n)
+{
+    const int t = coarse_shift(n);
+    return ((n >> t) + 1) * ((1ull << t) + 1);
+}
 
 static constexpr int SORT_TILE = 4096;     // keys per sort tile
 static constexpr int SCAN_TILE = 2048;     // elements per scan tile
@@ -67,9 +89,8 @@ static inline Workspace carve(void* base, uint64_t n)
     w.lookback    = reinterpret_cast<uint32_t*>(take(8 * sort_tiles * 256 * 4));
     w.tickets     = reinterpret_cast<uint32_t*>(take(32 * 4));
     w.scan_status = reinterpret_cast<double*>(take(2 * scan_tiles * 8 * 8));
-    w.rphi        = reinterpret_cast<double2*>(take(n * 16));
-    w.rphi_mid    = reinterpret_cast<double2*>(take((n / 8 + 1) * 16));
-    w.r_mid       = reinterpret_cast<double*>(take((n / 8 + 1) * 8));
+    w.nodes       = reinterpret_cast<Node*>(take((n + 2) * sizeof(Node)));
+    w.dir         = reinterpret_cast<uint16_t*>(take(dir_entries(n) * 2));
     w.total = off;
     return w;
 }

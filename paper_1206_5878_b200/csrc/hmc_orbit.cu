@@ -1,40 +1,43 @@
 // hmc_orbit.cu -- S3 turning points and S4 new-radius draw (Appendix A).
 //
 // The paper's GPU port ran one thread per star with plain bisection over the (r, Phi) arrays in
-// global memory.  What is kept: one thread per star, SoA streams, coalesced
-// per-star loads and stores.  What differs:
+// global memory: ~2 log2 N dependent random reads per star for the two
+// brackets, and log2 N more per rejection trial.  What is kept: SoA streams for the per-star
+// data, one star per thread at a time.  What differs:
 //
-//  * Search order.  The bracket predicate "Q(r_j) < 0" is monotone on either side of the star (Q
-//    is concave in 1/r), and "r_j <= r0" is monotone, so ANY search order finds the same index.
-//    The searches descend a GLOBAL implicit binary tree over node numbers (the pivot of an open
-//    interval is its element with the most trailing zero bits) instead of bisecting [0,k] /
-//    [k,N+1] per star, so all stars share the upper levels of that tree:
-//      - nodes that are multiples of 2^t  : staged once per CTA in shared memory (<= 216 KB)
-//      - nodes that are multiples of 8    : a dense "mid" table (N/8 entries, L2 resident)
-//      - the last three levels            : the full table; 8 consecutive entries = one line
-//  * S3 runs the pericentre and the apocentre search of a star interleaved, two independent load
-//    chains per thread.
+//  * The bracket predicate "Q(r_j) < 0" is monotone on either side of the star (Q is concave in
+//    1/r) and "r_j <= r0" is monotone, so ANY probe order finds the same index.  The searches
+//    therefore do not bisect.  They run in three tiers:
+//      1. coarse: the nodes that are multiples of S = 2^shift ((r, Phi) pairs, <= 216 KB) are staged
+//         once per CTA in shared memory; a bisection over them costs no global traffic and leaves
+//         an interval of at most S nodes.
+//      2. guess: inside that interval r^2 Q(r) is very nearly linear (the interval spans ~1e-4 of
+//         the cluster), so one secant step gives the root radius to a fraction of the node
+//         spacing (S3); S4 knows the radius it looks for.  A "radius directory" -- for every coarse
+//         interval, S equal-width radius buckets with the offset of the first node of each
+//         bucket, 2 bytes per star, L2 resident -- turns that radius into a node index.
+//      3. exact: the node table proper (r_j, Phi_j, G M_j, 1/r_j in one 32-byte sector) is
+//         probed at the guess and its neighbour; if the sign change is not there the search
+//         gallops away from the guess and bisects what is left.  Typical cost: one directory read
+//         and one or two adjacent sectors instead of ~20 dependent probes.
+//  * S3 runs the pericentre and the apocentre search of a star interleaved (independent chains).
 //  * S4 decides most trials without touching global memory ("squeeze"): Phi is monotone in r, so
-//    the shared-memory table brackets Phi(r0) and hence Q(r0) and g; a trial is rejected (or
-//    provisionally accepted) when the whole bracket, widened by 1e-11, lies on one side of F X'.
-//    Only provisionally accepted and undecided trials run the exact shell search and the exact
-//    test, with the oracle's expressions, so the outcome is identical to evaluating every trial.
+//    the shared-memory table brackets Phi(r0) and hence Q(r0) and g; a trial is rejected when the
+//    whole bracket, widened by 1e-11, lies on the far side of F X'.  Only the other trials run the
+//    exact shell look-up and the exact test, with the oracle's expressions, so the outcome is
+//    identical to evaluating every trial.
+//  * S4 keeps every lane busy: a lane whose star has been accepted takes the warp's next star at
+//    once instead of idling until the slowest of 32 rejection loops ends (the trial count is
+//    geometric: mean ~2.5, maximum over a warp ~8).
 //  * Random numbers are Philox4x32-10 keyed by (seed, step, star id), not per-thread streams.
 #include "hmc_common.cuh"
 
 namespace hmc {
 
 static constexpr int ORB_THREADS = 1024;
-static constexpr uint32_t COARSE_CAP = 13824;        // (r, Phi) pairs: 216 KB
-static constexpr int MID_SHIFT = 3;                  // mid tables hold every 8th node
-static constexpr uint32_t MID_MASK = (1u << MID_SHIFT) - 1u;
+static constexpr int ORB_WARPS = ORB_THREADS / 32;
 
-static int coarse_shift(uint64_t n, uint32_t cap)
-{
-    int t = 0;
-    while ((n >> t) + 2 > cap) ++t;
-    return t;
-}
+__device__ __forceinline__ double pos_inf() { return __longlong_as_double(0x7ff0000000000000ll); }
 
 // element of the open interval (lo, hi), hi - lo > 1, with the most trailing zeros
 __device__ __forceinline__ uint32_t pivot(uint32_t lo, uint32_t hi)
@@ -45,66 +48,176 @@ __device__ __forceinline__ uint32_t pivot(uint32_t lo, uint32_t hi)
     return b & (0xffffffffu << hb);
 }
 
-__device__ __forceinline__ double pos_inf() { return __longlong_as_double(0x7ff0000000000000ll); }
+__device__ __forceinline__ Node ld_node(const Node* __restrict__ p)
+{
+    Node e;
+    asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(e.r), "=d"(e.phi), "=d"(e.B), "=d"(e.u) : "l"(p));
+    return e;
+}
 
-// ---- table builders ---------------------------------------------------------------------------
-// rphi[a] = (r_a, Phi_a); rphi_mid[c] = node 8c = array element 8c - 1 (c >= 1)
-__global__ void __launch_bounds__(256) build_rphi_kernel(const double* __restrict__ r, const double* __restrict__ phi,
-                                                         double2* __restrict__ rphi, double2* __restrict__ rphi_mid,
-                                                         uint64_t n)
+// ---- radius directory -------------------------------------------------------------------------
+// Coarse interval c holds the nodes j with j >> shift == c (j >= 1); its radii lie in [Rl, Rh],
+// Rl = r of node c << shift (0 for c = 0), Rh = r of node (c+1) << shift (r_N in the last
+// interval).  bucket() maps a radius of the interval to one of K = 2^shift equal-width buckets;
+// it is monotone non-decreasing in x, which is all the look-up relies on.  row[b] = number of
+// nodes of the interval whose bucket is < b, b = 0..K.
+__device__ __forceinline__ float bucket_scale(double Rl, double Rh, uint32_t K) { return (float)K / (float)(Rh - Rl); }
+
+__device__ __forceinline__ uint32_t bucket(double x, double Rl, float scale, uint32_t K)
+{
+    float t = (float)(x - Rl) * scale;
+    uint32_t b = 0;                                        // t < 0 or NaN (Rh == Rl)
+    if (t >= 0.0f) b = (t < (float)K) ? (uint32_t)t : K - 1;
+    return b;
+}
+
+// nodes[j], j = 0..n+1
+__global__ void __launch_bounds__(256) build_nodes_kernel(const double* __restrict__ r, const double* __restrict__ phi,
+                                                          const double* __restrict__ m_cum, double G,
+                                                          Node* __restrict__ nodes, uint64_t n)
 {
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
-    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        double2 e = make_double2(__ldcs(r + i), __ldcs(phi + i));
-        rphi[i] = e;
-        if (((i + 1) & MID_MASK) == 0) rphi_mid[(i + 1) >> MID_SHIFT] = e;
+    for (uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; j <= n + 1; j += stride) {
+        Node e;
+        if (j == 0) { e.r = 0.0; e.phi = __ldg(phi); e.B = 0.0; e.u = 0.0; }
+        else if (j == n + 1) { e.r = pos_inf(); e.phi = 0.0; e.B = G * __ldg(m_cum + (n - 1)); e.u = 0.0; }
+        else {
+            const double rj = __ldcs(r + (j - 1));
+            e.r = rj; e.phi = __ldcs(phi + (j - 1)); e.B = G * __ldcs(m_cum + (j - 1)); e.u = 1.0 / rj;
+        }
+        nodes[j] = e;
     }
 }
 
-// r_mid[c] = r of node 8c
-__global__ void __launch_bounds__(256) build_rmid_kernel(const double* __restrict__ r, double* __restrict__ r_mid,
-                                                         uint64_t n)
+__global__ void __launch_bounds__(256) build_dir_kernel(const double* __restrict__ r, uint16_t* __restrict__ dir,
+                                                        uint32_t n, int shift)
 {
-    const uint64_t nm = n >> MID_SHIFT;
-    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
-    for (uint64_t c = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x + 1; c <= nm; c += stride)
-        r_mid[c] = __ldg(r + ((c << MID_SHIFT) - 1));
+    const uint32_t K = 1u << shift;
+    const uint32_t stride = gridDim.x * blockDim.x;
+    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x + 1; j <= n; j += stride) {
+        const uint32_t c = j >> shift;
+        const uint32_t j0 = max(c << shift, 1u);                     // first node of the interval
+        const uint32_t jn = min(((c + 1) << shift) - 1, n);          // last node of the interval
+        const double Rl = c ? __ldg(r + ((c << shift) - 1)) : 0.0;
+        const double Rh = (((uint64_t)(c + 1) << shift) <= n) ? __ldg(r + (((c + 1) << shift) - 1)) : __ldg(r + (n - 1));
+        const float scale = bucket_scale(Rl, Rh, K);
+        const uint32_t b = bucket(__ldg(r + (j - 1)), Rl, scale, K);
+        const int bprev = (j > j0) ? (int)bucket(__ldg(r + (j - 2)), Rl, scale, K) : -1;
+        uint16_t* row = dir + (size_t)c * (K + 1);
+        for (int bb = bprev + 1; bb <= (int)b; ++bb) row[bb] = (uint16_t)(j - j0);
+        if (j == jn)
+            for (uint32_t bb = b + 1; bb <= K; ++bb) row[bb] = (uint16_t)(j - j0 + 1);
+    }
 }
 
-// ---- S3 ---------------------------------------------------------------------------------------
-struct RPhiTable {
-    const double2* full;     // [n]   node j at full[j-1]
-    const double2* mid;      // [n/8+1] node 8c at mid[c]
-    const double2* coarse;   // shared memory, node c << shift at coarse[c]
-    uint32_t low_mask;       // (1 << shift) - 1
+// coarse[c] = (r, Phi) of node c << shift, c = 1..ncoarse; coarse[0] = (0, Phi_1) and
+// coarse[ncoarse + 1] = (+inf, 0) are the sentinel nodes 0 and N+1.
+__device__ __forceinline__ void stage_coarse(double2* coarse, const Node* __restrict__ nodes, uint32_t n, int shift)
+{
+    const uint32_t ncoarse = n >> shift;
+    for (uint32_t c = threadIdx.x; c <= ncoarse; c += ORB_THREADS) {
+        Node e = ld_node(nodes + ((uint64_t)c << shift));
+        coarse[c] = make_double2(e.r, e.phi);
+    }
+    if (threadIdx.x == 0) coarse[ncoarse + 1] = make_double2(pos_inf(), 0.0);
+    __syncthreads();
+}
+
+struct Tables {
+    const Node* nodes;       // [n + 2]
+    const uint16_t* dir;
+    const double2* coarse;   // shared memory
+    double r_last;           // r_N
+    uint32_t n, ncoarse, K;
     int shift;
-    __device__ __forceinline__ double2 global_node(uint32_t p) const
+    // upper radius of coarse interval c, as build_dir_kernel defines it
+    __device__ __forceinline__ double interval_rh(uint32_t c) const { return c < ncoarse ? coarse[c + 1].x : r_last; }
+    // nodes lo < hi with  r_lo <= x < r_hi  as far as the directory knows: every node of interval c
+    // outside (lo, hi) is on the side stated.  x must lie in the radius range of interval c for the
+    // result to be tight; for any x it is a valid starting point of an exact search.
+    __device__ __forceinline__ void dir_range(uint32_t c, double x, uint32_t& lo, uint32_t& hi) const
     {
-        return (p & MID_MASK) ? __ldg(full + (p - 1)) : __ldg(mid + (p >> MID_SHIFT));
+        const double Rl = coarse[c].x;
+        const uint32_t b = bucket(x, Rl, bucket_scale(Rl, interval_rh(c), K), K);
+        const uint16_t* row = dir + (size_t)c * (K + 1) + b;
+        const uint32_t o0 = __ldg(row), o1 = __ldg(row + 1);
+        const uint32_t j0 = max(c << shift, 1u);
+        lo = j0 + o0 - 1;
+        hi = j0 + o1;
     }
 };
 
+// ---- S3 ---------------------------------------------------------------------------------------
 // Q(r_p) < 0, division-free (R2):  2 (E - Phi_p) r_p^2 < J^2
-__device__ __forceinline__ bool q_negative(double2 e, double E, double J2)
+__device__ __forceinline__ bool q_negative(double rp, double phip, double E, double J2)
 {
-    return 2.0 * ((E - e.y) * (e.x * e.x)) < J2;
+    return 2.0 * ((E - phip) * (rp * rp)) < J2;
+}
+
+// One side of the bracket search after the coarse tier.  The invariant is: node lo is "inside the
+// class" (pericentre: Q < 0; apocentre: Q >= 0), node hi is not; done when hi - lo == 1.
+enum { MODE_GUESS = 0, MODE_UP = 1, MODE_DOWN = 2, MODE_BISECT = 3 };
+
+struct Side {
+    uint32_t lo, hi, step, guess;
+    int mode;
+    __device__ __forceinline__ bool active() const { return hi - lo > 1; }
+    // first node of the adjacent pair (p, p+1) to probe next; lo < p < hi
+    __device__ __forceinline__ uint32_t probe() const
+    {
+        uint32_t p;
+        if (mode == MODE_GUESS) p = guess;
+        else if (mode == MODE_UP) p = lo + step;
+        else if (mode == MODE_DOWN) p = (hi > step + 1) ? hi - step - 1 : 0;
+        else p = lo + (hi - lo) / 2;
+        return min(max(p, lo + 1), hi - 1);
+    }
+    // c0 / c1: node p / p+1 is inside the class (c1 is ignored when p + 1 == hi)
+    __device__ __forceinline__ void update(uint32_t p, bool c0, bool c1)
+    {
+        const bool two = p + 1 < hi;
+        if (two && c1) {                       // both inside: the sign change is above p+1
+            lo = p + 1;
+            if (mode == MODE_GUESS) { mode = MODE_UP; step = 1; }
+            else if (mode == MODE_UP) step *= 2;
+            else mode = MODE_BISECT;
+        } else if (c0) {                       // p inside, p+1 outside (or p+1 == hi)
+            lo = p;
+            if (two) hi = p + 1;
+            mode = MODE_BISECT;
+        } else {                               // p outside: the sign change is below p
+            hi = p;
+            if (mode == MODE_GUESS) { mode = MODE_DOWN; step = 1; }
+            else if (mode == MODE_DOWN) step *= 2;
+            else mode = MODE_BISECT;
+        }
+    }
+};
+
+// Secant estimate of the root of P(r) = r^2 Q(r) between two nodes with P_lo and P_hi of opposite
+// sign, turned into a node number through the directory.  Only a starting point: any value works.
+__device__ __forceinline__ uint32_t guess_node(const Tables& T, uint32_t lo, uint32_t hi, double r_lo, double P_lo,
+                                               double r_hi, double P_hi)
+{
+    const double x = r_lo + (r_hi - r_lo) * (P_lo / (P_lo - P_hi));
+    uint32_t a, b;
+    T.dir_range(lo >> T.shift, x, a, b);
+    return a;                                  // last node known to lie at or below x
 }
 
 __global__ void __launch_bounds__(ORB_THREADS, 1)
 turning_points_kernel(uint32_t n, double G, const double* __restrict__ r, const double* __restrict__ v_r,
                       const double* __restrict__ v_t, const double* __restrict__ phi,
-                      const double* __restrict__ m_cum, const double2* __restrict__ rphi,
-                      const double2* __restrict__ rphi_mid, int shift, double* __restrict__ E_out,
-                      double* __restrict__ J_out, double* __restrict__ rmin_out, double* __restrict__ rmax_out,
-                      uint32_t* __restrict__ kmin_out, uint32_t* __restrict__ kmax_out,
+                      const Node* __restrict__ nodes, const uint16_t* __restrict__ dir, int shift,
+                      double* __restrict__ E_out, double* __restrict__ J_out, double* __restrict__ rmin_out,
+                      double* __restrict__ rmax_out, uint32_t* __restrict__ kmin_out, uint32_t* __restrict__ kmax_out,
                       uint8_t* __restrict__ status_out, unsigned long long* __restrict__ counters)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double2* coarse = reinterpret_cast<double2*>(smem_raw);     // coarse[c] = node c << shift, c >= 1
-    const uint32_t ncoarse = n >> shift;
-    for (uint32_t c = threadIdx.x + 1; c <= ncoarse; c += ORB_THREADS) coarse[c] = rphi[((uint64_t)c << shift) - 1];
-    __syncthreads();
-    RPhiTable T{ rphi, rphi_mid, coarse, (1u << shift) - 1u, shift };
+    double2* coarse = reinterpret_cast<double2*>(smem_raw);
+    stage_coarse(coarse, nodes, n, shift);
+    Tables T{ nodes, dir, coarse, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift };
+    const uint32_t low_mask = T.K - 1u;
 
     const uint32_t stride = gridDim.x * ORB_THREADS;
     for (uint32_t a = blockIdx.x * ORB_THREADS + threadIdx.x; a < n; a += stride) {
@@ -123,44 +236,60 @@ turning_points_kernel(uint32_t n, double G, const double* __restrict__ r, const 
             rmax = (st & HMC_STAR_UNBOUND) ? pos_inf() : rk;
             kmin = k - 1; kmax = k;
         } else {
-            // pericentre bracket (lo1, hi1): Q_lo1 < 0 <= Q_hi1;  apocentre (lo2, hi2): Q_lo2 >= 0 > Q_hi2
-            uint32_t lo1 = 0, hi1 = k, lo2 = k, hi2 = n + 1;
-            // levels held in shared memory
-            while (hi1 - lo1 > 1) {
-                uint32_t p = pivot(lo1, hi1);
-                if (p & T.low_mask) break;
-                if (q_negative(coarse[p >> shift], E, J2)) lo1 = p; else hi1 = p;
+            // pericentre bracket (lo, hi): Q_lo < 0 <= Q_hi;  apocentre: Q_lo >= 0 > Q_hi
+            Side s1{ 0u, k, 1u, 0u, MODE_BISECT }, s2{ k, n + 1, 1u, 0u, MODE_BISECT };
+            // tier 1: the coarse nodes, in shared memory
+            while (s1.active()) {
+                uint32_t p = pivot(s1.lo, s1.hi);
+                if (p & low_mask) break;
+                double2 e = coarse[p >> shift];
+                if (q_negative(e.x, e.y, E, J2)) s1.lo = p; else s1.hi = p;
             }
-            while (hi2 - lo2 > 1) {
-                uint32_t p = pivot(lo2, hi2);
-                if (p & T.low_mask) break;
-                if (q_negative(coarse[p >> shift], E, J2)) hi2 = p; else lo2 = p;
+            while (s2.active()) {
+                uint32_t p = pivot(s2.lo, s2.hi);
+                if (p & low_mask) break;
+                double2 e = coarse[p >> shift];
+                if (q_negative(e.x, e.y, E, J2)) s2.hi = p; else s2.lo = p;
             }
-            // remaining levels from global memory, the two searches interleaved
+            // tier 2: secant guess.  The ends are coarse nodes or the star's own node, where
+            // P = r^2 Q = (r_k v_r)^2.  The first and last intervals (a sentinel at one end) bisect.
+            const double Pk = (rk * vr) * (rk * vr);
+            if (s1.hi - s1.lo > 2 && s1.lo > 0) {
+                double2 el = coarse[s1.lo >> shift];
+                double r_hi = rk, P_hi = Pk;
+                if (s1.hi != k) { double2 eh = coarse[s1.hi >> shift]; r_hi = eh.x; P_hi = 2.0 * ((E - eh.y) * (eh.x * eh.x)) - J2; }
+                s1.guess = guess_node(T, s1.lo, s1.hi, el.x, 2.0 * ((E - el.y) * (el.x * el.x)) - J2, r_hi, P_hi);
+                s1.mode = MODE_GUESS;
+            }
+            if (s2.hi - s2.lo > 2 && s2.hi <= n) {
+                double2 eh = coarse[s2.hi >> shift];
+                double r_lo = rk, P_lo = Pk;
+                if (s2.lo != k) { double2 el = coarse[s2.lo >> shift]; r_lo = el.x; P_lo = 2.0 * ((E - el.y) * (el.x * el.x)) - J2; }
+                s2.guess = guess_node(T, s2.lo, s2.hi, r_lo, P_lo, eh.x, 2.0 * ((E - eh.y) * (eh.x * eh.x)) - J2);
+                s2.mode = MODE_GUESS;
+            }
+            // tier 3: exact probes of adjacent node pairs, the two searches interleaved
             while (true) {
-                const bool a1 = hi1 - lo1 > 1, a2 = hi2 - lo2 > 1;
+                const bool a1 = s1.active(), a2 = s2.active();
                 if (!(a1 || a2)) break;
-                uint32_t p1 = a1 ? pivot(lo1, hi1) : 1u, p2 = a2 ? pivot(lo2, hi2) : 1u;
-                double2 e1, e2;
-                if (a1) e1 = T.global_node(p1);
-                if (a2) e2 = T.global_node(p2);
-                if (a1) { if (q_negative(e1, E, J2)) lo1 = p1; else hi1 = p1; }
-                if (a2) { if (q_negative(e2, E, J2)) hi2 = p2; else lo2 = p2; }
+                const uint32_t p1 = a1 ? s1.probe() : 0u, p2 = a2 ? s2.probe() : 0u;
+                Node e10, e11, e20, e21;
+                if (a1) { e10 = ld_node(nodes + p1); e11 = ld_node(nodes + p1 + 1); }
+                if (a2) { e20 = ld_node(nodes + p2); e21 = ld_node(nodes + p2 + 1); }
+                if (a1) s1.update(p1, q_negative(e10.r, e10.phi, E, J2), q_negative(e11.r, e11.phi, E, J2));
+                if (a2) s2.update(p2, !q_negative(e20.r, e20.phi, E, J2), !q_negative(e21.r, e21.phi, E, J2));
             }
-            kmin = lo1; kmax = lo2;
+            kmin = s1.lo; kmax = s2.lo;
             // closed-form roots of Q(u) = 2C + 2Bu - J^2 u^2 in the bracketing shells (R3)
-            double2 ea = (kmin == 0) ? make_double2(1.0, __ldg(phi)) : __ldg(rphi + (kmin - 1));
-            double2 eb = __ldg(rphi + (kmax - 1));                       // kmax >= k >= 1
-            double Ba = (kmin == 0) ? 0.0 : G * __ldg(m_cum + (kmin - 1));
-            double Bb = G * __ldg(m_cum + (kmax - 1));
-            double Ca = (kmin == 0) ? (E - ea.y) : ((E - ea.y) - Ba * (1.0 / ea.x));
-            double Cb = (E - eb.y) - Bb * (1.0 / eb.x);
-            double D = Ba * Ba + 2.0 * (J2 * Ca);
+            const Node ea = ld_node(nodes + kmin), eb = ld_node(nodes + kmax);
+            const double Ca = (E - ea.phi) - ea.B * ea.u;
+            const double Cb = (E - eb.phi) - eb.B * eb.u;
+            double D = ea.B * ea.B + 2.0 * (J2 * Ca);
             if (D < 0.0) D = 0.0;
-            rmin = J2 / (Ba + sqrt(D));
-            D = Bb * Bb + 2.0 * (J2 * Cb);
+            rmin = J2 / (ea.B + sqrt(D));
+            D = eb.B * eb.B + 2.0 * (J2 * Cb);
             if (D < 0.0) D = 0.0;
-            if (Cb < 0.0) rmax = (Bb + sqrt(D)) / (-2.0 * Cb);
+            if (Cb < 0.0) rmax = (eb.B + sqrt(D)) / (-2.0 * Cb);
             else { rmax = pos_inf(); st |= HMC_STAR_DEGENERATE; }
         }
         __stcs(E_out + a, E); __stcs(J_out + a, J); __stcs(rmin_out + a, rmin); __stcs(rmax_out + a, rmax);
@@ -190,7 +319,7 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 
 // ---- S4 ---------------------------------------------------------------------------------------
 struct Orbit {          // per-star constants of the draw
-    double E, J2, mid, quarter, three_q, F;
+    double E, J, J2, mid, quarter, three_q, F;
     uint32_t kmin, kmax, sid;
 };
 
@@ -213,30 +342,41 @@ __device__ __forceinline__ Trial make_trial(const Orbit& o, uint32_t seed_lo, ui
     return tr;
 }
 
-struct RTable {
-    const double* r;         // [n]
-    const double* r_mid;     // node 8c at r_mid[c]
-    const double* phi;
-    const double* m_cum;
-    double G;
-    __device__ __forceinline__ double node_r(uint32_t p) const
-    {
-        return (p & MID_MASK) ? __ldg(r + (p - 1)) : __ldg(r_mid + (p >> MID_SHIFT));
-    }
-};
-
-// exact evaluation of a trial, the oracle's expressions: shell j of r0 inside (lo, hi) (which must
-// satisfy r_lo <= r0 < r_hi in the clamped sense), Phi(r0) by Eq. 6 anchored at j, Q0, g.
-__device__ __forceinline__ void exact_trial(const RTable& T, const Orbit& o, const Trial& tr, uint32_t lo, uint32_t hi,
-                                            double& Q0, double& g)
+// coarse interval of r0, clamped to the orbit's own: largest c in [cl, ch] with coarse[c].r <= r0
+__device__ __forceinline__ uint32_t coarse_locate(const double2* coarse, uint32_t cl, uint32_t ch, double r0)
 {
+    uint32_t lo = cl, hi = ch + 1;
     while (hi - lo > 1) {
-        uint32_t p = pivot(lo, hi);
-        if (T.node_r(p) <= tr.r0) lo = p; else hi = p;
+        uint32_t m = (lo + hi) >> 1;
+        if (coarse[m].x <= r0) lo = m; else hi = m;
     }
-    double phi0;
-    if (lo == 0) phi0 = __ldg(T.phi);
-    else phi0 = __ldg(T.phi + (lo - 1)) - (T.G * __ldg(T.m_cum + (lo - 1))) * (1.0 / tr.r0 - 1.0 / __ldg(T.r + (lo - 1)));
+    return lo;
+}
+
+// Exact evaluation of a trial, the oracle's expressions: shell j = #{ i : r_i <= r0 } clamped to
+// [k_min, k_max], found from the directory of coarse interval c; Phi(r0) by Eq. 6 anchored at j; Q0; g.
+__device__ __forceinline__ void exact_trial(const Tables& T, const Orbit& o, const Trial& tr, uint32_t c, double& Q0, double& g)
+{
+    uint32_t lo, hi;
+    if (T.shift == 0) { lo = c; hi = c + 1; }          // the coarse table is the whole table
+    else {
+        T.dir_range(c, tr.r0, lo, hi);
+        lo = max(lo, o.kmin); hi = min(hi, o.kmax + 1);
+        if (hi <= lo) { lo = min(lo, o.kmax); hi = lo + 1; }
+    }
+    Node e = ld_node(T.nodes + lo);
+    if (hi - lo > 1) {
+        Node e1 = ld_node(T.nodes + lo + 1);
+        if (e1.r <= tr.r0) {
+            lo = lo + 1; e = e1;
+            while (hi - lo > 1) {
+                uint32_t p = (hi - lo > 4) ? lo + (hi - lo) / 2 : lo + 1;
+                Node ep = ld_node(T.nodes + p);
+                if (ep.r <= tr.r0) { lo = p; e = ep; } else hi = p;
+            }
+        }
+    }
+    const double phi0 = e.phi - e.B * (1.0 / tr.r0 - e.u);            // Eq. 6 anchored at node lo (R3)
     Q0 = 2.0 * (o.E - phi0) - o.J2 / (tr.r0 * tr.r0);                  // Eq. 12
     g = 0.0;
     if (Q0 > 0.0) g = (o.three_q * (1.0 - tr.s * tr.s)) / sqrt(Q0);
@@ -244,16 +384,17 @@ __device__ __forceinline__ void exact_trial(const RTable& T, const Orbit& o, con
 
 // Cold path, reached only if HMC_T_MAX trials were all rejected: redo the star exactly as the
 // oracle's loop does, every trial evaluated, remembering the last trial with Q0 > 0.
-__device__ __noinline__ void draw_exhaustive(const RTable& T, const Orbit& o, uint32_t seed_lo, uint32_t seed_hi,
+__device__ __noinline__ void draw_exhaustive(const Tables& T, const Orbit& o, uint32_t seed_lo, uint32_t seed_hi,
                                              uint32_t step, unsigned& st, bool& accepted, uint32_t& used,
                                              bool& have_good, double& good_r, double& good_Q, uint32_t& good_w3)
 {
     accepted = false; have_good = false;
+    const uint32_t cl = o.kmin >> T.shift, ch = o.kmax >> T.shift;
     uint32_t t = 0;
     for (; t < HMC_T_MAX; ++t) {
         Trial tr = make_trial(o, seed_lo, seed_hi, step, t);
         double Q0, g;
-        exact_trial(T, o, tr, o.kmin, o.kmax + 1, Q0, g);
+        exact_trial(T, o, tr, coarse_locate(T.coarse, cl, ch, tr.r0), Q0, g);
         if (Q0 > 0.0) {
             have_good = true; good_r = tr.r0; good_Q = Q0; good_w3 = tr.w3;
             if (g > o.F) st |= HMC_STAR_CLIPPED;
@@ -263,143 +404,169 @@ __device__ __noinline__ void draw_exhaustive(const RTable& T, const Orbit& o, ui
     used = accepted ? t + 1 : HMC_T_MAX;
 }
 
+struct SampleIO {
+    const double *r, *v_r, *v_t, *E, *J, *rmin, *rmax;
+    const uint32_t *kmin, *kmax, *id;
+    const uint8_t* status_in;
+    double *r_new, *v_r_new, *v_t_new;
+    uint16_t* n_try;
+    uint8_t* status_out;
+    unsigned long long* counters;
+};
+
+__device__ __forceinline__ void finish_star(const SampleIO& io, uint32_t a, double out_r, double out_vr, double out_vt,
+                                            uint32_t used, unsigned st)
+{
+    __stcs(io.r_new + a, out_r); __stcs(io.v_r_new + a, out_vr); __stcs(io.v_t_new + a, out_vt);
+    if (io.n_try) io.n_try[a] = (uint16_t)used;
+    io.status_out[a] = (uint8_t)st;
+    if (io.counters && (st & (HMC_STAR_CIRCULAR | HMC_STAR_MAXTRIES | HMC_STAR_CLIPPED))) {
+        if (st & HMC_STAR_CIRCULAR) atomicAdd(io.counters + HMC_CNT_CIRCULAR, 1ull);
+        if (st & HMC_STAR_MAXTRIES) atomicAdd(io.counters + HMC_CNT_MAXTRIES, 1ull);
+        if (st & HMC_STAR_CLIPPED) atomicAdd(io.counters + HMC_CNT_CLIPPED, 1ull);
+    }
+}
+
 __global__ void __launch_bounds__(ORB_THREADS, 1)
 sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_hi, uint32_t step,
-                         const double* __restrict__ r, const double* __restrict__ phi,
-                         const double* __restrict__ m_cum, const double* __restrict__ r_mid, int shift,
-                         const double* __restrict__ v_r, const double* __restrict__ v_t,
-                         const double* __restrict__ E_in, const double* __restrict__ J_in,
-                         const double* __restrict__ rmin_in, const double* __restrict__ rmax_in,
-                         const uint32_t* __restrict__ kmin_in, const uint32_t* __restrict__ kmax_in,
-                         const uint32_t* __restrict__ id, const uint8_t* __restrict__ status_in,
-                         double* __restrict__ r_new, double* __restrict__ v_r_new, double* __restrict__ v_t_new,
-                         uint16_t* __restrict__ n_try, uint8_t* __restrict__ status_out,
-                         unsigned long long* __restrict__ counters)
+                         const Node* __restrict__ nodes, const uint16_t* __restrict__ dir, int shift, SampleIO io)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    // coarse[c] = (r, Phi) of node c << shift for 1 <= c <= ncoarse; sentinels (0, Phi_1) and (inf, 0)
     double2* coarse = reinterpret_cast<double2*>(smem_raw);
-    const uint32_t ncoarse = n >> shift;
-    for (uint32_t c = threadIdx.x + 1; c <= ncoarse; c += ORB_THREADS) {
-        uint64_t a = ((uint64_t)c << shift) - 1;
-        coarse[c] = make_double2(__ldg(r + a), __ldg(phi + a));
-    }
-    if (threadIdx.x == 0) { coarse[0] = make_double2(0.0, __ldg(phi)); coarse[ncoarse + 1] = make_double2(pos_inf(), 0.0); }
-    __syncthreads();
-    RTable T{ r, r_mid, phi, m_cum, G };
+    stage_coarse(coarse, nodes, n, shift);
+    Tables T{ nodes, dir, coarse, __ldg(io.r + (n - 1)), n, n >> shift, 1u << shift, shift };
     unsigned long long my_trials = 0;
+    const unsigned lane_lt = lanemask_lt();
 
-    const uint32_t stride = gridDim.x * ORB_THREADS;
-    for (uint32_t a = blockIdx.x * ORB_THREADS + threadIdx.x; a < n; a += stride) {
-        unsigned st = status_in[a];
-        double out_r = 0.0, out_vr = 0.0, out_vt = 0.0;
-        bool moved = false;
-        uint32_t used = 0;
-        if (!(st & (HMC_STAR_UNBOUND | HMC_STAR_RADIAL | HMC_STAR_DEGENERATE))) {
-            Orbit o;
-            o.E = __ldcs(E_in + a);
-            const double J = __ldcs(J_in + a);
-            o.J2 = J * J;
-            const double rmin = __ldcs(rmin_in + a), rmax = __ldcs(rmax_in + a);
-            o.kmin = __ldcs(kmin_in + a); o.kmax = __ldcs(kmax_in + a);
-            const double delta = rmax - rmin;
-            bool ok = delta > 0.0;
-            o.F = 0.0;
-            if (ok) {
-                double Bmin = (o.kmin == 0) ? 0.0 : G * __ldg(m_cum + (o.kmin - 1));
-                double Bmax = (o.kmax == 0) ? 0.0 : G * __ldg(m_cum + (o.kmax - 1));
-                double q1 = (2.0 * (o.J2 / rmin - Bmin)) / (rmin * rmin);      // Q'(r_min) in shell k_min
-                double q2 = (2.0 * (o.J2 / rmax - Bmax)) / (rmax * rmax);      // Q'(r_max) in shell k_max
-                ok = (q1 > 0.0) && (q2 < 0.0);
-                if (ok) o.F = 1.2 * fmax(sqrt((3.0 * delta) / q1), sqrt((3.0 * delta) / (-q2)));
-            }
-            if (!ok) st |= HMC_STAR_CIRCULAR;
-            else {
-                o.mid = 0.5 * (rmin + rmax);
-                o.quarter = 0.25 * delta; o.three_q = 0.75 * delta;
-                o.sid = __ldcs(id + a);
-                const uint32_t cl = o.kmin >> shift, ch = o.kmax >> shift;
-                bool accepted = false, have_good = false;
-                double good_r = 0.0, good_Q = 0.0;
-                uint32_t good_w3 = 0, t = 0;
-                while (true) {
-                    // phase 1: trials decided from shared memory only, until one cannot be rejected
-                    Trial tr;
-                    uint32_t c = 0;
-                    bool cand = false;
-                    for (; t < HMC_T_MAX; ++t) {
-                        tr = make_trial(o, seed_lo, seed_hi, step, t);
-                        uint32_t lo = cl, hi = ch + 1;                 // coarse[lo].x <= r0 < coarse[hi].x (clamped)
-                        while (hi - lo > 1) {
-                            uint32_t m = (lo + hi) >> 1;
-                            if (coarse[m].x <= tr.r0) lo = m; else hi = m;
-                        }
-                        c = lo;
-                        // Phi(r0) lies in [coarse[c].y, coarse[c+1].y]; widen everything by ~1e-11
-                        const double u0 = 1.0 / tr.r0;
-                        const double cen = (o.J2 * u0) * u0;
-                        const double top = 2.0 * (o.E - coarse[c].y);
-                        const double tol = 1e-11 * (fabs(top) + cen);
-                        const double Qh = (top - cen) + tol;
-                        if (Qh <= 0.0) continue;                       // Q0 <= 0 for certain: rejected
-                        const double Ql = (2.0 * (o.E - coarse[c + 1].y) - cen) - tol;
-                        const double fx = o.F * tr.Xp, cc = o.three_q * (1.0 - tr.s * tr.s);
-                        if (Ql > 0.0 && (fx * fx) * Ql > (cc * cc) * (1.0 + 1e-10)) continue;   // F X' > g for certain
-                        cand = true;
-                        break;
-                    }
-                    if (!cand) break;
-                    // phase 2: the exact test for the candidate
-                    const uint32_t lo = max(o.kmin, c << shift);
-                    const uint32_t hi = (c >= ncoarse) ? (o.kmax + 1) : min(o.kmax + 1, (c + 1) << shift);
-                    double Q0, g;
-                    exact_trial(T, o, tr, lo, hi, Q0, g);
-                    ++t;
-                    if (Q0 > 0.0) {
-                        if (g > o.F) st |= HMC_STAR_CLIPPED;
-                        if (o.F * tr.Xp < g) {
-                            accepted = true; have_good = true; good_r = tr.r0; good_Q = Q0; good_w3 = tr.w3;
-                            break;
+    // each warp owns a contiguous run of stars (a multiple of 32) and deals them to its lanes
+    const uint32_t warps_total = gridDim.x * ORB_WARPS;
+    const uint32_t gw = blockIdx.x * ORB_WARPS + (threadIdx.x >> 5);
+    const uint32_t per = (uint32_t)((((uint64_t)n + warps_total - 1) / warps_total + 31) & ~31ull);
+    uint32_t next = (uint32_t)min((unsigned long long)n, (unsigned long long)gw * per);
+    const uint32_t end = (uint32_t)min((unsigned long long)n, (unsigned long long)next + per);
+
+    bool have = false;
+    uint32_t a = 0, t = 0, cl = 0, ch = 0;
+    unsigned st = 0;
+    Orbit o;
+    while (true) {
+        // ---- deal new stars to the free lanes
+        const unsigned need = __ballot_sync(0xffffffffu, !have);
+        if (need && next < end) {
+            const uint32_t mine = next + __popc(need & lane_lt);
+            next = min(end, next + (uint32_t)__popc(need));
+            if (!have && mine < end) {
+                a = mine;
+                st = io.status_in[a];
+                bool ok = !(st & (HMC_STAR_UNBOUND | HMC_STAR_RADIAL | HMC_STAR_DEGENERATE));
+                if (ok) {
+                    o.E = __ldcs(io.E + a);
+                    o.J = __ldcs(io.J + a);
+                    o.J2 = o.J * o.J;
+                    const double rmin = __ldcs(io.rmin + a), rmax = __ldcs(io.rmax + a);
+                    o.kmin = __ldcs(io.kmin + a); o.kmax = __ldcs(io.kmax + a);
+                    const double delta = rmax - rmin;
+                    ok = delta > 0.0;
+                    if (ok) {
+                        const double Bmin = ld_node(nodes + o.kmin).B, Bmax = ld_node(nodes + o.kmax).B;
+                        const double q1 = (2.0 * (o.J2 / rmin - Bmin)) / (rmin * rmin);      // Q'(r_min) in shell k_min
+                        const double q2 = (2.0 * (o.J2 / rmax - Bmax)) / (rmax * rmax);      // Q'(r_max) in shell k_max
+                        ok = (q1 > 0.0) && (q2 < 0.0);
+                        if (ok) {
+                            o.F = 1.2 * fmax(sqrt((3.0 * delta) / q1), sqrt((3.0 * delta) / (-q2)));
+                            o.mid = 0.5 * (rmin + rmax);
+                            o.quarter = 0.25 * delta; o.three_q = 0.75 * delta;
+                            o.sid = __ldcs(io.id + a);
+                            cl = o.kmin >> shift; ch = o.kmax >> shift;
+                            t = 0;
+                            have = true;
                         }
                     }
+                    if (!ok) st |= HMC_STAR_CIRCULAR;
                 }
-                used = t;
-                if (!accepted) draw_exhaustive(T, o, seed_lo, seed_hi, step, st, accepted, used, have_good, good_r, good_Q, good_w3);
+                if (!have) finish_star(io, a, __ldg(io.r + a), __ldcs(io.v_r + a), __ldcs(io.v_t + a), 0u, st);
+            }
+        }
+        if (!__any_sync(0xffffffffu, have)) {
+            if (next >= end) break;
+            continue;
+        }
+        // ---- one trial for every lane that holds a star
+        if (have) {
+            const Trial tr = make_trial(o, seed_lo, seed_hi, step, t);
+            const uint32_t c = coarse_locate(coarse, cl, ch, tr.r0);
+            ++t;
+            // squeeze: Phi(r0) lies in [coarse[c].Phi, coarse[c+1].Phi]; everything widened by ~1e-11.
+            // Written multiplied through by r0^2 > 0, so there is no division on this path.
+            const double r2 = tr.r0 * tr.r0;
+            const double top = 2.0 * (o.E - coarse[c].y) * r2;
+            const double tol = 1e-11 * (fabs(top) + o.J2);
+            const double Qh = (top - o.J2) + tol;                       // upper bound of r0^2 Q0
+            bool candidate = Qh > 0.0;
+            if (candidate) {
+                const double Ql = (2.0 * (o.E - coarse[c + 1].y) * r2 - o.J2) - tol;   // lower bound of r0^2 Q0
+                const double fx = o.F * tr.Xp, cc = o.three_q * (1.0 - tr.s * tr.s);
+                if (Ql > 0.0 && (fx * fx) * Ql > ((cc * cc) * r2) * (1.0 + 1e-10)) candidate = false;   // F X' > g for certain
+            }
+            bool done = false, accepted = false, have_good = false;
+            double good_r = 0.0, good_Q = 0.0;
+            uint32_t good_w3 = 0, used = t;
+            if (candidate) {
+                double Q0, g;
+                exact_trial(T, o, tr, c, Q0, g);
+                if (Q0 > 0.0) {
+                    if (g > o.F) st |= HMC_STAR_CLIPPED;
+                    if (o.F * tr.Xp < g) { done = accepted = have_good = true; good_r = tr.r0; good_Q = Q0; good_w3 = tr.w3; }
+                }
+            }
+            if (!done && t >= HMC_T_MAX) {
+                draw_exhaustive(T, o, seed_lo, seed_hi, step, st, accepted, used, have_good, good_r, good_Q, good_w3);
+                done = true;
+            }
+            if (done) {
                 my_trials += used;
                 if (!accepted) st |= HMC_STAR_MAXTRIES;
+                double out_r, out_vr, out_vt;
                 if (have_good) {
-                    moved = true;
                     out_r = good_r;
-                    out_vt = J / good_r;
-                    double vrn = sqrt(good_Q);                         // v_r = Q^(1/2)
+                    out_vt = o.J / good_r;
+                    const double vrn = sqrt(good_Q);                    // v_r = Q^(1/2)
                     out_vr = (good_w3 & 1u) ? -vrn : vrn;
-                }
+                } else { out_r = __ldg(io.r + a); out_vr = __ldcs(io.v_r + a); out_vt = __ldcs(io.v_t + a); }
+                finish_star(io, a, out_r, out_vr, out_vt, used, st);
+                have = false;
             }
         }
-        if (!moved) { out_r = __ldg(r + a); out_vr = __ldcs(v_r + a); out_vt = __ldcs(v_t + a); }
-        __stcs(r_new + a, out_r); __stcs(v_r_new + a, out_vr); __stcs(v_t_new + a, out_vt);
-        if (n_try) n_try[a] = (uint16_t)used;
-        status_out[a] = (uint8_t)st;
-        if (counters && (st & (HMC_STAR_CIRCULAR | HMC_STAR_MAXTRIES | HMC_STAR_CLIPPED))) {
-            if (st & HMC_STAR_CIRCULAR) atomicAdd(counters + HMC_CNT_CIRCULAR, 1ull);
-            if (st & HMC_STAR_MAXTRIES) atomicAdd(counters + HMC_CNT_MAXTRIES, 1ull);
-            if (st & HMC_STAR_CLIPPED) atomicAdd(counters + HMC_CNT_CLIPPED, 1ull);
-        }
     }
-    if (counters) {
+    if (io.counters) {
         for (int off = 16; off > 0; off >>= 1) my_trials += __shfl_down_sync(0xffffffffu, my_trials, off);
-        if ((threadIdx.x & 31) == 0 && my_trials) atomicAdd(counters + HMC_CNT_TRIALS, my_trials);
+        if ((threadIdx.x & 31) == 0 && my_trials) atomicAdd(io.counters + HMC_CNT_TRIALS, my_trials);
     }
 }
 
 // ---- host side --------------------------------------------------------------------------------
+static hmc_status build_tables(uint64_t n, double G, const double* r, const double* phi, const double* m_cum,
+                               const Workspace& ws, int shift, cudaStream_t st)
+{
+    const int sms = sm_count();
+    int blocks = (int)umin64((n + 2 + 255) / 256, (uint64_t)sms * 8);
+    build_nodes_kernel<<<blocks, 256, 0, st>>>(r, phi, m_cum, G, ws.nodes, n);
+    HMC_LAUNCH_CHECK();
+    if (shift > 0) {
+        blocks = (int)umin64((n + 255) / 256, (uint64_t)sms * 8);
+        build_dir_kernel<<<blocks, 256, 0, st>>>(r, ws.dir, (uint32_t)n, shift);
+        HMC_LAUNCH_CHECK();
+    }
+    return HMC_OK;
+}
+
 hmc_status turning_points(uint64_t n, double G, const double* r, const double* v_r, const double* v_t,
                           const double* phi, const double* m_cum, double* E, double* J, double* r_min,
                           double* r_max, uint32_t* k_min, uint32_t* k_max, uint8_t* status, uint64_t* counters,
                           const Workspace& ws, cudaStream_t st)
 {
     const int sms = sm_count();
-    const int shift = coarse_shift(n, COARSE_CAP);
+    const int shift = coarse_shift(n);
     const size_t smem = ((n >> shift) + 2) * sizeof(double2);
     static bool attr_done = false;
     if (!attr_done) {
@@ -407,12 +574,11 @@ hmc_status turning_points(uint64_t n, double G, const double* r, const double* v
                                           (int)(COARSE_CAP * sizeof(double2))));
         attr_done = true;
     }
-    int blocks = (int)umin64((n + 255) / 256, (uint64_t)sms * 8);
-    build_rphi_kernel<<<blocks, 256, 0, st>>>(r, phi, ws.rphi, ws.rphi_mid, n);
-    HMC_LAUNCH_CHECK();
-    blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
-    turning_points_kernel<<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, G, r, v_r, v_t, phi, m_cum, ws.rphi,
-                                                            ws.rphi_mid, shift, E, J, r_min, r_max, k_min, k_max, status,
+    hmc_status s = build_tables(n, G, r, phi, m_cum, ws, shift, st);
+    if (s != HMC_OK) return s;
+    const int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
+    turning_points_kernel<<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, G, r, v_r, v_t, phi, ws.nodes, ws.dir, shift,
+                                                            E, J, r_min, r_max, k_min, k_max, status,
                                                             reinterpret_cast<unsigned long long*>(counters));
     HMC_LAUNCH_CHECK();
     return HMC_OK;
@@ -427,7 +593,7 @@ hmc_status sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step,
                              cudaStream_t st)
 {
     const int sms = sm_count();
-    const int shift = coarse_shift(n, COARSE_CAP);
+    const int shift = coarse_shift(n);
     const size_t smem = ((n >> shift) + 2) * sizeof(double2);
     static bool attr_done = false;
     if (!attr_done) {
@@ -435,16 +601,13 @@ hmc_status sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step,
                                           (int)(COARSE_CAP * sizeof(double2))));
         attr_done = true;
     }
-    if ((n >> MID_SHIFT) > 0) {
-        int blocks = (int)umin64(((n >> MID_SHIFT) + 255) / 256, (uint64_t)sms * 8);
-        build_rmid_kernel<<<blocks, 256, 0, st>>>(r, ws.r_mid, n);
-        HMC_LAUNCH_CHECK();
-    }
-    int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
-    sample_new_radius_kernel<<<blocks, ORB_THREADS, smem, st>>>(
-        (uint32_t)n, G, (uint32_t)seed, (uint32_t)(seed >> 32), step, r, phi, m_cum, ws.r_mid, shift, v_r, v_t, E, J,
-        r_min, r_max, k_min, k_max, id, status_in, r_new, v_r_new, v_t_new, n_try, status_out,
-        reinterpret_cast<unsigned long long*>(counters));
+    hmc_status s = build_tables(n, G, r, phi, m_cum, ws, shift, st);
+    if (s != HMC_OK) return s;
+    SampleIO io{ r, v_r, v_t, E, J, r_min, r_max, k_min, k_max, id, status_in, r_new, v_r_new, v_t_new, n_try,
+                 status_out, reinterpret_cast<unsigned long long*>(counters) };
+    const int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
+    sample_new_radius_kernel<<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, G, (uint32_t)seed, (uint32_t)(seed >> 32),
+                                                               step, ws.nodes, ws.dir, shift, io);
     HMC_LAUNCH_CHECK();
     return HMC_OK;
 }

@@ -23,7 +23,7 @@ LIB_PATH = os.path.join(_HERE, "libhmc.so")
 ST_UNBOUND, ST_RADIAL, ST_DEGENERATE, ST_CIRCULAR, ST_MAXTRIES, ST_CLIPPED = 1, 2, 4, 8, 16, 32
 COUNTER_NAMES = ("unbound", "radial", "degenerate", "circular", "maxtries", "clipped", "trials", "reserved")
 NCOUNTERS = 8
-MAX_N = 1 << 30
+MAX_N = 1 << 28
 
 _lib = None
 
