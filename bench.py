@@ -164,6 +164,11 @@ def dist_sum(x: float, device="cpu") -> float:
     return float(t.item())
 
 
+def replica_seed(seed: int, rank: int) -> int:
+    """Replicas only: rank r runs an independent cluster with seed + 1000 r."""
+    return seed + 1000 * rank
+
+
 def aggregate_throughput(stars_this_rank: float, ms_this_rank: float, device="cpu"):
     """Whole-job stars/s: stars processed by all ranks / max-over-ranks time."""
     ms = dist_max(ms_this_rank, device)
@@ -252,9 +257,9 @@ def run_gpu(args, cfg):
     c = inputs.config(args.config, args.n)
     n = c["n"]
     if world > 1:   # independent replica per rank
-        c.update(inputs.plummer(n, c["seed"] + 1000 * rank, c["masses"]))
+        c.update(inputs.plummer(n, replica_seed(c["seed"], rank), c["masses"]))
     cluster = {k: c[k] for k in ("r", "v_r", "v_t", "m", "id")}
-    seed = c["seed"] + 1000 * rank
+    seed = replica_seed(c["seed"], rank)
     d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(devs)
     stepper = hmc.OrbitStepper(d(cluster["r"]), d(cluster["v_r"]), d(cluster["v_t"]), d(cluster["m"]),
                                d(cluster["id"].view(np.int32)), seed, with_n_try=False)
