@@ -279,7 +279,7 @@ def run_gpu(args, cfg):
         ev[3].record(stream)
         hmc.hmc_sample_new_radius(so["r"], stepper.phi, stepper.m_cum, so["v_r"], so["v_t"], stepper.tp, so["id"],
                                   stepper.seed, stepper.step_index, stepper.G, out=stepper.sample,
-                                  counters=stepper.counters, workspace=stepper.workspace)
+                                  counters=stepper.counters, workspace=stepper.workspace, reuse_tables=True)
         ev[4].record(stream)
         sm = stepper.sample
         s["r"], sm["r_new"] = sm["r_new"], s["r"]

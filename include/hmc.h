@@ -148,6 +148,11 @@ HMC_API hmc_status hmc_orbit_turning_points(uint64_t n, double G,
  *   outputs  r_new, v_r_new, v_t_new [n]; n_try[n] (trials used, may be NULL);
  *            star_status_out[n] (input bits plus CIRCULAR / MAXTRIES / CLIPPED)
  * v_t_new = J / r_new, v_r_new = +-sqrt(Q(r_new)) with the sign from a spare random bit.
+ *   reuse_tables  S3 and S4 search the same tables, which each call derives from (r_sorted, phi,
+ *            m_cum, G) into the workspace.  Non-zero: the caller states that the immediately
+ *            preceding libhmc call on this workspace was hmc_orbit_turning_points with the same
+ *            n, G, r_sorted, phi and m_cum (contents unchanged), so the tables are still there and
+ *            are not rebuilt.  Zero: always correct.
  */
 HMC_API hmc_status hmc_sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step,
         const double* r_sorted, const double* phi, const double* m_cum,
@@ -156,7 +161,7 @@ HMC_API hmc_status hmc_sample_new_radius(uint64_t n, double G, uint64_t seed, ui
         const uint32_t* k_min, const uint32_t* k_max, const uint32_t* id,
         const uint8_t* star_status_in,
         double* r_new, double* v_r_new, double* v_t_new, uint16_t* n_try,
-        uint8_t* star_status_out, uint64_t* counters,
+        uint8_t* star_status_out, uint64_t* counters, int32_t reuse_tables,
         void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*

@@ -148,8 +148,8 @@ hmc_status hmc_sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t s
                                  const double* E, const double* J, const double* r_min, const double* r_max,
                                  const uint32_t* k_min, const uint32_t* k_max, const uint32_t* id,
                                  const uint8_t* star_status_in, double* r_new, double* v_r_new, double* v_t_new,
-                                 uint16_t* n_try, uint8_t* star_status_out, uint64_t* counters, void* workspace,
-                                 size_t workspace_bytes, void* cuda_stream)
+                                 uint16_t* n_try, uint8_t* star_status_out, uint64_t* counters,
+                                 int32_t reuse_tables, void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
     if (n > HMC_MAX_N) return HMC_ERR_SIZE;
     if (n == 0) return HMC_OK;
@@ -166,7 +166,7 @@ hmc_status hmc_sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t s
     hmc_status s = check_ws(workspace, workspace_bytes, n);
     if (s != HMC_OK) return s;
     return sample_new_radius(n, G, seed, step, r_sorted, phi, m_cum, v_r, v_t, E, J, r_min, r_max, k_min, k_max, id,
-                             star_status_in, r_new, v_r_new, v_t_new, n_try, star_status_out, counters,
+                             star_status_in, r_new, v_r_new, v_t_new, n_try, star_status_out, counters, reuse_tables != 0,
                              carve(workspace, n), static_cast<cudaStream_t>(cuda_stream));
 }
 
@@ -202,7 +202,7 @@ hmc_status hmc_step_host(uint64_t n, double G, uint64_t seed, uint32_t step, con
                        a.counters, ws, st);
     if (s != HMC_OK) return s;
     s = sample_new_radius(n, G, seed, step, a.rs, a.phi, a.mcum, a.vrs, a.vts, a.E, a.J, a.rmin, a.rmax, a.kmin,
-                          a.kmax, a.ids, a.st0, a.rn, a.vrn, a.vtn, nullptr, a.st1, a.counters, ws, st);
+                          a.kmax, a.ids, a.st0, a.rn, a.vrn, a.vtn, nullptr, a.st1, a.counters, true, ws, st);
     if (s != HMC_OK) return s;
     HMC_CUDA_TRY(cudaMemcpyAsync(r_new, a.rn, n * 8, cudaMemcpyDeviceToHost, st));
     HMC_CUDA_TRY(cudaMemcpyAsync(v_r_new, a.vrn, n * 8, cudaMemcpyDeviceToHost, st));

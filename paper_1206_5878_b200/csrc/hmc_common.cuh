@@ -55,7 +55,7 @@ struct Workspace {
 };
 
 // ---- orbit tables: sizes shared by carve() and hmc_orbit.cu ---------------------------------
-static constexpr uint32_t COARSE_CAP = 13824;        // (r, Phi) pairs of the shared-memory coarse table: 216 KB
+static constexpr uint32_t COARSE_CAP = 10240;        // (r, Phi) pairs of the shared-memory coarse table: 160 KB
 
 // coarse nodes are the multiples of 2^shift; smallest shift with (n >> shift) + 2 <= COARSE_CAP
 static inline int coarse_shift(uint64_t n)
@@ -183,7 +183,7 @@ hmc_status sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step,
                              const double* E, const double* J, const double* r_min, const double* r_max,
                              const uint32_t* k_min, const uint32_t* k_max, const uint32_t* id,
                              const uint8_t* status_in, double* r_new, double* v_r_new, double* v_t_new,
-                             uint16_t* n_try, uint8_t* status_out, uint64_t* counters, const Workspace& ws,
-                             cudaStream_t st);
+                             uint16_t* n_try, uint8_t* status_out, uint64_t* counters, bool reuse_tables,
+                             const Workspace& ws, cudaStream_t st);
 
 }  // namespace hmc

@@ -166,7 +166,7 @@ def alloc_sample(n: int, device="cuda", with_n_try: bool = True):
 
 
 def hmc_sample_new_radius(r_sorted, phi, m_cum, v_r, v_t, tp, ids, seed: int, step: int, G: float = 1.0, *,
-                          out=None, counters=None, workspace=None):
+                          out=None, counters=None, workspace=None, reuse_tables: bool = False):
     """S4.  ``tp`` is the dict returned by hmc_orbit_turning_points.
     -> dict(r_new, v_r_new, v_t_new, n_try, status)"""
     n = r_sorted.numel()
@@ -184,7 +184,8 @@ def hmc_sample_new_radius(r_sorted, phi, m_cum, v_r, v_t, tp, ids, seed: int, st
         _dev(tp["status"], torch.uint8, n, "status_in"), _dev(out["r_new"], f, n, "r_new"),
         _dev(out["v_r_new"], f, n, "v_r_new"), _dev(out["v_t_new"], f, n, "v_t_new"),
         _dev(out.get("n_try"), torch.int16, n, "n_try"), _dev(out["status"], torch.uint8, n, "status_out"),
-        _dev(counters, torch.int64, NCOUNTERS, "counters"), wp, wb, _stream())
+        _dev(counters, torch.int64, NCOUNTERS, "counters"), ctypes.c_int32(1 if reuse_tables else 0), wp, wb,
+        _stream())
     _check(rc, "hmc_sample_new_radius")
     return out
 
@@ -222,7 +223,7 @@ class OrbitStepper:
                                  counters=self.counters, workspace=self.workspace)
         hmc_sample_new_radius(so["r"], self.phi, self.m_cum, so["v_r"], so["v_t"], self.tp, so["id"], self.seed,
                               self.step_index, self.G, out=self.sample, counters=self.counters,
-                              workspace=self.workspace)
+                              workspace=self.workspace, reuse_tables=True)
         # carried state for the next step: new phase-space coordinates, masses and ids in sorted order
         sm = self.sample
         s["r"], sm["r_new"] = sm["r_new"], s["r"]
