@@ -50,7 +50,8 @@ struct Workspace {
     double*   scan_status;   // [2][scan_tiles][8] (flag, agg_hi, agg_lo, inc_hi, inc_lo, pad)
     // orbit
     Node*     nodes;         // [n + 2] node table with sentinels (hmc_orbit.cu)
-    uint16_t* dir;           // radius directory, dir_entries(n) entries (hmc_orbit.cu)
+    uint32_t* dir;           // radius directory, dir_entries(n) entries (hmc_orbit.cu)
+    double2*  coarse;        // [COARSE_CAP] (r, Phi) of every 2^shift-th node, contiguous (hmc_orbit.cu)
     size_t    total;
 };
 
@@ -65,11 +66,11 @@ static inline int coarse_shift(uint64_t n)
     return t;
 }
 
-// the directory holds, for each of the (n >> shift) + 1 coarse intervals, 2^shift + 1 offsets
+// the directory holds, for each of the (n >> shift) + 1 coarse intervals, 2^shift 32-bit entries
 static inline uint64_t dir_entries(uint64_t n)
 {
     const int t = coarse_shift(n);
-    return ((n >> t) + 1) * ((1ull << t) + 1);
+    return ((n >> t) + 1) * (1ull << t);
 }
 
 static constexpr int SORT_TILE = 4096;     // keys per sort tile
@@ -90,7 +91,8 @@ static inline Workspace carve(void* base, uint64_t n)
     w.tickets     = reinterpret_cast<uint32_t*>(take(32 * 4));
     w.scan_status = reinterpret_cast<double*>(take(2 * scan_tiles * 8 * 8));
     w.nodes       = reinterpret_cast<Node*>(take((n + 2) * sizeof(Node)));
-    w.dir         = reinterpret_cast<uint16_t*>(take(dir_entries(n) * 2));
+    w.dir         = reinterpret_cast<uint32_t*>(take(dir_entries(n) * 4));
+    w.coarse      = reinterpret_cast<double2*>(take(COARSE_CAP * sizeof(double2)));
     w.total = off;
     return w;
 }

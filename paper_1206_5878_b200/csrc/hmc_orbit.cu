@@ -58,12 +58,20 @@ __device__ __forceinline__ Node ld_node(const Node* __restrict__ p)
     return e;
 }
 
+__device__ __forceinline__ uint32_t ld_u32_na(const uint32_t* __restrict__ p)
+{
+    uint32_t v;
+    asm("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
+
 // ---- radius directory -------------------------------------------------------------------------
 // Coarse interval c holds the nodes j with j >> shift == c (j >= 1); its radii lie in [Rl, Rh],
 // Rl = r of node c << shift (0 for c = 0), Rh = r of node (c+1) << shift (r_N in the last
 // interval).  bucket() maps a radius of the interval to one of K = 2^shift equal-width buckets;
-// it is monotone non-decreasing in x, which is all the look-up relies on.  row[b] = number of
-// nodes of the interval whose bucket is < b, b = 0..K.
+// it is monotone non-decreasing in x, which is all the look-up relies on.  With o_b = number of
+// nodes of the interval whose bucket is < b (b = 0..K), entry b of the interval's row is the
+// 32-bit word o_b | o_{b+1} << 16, b = 0..K-1: one load gives both ends of a bucket.
 __device__ __forceinline__ float bucket_scale(double Rl, double Rh, uint32_t K) { return (float)K / (float)(Rh - Rl); }
 
 __device__ __forceinline__ uint32_t bucket(double x, double Rl, float scale, uint32_t K)
@@ -77,8 +85,10 @@ __device__ __forceinline__ uint32_t bucket(double x, double Rl, float scale, uin
 // nodes[j], j = 0..n+1
 __global__ void __launch_bounds__(256) build_nodes_kernel(const double* __restrict__ r, const double* __restrict__ phi,
                                                           const double* __restrict__ m_cum, double G,
-                                                          Node* __restrict__ nodes, uint64_t n)
+                                                          Node* __restrict__ nodes, double2* __restrict__ coarse_g,
+                                                          int shift, uint64_t n)
 {
+    const uint64_t low_mask = (1ull << shift) - 1;
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
     for (uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; j <= n + 1; j += stride) {
         Node e;
@@ -89,10 +99,11 @@ __global__ void __launch_bounds__(256) build_nodes_kernel(const double* __restri
             e.r = rj; e.phi = __ldcs(phi + (j - 1)); e.B = G * __ldcs(m_cum + (j - 1)); e.u = 1.0 / rj;
         }
         nodes[j] = e;
+        if ((j & low_mask) == 0 && j <= n) coarse_g[j >> shift] = make_double2(e.r, e.phi);
     }
 }
 
-__global__ void __launch_bounds__(256) build_dir_kernel(const double* __restrict__ r, uint16_t* __restrict__ dir,
+__global__ void __launch_bounds__(256) build_dir_kernel(const double* __restrict__ r, uint32_t* __restrict__ dir,
                                                         uint32_t n, int shift)
 {
     const uint32_t K = 1u << shift;
@@ -106,29 +117,32 @@ __global__ void __launch_bounds__(256) build_dir_kernel(const double* __restrict
         const float scale = bucket_scale(Rl, Rh, K);
         const uint32_t b = bucket(__ldg(r + (j - 1)), Rl, scale, K);
         const int bprev = (j > j0) ? (int)bucket(__ldg(r + (j - 2)), Rl, scale, K) : -1;
-        uint16_t* row = dir + (size_t)c * (K + 1);
-        for (int bb = bprev + 1; bb <= (int)b; ++bb) row[bb] = (uint16_t)(j - j0);
+        uint16_t* row = reinterpret_cast<uint16_t*>(dir + (size_t)c * K);   // halves: [2b] = o_b, [2b+1] = o_{b+1}
+        for (int bb = bprev + 1; bb <= (int)b; ++bb) {               // o_bb = j - j0
+            if (bb < (int)K) row[2 * bb] = (uint16_t)(j - j0);
+            if (bb > 0) row[2 * bb - 1] = (uint16_t)(j - j0);
+        }
         if (j == jn)
-            for (uint32_t bb = b + 1; bb <= K; ++bb) row[bb] = (uint16_t)(j - j0 + 1);
+            for (uint32_t bb = b + 1; bb <= K; ++bb) {               // o_bb = number of nodes of the interval
+                if (bb < K) row[2 * bb] = (uint16_t)(j - j0 + 1);
+                row[2 * bb - 1] = (uint16_t)(j - j0 + 1);
+            }
     }
 }
 
 // coarse[c] = (r, Phi) of node c << shift, c = 1..ncoarse; coarse[0] = (0, Phi_1) and
 // coarse[ncoarse + 1] = (+inf, 0) are the sentinel nodes 0 and N+1.
-__device__ __forceinline__ void stage_coarse(double2* coarse, const Node* __restrict__ nodes, uint32_t n, int shift)
+__device__ __forceinline__ void stage_coarse(double2* coarse, const double2* __restrict__ coarse_g, uint32_t n, int shift)
 {
     const uint32_t ncoarse = n >> shift;
-    for (uint32_t c = threadIdx.x; c <= ncoarse; c += ORB_THREADS) {
-        Node e = ld_node(nodes + ((uint64_t)c << shift));
-        coarse[c] = make_double2(e.r, e.phi);
-    }
+    for (uint32_t c = threadIdx.x; c <= ncoarse; c += ORB_THREADS) coarse[c] = __ldg(coarse_g + c);
     if (threadIdx.x == 0) coarse[ncoarse + 1] = make_double2(pos_inf(), 0.0);
     __syncthreads();
 }
 
 struct Tables {
     const Node* nodes;       // [n + 2]
-    const uint16_t* dir;
+    const uint32_t* dir;
     const double2* coarse;   // shared memory
     double r_last;           // r_N
     uint32_t n, ncoarse, K;
@@ -142,8 +156,8 @@ struct Tables {
     {
         const double Rl = coarse[c].x;
         const uint32_t b = bucket(x, Rl, bucket_scale(Rl, interval_rh(c), K), K);
-        const uint16_t* row = dir + (size_t)c * (K + 1) + b;
-        const uint32_t o0 = __ldg(row), o1 = __ldg(row + 1);
+        const uint32_t w = ld_u32_na(dir + (size_t)c * K + b);
+        const uint32_t o0 = w & 0xffffu, o1 = w >> 16;
         const uint32_t j0 = max(c << shift, 1u);
         lo = j0 + o0 - 1;
         hi = j0 + o1;
@@ -211,14 +225,14 @@ __device__ __forceinline__ uint32_t guess_node(const Tables& T, uint32_t lo, uin
 __global__ void __launch_bounds__(ORB_THREADS, 1)
 turning_points_kernel(uint32_t n, double G, const double* __restrict__ r, const double* __restrict__ v_r,
                       const double* __restrict__ v_t, const double* __restrict__ phi,
-                      const Node* __restrict__ nodes, const uint16_t* __restrict__ dir, int shift,
-                      double* __restrict__ E_out, double* __restrict__ J_out, double* __restrict__ rmin_out,
+                      const Node* __restrict__ nodes, const double2* __restrict__ coarse_g,
+                      const uint32_t* __restrict__ dir, int shift, double* __restrict__ E_out, double* __restrict__ J_out, double* __restrict__ rmin_out,
                       double* __restrict__ rmax_out, uint32_t* __restrict__ kmin_out, uint32_t* __restrict__ kmax_out,
                       uint8_t* __restrict__ status_out, unsigned long long* __restrict__ counters)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* coarse = reinterpret_cast<double2*>(smem_raw);
-    stage_coarse(coarse, nodes, n, shift);
+    stage_coarse(coarse, coarse_g, n, shift);
     Tables T{ nodes, dir, coarse, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift };
     const uint32_t low_mask = T.K - 1u;
 
@@ -386,12 +400,20 @@ __device__ __forceinline__ void exact_trial(const Tables& T, const Orbit& o, con
 }
 
 // Cold path, reached only if HMC_T_MAX trials were all rejected: redo the star exactly as the
-// oracle's loop does, every trial evaluated, remembering the last trial with Q0 > 0.
-__device__ __noinline__ void draw_exhaustive(const Tables& T, const Orbit& o, uint32_t seed_lo, uint32_t seed_hi,
-                                             uint32_t step, unsigned& st, bool& accepted, uint32_t& used,
-                                             bool& have_good, double& good_r, double& good_Q, uint32_t& good_w3)
+// oracle's loop does, every trial evaluated, remembering the last trial with Q0 > 0.  Everything
+// goes in and out by value so that nothing of the hot loop has its address taken (which would
+// put it in local memory).
+struct Exhaustive {
+    double good_r, good_Q;
+    uint32_t good_w3, used;
+    unsigned st;
+    bool accepted, have_good;
+};
+
+__device__ __noinline__ Exhaustive draw_exhaustive(Tables T, Orbit o, uint32_t seed_lo, uint32_t seed_hi, uint32_t step,
+                                                   unsigned st)
 {
-    accepted = false; have_good = false;
+    Exhaustive x{ 0.0, 0.0, 0u, 0u, st, false, false };
     const uint32_t cl = o.kmin >> T.shift, ch = o.kmax >> T.shift;
     uint32_t t = 0;
     for (; t < HMC_T_MAX; ++t) {
@@ -399,12 +421,13 @@ __device__ __noinline__ void draw_exhaustive(const Tables& T, const Orbit& o, ui
         double Q0, g;
         exact_trial(T, o, tr, coarse_locate(T.coarse, cl, ch, tr.r0), Q0, g);
         if (Q0 > 0.0) {
-            have_good = true; good_r = tr.r0; good_Q = Q0; good_w3 = tr.w3;
-            if (g > o.F) st |= HMC_STAR_CLIPPED;
-            if (o.F * tr.Xp < g) { accepted = true; break; }
+            x.have_good = true; x.good_r = tr.r0; x.good_Q = Q0; x.good_w3 = tr.w3;
+            if (g > o.F) x.st |= HMC_STAR_CLIPPED;
+            if (o.F * tr.Xp < g) { x.accepted = true; break; }
         }
     }
-    used = accepted ? t + 1 : HMC_T_MAX;
+    x.used = x.accepted ? t + 1 : HMC_T_MAX;
+    return x;
 }
 
 struct SampleIO {
@@ -486,12 +509,13 @@ __device__ __forceinline__ uint32_t park_from_arrays(const Node* __restrict__ no
 
 __global__ void __launch_bounds__(ORB_THREADS, 1)
 sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_hi, uint32_t step,
-                         const Node* __restrict__ nodes, const uint16_t* __restrict__ dir, int shift, SampleIO io)
+                         const Node* __restrict__ nodes, const double2* __restrict__ coarse_g,
+                         const uint32_t* __restrict__ dir, int shift, SampleIO io)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Park& pk = reinterpret_cast<Park*>(smem_raw)[threadIdx.x >> 5];
     double2* coarse = reinterpret_cast<double2*>(smem_raw + ORB_WARPS * sizeof(Park));
-    stage_coarse(coarse, nodes, n, shift);
+    stage_coarse(coarse, coarse_g, n, shift);
     Tables T{ nodes, dir, coarse, __ldg(io.r + (n - 1)), n, n >> shift, 1u << shift, shift };
     unsigned long long my_trials = 0;
     const unsigned lane_lt = lanemask_lt();
@@ -565,7 +589,9 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
                 }
             }
             if (!done && t >= HMC_T_MAX) {
-                draw_exhaustive(T, o, seed_lo, seed_hi, step, st, accepted, used, have_good, good_r, good_Q, good_w3);
+                const Exhaustive x = draw_exhaustive(T, o, seed_lo, seed_hi, step, st);
+                st = x.st; accepted = x.accepted; used = x.used; have_good = x.have_good;
+                good_r = x.good_r; good_Q = x.good_Q; good_w3 = x.good_w3;
                 done = true;
             }
             if (done) {
@@ -595,7 +621,7 @@ static hmc_status build_tables(uint64_t n, double G, const double* r, const doub
 {
     const int sms = sm_count();
     int blocks = (int)umin64((n + 2 + 255) / 256, (uint64_t)sms * 8);
-    build_nodes_kernel<<<blocks, 256, 0, st>>>(r, phi, m_cum, G, ws.nodes, n);
+    build_nodes_kernel<<<blocks, 256, 0, st>>>(r, phi, m_cum, G, ws.nodes, ws.coarse, shift, n);
     HMC_LAUNCH_CHECK();
     if (shift > 0) {
         blocks = (int)umin64((n + 255) / 256, (uint64_t)sms * 8);
@@ -622,7 +648,7 @@ hmc_status turning_points(uint64_t n, double G, const double* r, const double* v
     hmc_status s = build_tables(n, G, r, phi, m_cum, ws, shift, st);
     if (s != HMC_OK) return s;
     const int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
-    turning_points_kernel<<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, G, r, v_r, v_t, phi, ws.nodes, ws.dir, shift,
+    turning_points_kernel<<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, G, r, v_r, v_t, phi, ws.nodes, ws.coarse, ws.dir, shift,
                                                             E, J, r_min, r_max, k_min, k_max, status,
                                                             reinterpret_cast<unsigned long long*>(counters));
     HMC_LAUNCH_CHECK();
@@ -654,7 +680,7 @@ hmc_status sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step,
                  status_out, reinterpret_cast<unsigned long long*>(counters) };
     const int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
     sample_new_radius_kernel<<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, G, (uint32_t)seed, (uint32_t)(seed >> 32),
-                                                               step, ws.nodes, ws.dir, shift, io);
+                                                               step, ws.nodes, ws.coarse, ws.dir, shift, io);
     HMC_LAUNCH_CHECK();
     return HMC_OK;
 }
