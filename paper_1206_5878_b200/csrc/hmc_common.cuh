@@ -46,6 +46,12 @@ struct Workspace {
     uint32_t* digit_hist;    // [8][256] global digit counts -> exclusive bin offsets
     uint32_t* lookback;      // [8][sort_tiles][256] tile status words
     uint32_t* tickets;       // [32]: sort tile tickets 0..7, sort pass_live 8..15, scan tickets 16..17
+    // sort, fast path (packed words, hmc_sort.cu)
+    uint64_t* pk_alt;        // [n] second packed-word buffer (the first is keys_alt)
+    unsigned char* rec;      // [n] 64-byte star records (r, columns, id)
+    uint64_t* sortctl;       // [8]: key minimum, key maximum, long-run flag
+    uint32_t* pk_hist;       // [5][256]
+    uint32_t* pk_tickets;    // [16]: tile tickets 0..4, pass_live 8..12
     // potential
     double*   scan_status;   // [2][scan_tiles][8] (flag, agg_hi, agg_lo, inc_hi, inc_lo, pad)
     // orbit
@@ -89,6 +95,11 @@ static inline Workspace carve(void* base, uint64_t n)
     w.digit_hist  = reinterpret_cast<uint32_t*>(take(8 * 256 * 4));
     w.lookback    = reinterpret_cast<uint32_t*>(take(8 * sort_tiles * 256 * 4));
     w.tickets     = reinterpret_cast<uint32_t*>(take(32 * 4));
+    w.pk_alt      = reinterpret_cast<uint64_t*>(take(n * 8));
+    w.rec         = reinterpret_cast<unsigned char*>(take(n * 64));
+    w.sortctl     = reinterpret_cast<uint64_t*>(take(8 * 8));
+    w.pk_hist     = reinterpret_cast<uint32_t*>(take(5 * 256 * 4));
+    w.pk_tickets  = reinterpret_cast<uint32_t*>(take(16 * 4));
     w.scan_status = reinterpret_cast<double*>(take(2 * scan_tiles * 8 * 8));
     w.nodes       = reinterpret_cast<Node*>(take((n + 2) * sizeof(Node)));
     w.dir         = reinterpret_cast<uint32_t*>(take(dir_entries(n) * 4));

@@ -20,6 +20,21 @@ static constexpr int SORT_WARPS = SORT_THREADS / 32;
 static constexpr int SORT_ITEMS = SORT_TILE / SORT_THREADS;   // 16
 static_assert(SORT_THREADS == RADIX, "thread d owns digit d");
 
+// The general sort runs after the fast path of hmc_sort_fast.cu and only if that path met a run
+// of near-equal keys it would not resolve (guard[2] != 0).  guard == nullptr: run always.
+__device__ __forceinline__ bool guard_open(const uint64_t* __restrict__ guard) { return guard == nullptr || guard[2] != 0; }
+
+// zero-fill of the look-back words, digit histograms and tickets, under the same guard
+__global__ void sort_zero_kernel(uint32_t* __restrict__ a, uint64_t na, uint32_t* __restrict__ b, uint64_t nb,
+                                 uint32_t* __restrict__ c, uint64_t nc, const uint64_t* __restrict__ guard)
+{
+    if (!guard_open(guard)) return;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x, t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (uint64_t i = t; i < na; i += stride) a[i] = 0;
+    for (uint64_t i = t; i < nb; i += stride) b[i] = 0;
+    for (uint64_t i = t; i < nc; i += stride) c[i] = 0;
+}
+
 static constexpr uint32_t FLAG_AGG = 1u << 30;
 static constexpr uint32_t FLAG_INC = 2u << 30;
 static constexpr uint32_t FLAG_MASK = 3u << 30;
@@ -33,8 +48,10 @@ static constexpr int HIST_COPIES = 4;
 static constexpr int HIST_SKEWED_FROM = 6;      // digits >= this are warp-aggregated
 
 __global__ void __launch_bounds__(HIST_THREADS) sort_histogram_kernel(const uint64_t* __restrict__ keys, uint64_t n,
-                                                                      uint32_t* __restrict__ hist /*[8][256]*/)
+                                                                      uint32_t* __restrict__ hist /*[8][256]*/,
+                                                                      const uint64_t* __restrict__ guard)
 {
+    if (!guard_open(guard)) return;
     __shared__ uint32_t sh[HIST_COPIES][NPASS * RADIX];
     for (int i = threadIdx.x; i < HIST_COPIES * NPASS * RADIX; i += HIST_THREADS) (&sh[0][0])[i] = 0;
     __syncthreads();
@@ -67,8 +84,10 @@ __global__ void __launch_bounds__(HIST_THREADS) sort_histogram_kernel(const uint
 }
 
 // exclusive scan of each digit's 256 counts; pass_live[p] = 0 when one bin holds every key
-__global__ void sort_scan_hist_kernel(uint32_t* __restrict__ hist, uint64_t n, uint32_t* __restrict__ pass_live)
+__global__ void sort_scan_hist_kernel(uint32_t* __restrict__ hist, uint64_t n, uint32_t* __restrict__ pass_live,
+                                      const uint64_t* __restrict__ guard)
 {
+    if (!guard_open(guard)) return;
     __shared__ uint32_t sh[RADIX];
     const int p = blockIdx.x, d = threadIdx.x;
     uint32_t c = hist[p * RADIX + d];
@@ -110,8 +129,10 @@ struct SortBuffers {
 __global__ void __launch_bounds__(SORT_THREADS, 2)
 sort_onesweep_kernel(SortBuffers buf, uint32_t n, int shift,
                      const uint32_t* __restrict__ bin_offset /*[256] exclusive*/, uint32_t* __restrict__ lookback,
-                     uint32_t* __restrict__ ticket, const uint32_t* __restrict__ pass_live, int pass)
+                     uint32_t* __restrict__ ticket, const uint32_t* __restrict__ pass_live, int pass,
+                     const uint64_t* __restrict__ guard)
 {
+    if (!guard_open(guard)) return;
     if (!pass_live[pass]) return;
     int live_before = 0, live_total = 0;
 #pragma unroll
@@ -226,8 +247,10 @@ sort_onesweep_kernel(SortBuffers buf, uint32_t n, int shift,
 
 // ---- copy-through for the degenerate case "every pass skipped" and final gather ---------------
 __global__ void sort_iota_copy_kernel(const uint64_t* __restrict__ keys_in, uint64_t* __restrict__ keys_out,
-                                      uint32_t* __restrict__ perm, uint64_t n, const uint32_t* __restrict__ pass_live)
+                                      uint32_t* __restrict__ perm, uint64_t n, const uint32_t* __restrict__ pass_live,
+                                      const uint64_t* __restrict__ guard)
 {
+    if (!guard_open(guard)) return;
     // runs only when no pass was live (all keys equal): identity permutation
     uint32_t any = 0;
     for (int p = 0; p < NPASS; ++p) any |= pass_live[p];
@@ -247,8 +270,10 @@ struct GatherCols {
     int ncols;
 };
 
-__global__ void __launch_bounds__(256) sort_gather_kernel(GatherCols g, const uint32_t* __restrict__ perm, uint64_t n)
+__global__ void __launch_bounds__(256) sort_gather_kernel(GatherCols g, const uint32_t* __restrict__ perm, uint64_t n,
+                                                          const uint64_t* __restrict__ guard)
 {
+    if (!guard_open(guard)) return;
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
     for (uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += stride) {
         uint32_t src = perm[k];
@@ -264,23 +289,28 @@ __global__ void __launch_bounds__(256) sort_gather_kernel(GatherCols g, const ui
     }
 }
 
-hmc_status sort_by_radius(uint64_t n, const double* r_in, double* r_sorted, uint32_t* perm, int ncols,
-                          const double* const* cols_in, double* const* cols_out, const uint32_t* id_in,
-                          uint32_t* id_out, const Workspace& ws, cudaStream_t st)
+hmc_status sort_fast(uint64_t n, const double* r_in, double* r_sorted, uint32_t* perm, int ncols,
+                     const double* const* cols_in, double* const* cols_out, const uint32_t* id_in, uint32_t* id_out,
+                     const Workspace& ws, cudaStream_t st);
+
+// the general eight-pass sort; with a guard it is enqueued but does nothing unless the guard is set
+static hmc_status sort_general(uint64_t n, const double* r_in, double* r_sorted, uint32_t* perm, int ncols,
+                               const double* const* cols_in, double* const* cols_out, const uint32_t* id_in,
+                               uint32_t* id_out, const Workspace& ws, const uint64_t* guard, cudaStream_t st)
 {
     const uint32_t tiles = (uint32_t)((n + SORT_TILE - 1) / SORT_TILE);
     uint32_t* pass_live = ws.tickets + 8;    // [8] words after the 8 sort tickets
-    HMC_CUDA_TRY(cudaMemsetAsync(ws.digit_hist, 0, NPASS * RADIX * 4, st));
-    HMC_CUDA_TRY(cudaMemsetAsync(ws.tickets, 0, 16 * 4, st));
-    HMC_CUDA_TRY(cudaMemsetAsync(ws.lookback, 0, (size_t)NPASS * tiles * RADIX * 4, st));
-
     const int sms = sm_count();
+    const int copy_blocks = (int)umin64((n + 255) / 256, (uint64_t)sms * 8);
+    sort_zero_kernel<<<copy_blocks, 256, 0, st>>>(ws.lookback, (uint64_t)NPASS * tiles * RADIX, ws.digit_hist, NPASS * RADIX,
+                                                 ws.tickets, 16, guard);
+    HMC_LAUNCH_CHECK();
     const uint64_t* keys0 = reinterpret_cast<const uint64_t*>(r_in);
     {
         int blocks = (int)umin64((n + HIST_THREADS - 1) / HIST_THREADS, (uint64_t)sms * 3);
-        sort_histogram_kernel<<<blocks, HIST_THREADS, 0, st>>>(keys0, n, ws.digit_hist);
+        sort_histogram_kernel<<<blocks, HIST_THREADS, 0, st>>>(keys0, n, ws.digit_hist, guard);
         HMC_LAUNCH_CHECK();
-        sort_scan_hist_kernel<<<NPASS, RADIX, 0, st>>>(ws.digit_hist, n, pass_live);
+        sort_scan_hist_kernel<<<NPASS, RADIX, 0, st>>>(ws.digit_hist, n, pass_live, guard);
         HMC_LAUNCH_CHECK();
     }
     static bool attr_done = false;
@@ -293,24 +323,33 @@ hmc_status sort_by_radius(uint64_t n, const double* r_in, double* r_sorted, uint
     buf.keys_src = keys0;
     buf.keys[0] = ws.keys_alt; buf.keys[1] = reinterpret_cast<uint64_t*>(r_sorted);
     buf.vals[0] = ws.vals_alt; buf.vals[1] = perm;
-    const int copy_blocks = (int)umin64((n + 255) / 256, (uint64_t)sms * 8);
     for (int p = 0; p < NPASS; ++p) {
         sort_onesweep_kernel<<<tiles, SORT_THREADS, sizeof(SortSmem), st>>>(
             buf, (uint32_t)n, p * RADIX_BITS, ws.digit_hist + p * RADIX, ws.lookback + (size_t)p * tiles * RADIX,
-            ws.tickets + p, pass_live, p);
+            ws.tickets + p, pass_live, p, guard);
         HMC_LAUNCH_CHECK();
     }
-    sort_iota_copy_kernel<<<copy_blocks, 256, 0, st>>>(keys0, buf.keys[1], perm, n, pass_live);
+    sort_iota_copy_kernel<<<copy_blocks, 256, 0, st>>>(keys0, buf.keys[1], perm, n, pass_live, guard);
     HMC_LAUNCH_CHECK();
     if (ncols > 0 || id_in) {
         GatherCols g{};
         g.ncols = ncols;
         for (int c = 0; c < ncols; ++c) { g.in[c] = cols_in[c]; g.out[c] = cols_out[c]; }
         g.id_in = id_in; g.id_out = id_out;
-        sort_gather_kernel<<<copy_blocks, 256, 0, st>>>(g, perm, n);
+        sort_gather_kernel<<<copy_blocks, 256, 0, st>>>(g, perm, n, guard);
         HMC_LAUNCH_CHECK();
     }
     return HMC_OK;
+}
+
+hmc_status sort_by_radius(uint64_t n, const double* r_in, double* r_sorted, uint32_t* perm, int ncols,
+                          const double* const* cols_in, double* const* cols_out, const uint32_t* id_in,
+                          uint32_t* id_out, const Workspace& ws, cudaStream_t st)
+{
+    if (n < 2) return sort_general(n, r_in, r_sorted, perm, ncols, cols_in, cols_out, id_in, id_out, ws, nullptr, st);
+    hmc_status s = sort_fast(n, r_in, r_sorted, perm, ncols, cols_in, cols_out, id_in, id_out, ws, st);
+    if (s != HMC_OK) return s;
+    return sort_general(n, r_in, r_sorted, perm, ncols, cols_in, cols_out, id_in, id_out, ws, ws.sortctl, st);
 }
 
 }  // namespace hmc
