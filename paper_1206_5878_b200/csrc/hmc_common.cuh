@@ -57,6 +57,7 @@ struct Workspace {
     // orbit
     Node*     nodes;         // [n + 2] node table with sentinels (hmc_orbit.cu)
     uint32_t* dir;           // radius directory, dir_entries(n) entries (hmc_orbit.cu)
+    double*   orbitF;        // [n] S3's rejection bound F per star, read by S4 with reuse_tables (hmc_orbit.cu)
     double2*  coarse;        // [COARSE_CAP] (r, Phi) of every 2^shift-th node, contiguous (hmc_orbit.cu)
     size_t    total;
 };
@@ -93,7 +94,7 @@ static inline Workspace carve(void* base, uint64_t n)
     w.keys_alt    = reinterpret_cast<uint64_t*>(take(n * 8));
     w.vals_alt    = reinterpret_cast<uint32_t*>(take(n * 4));
     w.digit_hist  = reinterpret_cast<uint32_t*>(take(8 * 256 * 4));
-    w.lookback    = reinterpret_cast<uint32_t*>(take(8 * sort_tiles * 256 * 4));
+    w.lookback    = reinterpret_cast<uint32_t*>(take(16 * sort_tiles * 256 * 4));   // enough for 5 passes over tiles of 1024
     w.tickets     = reinterpret_cast<uint32_t*>(take(32 * 4));
     w.pk_alt      = reinterpret_cast<uint64_t*>(take(n * 8));
     w.rec         = reinterpret_cast<unsigned char*>(take(n * 64));
@@ -104,6 +105,7 @@ static inline Workspace carve(void* base, uint64_t n)
     w.nodes       = reinterpret_cast<Node*>(take((n + 2) * sizeof(Node)));
     w.dir         = reinterpret_cast<uint32_t*>(take(dir_entries(n) * 4));
     w.coarse      = reinterpret_cast<double2*>(take(COARSE_CAP * sizeof(double2)));
+    w.orbitF      = reinterpret_cast<double*>(take(n * 8));
     w.total = off;
     return w;
 }

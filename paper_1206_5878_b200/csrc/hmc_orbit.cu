@@ -228,7 +228,8 @@ turning_points_kernel(uint32_t n, double G, const double* __restrict__ r, const 
                       const Node* __restrict__ nodes, const double2* __restrict__ coarse_g,
                       const uint32_t* __restrict__ dir, int shift, double* __restrict__ E_out, double* __restrict__ J_out, double* __restrict__ rmin_out,
                       double* __restrict__ rmax_out, uint32_t* __restrict__ kmin_out, uint32_t* __restrict__ kmax_out,
-                      uint8_t* __restrict__ status_out, unsigned long long* __restrict__ counters)
+                      uint8_t* __restrict__ status_out, double* __restrict__ F_ws,
+                      unsigned long long* __restrict__ counters)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* coarse = reinterpret_cast<double2*>(smem_raw);
@@ -246,7 +247,7 @@ turning_points_kernel(uint32_t n, double G, const double* __restrict__ r, const 
         unsigned st = 0;
         if (!(E < 0.0)) st |= HMC_STAR_UNBOUND;
         if (J2 == 0.0) st |= HMC_STAR_RADIAL;
-        double rmin, rmax;
+        double rmin, rmax, Fv = 0.0;
         uint32_t kmin, kmax;
         if (st) {
             rmin = (st & HMC_STAR_RADIAL) ? 0.0 : rk;
@@ -308,7 +309,17 @@ turning_points_kernel(uint32_t n, double G, const double* __restrict__ r, const 
             if (D < 0.0) D = 0.0;
             if (Cb < 0.0) rmax = (eb.B + sqrt(D)) / (-2.0 * Cb);
             else { rmax = pos_inf(); st |= HMC_STAR_DEGENERATE; }
+            // S4's bound F (R7) needs G M at both bracketing shells, which are in registers here and
+            // would cost S4 two random node reads per star: computed here, with S4's expressions,
+            // and left in the workspace for a following S4 call with reuse_tables (0 = no draw).
+            const double delta = rmax - rmin;
+            if (!(st & HMC_STAR_DEGENERATE) && delta > 0.0) {
+                const double q1 = (2.0 * (J2 / rmin - ea.B)) / (rmin * rmin);      // Q'(r_min) in shell k_min
+                const double q2 = (2.0 * (J2 / rmax - eb.B)) / (rmax * rmax);      // Q'(r_max) in shell k_max
+                if ((q1 > 0.0) && (q2 < 0.0)) Fv = 1.2 * fmax(sqrt((3.0 * delta) / q1), sqrt((3.0 * delta) / (-q2)));
+            }
         }
+        __stcs(F_ws + a, Fv);
         __stcs(E_out + a, E); __stcs(J_out + a, J); __stcs(rmin_out + a, rmin); __stcs(rmax_out + a, rmax);
         __stcs(kmin_out + a, kmin); __stcs(kmax_out + a, kmax); status_out[a] = (uint8_t)st;
         if (st && counters) {
@@ -434,6 +445,7 @@ struct SampleIO {
     const double *r, *v_r, *v_t, *E, *J, *rmin, *rmax;
     const uint32_t *kmin, *kmax, *id;
     const uint8_t* status_in;
+    const double* F_ws;      // S3's bound F per star (workspace), or nullptr: compute it here
     double *r_new, *v_r_new, *v_t_new;
     uint16_t* n_try;
     uint8_t* status_out;
@@ -472,7 +484,7 @@ __device__ __forceinline__ uint32_t park_from_arrays(const Node* __restrict__ no
     const uint32_t a = base + lane;
     const bool in = a < end;
     unsigned st = 0;
-    double E = 0.0, J = 0.0, rmin = 0.0, rmax = 0.0;
+    double E = 0.0, J = 0.0, rmin = 0.0, rmax = 0.0, F = 0.0;
     uint32_t kmin = 0, kmax = 0, sid = 0;
     if (in) {
         st = io.status_in[a];
@@ -480,13 +492,14 @@ __device__ __forceinline__ uint32_t park_from_arrays(const Node* __restrict__ no
         rmin = __ldcs(io.rmin + a); rmax = __ldcs(io.rmax + a);
         kmin = __ldcs(io.kmin + a); kmax = __ldcs(io.kmax + a);
         sid = __ldcs(io.id + a);
+        if (io.F_ws) F = __ldcs(io.F_ws + a);
     }
     bool ok = in && !(st & (HMC_STAR_UNBOUND | HMC_STAR_RADIAL | HMC_STAR_DEGENERATE));
     const double delta = rmax - rmin;
-    double F = 0.0;
     if (ok) {
         ok = delta > 0.0;
-        if (ok) {
+        if (ok && io.F_ws) ok = F > 0.0;
+        else if (ok) {
             const double J2 = J * J;
             const double Bmin = ld_node(nodes + kmin).B, Bmax = ld_node(nodes + kmax).B;
             const double q1 = (2.0 * (J2 / rmin - Bmin)) / (rmin * rmin);      // Q'(r_min) in shell k_min
@@ -649,7 +662,7 @@ hmc_status turning_points(uint64_t n, double G, const double* r, const double* v
     if (s != HMC_OK) return s;
     const int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
     turning_points_kernel<<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, G, r, v_r, v_t, phi, ws.nodes, ws.coarse, ws.dir, shift,
-                                                            E, J, r_min, r_max, k_min, k_max, status,
+                                                            E, J, r_min, r_max, k_min, k_max, status, ws.orbitF,
                                                             reinterpret_cast<unsigned long long*>(counters));
     HMC_LAUNCH_CHECK();
     return HMC_OK;
@@ -676,7 +689,7 @@ hmc_status sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step,
         hmc_status s = build_tables(n, G, r, phi, m_cum, ws, shift, st);
         if (s != HMC_OK) return s;
     }
-    SampleIO io{ r, v_r, v_t, E, J, r_min, r_max, k_min, k_max, id, status_in, r_new, v_r_new, v_t_new, n_try,
+    SampleIO io{ r, v_r, v_t, E, J, r_min, r_max, k_min, k_max, id, status_in, reuse_tables ? ws.orbitF : nullptr, r_new, v_r_new, v_t_new, n_try,
                  status_out, reinterpret_cast<unsigned long long*>(counters) };
     const int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
     sample_new_radius_kernel<<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, G, (uint32_t)seed, (uint32_t)(seed >> 32),
