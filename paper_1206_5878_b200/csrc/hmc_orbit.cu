@@ -235,7 +235,6 @@ turning_points_kernel(uint32_t n, double G, const double* __restrict__ r, const 
     double2* coarse = reinterpret_cast<double2*>(smem_raw);
     stage_coarse(coarse, coarse_g, n, shift);
     Tables T{ nodes, dir, coarse, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift };
-    const uint32_t low_mask = T.K - 1u;
 
     const uint32_t stride = gridDim.x * ORB_THREADS;
     for (uint32_t a = blockIdx.x * ORB_THREADS + threadIdx.x; a < n; a += stride) {
@@ -256,18 +255,24 @@ turning_points_kernel(uint32_t n, double G, const double* __restrict__ r, const 
         } else {
             // pericentre bracket (lo, hi): Q_lo < 0 <= Q_hi;  apocentre: Q_lo >= 0 > Q_hi
             Side s1{ 0u, k, 1u, 0u, MODE_BISECT }, s2{ k, n + 1, 1u, 0u, MODE_BISECT };
-            // tier 1: the coarse nodes, in shared memory
-            while (s1.active()) {
-                uint32_t p = pivot(s1.lo, s1.hi);
-                if (p & low_mask) break;
-                double2 e = coarse[p >> shift];
-                if (q_negative(e.x, e.y, E, J2)) s1.lo = p; else s1.hi = p;
-            }
-            while (s2.active()) {
-                uint32_t p = pivot(s2.lo, s2.hi);
-                if (p & low_mask) break;
-                double2 e = coarse[p >> shift];
-                if (q_negative(e.x, e.y, E, J2)) s2.hi = p; else s2.lo = p;
+            // tier 1: the coarse nodes, in shared memory; both searches advance together (two
+            // independent chains of dependent shared-memory loads instead of one after the other).
+            // Pericentre: largest coarse c in [0, ck] with Q < 0 (c = 0 is node 0, always < 0).
+            // Apocentre: smallest coarse c in [cka, ncoarse + 1] with Q < 0 (ncoarse + 1 stands for node N+1).
+            {
+                const uint32_t ck = (k - 1) >> shift, cka = (k >> shift) + 1;
+                uint32_t l1 = 0, h1 = ck + 1, l2 = cka - 1, h2 = T.ncoarse + 1;
+                while (true) {
+                    const bool a1 = h1 - l1 > 1, a2 = h2 - l2 > 1;
+                    if (!(a1 || a2)) break;
+                    const uint32_t m1 = (l1 + h1) >> 1, m2 = (l2 + h2) >> 1;
+                    const double2 e1 = coarse[a1 ? m1 : 0u], e2 = coarse[a2 ? m2 : 0u];
+                    const bool n1 = q_negative(e1.x, e1.y, E, J2), n2 = q_negative(e2.x, e2.y, E, J2);
+                    l1 = (a1 && n1) ? m1 : l1; h1 = (a1 && !n1) ? m1 : h1;
+                    h2 = (a2 && n2) ? m2 : h2; l2 = (a2 && !n2) ? m2 : l2;
+                }
+                s1.lo = l1 << shift; s1.hi = (l1 == ck) ? k : ((l1 + 1) << shift);
+                s2.hi = (h2 <= T.ncoarse) ? (h2 << shift) : n + 1; s2.lo = (h2 == cka) ? k : ((h2 - 1) << shift);
             }
             // tier 2: secant guess.  The ends are coarse nodes or the star's own node, where
             // P = r^2 Q = (r_k v_r)^2.  The first and last intervals (a sentinel at one end) bisect.
