@@ -151,10 +151,16 @@ sort_onesweep_kernel(SortBuffers buf, uint32_t n, int shift,
     SortSmem& s = *reinterpret_cast<SortSmem*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
+    // persistent CTAs: tiles are taken in ticket order until none is left (the grid is a few CTAs
+    // per SM, so that a guarded launch that has nothing to do costs next to nothing)
+    const uint32_t tiles = (n + SORT_TILE - 1) / SORT_TILE;
+    for (;;) {
+    __syncthreads();                                            // previous tile's shared memory is no longer read
     if (tid == 0) s.tile = atomicAdd(ticket, 1u);
     for (int i = tid; i < SORT_WARPS * RADIX; i += SORT_THREADS) (&s.warp_counts[0][0])[i] = 0;
     __syncthreads();
     const uint32_t tile = s.tile;
+    if (tile >= tiles) break;
     const uint32_t tile_base = tile * SORT_TILE;
     const uint32_t valid = min((uint32_t)SORT_TILE, n - tile_base);
 
@@ -243,6 +249,7 @@ sort_onesweep_kernel(SortBuffers buf, uint32_t n, int shift,
             vals_out[g] = s.vals[pos];
         }
     }
+    }   // tile loop
 }
 
 // ---- copy-through for the degenerate case "every pass skipped" and final gather ---------------
@@ -324,7 +331,7 @@ static hmc_status sort_general(uint64_t n, const double* r_in, double* r_sorted,
     buf.keys[0] = ws.keys_alt; buf.keys[1] = reinterpret_cast<uint64_t*>(r_sorted);
     buf.vals[0] = ws.vals_alt; buf.vals[1] = perm;
     for (int p = 0; p < NPASS; ++p) {
-        sort_onesweep_kernel<<<tiles, SORT_THREADS, sizeof(SortSmem), st>>>(
+        sort_onesweep_kernel<<<(int)umin64(tiles, (uint64_t)sms * 2), SORT_THREADS, sizeof(SortSmem), st>>>(
             buf, (uint32_t)n, p * RADIX_BITS, ws.digit_hist + p * RADIX, ws.lookback + (size_t)p * tiles * RADIX,
             ws.tickets + p, pass_live, p, guard);
         HMC_LAUNCH_CHECK();

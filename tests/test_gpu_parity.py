@@ -82,6 +82,54 @@ def test_sort_adversarial_keys(oracle, kind):
     assert np.array_equal(host(rs), o_rs)
 
 
+def _clustered_keys(n, cluster, g):
+    """Radii over ~8 binades in which groups of `cluster` stars differ only in their lowest
+    mantissa bits (and some are exactly equal): the packed-word fast path cannot separate them
+    by its leading key bits and has to resolve each run from the full keys."""
+    base = np.exp(g.uniform(np.log(0.01), np.log(3.0), n // cluster + 1))
+    r = np.repeat(base, cluster)[:n].copy()
+    bits = r.view(np.uint64)
+    bits += g.integers(0, 6, n).astype(np.uint64)          # 0..5 ulps: near-ties and exact ties
+    g.shuffle(r)
+    return r
+
+
+@pytest.mark.parametrize("cluster", [2, 7, 32, 33, 200])
+def test_sort_runs_of_near_equal_keys(oracle, cluster):
+    """cluster <= 32: runs resolved inside the fast path; > 32: the guarded general sort redoes the call."""
+    g = np.random.default_rng(11 + cluster)
+    n = 300_017
+    r = _clustered_keys(n, cluster, g)
+    v = g.random(n)
+    ids = np.arange(n, dtype=np.uint32)[::-1].copy()
+    rs, perm, cols, ids_s = hmc.hmc_sort_by_radius(dev(r), (dev(v),), dev(ids.view(np.int32)))
+    o_rs, o_perm, o_cols, o_ids = oracle.sort_by_radius(r, (v,), ids)
+    assert np.array_equal(host(perm, np.uint32), o_perm)
+    assert np.array_equal(host(rs), o_rs)
+    assert np.array_equal(host(cols[0]), o_cols[0])
+    assert np.array_equal(host(ids_s, np.uint32), o_ids)
+
+
+@pytest.mark.parametrize("ncols,with_id", [(0, False), (0, True), (1, False), (6, True), (7, True), (8, False)])
+def test_sort_column_counts(oracle, ncols, with_id):
+    """0..8 record columns, with and without the id column (up to 6 columns travel as 64-byte records,
+    more are gathered column by column)."""
+    g = np.random.default_rng(3 + ncols)
+    n = 70_001
+    r = np.exp(g.uniform(-5, 5, n))
+    cols = [g.random(n) for _ in range(ncols)]
+    ids = g.permutation(n).astype(np.uint32)
+    rs, perm, cols_s, ids_s = hmc.hmc_sort_by_radius(dev(r), [dev(c) for c in cols],
+                                                     dev(ids.view(np.int32)) if with_id else None)
+    o_rs, o_perm, o_cols, o_ids = oracle.sort_by_radius(r, tuple(cols), ids if with_id else None)
+    assert np.array_equal(host(perm, np.uint32), o_perm)
+    assert np.array_equal(host(rs), o_rs)
+    for a, b in zip(cols_s, o_cols):
+        assert np.array_equal(host(a), b)
+    if with_id:
+        assert np.array_equal(host(ids_s, np.uint32), o_ids)
+
+
 def test_sort_empty_and_errors():
     e = torch.empty(0, dtype=torch.float64, device="cuda")
     rs, perm, _, _ = hmc.hmc_sort_by_radius(e)
@@ -159,6 +207,13 @@ def test_orbit_stage_isolation_on_oracle_tables(oracle, n, masses, seed):
     check_orbit_against(oracle, o, tp, sm, report="isolated n=%d" % n)
     cnt = host(counters)
     assert cnt[hmc.COUNTER_NAMES.index("trials")] == o["sample"]["trials"]
+    # the same two calls sharing one workspace, S4 reusing S3's tables and per-star bound F
+    ws = hmc.alloc_workspace(n)
+    tp2 = hmc.hmc_orbit_turning_points(rs, vrs, vts, phi, mc, 1.0, workspace=ws)
+    sm2 = hmc.hmc_sample_new_radius(rs, phi, mc, vrs, vts, tp2, dev(o["id"].view(np.int32)), seed, 2, 1.0,
+                                    workspace=ws, reuse_tables=True)
+    for key in ("r_new", "v_r_new", "v_t_new", "n_try", "status"):
+        assert torch.equal(sm[key], sm2[key]), key
 
 
 def test_config1_whole_step_chained(oracle):
