@@ -195,10 +195,14 @@ sort_pk_pass_kernel(PkBuffers b, uint32_t n, const uint64_t* __restrict__ ctl,
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PkSmem& s = *reinterpret_cast<PkSmem*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t tiles = (n + PK_TILE - 1) / PK_TILE;
+    for (;;) {                                                  // persistent CTAs: tiles in ticket order
+    __syncthreads();                                            // previous tile's shared memory is no longer read
     if (tid == 0) s.tile = atomicAdd(ticket, 1u);
     for (int i = tid; i < PK_WARPS * PK_RADIX; i += PK_THREADS) (&s.warp_counts[0][0])[i] = 0;
     __syncthreads();
     const uint32_t tile = s.tile;
+    if (tile >= tiles) break;
     const uint32_t tile_base = tile * PK_TILE;
     const uint32_t valid = min((uint32_t)PK_TILE, n - tile_base);
 
@@ -281,6 +285,7 @@ sort_pk_pass_kernel(PkBuffers b, uint32_t n, const uint64_t* __restrict__ ctl,
             out[s.global_base[(uint32_t)(v >> shift) & 255u] + pos] = v;
         }
     }
+    }   // tile loop
 }
 
 // ---- 64-byte star records -------------------------------------------------------------------------
@@ -387,7 +392,7 @@ sort_pk_finish_kernel(PkBuffers b, const double* __restrict__ rec, PkCols g, uin
                 if (in_j) {
                     double v[4];
                     const double* p = rec + (size_t)idx_j * 8 + h * 4;
-                    asm("ld.global.nc.L1::no_allocate.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3]) : "l"(p));
+                    asm("ld.global.nc.L1::no_allocate.L2::64B.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3]) : "l"(p));
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
                         const int slot = h * 4 + q;
@@ -453,7 +458,7 @@ hmc_status sort_fast(uint64_t n, const double* r_in, double* r_sorted, uint32_t*
     if (key_bits > 64 - idx_bits) key_bits = 64 - idx_bits;
     const int npass = (key_bits + 7) / 8;                                   // later digits are constant
     for (int p = 0; p < npass; ++p) {
-        sort_pk_pass_kernel<<<tiles, PK_THREADS, sizeof(PkSmem), st>>>(b, (uint32_t)n, ws.sortctl, ws.pk_hist + p * PK_RADIX,
+        sort_pk_pass_kernel<<<(int)umin64(tiles, (uint64_t)sms * 2), PK_THREADS, sizeof(PkSmem), st>>>(b, (uint32_t)n, ws.sortctl, ws.pk_hist + p * PK_RADIX,
                                                                        ws.lookback + (size_t)p * tiles * PK_RADIX,
                                                                        ws.pk_tickets + p, pass_live, p);
         HMC_LAUNCH_CHECK();

@@ -190,13 +190,30 @@ def hmc_sample_new_radius(r_sorted, phi, m_cum, v_r, v_t, tp, ids, seed: int, st
     return out
 
 
+def kernel_launches_per_step(n: int, ncols: int = 3, with_id: bool = True) -> int:
+    """How many kernels of libhmc one orbit step (the four calls, S4 with reuse_tables) launches for
+    n stars; mirrors the host code of csrc/*.cu (memsets are not counted)."""
+    if n < 2:
+        return (14 if (ncols or with_id) else 13) + 3 + 3 + 1
+    ib = max(1, (n - 1).bit_length())
+    idx_bits = max(24, ib)
+    key_bits = min(((ib + 8 + 7) // 8) * 8, 40, 64 - idx_bits)
+    npass = (key_bits + 7) // 8
+    rec = 1 if ((ncols or with_id) and ncols <= 6) else 0
+    fast = 3 + rec + npass + 1                       # range, histogram, bin scan, records, digit passes, finish
+    general = 1 + 2 + 8 + 1 + (1 if (ncols or with_id) else 0)   # guarded: zero, histogram, bin scan, 8 passes, identity, gather
+    shift = 0
+    while (n >> shift) + 2 > 10240:
+        shift += 1
+    tables = 2 if shift > 0 else 1
+    return fast + general + 3 + (tables + 1) + 1     # + potential (3) + S3 (tables, search) + S4 (1)
+
+
 class OrbitStepper:
     """Pre-allocated device state for repeated orbit steps (sort -> potential -> turning points ->
     new radius), the loop of BASELINE.json's multi-step configs.  Holds the carried state
     (r, v_r, v_t, m, id) and every intermediate; ``step()`` makes the four C-ABI calls on the
     current stream and swaps (r, v_r, v_t) <- (r_new, v_r', v_t'); m and id follow the sort."""
-
-    KERNELS_PER_STEP = 2 + 8 + 1 + 1 + 2 + 2 + 1   # hist, scan, 8 passes, iota, gather, 2 scans, table, S3, S4
 
     def __init__(self, r, v_r, v_t, m, ids, seed: int, G: float = 1.0, with_n_try: bool = True):
         self.n = n = r.numel()
