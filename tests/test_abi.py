@@ -41,7 +41,7 @@ def test_host_only_entry_points(libhmc):
     libhmc.hmc_status_string.restype = ctypes.c_char_p
     w5, w7 = libhmc.hmc_workspace_bytes(10 ** 5), libhmc.hmc_workspace_bytes(10 ** 7)
     assert 0 < w5 < w7 and w5 % 256 == 0
-    assert w7 < 64 * 10 ** 7                      # scratch stays below 64 B/star
+    assert w7 < 160 * 10 ** 7                     # scratch stays below 160 B/star (64 of them the sort's star records)
     assert libhmc.hmc_step_host_arena_bytes(10 ** 5) > w5
     assert libhmc.hmc_status_string(0) == b"HMC_OK"
     for code in (-1, -2, -3, -4, -5):
