@@ -95,8 +95,13 @@ HMC_API int32_t hmc_version(void);
  *   ncols          0..HMC_MAX_COLS record columns to carry along
  *   cols_in/out    HOST arrays of ncols DEVICE pointers: cols_out[c][k] = cols_in[c][perm[k]]
  *   id_in/id_out   optional (both or neither NULL) persistent star-id column, gathered likewise
- * Method: least-significant-digit radix sort of (key, index) pairs, 8-bit digits, one
- * decoupled-look-back sweep per digit, then one gather of the record columns by perm.
+ * Method: each star is one 64-bit word (leading key bits above the smallest key | index); a stable
+ * least-significant-digit radix sort of those words (8-bit digits, one decoupled-look-back sweep
+ * per digit), then one kernel that resolves runs of stars agreeing in the kept key bits from
+ * their full keys and moves the record columns (as one 64-byte record per star when ncols <= 6).
+ * A run of more than 32 such stars makes the general sort (eight passes over 64-bit key +
+ * 32-bit index, enqueued behind a device-side flag) redo the call.  The result is the same
+ * unique permutation either way.
  */
 HMC_API hmc_status hmc_sort_by_radius(uint64_t n,
         const double* r_in, double* r_sorted, uint32_t* perm,
