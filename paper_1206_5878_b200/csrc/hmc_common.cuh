@@ -57,12 +57,14 @@ struct Workspace {
     // orbit
     Node*     nodes;         // [n + 2] node table with sentinels (hmc_orbit.cu)
     uint32_t* dir;           // radius directory, dir_entries(n) entries (hmc_orbit.cu)
+    double2*  mid;           // [(n >> MID_SHIFT) + 2] (r, Phi) of every 1024-th node (hmc_orbit.cu, large n only)
     double*   orbitF;        // [n] S3's rejection bound F per star, read by S4 with reuse_tables (hmc_orbit.cu)
     double2*  coarse;        // [COARSE_CAP] (r, Phi) of every 2^shift-th node, contiguous (hmc_orbit.cu)
     size_t    total;
 };
 
 // ---- orbit tables: sizes shared by carve() and hmc_orbit.cu ---------------------------------
+static constexpr int MID_SHIFT = 10;                 // S3's second search table: every 1024-th node, used when the coarse spacing is wider
 static constexpr uint32_t COARSE_CAP = 10240;        // (r, Phi) pairs of the shared-memory coarse table: 160 KB
 
 // coarse nodes are the multiples of 2^shift; smallest shift with (n >> shift) + 2 <= COARSE_CAP
@@ -106,6 +108,7 @@ static inline Workspace carve(void* base, uint64_t n)
     w.dir         = reinterpret_cast<uint32_t*>(take(dir_entries(n) * 4));
     w.coarse      = reinterpret_cast<double2*>(take(COARSE_CAP * sizeof(double2)));
     w.orbitF      = reinterpret_cast<double*>(take(n * 8));
+    w.mid         = reinterpret_cast<double2*>(take(((n >> MID_SHIFT) + 2) * sizeof(double2)));
     w.total = off;
     return w;
 }

@@ -58,6 +58,13 @@ __device__ __forceinline__ Node ld_node(const Node* __restrict__ p)
     return e;
 }
 
+__device__ __forceinline__ double2 ld_d2_na(const double2* __restrict__ p)
+{
+    double2 v;
+    asm("ld.global.nc.L1::no_allocate.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+
 __device__ __forceinline__ uint32_t ld_u32_na(const uint32_t* __restrict__ p)
 {
     uint32_t v;
@@ -86,7 +93,7 @@ __device__ __forceinline__ uint32_t bucket(double x, double Rl, float scale, uin
 __global__ void __launch_bounds__(256) build_nodes_kernel(const double* __restrict__ r, const double* __restrict__ phi,
                                                           const double* __restrict__ m_cum, double G,
                                                           Node* __restrict__ nodes, double2* __restrict__ coarse_g,
-                                                          int shift, uint64_t n)
+                                                          double2* __restrict__ mid_g, int shift, uint64_t n)
 {
     const uint64_t low_mask = (1ull << shift) - 1;
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
@@ -100,6 +107,7 @@ __global__ void __launch_bounds__(256) build_nodes_kernel(const double* __restri
         }
         nodes[j] = e;
         if ((j & low_mask) == 0 && j <= n) coarse_g[j >> shift] = make_double2(e.r, e.phi);
+        if (shift > MID_SHIFT && (j & ((1u << MID_SHIFT) - 1)) == 0 && j <= n) mid_g[j >> MID_SHIFT] = make_double2(e.r, e.phi);
     }
 }
 
@@ -144,9 +152,12 @@ struct Tables {
     const Node* nodes;       // [n + 2]
     const uint32_t* dir;
     const double2* coarse;   // shared memory
+    const double2* mid;      // global (L2): (r, Phi) of every 2^MID_SHIFT-th node when shift > MID_SHIFT, else nullptr
     double r_last;           // r_N
     uint32_t n, ncoarse, K;
     int shift;
+    // (r, Phi) of node j, j a multiple of the finest table spacing in use
+    __device__ __forceinline__ double2 aligned_node(uint32_t j) const { return mid ? ld_d2_na(mid + (j >> MID_SHIFT)) : coarse[j >> shift]; }
     // upper radius of coarse interval c, as build_dir_kernel defines it
     __device__ __forceinline__ double interval_rh(uint32_t c) const { return c < ncoarse ? coarse[c + 1].x : r_last; }
     // nodes lo < hi with  r_lo <= x < r_hi  as far as the directory knows: every node of interval c
@@ -226,7 +237,7 @@ __global__ void __launch_bounds__(ORB_THREADS, 1)
 turning_points_kernel(uint32_t n, double G, const double* __restrict__ r, const double* __restrict__ v_r,
                       const double* __restrict__ v_t, const double* __restrict__ phi,
                       const Node* __restrict__ nodes, const double2* __restrict__ coarse_g,
-                      const uint32_t* __restrict__ dir, int shift, double* __restrict__ E_out, double* __restrict__ J_out, double* __restrict__ rmin_out,
+                      const double2* __restrict__ mid_g, const uint32_t* __restrict__ dir, int shift, double* __restrict__ E_out, double* __restrict__ J_out, double* __restrict__ rmin_out,
                       double* __restrict__ rmax_out, uint32_t* __restrict__ kmin_out, uint32_t* __restrict__ kmax_out,
                       uint8_t* __restrict__ status_out, double* __restrict__ F_ws,
                       unsigned long long* __restrict__ counters)
@@ -234,7 +245,7 @@ turning_points_kernel(uint32_t n, double G, const double* __restrict__ r, const 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* coarse = reinterpret_cast<double2*>(smem_raw);
     stage_coarse(coarse, coarse_g, n, shift);
-    Tables T{ nodes, dir, coarse, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift };
+    Tables T{ nodes, dir, coarse, shift > MID_SHIFT ? mid_g : nullptr, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift };
 
     const uint32_t stride = gridDim.x * ORB_THREADS;
     for (uint32_t a = blockIdx.x * ORB_THREADS + threadIdx.x; a < n; a += stride) {
@@ -274,20 +285,38 @@ turning_points_kernel(uint32_t n, double G, const double* __restrict__ r, const 
                 s1.lo = l1 << shift; s1.hi = (l1 == ck) ? k : ((l1 + 1) << shift);
                 s2.hi = (h2 <= T.ncoarse) ? (h2 << shift) : n + 1; s2.lo = (h2 == cka) ? k : ((h2 - 1) << shift);
             }
-            // tier 2: secant guess.  The ends are coarse nodes or the star's own node, where
+            // tier 1b (large N only, shift > MID_SHIFT): a coarse interval then holds 2^shift >> 1024 nodes and
+            // r^2 Q is no longer linear across it; bisect on over every 1024-th node, a table small
+            // enough to stay in L2, both sides together.
+            if (T.mid) {
+                uint32_t l1 = s1.lo >> MID_SHIFT, h1 = (s1.hi + ((1u << MID_SHIFT) - 1)) >> MID_SHIFT;
+                uint32_t l2 = s2.lo >> MID_SHIFT, h2 = (s2.hi > n) ? (n >> MID_SHIFT) + 1 : (s2.hi >> MID_SHIFT);
+                while (true) {
+                    const bool a1 = h1 - l1 > 1, a2 = h2 - l2 > 1;
+                    if (!(a1 || a2)) break;
+                    const uint32_t m1 = (l1 + h1) >> 1, m2 = (l2 + h2) >> 1;
+                    const double2 e1 = ld_d2_na(T.mid + (a1 ? m1 : 0u)), e2 = ld_d2_na(T.mid + (a2 ? m2 : 0u));
+                    const bool n1 = q_negative(e1.x, e1.y, E, J2), n2 = q_negative(e2.x, e2.y, E, J2);
+                    l1 = (a1 && n1) ? m1 : l1; h1 = (a1 && !n1) ? m1 : h1;
+                    h2 = (a2 && n2) ? m2 : h2; l2 = (a2 && !n2) ? m2 : l2;
+                }
+                s1.lo = max(s1.lo, l1 << MID_SHIFT); s1.hi = min(s1.hi, h1 << MID_SHIFT);
+                s2.lo = max(s2.lo, l2 << MID_SHIFT); if (h2 <= (n >> MID_SHIFT)) s2.hi = min(s2.hi, h2 << MID_SHIFT);
+            }
+            // tier 2: secant guess.  The ends are table nodes or the star's own node, where
             // P = r^2 Q = (r_k v_r)^2.  The first and last intervals (a sentinel at one end) bisect.
             const double Pk = (rk * vr) * (rk * vr);
             if (s1.hi - s1.lo > 2 && s1.lo > 0) {
-                double2 el = coarse[s1.lo >> shift];
+                double2 el = T.aligned_node(s1.lo);
                 double r_hi = rk, P_hi = Pk;
-                if (s1.hi != k) { double2 eh = coarse[s1.hi >> shift]; r_hi = eh.x; P_hi = 2.0 * ((E - eh.y) * (eh.x * eh.x)) - J2; }
+                if (s1.hi != k) { double2 eh = T.aligned_node(s1.hi); r_hi = eh.x; P_hi = 2.0 * ((E - eh.y) * (eh.x * eh.x)) - J2; }
                 s1.guess = guess_node(T, s1.lo, s1.hi, el.x, 2.0 * ((E - el.y) * (el.x * el.x)) - J2, r_hi, P_hi);
                 s1.mode = MODE_GUESS;
             }
             if (s2.hi - s2.lo > 2 && s2.hi <= n) {
-                double2 eh = coarse[s2.hi >> shift];
+                double2 eh = T.aligned_node(s2.hi);
                 double r_lo = rk, P_lo = Pk;
-                if (s2.lo != k) { double2 el = coarse[s2.lo >> shift]; r_lo = el.x; P_lo = 2.0 * ((E - el.y) * (el.x * el.x)) - J2; }
+                if (s2.lo != k) { double2 el = T.aligned_node(s2.lo); r_lo = el.x; P_lo = 2.0 * ((E - el.y) * (el.x * el.x)) - J2; }
                 s2.guess = guess_node(T, s2.lo, s2.hi, r_lo, P_lo, eh.x, 2.0 * ((E - eh.y) * (eh.x * eh.x)) - J2);
                 s2.mode = MODE_GUESS;
             }
@@ -534,7 +563,7 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
     Park& pk = reinterpret_cast<Park*>(smem_raw)[threadIdx.x >> 5];
     double2* coarse = reinterpret_cast<double2*>(smem_raw + ORB_WARPS * sizeof(Park));
     stage_coarse(coarse, coarse_g, n, shift);
-    Tables T{ nodes, dir, coarse, __ldg(io.r + (n - 1)), n, n >> shift, 1u << shift, shift };
+    Tables T{ nodes, dir, coarse, nullptr, __ldg(io.r + (n - 1)), n, n >> shift, 1u << shift, shift };
     unsigned long long my_trials = 0;
     const unsigned lane_lt = lanemask_lt();
     const uint32_t lane = threadIdx.x & 31;
@@ -639,7 +668,7 @@ static hmc_status build_tables(uint64_t n, double G, const double* r, const doub
 {
     const int sms = sm_count();
     int blocks = (int)umin64((n + 2 + 255) / 256, (uint64_t)sms * 8);
-    build_nodes_kernel<<<blocks, 256, 0, st>>>(r, phi, m_cum, G, ws.nodes, ws.coarse, shift, n);
+    build_nodes_kernel<<<blocks, 256, 0, st>>>(r, phi, m_cum, G, ws.nodes, ws.coarse, ws.mid, shift, n);
     HMC_LAUNCH_CHECK();
     if (shift > 0) {
         blocks = (int)umin64((n + 255) / 256, (uint64_t)sms * 8);
@@ -666,7 +695,7 @@ hmc_status turning_points(uint64_t n, double G, const double* r, const double* v
     hmc_status s = build_tables(n, G, r, phi, m_cum, ws, shift, st);
     if (s != HMC_OK) return s;
     const int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
-    turning_points_kernel<<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, G, r, v_r, v_t, phi, ws.nodes, ws.coarse, ws.dir, shift,
+    turning_points_kernel<<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, G, r, v_r, v_t, phi, ws.nodes, ws.coarse, ws.mid, ws.dir, shift,
                                                             E, J, r_min, r_max, k_min, k_max, status, ws.orbitF,
                                                             reinterpret_cast<unsigned long long*>(counters));
     HMC_LAUNCH_CHECK();

@@ -33,8 +33,8 @@ def rel(a, b):
     return d
 
 
-def run_fullsize(oracle, index, steps=1):
-    cfg = inputs.config(index)
+def run_fullsize(oracle, index, steps=1, n_override=None):
+    cfg = inputs.config(index, n_override)
     n, seed = cfg["n"], cfg["seed"]
     free, _ = torch.cuda.mem_get_info()
     if free < 260 * n:
@@ -110,6 +110,12 @@ def test_config4_salpeter_1e7(oracle):
     run_fullsize(oracle, 3, steps=1)
 
 
+def test_second_search_table_just_above_the_coarse_capacity(oracle):
+    """N = 1.2e7 (recipe of configs[2]): the coarse table's spacing becomes 2048 nodes, so S3's second
+    table (every 1024-th node, in L2) does one bisection step -- the smallest case of the large-N path."""
+    run_fullsize(oracle, 2, steps=1, n_override=12_000_000)
+
+
 def test_config5_1e8(oracle):
-    """BASELINE.json configs[4]: N = 1e8 equal-mass, seed 5 (table far beyond L2, shift = 13)."""
+    """BASELINE.json configs[4]: N = 1e8 equal-mass, seed 5 (tables far beyond L2, coarse spacing 2^14)."""
     run_fullsize(oracle, 4, steps=1)
