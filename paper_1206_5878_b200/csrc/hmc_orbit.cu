@@ -173,6 +173,19 @@ struct Tables {
         lo = j0 + o0 - 1;
         hi = j0 + o1;
     }
+    // Most likely last node at or below x: the nodes strictly inside dir_range's (lo, hi) share x's
+    // bucket, and about the fraction of the bucket that lies below x of them are below x.  A guess only.
+    __device__ __forceinline__ uint32_t dir_guess(uint32_t c, double x) const
+    {
+        const double Rl = coarse[c].x;
+        const float scale = bucket_scale(Rl, interval_rh(c), K);
+        const uint32_t b = bucket(x, Rl, scale, K);
+        const uint32_t w = ld_u32_na(dir + (size_t)c * K + b);
+        const uint32_t o0 = w & 0xffffu, o1 = w >> 16;
+        float frac = (float)(x - Rl) * scale - (float)b;
+        frac = fminf(fmaxf(frac, 0.0f), 1.0f);
+        return max(c << shift, 1u) + o0 - 1 + (uint32_t)(frac * (float)(o1 - o0) + 0.5f);
+    }
 };
 
 // ---- S3 ---------------------------------------------------------------------------------------
@@ -228,9 +241,7 @@ __device__ __forceinline__ uint32_t guess_node(const Tables& T, uint32_t lo, uin
                                                double r_hi, double P_hi)
 {
     const double x = r_lo + (r_hi - r_lo) * (P_lo / (P_lo - P_hi));
-    uint32_t a, b;
-    T.dir_range(lo >> T.shift, x, a, b);
-    return a;                                  // last node known to lie at or below x
+    return T.dir_guess(lo >> T.shift, x);
 }
 
 __global__ void __launch_bounds__(ORB_THREADS, 1)
@@ -394,10 +405,13 @@ __device__ __forceinline__ Trial make_trial(const Orbit& o, uint32_t seed_lo, ui
 {
     uint32_t w[4];
     philox4x32_10(o.sid, 0u, step, t, seed_lo, seed_hi, w);
-    const double two_m53 = 1.0 / 9007199254740992.0;
-    double X = (double)((((unsigned long long)w[0] << 32) | w[1]) >> 11) * two_m53;
+    // X = ((w0 * 2^32 + w1) >> 11) * 2^-53 (R9).  The 53-bit integer is split into its top 21 and low 32
+    // bits, converted separately (both exact) and added (exact: 53 bits): the same value as converting the
+    // 64-bit integer, without the slow 64-bit integer-to-double conversion.
+    const double two_m21 = 1.0 / 2097152.0, two_m53 = 1.0 / 9007199254740992.0;
+    const double X = __uint2double_rn(w[0] >> 11) * two_m21 + __uint2double_rn((w[0] << 21) | (w[1] >> 11)) * two_m53;
     Trial tr;
-    tr.Xp = (double)((((unsigned long long)w[2] << 32) | w[3]) >> 11) * two_m53;
+    tr.Xp = __uint2double_rn(w[2] >> 11) * two_m21 + __uint2double_rn((w[2] << 21) | (w[3] >> 11)) * two_m53;
     tr.s = 2.0 * X - 1.0;
     tr.r0 = o.mid + o.quarter * (3.0 * tr.s - (tr.s * tr.s) * tr.s);     // replaces Eq. 14 (R7)
     tr.w3 = w[3];
