@@ -244,6 +244,128 @@ __device__ __forceinline__ uint32_t guess_node(const Tables& T, uint32_t lo, uin
     return T.dir_guess(lo >> T.shift, x);
 }
 
+// One star of S3: brackets, turning points, status, and S4's bound F (0 = no draw).  a = position in the
+// sorted arrays (star k = a + 1); rk, vr, vt, phik its radius, velocities and potential.
+struct Solved {
+    double E, J, rmin, rmax, Fv;
+    uint32_t kmin, kmax;
+    unsigned st;
+};
+
+__device__ __forceinline__ Solved solve_star(const Tables& T, uint32_t a, double rk, double vr, double vt, double phik)
+{
+    const uint32_t n = T.n;
+    const int shift = T.shift;
+    const Node* __restrict__ nodes = T.nodes;
+    const double2* coarse = T.coarse;
+    double E, J, rmin, rmax, Fv;
+    uint32_t kmin, kmax;
+    unsigned st;
+    const uint32_t k = a + 1;
+        E = phik + 0.5 * (vr * vr + vt * vt);      // Eq. 16
+    J = rk * vt;
+    const double J2 = J * J;
+    st = 0;
+    if (!(E < 0.0)) st |= HMC_STAR_UNBOUND;
+    if (J2 == 0.0) st |= HMC_STAR_RADIAL;
+    Fv = 0.0;
+    if (st) {
+        rmin = (st & HMC_STAR_RADIAL) ? 0.0 : rk;
+        rmax = (st & HMC_STAR_UNBOUND) ? pos_inf() : rk;
+        kmin = k - 1; kmax = k;
+    } else {
+        // pericentre bracket (lo, hi): Q_lo < 0 <= Q_hi;  apocentre: Q_lo >= 0 > Q_hi
+        Side s1{ 0u, k, 1u, 0u, MODE_BISECT }, s2{ k, n + 1, 1u, 0u, MODE_BISECT };
+        // tier 1: the coarse nodes, in shared memory; both searches advance together (two
+        // independent chains of dependent shared-memory loads instead of one after the other).
+        // Pericentre: largest coarse c in [0, ck] with Q < 0 (c = 0 is node 0, always < 0).
+        // Apocentre: smallest coarse c in [cka, ncoarse + 1] with Q < 0 (ncoarse + 1 stands for node N+1).
+        {
+            const uint32_t ck = (k - 1) >> shift, cka = (k >> shift) + 1;
+            uint32_t l1 = 0, h1 = ck + 1, l2 = cka - 1, h2 = T.ncoarse + 1;
+            while (true) {
+                const bool a1 = h1 - l1 > 1, a2 = h2 - l2 > 1;
+                if (!(a1 || a2)) break;
+                const uint32_t m1 = (l1 + h1) >> 1, m2 = (l2 + h2) >> 1;
+                const double2 e1 = coarse[a1 ? m1 : 0u], e2 = coarse[a2 ? m2 : 0u];
+                const bool n1 = q_negative(e1.x, e1.y, E, J2), n2 = q_negative(e2.x, e2.y, E, J2);
+                l1 = (a1 && n1) ? m1 : l1; h1 = (a1 && !n1) ? m1 : h1;
+                h2 = (a2 && n2) ? m2 : h2; l2 = (a2 && !n2) ? m2 : l2;
+            }
+            s1.lo = l1 << shift; s1.hi = (l1 == ck) ? k : ((l1 + 1) << shift);
+            s2.hi = (h2 <= T.ncoarse) ? (h2 << shift) : n + 1; s2.lo = (h2 == cka) ? k : ((h2 - 1) << shift);
+        }
+        // tier 1b (large N only, shift > MID_SHIFT): a coarse interval then holds 2^shift >> 1024 nodes and
+        // r^2 Q is no longer linear across it; bisect on over every 1024-th node, a table small
+        // enough to stay in L2, both sides together.
+        if (T.mid) {
+            uint32_t l1 = s1.lo >> MID_SHIFT, h1 = (s1.hi + ((1u << MID_SHIFT) - 1)) >> MID_SHIFT;
+            uint32_t l2 = s2.lo >> MID_SHIFT, h2 = (s2.hi > n) ? (n >> MID_SHIFT) + 1 : (s2.hi >> MID_SHIFT);
+            while (true) {
+                const bool a1 = h1 - l1 > 1, a2 = h2 - l2 > 1;
+                if (!(a1 || a2)) break;
+                const uint32_t m1 = (l1 + h1) >> 1, m2 = (l2 + h2) >> 1;
+                const double2 e1 = ld_d2_na(T.mid + (a1 ? m1 : 0u)), e2 = ld_d2_na(T.mid + (a2 ? m2 : 0u));
+                const bool n1 = q_negative(e1.x, e1.y, E, J2), n2 = q_negative(e2.x, e2.y, E, J2);
+                l1 = (a1 && n1) ? m1 : l1; h1 = (a1 && !n1) ? m1 : h1;
+                h2 = (a2 && n2) ? m2 : h2; l2 = (a2 && !n2) ? m2 : l2;
+            }
+            s1.lo = max(s1.lo, l1 << MID_SHIFT); s1.hi = min(s1.hi, h1 << MID_SHIFT);
+            s2.lo = max(s2.lo, l2 << MID_SHIFT); if (h2 <= (n >> MID_SHIFT)) s2.hi = min(s2.hi, h2 << MID_SHIFT);
+        }
+        // tier 2: secant guess.  The ends are table nodes or the star's own node, where
+        // P = r^2 Q = (r_k v_r)^2.  The first and last intervals (a sentinel at one end) bisect.
+        const double Pk = (rk * vr) * (rk * vr);
+        if (s1.hi - s1.lo > 2 && s1.lo > 0) {
+            double2 el = T.aligned_node(s1.lo);
+            double r_hi = rk, P_hi = Pk;
+            if (s1.hi != k) { double2 eh = T.aligned_node(s1.hi); r_hi = eh.x; P_hi = 2.0 * ((E - eh.y) * (eh.x * eh.x)) - J2; }
+            s1.guess = guess_node(T, s1.lo, s1.hi, el.x, 2.0 * ((E - el.y) * (el.x * el.x)) - J2, r_hi, P_hi);
+            s1.mode = MODE_GUESS;
+        }
+        if (s2.hi - s2.lo > 2 && s2.hi <= n) {
+            double2 eh = T.aligned_node(s2.hi);
+            double r_lo = rk, P_lo = Pk;
+            if (s2.lo != k) { double2 el = T.aligned_node(s2.lo); r_lo = el.x; P_lo = 2.0 * ((E - el.y) * (el.x * el.x)) - J2; }
+            s2.guess = guess_node(T, s2.lo, s2.hi, r_lo, P_lo, eh.x, 2.0 * ((E - eh.y) * (eh.x * eh.x)) - J2);
+            s2.mode = MODE_GUESS;
+        }
+        // tier 3: exact probes of adjacent node pairs, the two searches interleaved
+        while (true) {
+            const bool a1 = s1.active(), a2 = s2.active();
+            if (!(a1 || a2)) break;
+            const uint32_t p1 = a1 ? s1.probe() : 0u, p2 = a2 ? s2.probe() : 0u;
+            Node e10, e11, e20, e21;
+            if (a1) { e10 = ld_node(nodes + p1); e11 = ld_node(nodes + p1 + 1); }
+            if (a2) { e20 = ld_node(nodes + p2); e21 = ld_node(nodes + p2 + 1); }
+            if (a1) s1.update(p1, q_negative(e10.r, e10.phi, E, J2), q_negative(e11.r, e11.phi, E, J2));
+            if (a2) s2.update(p2, !q_negative(e20.r, e20.phi, E, J2), !q_negative(e21.r, e21.phi, E, J2));
+        }
+        kmin = s1.lo; kmax = s2.lo;
+        // closed-form roots of Q(u) = 2C + 2Bu - J^2 u^2 in the bracketing shells (R3)
+        const Node ea = ld_node(nodes + kmin), eb = ld_node(nodes + kmax);
+        const double Ca = (E - ea.phi) - ea.B * ea.u;
+        const double Cb = (E - eb.phi) - eb.B * eb.u;
+        double D = ea.B * ea.B + 2.0 * (J2 * Ca);
+        if (D < 0.0) D = 0.0;
+        rmin = J2 / (ea.B + sqrt(D));
+        D = eb.B * eb.B + 2.0 * (J2 * Cb);
+        if (D < 0.0) D = 0.0;
+        if (Cb < 0.0) rmax = (eb.B + sqrt(D)) / (-2.0 * Cb);
+        else { rmax = pos_inf(); st |= HMC_STAR_DEGENERATE; }
+        // S4's bound F (R7) needs G M at both bracketing shells, which are in registers here and
+        // would cost S4 two random node reads per star: computed here, with S4's expressions,
+        // and left in the workspace for a following S4 call with reuse_tables (0 = no draw).
+        const double delta = rmax - rmin;
+        if (!(st & HMC_STAR_DEGENERATE) && delta > 0.0) {
+            const double q1 = (2.0 * (J2 / rmin - ea.B)) / (rmin * rmin);      // Q'(r_min) in shell k_min
+            const double q2 = (2.0 * (J2 / rmax - eb.B)) / (rmax * rmax);      // Q'(r_max) in shell k_max
+            if ((q1 > 0.0) && (q2 < 0.0)) Fv = 1.2 * fmax(sqrt((3.0 * delta) / q1), sqrt((3.0 * delta) / (-q2)));
+        }
+    }
+    return Solved{ E, J, rmin, rmax, Fv, kmin, kmax, st };
+}
+
 __global__ void __launch_bounds__(ORB_THREADS, 1)
 turning_points_kernel(uint32_t n, double G, const double* __restrict__ r, const double* __restrict__ v_r,
                       const double* __restrict__ v_t, const double* __restrict__ phi,
@@ -260,110 +382,10 @@ turning_points_kernel(uint32_t n, double G, const double* __restrict__ r, const 
 
     const uint32_t stride = gridDim.x * ORB_THREADS;
     for (uint32_t a = blockIdx.x * ORB_THREADS + threadIdx.x; a < n; a += stride) {
-        const uint32_t k = a + 1;
-        const double rk = __ldcs(r + a), vr = __ldcs(v_r + a), vt = __ldcs(v_t + a), phik = __ldcs(phi + a);
-        const double E = phik + 0.5 * (vr * vr + vt * vt);      // Eq. 16
-        const double J = rk * vt;
-        const double J2 = J * J;
-        unsigned st = 0;
-        if (!(E < 0.0)) st |= HMC_STAR_UNBOUND;
-        if (J2 == 0.0) st |= HMC_STAR_RADIAL;
-        double rmin, rmax, Fv = 0.0;
-        uint32_t kmin, kmax;
-        if (st) {
-            rmin = (st & HMC_STAR_RADIAL) ? 0.0 : rk;
-            rmax = (st & HMC_STAR_UNBOUND) ? pos_inf() : rk;
-            kmin = k - 1; kmax = k;
-        } else {
-            // pericentre bracket (lo, hi): Q_lo < 0 <= Q_hi;  apocentre: Q_lo >= 0 > Q_hi
-            Side s1{ 0u, k, 1u, 0u, MODE_BISECT }, s2{ k, n + 1, 1u, 0u, MODE_BISECT };
-            // tier 1: the coarse nodes, in shared memory; both searches advance together (two
-            // independent chains of dependent shared-memory loads instead of one after the other).
-            // Pericentre: largest coarse c in [0, ck] with Q < 0 (c = 0 is node 0, always < 0).
-            // Apocentre: smallest coarse c in [cka, ncoarse + 1] with Q < 0 (ncoarse + 1 stands for node N+1).
-            {
-                const uint32_t ck = (k - 1) >> shift, cka = (k >> shift) + 1;
-                uint32_t l1 = 0, h1 = ck + 1, l2 = cka - 1, h2 = T.ncoarse + 1;
-                while (true) {
-                    const bool a1 = h1 - l1 > 1, a2 = h2 - l2 > 1;
-                    if (!(a1 || a2)) break;
-                    const uint32_t m1 = (l1 + h1) >> 1, m2 = (l2 + h2) >> 1;
-                    const double2 e1 = coarse[a1 ? m1 : 0u], e2 = coarse[a2 ? m2 : 0u];
-                    const bool n1 = q_negative(e1.x, e1.y, E, J2), n2 = q_negative(e2.x, e2.y, E, J2);
-                    l1 = (a1 && n1) ? m1 : l1; h1 = (a1 && !n1) ? m1 : h1;
-                    h2 = (a2 && n2) ? m2 : h2; l2 = (a2 && !n2) ? m2 : l2;
-                }
-                s1.lo = l1 << shift; s1.hi = (l1 == ck) ? k : ((l1 + 1) << shift);
-                s2.hi = (h2 <= T.ncoarse) ? (h2 << shift) : n + 1; s2.lo = (h2 == cka) ? k : ((h2 - 1) << shift);
-            }
-            // tier 1b (large N only, shift > MID_SHIFT): a coarse interval then holds 2^shift >> 1024 nodes and
-            // r^2 Q is no longer linear across it; bisect on over every 1024-th node, a table small
-            // enough to stay in L2, both sides together.
-            if (T.mid) {
-                uint32_t l1 = s1.lo >> MID_SHIFT, h1 = (s1.hi + ((1u << MID_SHIFT) - 1)) >> MID_SHIFT;
-                uint32_t l2 = s2.lo >> MID_SHIFT, h2 = (s2.hi > n) ? (n >> MID_SHIFT) + 1 : (s2.hi >> MID_SHIFT);
-                while (true) {
-                    const bool a1 = h1 - l1 > 1, a2 = h2 - l2 > 1;
-                    if (!(a1 || a2)) break;
-                    const uint32_t m1 = (l1 + h1) >> 1, m2 = (l2 + h2) >> 1;
-                    const double2 e1 = ld_d2_na(T.mid + (a1 ? m1 : 0u)), e2 = ld_d2_na(T.mid + (a2 ? m2 : 0u));
-                    const bool n1 = q_negative(e1.x, e1.y, E, J2), n2 = q_negative(e2.x, e2.y, E, J2);
-                    l1 = (a1 && n1) ? m1 : l1; h1 = (a1 && !n1) ? m1 : h1;
-                    h2 = (a2 && n2) ? m2 : h2; l2 = (a2 && !n2) ? m2 : l2;
-                }
-                s1.lo = max(s1.lo, l1 << MID_SHIFT); s1.hi = min(s1.hi, h1 << MID_SHIFT);
-                s2.lo = max(s2.lo, l2 << MID_SHIFT); if (h2 <= (n >> MID_SHIFT)) s2.hi = min(s2.hi, h2 << MID_SHIFT);
-            }
-            // tier 2: secant guess.  The ends are table nodes or the star's own node, where
-            // P = r^2 Q = (r_k v_r)^2.  The first and last intervals (a sentinel at one end) bisect.
-            const double Pk = (rk * vr) * (rk * vr);
-            if (s1.hi - s1.lo > 2 && s1.lo > 0) {
-                double2 el = T.aligned_node(s1.lo);
-                double r_hi = rk, P_hi = Pk;
-                if (s1.hi != k) { double2 eh = T.aligned_node(s1.hi); r_hi = eh.x; P_hi = 2.0 * ((E - eh.y) * (eh.x * eh.x)) - J2; }
-                s1.guess = guess_node(T, s1.lo, s1.hi, el.x, 2.0 * ((E - el.y) * (el.x * el.x)) - J2, r_hi, P_hi);
-                s1.mode = MODE_GUESS;
-            }
-            if (s2.hi - s2.lo > 2 && s2.hi <= n) {
-                double2 eh = T.aligned_node(s2.hi);
-                double r_lo = rk, P_lo = Pk;
-                if (s2.lo != k) { double2 el = T.aligned_node(s2.lo); r_lo = el.x; P_lo = 2.0 * ((E - el.y) * (el.x * el.x)) - J2; }
-                s2.guess = guess_node(T, s2.lo, s2.hi, r_lo, P_lo, eh.x, 2.0 * ((E - eh.y) * (eh.x * eh.x)) - J2);
-                s2.mode = MODE_GUESS;
-            }
-            // tier 3: exact probes of adjacent node pairs, the two searches interleaved
-            while (true) {
-                const bool a1 = s1.active(), a2 = s2.active();
-                if (!(a1 || a2)) break;
-                const uint32_t p1 = a1 ? s1.probe() : 0u, p2 = a2 ? s2.probe() : 0u;
-                Node e10, e11, e20, e21;
-                if (a1) { e10 = ld_node(nodes + p1); e11 = ld_node(nodes + p1 + 1); }
-                if (a2) { e20 = ld_node(nodes + p2); e21 = ld_node(nodes + p2 + 1); }
-                if (a1) s1.update(p1, q_negative(e10.r, e10.phi, E, J2), q_negative(e11.r, e11.phi, E, J2));
-                if (a2) s2.update(p2, !q_negative(e20.r, e20.phi, E, J2), !q_negative(e21.r, e21.phi, E, J2));
-            }
-            kmin = s1.lo; kmax = s2.lo;
-            // closed-form roots of Q(u) = 2C + 2Bu - J^2 u^2 in the bracketing shells (R3)
-            const Node ea = ld_node(nodes + kmin), eb = ld_node(nodes + kmax);
-            const double Ca = (E - ea.phi) - ea.B * ea.u;
-            const double Cb = (E - eb.phi) - eb.B * eb.u;
-            double D = ea.B * ea.B + 2.0 * (J2 * Ca);
-            if (D < 0.0) D = 0.0;
-            rmin = J2 / (ea.B + sqrt(D));
-            D = eb.B * eb.B + 2.0 * (J2 * Cb);
-            if (D < 0.0) D = 0.0;
-            if (Cb < 0.0) rmax = (eb.B + sqrt(D)) / (-2.0 * Cb);
-            else { rmax = pos_inf(); st |= HMC_STAR_DEGENERATE; }
-            // S4's bound F (R7) needs G M at both bracketing shells, which are in registers here and
-            // would cost S4 two random node reads per star: computed here, with S4's expressions,
-            // and left in the workspace for a following S4 call with reuse_tables (0 = no draw).
-            const double delta = rmax - rmin;
-            if (!(st & HMC_STAR_DEGENERATE) && delta > 0.0) {
-                const double q1 = (2.0 * (J2 / rmin - ea.B)) / (rmin * rmin);      // Q'(r_min) in shell k_min
-                const double q2 = (2.0 * (J2 / rmax - eb.B)) / (rmax * rmax);      // Q'(r_max) in shell k_max
-                if ((q1 > 0.0) && (q2 < 0.0)) Fv = 1.2 * fmax(sqrt((3.0 * delta) / q1), sqrt((3.0 * delta) / (-q2)));
-            }
-        }
+        const Solved v = solve_star(T, a, __ldcs(r + a), __ldcs(v_r + a), __ldcs(v_t + a), __ldcs(phi + a));
+        const double E = v.E, J = v.J, rmin = v.rmin, rmax = v.rmax, Fv = v.Fv;
+        const uint32_t kmin = v.kmin, kmax = v.kmax;
+        const unsigned st = v.st;
         __stcs(F_ws + a, Fv);
         __stcs(E_out + a, E); __stcs(J_out + a, J); __stcs(rmin_out + a, rmin); __stcs(rmax_out + a, rmax);
         __stcs(kmin_out + a, kmin); __stcs(kmax_out + a, kmax); status_out[a] = (uint8_t)st;
