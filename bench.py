@@ -272,12 +272,18 @@ def run_gpu(args, cfg):
         ev[1].record(stream)
         hmc.hmc_potential(so["r"], so["m"], stepper.G, phi=stepper.phi, m_cum=stepper.m_cum, workspace=stepper.workspace)
         ev[2].record(stream)
-        hmc.hmc_orbit_turning_points(so["r"], so["v_r"], so["v_t"], stepper.phi, stepper.m_cum, stepper.G,
-                                     out=stepper.tp, counters=stepper.counters, workspace=stepper.workspace)
-        ev[3].record(stream)
-        hmc.hmc_sample_new_radius(so["r"], stepper.phi, stepper.m_cum, so["v_r"], so["v_t"], stepper.tp, so["id"],
-                                  stepper.seed, stepper.step_index, stepper.G, out=stepper.sample,
-                                  counters=stepper.counters, workspace=stepper.workspace, reuse_tables=True)
+        if args.fused:
+            ev[3].record(stream)      # "turning_points" reads 0; "sampling" is the fused S3 + S4 call
+            hmc.hmc_orbit_step(so["r"], so["v_r"], so["v_t"], stepper.phi, stepper.m_cum, so["id"], stepper.seed,
+                               stepper.step_index, stepper.G, tp=stepper.tp, out=stepper.sample,
+                               counters=stepper.counters, workspace=stepper.workspace)
+        else:
+            hmc.hmc_orbit_turning_points(so["r"], so["v_r"], so["v_t"], stepper.phi, stepper.m_cum, stepper.G,
+                                         out=stepper.tp, counters=stepper.counters, workspace=stepper.workspace)
+            ev[3].record(stream)
+            hmc.hmc_sample_new_radius(so["r"], stepper.phi, stepper.m_cum, so["v_r"], so["v_t"], stepper.tp, so["id"],
+                                      stepper.seed, stepper.step_index, stepper.G, out=stepper.sample,
+                                      counters=stepper.counters, workspace=stepper.workspace, reuse_tables=True)
         ev[4].record(stream)
         sm = stepper.sample
         s["r"], sm["r_new"] = sm["r_new"], s["r"]
@@ -395,6 +401,7 @@ def main(argv=None):
     ap.add_argument("--n", type=int, default=None, help="override N (same recipe and seed); not a bench line")
     ap.add_argument("--ref-stride", type=int, default=4, help="oracle legs: orbit stages on every k-th star")
     ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--fused", action="store_true", help="S3 and S4 as the single call hmc_orbit_step")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args(argv)

@@ -8,6 +8,7 @@
  *   hmc_potential             PAPER.md:67-79 (step 1, Eq. 1-5)
  *   hmc_orbit_turning_points  PAPER.md:117-124 (step 5, Eq. 12, bracket + analytic roots)
  *   hmc_sample_new_radius     PAPER.md:126-137 (step 5, Eq. 13-15, rejection sampling)
+ * (hmc_orbit_step does the last two in one launch.)
  *
  * Conventions common to all calls
  * -------------------------------
@@ -167,6 +168,23 @@ HMC_API hmc_status hmc_sample_new_radius(uint64_t n, double G, uint64_t seed, ui
         const uint8_t* star_status_in,
         double* r_new, double* v_r_new, double* v_t_new, uint16_t* n_try,
         uint8_t* star_status_out, uint64_t* counters, int32_t reuse_tables,
+        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * S3 + S4 in one launch (the two calls above fused).  Computes exactly what
+ * hmc_orbit_turning_points followed by hmc_sample_new_radius compute, bit for bit, and writes every
+ * output of both (E .. star_status are S3's, r_new .. star_status_out S4's): each warp solves 32 stars,
+ * keeps their orbits on chip and draws their new radii, so S3's outputs are never read back and
+ * searching and drawing warps share an SM.  Arguments as in the two calls.  Measured on B200 at N = 1e7 it is
+ * SLOWER than the two calls (3.1 ms against 1.05 + 1.08 ms), so nothing else here uses it.
+ */
+HMC_API hmc_status hmc_orbit_step(uint64_t n, double G, uint64_t seed, uint32_t step,
+        const double* r_sorted, const double* v_r, const double* v_t,
+        const double* phi, const double* m_cum, const uint32_t* id,
+        double* E, double* J, double* r_min, double* r_max,
+        uint32_t* k_min, uint32_t* k_max, uint8_t* star_status,
+        double* r_new, double* v_r_new, double* v_t_new, uint16_t* n_try,
+        uint8_t* star_status_out, uint64_t* counters,
         void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*

@@ -204,4 +204,10 @@ hmc_status sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step,
                              uint16_t* n_try, uint8_t* status_out, uint64_t* counters, bool reuse_tables,
                              const Workspace& ws, cudaStream_t st);
 
+hmc_status orbit_step(uint64_t n, double G, uint64_t seed, uint32_t step, const double* r, const double* v_r,
+                      const double* v_t, const double* phi, const double* m_cum, const uint32_t* id, double* E,
+                      double* J, double* r_min, double* r_max, uint32_t* k_min, uint32_t* k_max, uint8_t* status,
+                      double* r_new, double* v_r_new, double* v_t_new, uint16_t* n_try, uint8_t* status_out,
+                      uint64_t* counters, const Workspace& ws, cudaStream_t st);
+
 }  // namespace hmc

@@ -516,6 +516,11 @@ struct SampleIO {
     const uint32_t *kmin, *kmax, *id;
     const uint8_t* status_in;
     const double* F_ws;      // S3's bound F per star (workspace), or nullptr: compute it here
+    // fused S3 + S4 only: S3's table input and where its outputs go
+    const double* phi;
+    double *E_w, *J_w, *rmin_w, *rmax_w;
+    uint32_t *kmin_w, *kmax_w;
+    uint8_t* status_w;
     double *r_new, *v_r_new, *v_t_new;
     uint16_t* n_try;
     uint8_t* status_out;
@@ -590,16 +595,55 @@ __device__ __forceinline__ uint32_t park_from_arrays(const Node* __restrict__ no
     return (uint32_t)__popc(valid);
 }
 
+// Fused S3 + S4: prepare stars base .. base+31 by SOLVING them (S3's work, all 32 lanes busy), write S3's
+// outputs, and park the orbits that take a draw; nothing of S3's output is read back.
+__device__ __forceinline__ uint32_t park_by_solving(const Tables& T, const SampleIO& io, Park& pk, uint32_t base,
+                                                    uint32_t end, uint32_t lane, unsigned lane_lt)
+{
+    const uint32_t a = base + lane;
+    const bool in = a < end;
+    bool ok = false;
+    Solved v{ 0.0, 0.0, 0.0, 0.0, 0.0, 0u, 0u, 0u };
+    uint32_t sid = 0;
+    if (in) {
+        const double rk = __ldcs(io.r + a), vr = __ldcs(io.v_r + a), vt = __ldcs(io.v_t + a), phik = __ldcs(io.phi + a);
+        sid = __ldcs(io.id + a);
+        v = solve_star(T, a, rk, vr, vt, phik);
+        __stcs(io.E_w + a, v.E); __stcs(io.J_w + a, v.J); __stcs(io.rmin_w + a, v.rmin); __stcs(io.rmax_w + a, v.rmax);
+        __stcs(io.kmin_w + a, v.kmin); __stcs(io.kmax_w + a, v.kmax); io.status_w[a] = (uint8_t)v.st;
+        if (v.st && io.counters) {
+            if (v.st & HMC_STAR_UNBOUND) atomicAdd(io.counters + HMC_CNT_UNBOUND, 1ull);
+            if (v.st & HMC_STAR_RADIAL) atomicAdd(io.counters + HMC_CNT_RADIAL, 1ull);
+            if (v.st & HMC_STAR_DEGENERATE) atomicAdd(io.counters + HMC_CNT_DEGENERATE, 1ull);
+        }
+        ok = !(v.st & (HMC_STAR_UNBOUND | HMC_STAR_RADIAL | HMC_STAR_DEGENERATE));
+        if (ok) {
+            ok = v.Fv > 0.0;                               // as S4 reading S3's F: 0 = empty interval or wrong end slopes
+            if (!ok) v.st |= HMC_STAR_CIRCULAR;
+        }
+        if (!ok) finish_star(io, a, rk, vr, vt, 0u, v.st);
+    }
+    const unsigned valid = __ballot_sync(0xffffffffu, ok);
+    if (ok) {
+        const uint32_t slot = __popc(valid & lane_lt);
+        pk.E[slot] = v.E; pk.J[slot] = v.J; pk.mid[slot] = 0.5 * (v.rmin + v.rmax); pk.delta[slot] = v.rmax - v.rmin; pk.F[slot] = v.Fv;
+        pk.kmin[slot] = v.kmin; pk.kmax[slot] = v.kmax; pk.sid[slot] = sid; pk.a[slot] = a; pk.st[slot] = v.st;
+    }
+    __syncwarp();
+    return (uint32_t)__popc(valid);
+}
+
+template <bool FUSED>
 __global__ void __launch_bounds__(ORB_THREADS, 1)
 sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_hi, uint32_t step,
                          const Node* __restrict__ nodes, const double2* __restrict__ coarse_g,
-                         const uint32_t* __restrict__ dir, int shift, SampleIO io)
+                         const double2* __restrict__ mid_g, const uint32_t* __restrict__ dir, int shift, SampleIO io)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Park& pk = reinterpret_cast<Park*>(smem_raw)[threadIdx.x >> 5];
     double2* coarse = reinterpret_cast<double2*>(smem_raw + ORB_WARPS * sizeof(Park));
     stage_coarse(coarse, coarse_g, n, shift);
-    Tables T{ nodes, dir, coarse, nullptr, __ldg(io.r + (n - 1)), n, n >> shift, 1u << shift, shift };
+    Tables T{ nodes, dir, coarse, (FUSED && shift > MID_SHIFT) ? mid_g : nullptr, __ldg(io.r + (n - 1)), n, n >> shift, 1u << shift, shift };
     unsigned long long my_trials = 0;
     const unsigned lane_lt = lanemask_lt();
     const uint32_t lane = threadIdx.x & 31;
@@ -622,7 +666,8 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
         while (need) {
             if (head == parked) {
                 if (next >= end) break;
-                parked = park_from_arrays(nodes, io, pk, next, end, lane, lane_lt);
+                parked = FUSED ? park_by_solving(T, io, pk, next, end, lane, lane_lt)
+                               : park_from_arrays(nodes, io, pk, next, end, lane, lane_lt);
                 head = 0;
                 next = min(end, next + 32u);
                 continue;
@@ -738,6 +783,29 @@ hmc_status turning_points(uint64_t n, double G, const double* r, const double* v
     return HMC_OK;
 }
 
+static hmc_status launch_sampler(bool fused, uint64_t n, double G, uint64_t seed, uint32_t step, int shift, const SampleIO& io,
+                                 const Workspace& ws, cudaStream_t st)
+{
+    const int sms = sm_count();
+    const size_t smem = ORB_WARPS * sizeof(Park) + ((n >> shift) + 2) * sizeof(double2);
+    static bool attr_done = false;
+    if (!attr_done) {
+        const int cap = (int)(ORB_WARPS * sizeof(Park) + COARSE_CAP * sizeof(double2));
+        HMC_CUDA_TRY(cudaFuncSetAttribute(sample_new_radius_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap));
+        HMC_CUDA_TRY(cudaFuncSetAttribute(sample_new_radius_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap));
+        attr_done = true;
+    }
+    const int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
+    if (fused)
+        sample_new_radius_kernel<true><<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, G, (uint32_t)seed, (uint32_t)(seed >> 32), step,
+                                                                         ws.nodes, ws.coarse, ws.mid, ws.dir, shift, io);
+    else
+        sample_new_radius_kernel<false><<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, G, (uint32_t)seed, (uint32_t)(seed >> 32), step,
+                                                                          ws.nodes, ws.coarse, ws.mid, ws.dir, shift, io);
+    HMC_LAUNCH_CHECK();
+    return HMC_OK;
+}
+
 hmc_status sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step, const double* r,
                              const double* phi, const double* m_cum, const double* v_r, const double* v_t,
                              const double* E, const double* J, const double* r_min, const double* r_max,
@@ -746,26 +814,36 @@ hmc_status sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step,
                              uint16_t* n_try, uint8_t* status_out, uint64_t* counters, bool reuse_tables,
                              const Workspace& ws, cudaStream_t st)
 {
-    const int sms = sm_count();
     const int shift = coarse_shift(n);
-    const size_t smem = ORB_WARPS * sizeof(Park) + ((n >> shift) + 2) * sizeof(double2);
-    static bool attr_done = false;
-    if (!attr_done) {
-        HMC_CUDA_TRY(cudaFuncSetAttribute(sample_new_radius_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)(ORB_WARPS * sizeof(Park) + COARSE_CAP * sizeof(double2))));
-        attr_done = true;
-    }
     if (!reuse_tables) {
         hmc_status s = build_tables(n, G, r, phi, m_cum, ws, shift, st);
         if (s != HMC_OK) return s;
     }
-    SampleIO io{ r, v_r, v_t, E, J, r_min, r_max, k_min, k_max, id, status_in, reuse_tables ? ws.orbitF : nullptr, r_new, v_r_new, v_t_new, n_try,
-                 status_out, reinterpret_cast<unsigned long long*>(counters) };
-    const int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
-    sample_new_radius_kernel<<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, G, (uint32_t)seed, (uint32_t)(seed >> 32),
-                                                               step, ws.nodes, ws.coarse, ws.dir, shift, io);
-    HMC_LAUNCH_CHECK();
-    return HMC_OK;
+    SampleIO io{};
+    io.r = r; io.v_r = v_r; io.v_t = v_t; io.E = E; io.J = J; io.rmin = r_min; io.rmax = r_max;
+    io.kmin = k_min; io.kmax = k_max; io.id = id; io.status_in = status_in;
+    io.F_ws = reuse_tables ? ws.orbitF : nullptr;
+    io.r_new = r_new; io.v_r_new = v_r_new; io.v_t_new = v_t_new; io.n_try = n_try; io.status_out = status_out;
+    io.counters = reinterpret_cast<unsigned long long*>(counters);
+    return launch_sampler(false, n, G, seed, step, shift, io, ws, st);
+}
+
+// S3 + S4 in one launch: same outputs as the two calls.
+hmc_status orbit_step(uint64_t n, double G, uint64_t seed, uint32_t step, const double* r, const double* v_r,
+                      const double* v_t, const double* phi, const double* m_cum, const uint32_t* id, double* E,
+                      double* J, double* r_min, double* r_max, uint32_t* k_min, uint32_t* k_max, uint8_t* status,
+                      double* r_new, double* v_r_new, double* v_t_new, uint16_t* n_try, uint8_t* status_out,
+                      uint64_t* counters, const Workspace& ws, cudaStream_t st)
+{
+    const int shift = coarse_shift(n);
+    hmc_status s = build_tables(n, G, r, phi, m_cum, ws, shift, st);
+    if (s != HMC_OK) return s;
+    SampleIO io{};
+    io.r = r; io.v_r = v_r; io.v_t = v_t; io.id = id; io.phi = phi;
+    io.E_w = E; io.J_w = J; io.rmin_w = r_min; io.rmax_w = r_max; io.kmin_w = k_min; io.kmax_w = k_max; io.status_w = status;
+    io.r_new = r_new; io.v_r_new = v_r_new; io.v_t_new = v_t_new; io.n_try = n_try; io.status_out = status_out;
+    io.counters = reinterpret_cast<unsigned long long*>(counters);
+    return launch_sampler(true, n, G, seed, step, shift, io, ws, st);
 }
 
 }  // namespace hmc

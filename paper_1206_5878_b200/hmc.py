@@ -48,7 +48,7 @@ def lib() -> ctypes.CDLL:
         L.hmc_status_string.argtypes = [ctypes.c_int32]
         L.hmc_version.restype = ctypes.c_int32
         for name in ("hmc_sort_by_radius", "hmc_potential", "hmc_orbit_turning_points", "hmc_sample_new_radius",
-                     "hmc_step_host"):
+                     "hmc_orbit_step", "hmc_step_host"):
             getattr(L, name).restype = ctypes.c_int32
         _lib = L
     return _lib
@@ -190,7 +190,29 @@ def hmc_sample_new_radius(r_sorted, phi, m_cum, v_r, v_t, tp, ids, seed: int, st
     return out
 
 
-def kernel_launches_per_step(n: int, ncols: int = 3, with_id: bool = True) -> int:
+def hmc_orbit_step(r_sorted, v_r, v_t, phi, m_cum, ids, seed: int, step: int, G: float = 1.0, *, tp=None, out=None,
+                   counters=None, workspace=None):
+    """S3 + S4 in one launch (same outputs as the two calls).  -> (tp dict, sample dict)"""
+    n = r_sorted.numel()
+    dev = r_sorted.device
+    tp = alloc_turning_points(n, dev) if tp is None else tp
+    out = alloc_sample(n, dev) if out is None else out
+    workspace, wp, wb = _ws(workspace, n, dev)
+    f = torch.float64
+    rc = lib().hmc_orbit_step(
+        ctypes.c_uint64(n), ctypes.c_double(G), ctypes.c_uint64(seed), ctypes.c_uint32(step),
+        _dev(r_sorted, f, n, "r_sorted"), _dev(v_r, f, n, "v_r"), _dev(v_t, f, n, "v_t"), _dev(phi, f, n, "phi"),
+        _dev(m_cum, f, n, "m_cum"), _dev(ids, torch.int32, n, "ids"), _dev(tp["E"], f, n, "E"), _dev(tp["J"], f, n, "J"),
+        _dev(tp["r_min"], f, n, "r_min"), _dev(tp["r_max"], f, n, "r_max"), _dev(tp["k_min"], torch.int32, n, "k_min"),
+        _dev(tp["k_max"], torch.int32, n, "k_max"), _dev(tp["status"], torch.uint8, n, "status"),
+        _dev(out["r_new"], f, n, "r_new"), _dev(out["v_r_new"], f, n, "v_r_new"), _dev(out["v_t_new"], f, n, "v_t_new"),
+        _dev(out.get("n_try"), torch.int16, n, "n_try"), _dev(out["status"], torch.uint8, n, "status_out"),
+        _dev(counters, torch.int64, NCOUNTERS, "counters"), wp, wb, _stream())
+    _check(rc, "hmc_orbit_step")
+    return tp, out
+
+
+def kernel_launches_per_step(n: int, ncols: int = 3, with_id: bool = True, fused: bool = False) -> int:
     """How many kernels of libhmc one orbit step (the four calls, S4 with reuse_tables) launches for
     n stars; mirrors the host code of csrc/*.cu (memsets are not counted)."""
     if n < 2:
@@ -206,6 +228,8 @@ def kernel_launches_per_step(n: int, ncols: int = 3, with_id: bool = True) -> in
     while (n >> shift) + 2 > 10240:
         shift += 1
     tables = 2 if shift > 0 else 1
+    if fused:
+        return fast + general + 3 + (tables + 1)     # + potential (3) + tables and the fused S3/S4 kernel
     return fast + general + 3 + (tables + 1) + 1     # + potential (3) + S3 (tables, search) + S4 (1)
 
 
@@ -231,16 +255,22 @@ class OrbitStepper:
         self.counters = alloc_counters(dev)
         self.workspace = alloc_workspace(n, dev)
 
-    def step(self):
+    def step(self, fused: bool = False):
+        """One orbit step.  fused=False: the four C-ABI calls; fused=True: S3 and S4 as the single
+        call hmc_orbit_step (same results)."""
         s, so = self.state, self.sorted
         hmc_sort_by_radius(s["r"], (s["v_r"], s["v_t"], s["m"]), s["id"], r_sorted=so["r"], perm=so["perm"],
                            cols_out=(so["v_r"], so["v_t"], so["m"]), ids_out=so["id"], workspace=self.workspace)
         hmc_potential(so["r"], so["m"], self.G, phi=self.phi, m_cum=self.m_cum, workspace=self.workspace)
-        hmc_orbit_turning_points(so["r"], so["v_r"], so["v_t"], self.phi, self.m_cum, self.G, out=self.tp,
-                                 counters=self.counters, workspace=self.workspace)
-        hmc_sample_new_radius(so["r"], self.phi, self.m_cum, so["v_r"], so["v_t"], self.tp, so["id"], self.seed,
-                              self.step_index, self.G, out=self.sample, counters=self.counters,
-                              workspace=self.workspace, reuse_tables=True)
+        if fused:
+            hmc_orbit_step(so["r"], so["v_r"], so["v_t"], self.phi, self.m_cum, so["id"], self.seed, self.step_index,
+                           self.G, tp=self.tp, out=self.sample, counters=self.counters, workspace=self.workspace)
+        else:
+            hmc_orbit_turning_points(so["r"], so["v_r"], so["v_t"], self.phi, self.m_cum, self.G, out=self.tp,
+                                     counters=self.counters, workspace=self.workspace)
+            hmc_sample_new_radius(so["r"], self.phi, self.m_cum, so["v_r"], so["v_t"], self.tp, so["id"], self.seed,
+                                  self.step_index, self.G, out=self.sample, counters=self.counters,
+                                  workspace=self.workspace, reuse_tables=True)
         # carried state for the next step: new phase-space coordinates, masses and ids in sorted order
         sm = self.sample
         s["r"], sm["r_new"] = sm["r_new"], s["r"]

@@ -216,6 +216,25 @@ def test_orbit_stage_isolation_on_oracle_tables(oracle, n, masses, seed):
         assert torch.equal(sm[key], sm2[key]), key
 
 
+@pytest.mark.parametrize("n,masses", [(1, "equal"), (33, "equal"), (100_000, "equal"), (300_001, "salpeter")])
+def test_fused_orbit_step_equals_the_two_calls(n, masses):
+    """hmc_orbit_step (S3 + S4 in one launch) writes bit for bit what the two calls write, counters included."""
+    c = inputs.plummer(n, 21, masses)
+    rs, perm, (vrs, vts, ms), ids = hmc.hmc_sort_by_radius(dev(c["r"]), (dev(c["v_r"]), dev(c["v_t"]), dev(c["m"])),
+                                                           dev(c["id"].view(np.int32)))
+    phi, mc = hmc.hmc_potential(rs, ms)
+    c1, c2 = hmc.alloc_counters(), hmc.alloc_counters()
+    ws = hmc.alloc_workspace(n)
+    tp = hmc.hmc_orbit_turning_points(rs, vrs, vts, phi, mc, counters=c1, workspace=ws)
+    sm = hmc.hmc_sample_new_radius(rs, phi, mc, vrs, vts, tp, ids, 21, 5, counters=c1, workspace=ws, reuse_tables=True)
+    tp2, sm2 = hmc.hmc_orbit_step(rs, vrs, vts, phi, mc, ids, 21, 5, counters=c2)
+    for key in tp:
+        assert torch.equal(tp[key], tp2[key]), key
+    for key in sm:
+        assert torch.equal(sm[key], sm2[key]), key
+    assert torch.equal(c1, c2)
+
+
 def test_config1_whole_step_chained(oracle):
     """BASELINE.json configs[0]: Plummer N = 1e5, seed 1, one orbit step -- all four GPU stages chained."""
     cfg = inputs.config(0)
