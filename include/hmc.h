@@ -195,7 +195,8 @@ HMC_API hmc_status hmc_orbit_step(uint64_t n, double G, uint64_t seed, uint32_t 
  * `device_arena` is a DEVICE buffer of at least hmc_step_host_arena_bytes(n) bytes (256-byte
  * aligned) holding the staged columns, every intermediate and the workspace.
  * The call enqueues H2D copies, the four stages and D2H copies on `cuda_stream`; the host arrays
- * are valid after the caller synchronises the stream.  counters_host (HOST uint64[HMC_NCOUNTERS],
+ * are valid after the caller synchronises the stream (m_out and id_out travel on a second, library-owned
+ * stream, created at first use per host thread, which `cuda_stream` waits for before the call's work ends).  counters_host (HOST uint64[HMC_NCOUNTERS],
  * may be NULL) receives the step's counters.
  */
 HMC_API size_t hmc_step_host_arena_bytes(uint64_t n);

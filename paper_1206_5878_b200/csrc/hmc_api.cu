@@ -63,6 +63,30 @@ static Arena carve_arena(void* base, uint64_t n)
     return a;
 }
 
+// hmc_step_host only: a second stream on which the sorted masses and ids go back to the host while the
+// potential and orbit stages run (the two directions and the kernels then overlap).  One per host thread and
+// device, created at first use, never destroyed.
+struct SideStream {
+    int device = -1;
+    cudaStream_t stream = nullptr;
+    cudaEvent_t sorted = nullptr, copied = nullptr;
+};
+
+static hmc_status side_stream(SideStream** out)
+{
+    static thread_local SideStream ss;
+    int dev = 0;
+    HMC_CUDA_TRY(cudaGetDevice(&dev));
+    if (ss.device != dev) {
+        HMC_CUDA_TRY(cudaStreamCreateWithFlags(&ss.stream, cudaStreamNonBlocking));
+        HMC_CUDA_TRY(cudaEventCreateWithFlags(&ss.sorted, cudaEventDisableTiming));
+        HMC_CUDA_TRY(cudaEventCreateWithFlags(&ss.copied, cudaEventDisableTiming));
+        ss.device = dev;
+    }
+    *out = &ss;
+    return HMC_OK;
+}
+
 }  // namespace hmc
 
 using namespace hmc;
@@ -220,6 +244,14 @@ hmc_status hmc_step_host(uint64_t n, double G, uint64_t seed, uint32_t step, con
     double* cout[3] = { a.vrs, a.vts, a.ms };
     hmc_status s = sort_by_radius(n, a.r, a.rs, a.perm, 3, cin, cout, a.id, a.ids, ws, st);
     if (s != HMC_OK) return s;
+    SideStream* side = nullptr;
+    s = side_stream(&side);
+    if (s != HMC_OK) return s;
+    HMC_CUDA_TRY(cudaEventRecord(side->sorted, st));
+    HMC_CUDA_TRY(cudaStreamWaitEvent(side->stream, side->sorted, 0));
+    HMC_CUDA_TRY(cudaMemcpyAsync(m_out, a.ms, n * 8, cudaMemcpyDeviceToHost, side->stream));
+    HMC_CUDA_TRY(cudaMemcpyAsync(id_out, a.ids, n * 4, cudaMemcpyDeviceToHost, side->stream));
+    HMC_CUDA_TRY(cudaEventRecord(side->copied, side->stream));
     s = potential(n, G, a.rs, a.ms, a.phi, a.mcum, ws, st);
     if (s != HMC_OK) return s;
     s = turning_points(n, G, a.rs, a.vrs, a.vts, a.phi, a.mcum, a.E, a.J, a.rmin, a.rmax, a.kmin, a.kmax, a.st0,
@@ -231,10 +263,9 @@ hmc_status hmc_step_host(uint64_t n, double G, uint64_t seed, uint32_t step, con
     HMC_CUDA_TRY(cudaMemcpyAsync(r_new, a.rn, n * 8, cudaMemcpyDeviceToHost, st));
     HMC_CUDA_TRY(cudaMemcpyAsync(v_r_new, a.vrn, n * 8, cudaMemcpyDeviceToHost, st));
     HMC_CUDA_TRY(cudaMemcpyAsync(v_t_new, a.vtn, n * 8, cudaMemcpyDeviceToHost, st));
-    HMC_CUDA_TRY(cudaMemcpyAsync(m_out, a.ms, n * 8, cudaMemcpyDeviceToHost, st));
-    HMC_CUDA_TRY(cudaMemcpyAsync(id_out, a.ids, n * 4, cudaMemcpyDeviceToHost, st));
     if (counters_host)
         HMC_CUDA_TRY(cudaMemcpyAsync(counters_host, a.counters, HMC_NCOUNTERS * 8, cudaMemcpyDeviceToHost, st));
+    HMC_CUDA_TRY(cudaStreamWaitEvent(st, side->copied, 0));      // the caller's stream completes after the side copies
     return HMC_OK;
 }
 
