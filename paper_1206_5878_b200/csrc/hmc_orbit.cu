@@ -516,6 +516,7 @@ struct SampleIO {
     const uint32_t *kmin, *kmax, *id;
     const uint8_t* status_in;
     const double* F_ws;      // S3's bound F per star (workspace), or nullptr: compute it here
+    uint32_t* batch_counter; // workspace word, zero at launch: next unclaimed star
     // fused S3 + S4 only: S3's table input and where its outputs go
     const double* phi;
     double *E_w, *J_w, *rmin_w, *rmax_w;
@@ -648,12 +649,9 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
     const unsigned lane_lt = lanemask_lt();
     const uint32_t lane = threadIdx.x & 31;
 
-    // each warp owns a contiguous run of stars (a multiple of 32) and deals them to its lanes
-    const uint32_t warps_total = gridDim.x * ORB_WARPS;
-    const uint32_t gw = blockIdx.x * ORB_WARPS + (threadIdx.x >> 5);
-    const uint32_t per = (uint32_t)((((uint64_t)n + warps_total - 1) / warps_total + 31) & ~31ull);
-    uint32_t next = (uint32_t)min((unsigned long long)n, (unsigned long long)gw * per);
-    const uint32_t end = (uint32_t)min((unsigned long long)n, (unsigned long long)next + per);
+    // warps take batches of 32 consecutive stars from a global counter (the draws of some regions of the
+    // cluster take longer than others: a static split leaves SMs idle at the end) and deal them to their lanes
+    bool exhausted = false;
     uint32_t parked = 0, head = 0;          // park slots head .. parked-1 are waiting
 
     bool have = false;
@@ -665,11 +663,14 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
         unsigned need = __ballot_sync(0xffffffffu, !have);
         while (need) {
             if (head == parked) {
-                if (next >= end) break;
-                parked = FUSED ? park_by_solving(T, io, pk, next, end, lane, lane_lt)
-                               : park_from_arrays(nodes, io, pk, next, end, lane, lane_lt);
+                if (exhausted) break;
+                uint32_t base = 0;
+                if (lane == 0) base = atomicAdd(io.batch_counter, 32u);
+                base = __shfl_sync(0xffffffffu, base, 0);
+                if (base >= n) { exhausted = true; break; }
+                parked = FUSED ? park_by_solving(T, io, pk, base, n, lane, lane_lt)
+                               : park_from_arrays(nodes, io, pk, base, n, lane, lane_lt);
                 head = 0;
-                next = min(end, next + 32u);
                 continue;
             }
             const uint32_t slot = head + __popc(need & lane_lt);
@@ -783,7 +784,7 @@ hmc_status turning_points(uint64_t n, double G, const double* r, const double* v
     return HMC_OK;
 }
 
-static hmc_status launch_sampler(bool fused, uint64_t n, double G, uint64_t seed, uint32_t step, int shift, const SampleIO& io,
+static hmc_status launch_sampler(bool fused, uint64_t n, double G, uint64_t seed, uint32_t step, int shift, const SampleIO& io_in,
                                  const Workspace& ws, cudaStream_t st)
 {
     const int sms = sm_count();
@@ -796,6 +797,9 @@ static hmc_status launch_sampler(bool fused, uint64_t n, double G, uint64_t seed
         attr_done = true;
     }
     const int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
+    HMC_CUDA_TRY(cudaMemsetAsync(ws.tickets + 16, 0, 4, st));
+    SampleIO io = io_in;
+    io.batch_counter = ws.tickets + 16;
     if (fused)
         sample_new_radius_kernel<true><<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, G, (uint32_t)seed, (uint32_t)(seed >> 32), step,
                                                                          ws.nodes, ws.coarse, ws.mid, ws.dir, shift, io);
