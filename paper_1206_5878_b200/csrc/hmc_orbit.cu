@@ -58,6 +58,8 @@ __device__ __forceinline__ Node ld_node(const Node* __restrict__ p)
     return e;
 }
 
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 __device__ __forceinline__ double2 ld_d2_na(const double2* __restrict__ p)
 {
     double2 v;
@@ -635,6 +637,17 @@ __device__ __forceinline__ uint32_t park_by_solving(const Tables& T, const Sampl
 }
 
 template <bool FUSED>
+__device__ __forceinline__ void prefetch_inputs(const SampleIO& io, uint32_t a)
+{
+    if (FUSED) { prefetch_l2(io.r + a); prefetch_l2(io.v_r + a); prefetch_l2(io.v_t + a); prefetch_l2(io.phi + a); prefetch_l2(io.id + a); }
+    else {
+        prefetch_l2(io.E + a); prefetch_l2(io.J + a); prefetch_l2(io.rmin + a); prefetch_l2(io.rmax + a);
+        prefetch_l2(io.kmin + a); prefetch_l2(io.kmax + a); prefetch_l2(io.id + a); prefetch_l2(io.status_in + a);
+        if (io.F_ws) prefetch_l2(io.F_ws + a);
+    }
+}
+
+template <bool FUSED>
 __global__ void __launch_bounds__(ORB_THREADS, 1)
 sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_hi, uint32_t step,
                          const Node* __restrict__ nodes, const double2* __restrict__ coarse_g,
@@ -653,6 +666,9 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
     // cluster take longer than others: a static split leaves SMs idle at the end) and deal them to their lanes
     bool exhausted = false;
     uint32_t parked = 0, head = 0;          // park slots head .. parked-1 are waiting
+    uint32_t next_base = 0;
+    if (lane == 0) next_base = atomicAdd(io.batch_counter, 32u);
+    next_base = __shfl_sync(0xffffffffu, next_base, 0);
 
     bool have = false;
     uint32_t a = 0, t = 0, cl = 0, ch = 0;
@@ -664,10 +680,13 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
         while (need) {
             if (head == parked) {
                 if (exhausted) break;
-                uint32_t base = 0;
-                if (lane == 0) base = atomicAdd(io.batch_counter, 32u);
-                base = __shfl_sync(0xffffffffu, base, 0);
+                // the batch claimed one round ago is prepared now; the next one is claimed here and its
+                // per-star inputs are pulled into L2 meanwhile
+                const uint32_t base = next_base;
                 if (base >= n) { exhausted = true; break; }
+                if (lane == 0) next_base = atomicAdd(io.batch_counter, 32u);
+                next_base = __shfl_sync(0xffffffffu, next_base, 0);
+                if (next_base + lane < n) prefetch_inputs<FUSED>(io, next_base + lane);
                 parked = FUSED ? park_by_solving(T, io, pk, base, n, lane, lane_lt)
                                : park_from_arrays(nodes, io, pk, base, n, lane, lane_lt);
                 head = 0;
