@@ -136,6 +136,22 @@ def sample_new_radius(r, phi, m_cum, r_self, v_r_self, v_t_self, E, J, r_min, r_
     return o
 
 
+DIAG_NAMES = ("M", "T", "W", "E_tot", "virial_ratio", "r_h", "t_rh")
+
+
+def diagnostics(r, v_r, v_t, m, phi, m_cum, fractions=(), G=1.0):
+    """Diagnostics on the radius-sorted arrays -> dict(M, T, W, E_tot, virial_ratio, r_h, t_rh, lagrange=[...])."""
+    r, v_r, v_t, m, phi, m_cum = map(_f64, (r, v_r, v_t, m, phi, m_cum))
+    fr = np.ascontiguousarray(np.asarray(fractions, dtype=np.float64))
+    out = np.empty(7 + fr.shape[0], np.float64)
+    rc = lib().hmc_ref_diagnostics(ctypes.c_uint64(r.shape[0]), ctypes.c_double(G), _p(r), _p(v_r), _p(v_t), _p(m),
+                                   _p(phi), _p(m_cum), ctypes.c_int(fr.shape[0]), _p(fr), _p(out))
+    assert rc == 0
+    d = dict(zip(DIAG_NAMES, out[:7].tolist()))
+    d["lagrange"] = out[7:].copy()
+    return d
+
+
 def orbit_step(r, v_r, v_t, m, ids, seed, step, G=1.0, sample=None):
     """One pass of the whole path: sort -> potential -> turning points -> new radius.
 

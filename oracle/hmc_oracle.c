@@ -28,6 +28,8 @@
  *                 Kepler closed form, circular orbit
  *   sampling    : energy identity, KS vs Kepler time-weighted CDF, closed-form
  *                 acceptance rate, order independence
+ *   diagnostics : exact rational pair sums for T and W, numpy searchsorted for the
+ *                 Lagrange radii, two-star hand case, Plummer closed forms, scaling laws
  * No function in this file is "parity unpinned".
  */
 #include <math.h>
@@ -353,5 +355,54 @@ int hmc_ref_sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step
         status_out[i] = (uint8_t)st;
     }
     if (counters) counters[0] += total_trials;
+    return 0;
+}
+
+/* ------------------------------------------------------------------------ */
+/* Diagnostics on the radius-sorted arrays ("half-mass radius   */
+/* ... that control program termination"; :346 Eq. 20; :354 total energy).   */
+/* SURVEY.md 8(f) item 4.  Readings (R15-R17):                    */
+/*  - kinetic energy T = sum_k m_k * (0.5 * (v_r^2 + v_t^2)), potential     */
+/*    energy W = sum_k 0.5 * (m_k * Phi_k) (Phi_k of Eq. 1 contains the      */
+/*    star's own term, as the paper's potential does); each term is the     */
+/*    binary64 value of the expression written, the SUM is exact, rounded   */
+/*    once (binary128 accumulator, as for Eq. 3-5);                          */
+/*  - E_tot = T + W, virial ratio = (2 T) / |W|;                            */
+/*  - Lagrange radius of mass fraction f: r_k of the first star k with      */
+/*    M_k >= f * M_N (binary64 product); half-mass radius r_h = f = 1/2;    */
+/*  - t_rh = 0.138 N / ln(0.1 N) * (r_h^3 / (G M_N))^(1/2), Eq. 20.         */
+/* out: [0] M_N, [1] T, [2] W, [3] E_tot, [4] virial ratio, [5] r_h,        */
+/*      [6] t_rh, [7 .. 7 + nfrac) Lagrange radii of fractions[].           */
+/* ------------------------------------------------------------------------ */
+static double lagrange_radius(uint64_t n, const double *r, const double *m_cum, double f)
+{
+    double target = f * m_cum[n - 1];
+    uint64_t k = 0;
+    while (k + 1 < n && !(m_cum[k] >= target)) ++k;      /* first k with M_k >= target, else the last star */
+    return r[k];
+}
+
+int hmc_ref_diagnostics(uint64_t n, double G, const double *r, const double *v_r, const double *v_t,
+                        const double *m, const double *phi, const double *m_cum,
+                        int nfrac, const double *fractions, double *out)
+{
+    if (n == 0) return -2;
+    __float128 accT = 0, accW = 0;
+    for (uint64_t a = 0; a < n; ++a) {
+        double t = m[a] * (0.5 * (v_r[a] * v_r[a] + v_t[a] * v_t[a]));
+        double w = 0.5 * (m[a] * phi[a]);
+        accT += (__float128)t;
+        accW += (__float128)w;
+    }
+    double M = m_cum[n - 1], T = (double)accT, W = (double)accW;
+    double rh = lagrange_radius(n, r, m_cum, 0.5);
+    out[0] = M;
+    out[1] = T;
+    out[2] = W;
+    out[3] = T + W;
+    out[4] = (2.0 * T) / fabs(W);
+    out[5] = rh;
+    out[6] = ((0.138 * (double)n) / log(0.1 * (double)n)) * sqrt(((rh * rh) * rh) / (G * M));
+    for (int i = 0; i < nfrac; ++i) out[7 + i] = lagrange_radius(n, r, m_cum, fractions[i]);
     return 0;
 }
