@@ -188,6 +188,30 @@ HMC_API hmc_status hmc_orbit_step(uint64_t n, double G, uint64_t seed, uint32_t 
         void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*
+ * Diagnostics on the radius-sorted arrays (PAPER.md:140 "half-mass radius ..."; :346 Eq. 20; :354
+ * total energy; R15-R17).  out is a DEVICE array of HMC_DIAG_LAGRANGE + nfrac doubles:
+ *   out[HMC_DIAG_M]      M_N, total mass
+ *   out[HMC_DIAG_T]      T = sum_k m_k (v_r^2 + v_t^2) / 2          (exact sum of the binary64 terms, rounded once)
+ *   out[HMC_DIAG_W]      W = sum_k m_k Phi_k / 2                    (likewise; Phi_k includes the star's own term)
+ *   out[HMC_DIAG_ETOT]   T + W
+ *   out[HMC_DIAG_VIRIAL] 2 T / |W|
+ *   out[HMC_DIAG_RH]     half-mass radius: r_k of the first star with M_k >= M_N / 2
+ *   out[HMC_DIAG_TRH]    0.138 N / ln(0.1 N) * (r_h^3 / (G M_N))^(1/2)   (Eq. 20)
+ *   out[HMC_DIAG_LAGRANGE + i]  Lagrange radius of mass_fractions[i]: r_k of the first star with
+ *                        M_k >= mass_fractions[i] * M_N (the outermost star if there is none)
+ * mass_fractions is a HOST array of nfrac values, 0 <= nfrac <= HMC_DIAG_MAX_FRACTIONS (may be NULL if 0).
+ * Preconditions: m >= 0 (M_cum ascending), n >= 1.
+ */
+#define HMC_DIAG_MAX_FRACTIONS 16
+enum { HMC_DIAG_M = 0, HMC_DIAG_T, HMC_DIAG_W, HMC_DIAG_ETOT, HMC_DIAG_VIRIAL, HMC_DIAG_RH, HMC_DIAG_TRH, HMC_DIAG_LAGRANGE };
+
+HMC_API hmc_status hmc_diagnostics(uint64_t n, double G,
+        const double* r_sorted, const double* v_r, const double* v_t, const double* m_sorted,
+        const double* phi, const double* m_cum,
+        int32_t nfrac, const double* mass_fractions, double* out,
+        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
  * Host-buffer variant of one whole orbit step (the four calls above, in order), for callers
  * whose star data lives in HOST memory.  r, v_r, v_t, m, id are HOST arrays [n] (unsorted);
  * r_new, v_r_new, v_t_new, m_out, id_out are HOST arrays [n] receiving the stars in radius-sorted

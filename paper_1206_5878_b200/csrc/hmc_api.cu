@@ -218,6 +218,23 @@ hmc_status hmc_orbit_step(uint64_t n, double G, uint64_t seed, uint32_t step, co
                       static_cast<cudaStream_t>(cuda_stream));
 }
 
+hmc_status hmc_diagnostics(uint64_t n, double G, const double* r_sorted, const double* v_r, const double* v_t,
+                           const double* m_sorted, const double* phi, const double* m_cum, int32_t nfrac,
+                           const double* mass_fractions, double* out, void* workspace, size_t workspace_bytes,
+                           void* cuda_stream)
+{
+    if (n == 0 || n > HMC_MAX_N || nfrac < 0 || nfrac > HMC_DIAG_MAX_FRACTIONS) return HMC_ERR_SIZE;
+    REQUIRE_PTR(r_sorted); REQUIRE_PTR(v_r); REQUIRE_PTR(v_t); REQUIRE_PTR(m_sorted); REQUIRE_PTR(phi); REQUIRE_PTR(m_cum);
+    REQUIRE_PTR(out);
+    if (nfrac > 0) REQUIRE_PTR(mass_fractions);
+    REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(v_r, 8); REQUIRE_ALIGN(v_t, 8); REQUIRE_ALIGN(m_sorted, 8); REQUIRE_ALIGN(phi, 8);
+    REQUIRE_ALIGN(m_cum, 8); REQUIRE_ALIGN(out, 8);
+    hmc_status s = check_ws(workspace, workspace_bytes, n);
+    if (s != HMC_OK) return s;
+    return diagnostics(n, G, r_sorted, v_r, v_t, m_sorted, phi, m_cum, nfrac, mass_fractions, out, carve(workspace, n),
+                       static_cast<cudaStream_t>(cuda_stream));
+}
+
 size_t hmc_step_host_arena_bytes(uint64_t n) { return carve_arena(nullptr, n).total; }
 
 hmc_status hmc_step_host(uint64_t n, double G, uint64_t seed, uint32_t step, const double* r, const double* v_r,

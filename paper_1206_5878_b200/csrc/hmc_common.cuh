@@ -210,4 +210,8 @@ hmc_status orbit_step(uint64_t n, double G, uint64_t seed, uint32_t step, const 
                       double* r_new, double* v_r_new, double* v_t_new, uint16_t* n_try, uint8_t* status_out,
                       uint64_t* counters, const Workspace& ws, cudaStream_t st);
 
+hmc_status diagnostics(uint64_t n, double G, const double* r, const double* v_r, const double* v_t, const double* m,
+                       const double* phi, const double* m_cum, int nfrac, const double* fractions, double* out,
+                       const Workspace& ws, cudaStream_t st);
+
 }  // namespace hmc

@@ -48,7 +48,7 @@ def lib() -> ctypes.CDLL:
         L.hmc_status_string.argtypes = [ctypes.c_int32]
         L.hmc_version.restype = ctypes.c_int32
         for name in ("hmc_sort_by_radius", "hmc_potential", "hmc_orbit_turning_points", "hmc_sample_new_radius",
-                     "hmc_orbit_step", "hmc_step_host"):
+                     "hmc_orbit_step", "hmc_diagnostics", "hmc_step_host"):
             getattr(L, name).restype = ctypes.c_int32
         _lib = L
     return _lib
@@ -212,6 +212,29 @@ def hmc_orbit_step(r_sorted, v_r, v_t, phi, m_cum, ids, seed: int, step: int, G:
     return tp, out
 
 
+DIAG_NAMES = ("M", "T", "W", "E_tot", "virial_ratio", "r_h", "t_rh")
+DIAG_MAX_FRACTIONS = 16
+
+
+def hmc_diagnostics(r_sorted, v_r, v_t, m_sorted, phi, m_cum, fractions: Sequence[float] = (), G: float = 1.0, *,
+                    out=None, workspace=None):
+    """Diagnostics (Eq. 20).  -> device float64 tensor [7 + len(fractions)]:
+    M, T, W, E_tot, virial ratio, r_h, t_rh, then the Lagrange radii of ``fractions`` (host floats)."""
+    n = r_sorted.numel()
+    dev = r_sorted.device
+    nf = len(fractions)
+    out = torch.empty(7 + nf, dtype=torch.float64, device=dev) if out is None else out
+    fr = (ctypes.c_double * max(nf, 1))(*[float(x) for x in fractions])
+    workspace, wp, wb = _ws(workspace, n, dev)
+    f = torch.float64
+    rc = lib().hmc_diagnostics(ctypes.c_uint64(n), ctypes.c_double(G), _dev(r_sorted, f, n, "r_sorted"),
+                               _dev(v_r, f, n, "v_r"), _dev(v_t, f, n, "v_t"), _dev(m_sorted, f, n, "m_sorted"),
+                               _dev(phi, f, n, "phi"), _dev(m_cum, f, n, "m_cum"), ctypes.c_int32(nf), fr,
+                               _dev(out, f, 7 + nf, "out"), wp, wb, _stream())
+    _check(rc, "hmc_diagnostics")
+    return out
+
+
 def kernel_launches_per_step(n: int, ncols: int = 3, with_id: bool = True, fused: bool = False) -> int:
     """How many kernels of libhmc one orbit step (the four calls, S4 with reuse_tables) launches for
     n stars; mirrors the host code of csrc/*.cu (memsets are not counted)."""
@@ -279,6 +302,13 @@ class OrbitStepper:
         s["m"], so["m"] = so["m"], s["m"]
         s["id"], so["id"] = so["id"], s["id"]
         self.step_index += 1
+
+    def diagnostics(self, fractions=()):
+        """hmc_diagnostics of the cluster as the last step's S1/S2 saw it: the sorted radii and velocities the
+        step started from, that step's potential (after step() the sorted masses are in state["m"])."""
+        so = self.sorted
+        return hmc_diagnostics(so["r"], so["v_r"], so["v_t"], self.state["m"], self.phi, self.m_cum, fractions,
+                               self.G, workspace=self.workspace)
 
 
 def step_host_arena_bytes(n: int) -> int:

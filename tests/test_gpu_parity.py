@@ -335,3 +335,42 @@ def test_host_buffer_step_matches_device_step(oracle):
     d = rel(out["r_new"].numpy(), o["sample"]["r_new"])
     assert (d <= TOL_RNEW).mean() >= FRAC_RNEW
     assert int(cnt[hmc.COUNTER_NAMES.index("trials")]) == o["sample"]["trials"]
+
+
+# ----------------------------------------------------------------------------- diagnostics
+@pytest.mark.parametrize("n,masses", [(1, "equal"), (2, "equal"), (255, "equal"), (100_000, "equal"), (1_000_003, "salpeter")])
+def test_diagnostics_match_oracle(oracle, n, masses):
+    """M, T, W, E_tot, virial ratio, r_h and the Lagrange radii bit for bit (exact sums rounded once on both sides,
+    index work for the radii); t_rh to 1e-14 (one logarithm from two different math libraries)."""
+    c = inputs.plummer(n, 31, masses)
+    rs, perm, (vrs, vts, ms), ids = oracle.sort_by_radius(c["r"], (c["v_r"], c["v_t"], c["m"]), c["id"])
+    phi, mc = oracle.potential(rs, ms)
+    fr = [1e-6, 0.01, 0.1, 0.25, 0.5, 0.75, 0.9, 0.99, 1.0]
+    o = oracle.diagnostics(rs, vrs, vts, ms, phi, mc, fr)
+    out = host(hmc.hmc_diagnostics(dev(rs), dev(vrs), dev(vts), dev(ms), dev(phi), dev(mc), fr))
+    for i, name in enumerate(hmc.DIAG_NAMES):
+        if name == "t_rh":
+            assert out[i] == o[name] or abs(out[i] - o[name]) <= 1e-14 * abs(o[name]) or (np.isnan(out[i]) and np.isnan(o[name])), name
+        else:
+            assert out[i] == o[name] or (np.isnan(out[i]) and np.isnan(o[name])), (name, out[i], o[name])
+    assert np.array_equal(out[7:], o["lagrange"])
+    # no fractions asked for
+    out0 = host(hmc.hmc_diagnostics(dev(rs), dev(vrs), dev(vts), dev(ms), dev(phi), dev(mc)))
+    assert np.array_equal(out0[:6], out[:6])
+
+
+def test_diagnostics_errors():
+    z = torch.ones(4, dtype=torch.float64, device="cuda")
+    with pytest.raises(hmc.HmcError):
+        hmc.hmc_diagnostics(z, z, z, z, z, z, [0.5] * 17)          # more than HMC_DIAG_MAX_FRACTIONS
+
+
+def test_stepper_diagnostics_after_a_step(oracle):
+    c = inputs.plummer(50_000, 17)
+    st = hmc.OrbitStepper(dev(c["r"]), dev(c["v_r"]), dev(c["v_t"]), dev(c["m"]), dev(c["id"].view(np.int32)), 17)
+    st.step()
+    o = oracle_chain(oracle, c, 17, 0)
+    od = oracle.diagnostics(o["r"], o["v_r"], o["v_t"], o["m"], o["phi"], o["m_cum"], [0.1, 0.5])
+    out = host(st.diagnostics([0.1, 0.5]))
+    assert [out[i] for i in range(6)] == [od[k] for k in hmc.DIAG_NAMES[:6]]
+    assert np.array_equal(out[7:], od["lagrange"])
