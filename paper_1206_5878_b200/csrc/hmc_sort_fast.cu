@@ -105,6 +105,7 @@ __global__ void __launch_bounds__(512) sort_minmax_kernel(const uint64_t* __rest
 // ---- digit histograms of the key part, all passes in one read -------------------------------------
 static constexpr int PKH_THREADS = 512;
 static constexpr int PKH_COPIES = 4;
+static constexpr int PKH_UNROLL = 4;
 
 __global__ void __launch_bounds__(PKH_THREADS) sort_pk_histogram_kernel(const uint64_t* __restrict__ keys, uint32_t n,
                                                                         const uint64_t* __restrict__ ctl,
@@ -115,25 +116,41 @@ __global__ void __launch_bounds__(PKH_THREADS) sort_pk_histogram_kernel(const ui
     __syncthreads();
     const Packing pk = packing_of(n, ctl);
     uint32_t* mine = sh[(threadIdx.x >> 5) % PKH_COPIES];
+    const int npass = (pk.key_bits + 7) / 8;                    // digits beyond are zero for every key
     const uint32_t stride = gridDim.x * PKH_THREADS;
     const uint32_t iters = (n + stride - 1) / stride;           // same trip count for every thread
     uint32_t i = blockIdx.x * PKH_THREADS + threadIdx.x;
-    for (uint32_t it = 0; it < iters; ++it, i += stride) {
-        const bool ok = i < n;
-        const uint64_t kp = ok ? pk.key_part(__ldg(keys + i)) : 0ull;
-        if (ok) {
+    for (uint32_t it = 0; it < iters; it += PKH_UNROLL) {
+        uint64_t kp[PKH_UNROLL];
+        bool ok[PKH_UNROLL];
 #pragma unroll
-            for (int p = 0; p < PK_MAXPASS - 2; ++p) atomicAdd(&mine[p * PK_RADIX + ((uint32_t)(kp >> (8 * p)) & 255u)], 1u);
+        for (int u = 0; u < PKH_UNROLL; ++u) {                  // all loads first: several keys in flight per thread
+            const uint32_t iu = i + u * stride;
+            ok[u] = (it + u < iters) && iu < n;
+            kp[u] = ok[u] ? __ldcs(keys + iu) : 0ull;
         }
-        // the two leading digits take few distinct values: aggregate across the warp first
 #pragma unroll
-        for (int p = PK_MAXPASS - 2; p < PK_MAXPASS; ++p) {
-            const uint32_t d = (uint32_t)(kp >> (8 * p)) & 255u;
-            const unsigned live = __ballot_sync(0xffffffffu, ok);
-            const unsigned peers = match_digit(d) & live;
-            if (ok && (peers & lanemask_lt()) == 0) atomicAdd(&mine[p * PK_RADIX + d], (uint32_t)__popc(peers));
+        for (int u = 0; u < PKH_UNROLL; ++u) {
+            if (it + u >= iters) break;                         // uniform over the warp
+            const uint64_t k = pk.key_part(kp[u]);
+            if (ok[u]) {
+#pragma unroll
+                for (int p = 0; p < PK_MAXPASS - 2; ++p) atomicAdd(&mine[p * PK_RADIX + ((uint32_t)(k >> (8 * p)) & 255u)], 1u);
+            }
+            // the leading digits take few distinct values: aggregate across the warp first
+            const unsigned live = __ballot_sync(0xffffffffu, ok[u]);
+#pragma unroll
+            for (int p = PK_MAXPASS - 2; p < PK_MAXPASS; ++p) {
+                if (p >= npass) break;
+                const uint32_t d = (uint32_t)(k >> (8 * p)) & 255u;
+                const unsigned peers = match_digit(d) & live;
+                if (ok[u] && (peers & lanemask_lt()) == 0) atomicAdd(&mine[p * PK_RADIX + d], (uint32_t)__popc(peers));
+            }
         }
+        i += PKH_UNROLL * stride;
     }
+    // digits beyond the kept key bits: every key has digit 0
+    if (blockIdx.x == 0 && threadIdx.x < PK_MAXPASS && (int)threadIdx.x >= max(npass, PK_MAXPASS - 2)) atomicAdd(&hist[threadIdx.x * PK_RADIX], n);
     __syncthreads();
     for (int b = threadIdx.x; b < PK_MAXPASS * PK_RADIX; b += PKH_THREADS) {
         uint32_t c = 0;
