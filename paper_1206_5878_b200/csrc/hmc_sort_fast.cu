@@ -179,6 +179,58 @@ __global__ void sort_pk_scan_hist_kernel(uint32_t* __restrict__ hist, uint32_t n
     if (d == 0) pass_live[p] = single ? 0u : 1u;
 }
 
+// ---- 64-byte star records -------------------------------------------------------------------------
+// record i = { r_i, cols[0][i], ..., cols[ncols-1][i], (uint32) id_i, padding }, ncols <= PK_REC_COLS
+static constexpr int PK_REC_COLS = 6;
+
+struct PkCols {
+    const double* in[HMC_MAX_COLS];
+    double* out[HMC_MAX_COLS];
+    const uint32_t* id_in;
+    uint32_t* id_out;
+    int ncols;
+};
+
+// Records of the 32 stars base .. base+31 (< n), written by one warp.  Lane l owns slot l & 7 (its source
+// array is chosen once) and, in each of 8 steps, star 4*step + (l >> 3): every load instruction reads one
+// full sector from each array, every store instruction writes 256 contiguous bytes.
+__device__ __forceinline__ void write_records_32(const double* __restrict__ r, const PkCols& g, double* __restrict__ rec,
+                                                 uint32_t base, uint32_t n, uint32_t lane)
+{
+    const uint32_t slot = lane & 7, sub = lane >> 3;
+    const double* src = nullptr;
+    if (slot == 0) src = r;
+    else if ((int)slot <= g.ncols) src = g.in[slot - 1];
+    const uint32_t* src_id = ((int)slot == g.ncols + 1) ? g.id_in : nullptr;
+    double v[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        const uint32_t i = base + 4 * j + sub;
+        v[j] = 0.0;
+        if (i < n) {
+            if (src) v[j] = __ldcs(src + i);
+            else if (src_id) v[j] = __longlong_as_double((long long)(unsigned long long)__ldcs(src_id + i));
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        const uint32_t i = base + 4 * j + sub;
+        if (i < n) __stcs(rec + (size_t)i * 8 + slot, v[j]);
+    }
+}
+
+// Stand-alone record pass, needed only when no digit pass is live (all key parts equal): otherwise the
+// first live digit pass, which walks the stars in input order anyway and leaves the memory system idle,
+// writes the records of its tiles.
+__global__ void __launch_bounds__(256) sort_pk_records_kernel(const double* __restrict__ r, PkCols g, uint32_t n,
+                                                              double* __restrict__ rec, const uint32_t* __restrict__ pass_live)
+{
+    for (int p = 0; p < PK_MAXPASS; ++p)
+        if (pass_live[p]) return;
+    const uint32_t warps = (gridDim.x * blockDim.x) >> 5, gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    for (uint32_t base = gw * 32; base < n; base += warps * 32) write_records_32(r, g, rec, base, n, threadIdx.x & 31);
+}
+
 // ---- one digit pass over the packed words -------------------------------------------------------
 // Same scheme as the general sort (tiles in ticket order, stable warp-level ranking, decoupled
 // look-back over per-tile digit counts, scatter through shared memory), but 8 bytes per star.
@@ -198,7 +250,8 @@ struct PkBuffers {
 __global__ void __launch_bounds__(PK_THREADS, 2)
 sort_pk_pass_kernel(PkBuffers b, uint32_t n, const uint64_t* __restrict__ ctl,
                     const uint32_t* __restrict__ bin_offset /*[256] exclusive*/, uint32_t* __restrict__ lookback,
-                    uint32_t* __restrict__ ticket, const uint32_t* __restrict__ pass_live, int pass)
+                    uint32_t* __restrict__ ticket, const uint32_t* __restrict__ pass_live, int pass, PkCols g,
+                    double* __restrict__ rec /* nullptr: no records wanted */)
 {
     if (!pass_live[pass]) return;
     int live_before = 0;
@@ -222,6 +275,10 @@ sort_pk_pass_kernel(PkBuffers b, uint32_t n, const uint64_t* __restrict__ ctl,
     if (tile >= tiles) break;
     const uint32_t tile_base = tile * PK_TILE;
     const uint32_t valid = min((uint32_t)PK_TILE, n - tile_base);
+    if (first && rec) {                                         // the star records of this tile (input order)
+        for (int round = 0; round < PK_ITEMS; ++round)
+            write_records_32(reinterpret_cast<const double*>(b.keys_src), g, rec, tile_base + warp * (32 * PK_ITEMS) + round * 32, n, lane);
+    }
 
     // load, warp-striped: item i of lane l sits at tile position warp*256 + i*32 + l
     uint64_t w[PK_ITEMS];
@@ -303,49 +360,6 @@ sort_pk_pass_kernel(PkBuffers b, uint32_t n, const uint64_t* __restrict__ ctl,
         }
     }
     }   // tile loop
-}
-
-// ---- 64-byte star records -------------------------------------------------------------------------
-// record i = { r_i, cols[0][i], ..., cols[ncols-1][i], (uint32) id_i, padding }, ncols <= PK_REC_COLS
-static constexpr int PK_REC_COLS = 6;
-
-struct PkCols {
-    const double* in[HMC_MAX_COLS];
-    double* out[HMC_MAX_COLS];
-    const uint32_t* id_in;
-    uint32_t* id_out;
-    int ncols;
-};
-
-// Lane l of a warp owns slot l & 7 (its source array is chosen once) and, in each of the 8 steps
-// of a round, star 4*step + (l >> 3) of the warp's 32: every load instruction reads one full
-// sector from each array, every store instruction writes 256 contiguous bytes.
-__global__ void __launch_bounds__(256) sort_pk_records_kernel(const double* __restrict__ r, PkCols g, uint32_t n,
-                                                              double* __restrict__ rec)
-{
-    const uint32_t lane = threadIdx.x & 31, slot = lane & 7, sub = lane >> 3;
-    const double* src = nullptr;
-    if (slot == 0) src = r;
-    else if ((int)slot <= g.ncols) src = g.in[slot - 1];
-    const uint32_t* src_id = ((int)slot == g.ncols + 1) ? g.id_in : nullptr;
-    const uint32_t warps = (gridDim.x * blockDim.x) >> 5, gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    for (uint32_t base = gw * 32; base < n; base += warps * 32) {
-        double v[8];
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            const uint32_t i = base + 4 * j + sub;
-            v[j] = 0.0;
-            if (i < n) {
-                if (src) v[j] = __ldcs(src + i);
-                else if (src_id) v[j] = __longlong_as_double((long long)(unsigned long long)__ldcs(src_id + i));
-            }
-        }
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            const uint32_t i = base + 4 * j + sub;
-            if (i < n) __stcs(rec + (size_t)i * 8 + slot, v[j]);
-        }
-    }
 }
 
 // ---- final kernel: resolve runs, move the records ---------------------------------------------------
@@ -457,10 +471,6 @@ hmc_status sort_fast(uint64_t n, const double* r_in, double* r_sorted, uint32_t*
     g.id_in = id_in; g.id_out = id_out;
     const bool use_rec = (ncols > 0 || id_in) && ncols <= PK_REC_COLS;
     const int copy_blocks = (int)umin64((n + 255) / 256, (uint64_t)sms * 8);
-    if (use_rec) {
-        sort_pk_records_kernel<<<copy_blocks, 256, 0, st>>>(r_in, g, (uint32_t)n, reinterpret_cast<double*>(ws.rec));
-        HMC_LAUNCH_CHECK();
-    }
     static bool attr_done = false;
     if (!attr_done) {
         HMC_CUDA_TRY(cudaFuncSetAttribute(sort_pk_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PkSmem)));
@@ -477,7 +487,11 @@ hmc_status sort_fast(uint64_t n, const double* r_in, double* r_sorted, uint32_t*
     for (int p = 0; p < npass; ++p) {
         sort_pk_pass_kernel<<<(int)umin64(tiles, (uint64_t)sms * 2), PK_THREADS, sizeof(PkSmem), st>>>(b, (uint32_t)n, ws.sortctl, ws.pk_hist + p * PK_RADIX,
                                                                        ws.lookback + (size_t)p * tiles * PK_RADIX,
-                                                                       ws.pk_tickets + p, pass_live, p);
+                                                                       ws.pk_tickets + p, pass_live, p, g, use_rec ? reinterpret_cast<double*>(ws.rec) : nullptr);
+        HMC_LAUNCH_CHECK();
+    }
+    if (use_rec) {                                                          // returns at once unless no pass was live
+        sort_pk_records_kernel<<<copy_blocks, 256, 0, st>>>(r_in, g, (uint32_t)n, reinterpret_cast<double*>(ws.rec), pass_live);
         HMC_LAUNCH_CHECK();
     }
     if (use_rec)
