@@ -60,13 +60,16 @@ def measured_peak_gbs():
 
 
 def ncu_traffic_bytes(kernel: str, n: int):
-    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture, if any."""
-    p = os.path.join(ROOT, "profiles", "dram_traffic.json")
+    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture (profiles/dram_traffic.csv), if any."""
+    p = os.path.join(ROOT, "profiles", "dram_traffic.csv")
     try:
-        rec = json.load(open(p))
-        return rec.get(str(n), {}).get(kernel)
+        for line in open(p):
+            f = line.strip().split(",")
+            if len(f) == 3 and f[0] == str(n) and f[1].split("<")[0] == kernel:
+                return int(f[2])
     except Exception:
-        return None
+        pass
+    return None
 
 
 # --------------------------------------------------------------------------- clocks
