@@ -77,7 +77,9 @@ enum {
     HMC_NCOUNTERS
 };
 
-/* Bytes of scratch any of the calls below may need for n stars (the maximum over the calls). */
+/* Bytes of scratch any of the calls below may need for n stars (the maximum over the calls; about
+ * 132 bytes per star: the sort's packed words and 64-byte star records, the 32-byte search nodes of the
+ * orbit calls, their radius directory, and S3's per-star bound for S4). */
 HMC_API size_t hmc_workspace_bytes(uint64_t n);
 
 /* Static string for a status code. */
@@ -157,8 +159,10 @@ HMC_API hmc_status hmc_orbit_turning_points(uint64_t n, double G,
  *   reuse_tables  S3 and S4 search the same tables, which each call derives from (r_sorted, phi,
  *            m_cum, G) into the workspace.  Non-zero: the caller states that the immediately
  *            preceding libhmc call on this workspace was hmc_orbit_turning_points with the same
- *            n, G, r_sorted, phi and m_cum (contents unchanged), so the tables are still there and
- *            are not rebuilt.  Zero: always correct.
+ *            n, G, r_sorted, phi and m_cum and the same per-star inputs (contents unchanged), so the
+ *            tables are still there and are not rebuilt, and the rejection bound F of every star,
+ *            which that call also left in the workspace, is read instead of recomputed from two more
+ *            table look-ups per star (same expressions, same bits).  Zero: always correct.
  */
 HMC_API hmc_status hmc_sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step,
         const double* r_sorted, const double* phi, const double* m_cum,
