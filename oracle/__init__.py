@@ -152,6 +152,18 @@ def diagnostics(r, v_r, v_t, m, phi, m_cum, fractions=(), G=1.0):
     return d
 
 
+def energy_correction(r, phi, m_cum, E_old, r_old, p_old, v_r, v_t, G=1.0):
+    """Energy correction for the time-varying potential, arrays in the NEW sorted order.
+    -> (v_r', v_t', status)"""
+    r, phi, m_cum, E_old, r_old, p_old, v_r, v_t = map(_f64, (r, phi, m_cum, E_old, r_old, p_old, v_r, v_t))
+    n = r.shape[0]
+    vro, vto, st = np.empty(n), np.empty(n), np.empty(n, np.uint8)
+    rc = lib().hmc_ref_energy_correction(ctypes.c_uint64(n), ctypes.c_double(G), _p(r), _p(phi), _p(m_cum), _p(E_old),
+                                         _p(r_old), _p(p_old), _p(v_r), _p(v_t), _p(vro), _p(vto), _p(st))
+    assert rc == 0
+    return vro, vto, st
+
+
 def orbit_step(r, v_r, v_t, m, ids, seed, step, G=1.0, sample=None):
     """One pass of the whole path: sort -> potential -> turning points -> new radius.
 

@@ -30,6 +30,9 @@
  *                 acceptance rate, order independence
  *   diagnostics : exact rational pair sums for T and W, numpy searchsorted for the
  *                 Lagrange radii, two-star hand case, Plummer closed forms, scaling laws
+ *   energy corr.: exact invariance of T + W over a corrected step (pair-sum symmetry
+ *                 of the shell potential), identity when the potential does not change,
+ *                 v_r/v_t preserved, ten-step drift against the uncorrected run
  * No function in this file is "parity unpinned".
  */
 #include <math.h>
@@ -404,5 +407,57 @@ int hmc_ref_diagnostics(uint64_t n, double G, const double *r, const double *v_r
     out[5] = rh;
     out[6] = ((0.138 * (double)n) / log(0.1 * (double)n)) * sqrt(((rh * rh) * rh) / (G * M));
     for (int i = 0; i < nfrac; ++i) out[7 + i] = lagrange_radius(n, r, m_cum, fractions[i]);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------ */
+/* Energy correction for the time-varying potential ("corrections */
+/* are made to the kinetic energy of each particle that account for the fact  */
+/* that the new orbit has been calculated in the old potential ... adjusting   */
+/* the stellar velocities according to the mechanical work done on the stellar */
+/* orbit by the time varying potential ... such that the ratio v_r/v_t is      */
+/* preserved"; formula deferred to Stodolkiewicz 1982 / Fregeau & Rasio 2007,  */
+/* not in the paper's text).  SURVEY.md 8(f) item 2.  Reading DESIGN.md R18:   */
+/* dE/dt = dPhi/dt along the orbit, integrated over the step by the mean of    */
+/* the potential change at the two positions known, the old and the new one:   */
+/*   dE = 1/2 [ (Phi'(r_old) - Phi(r_old)) + (Phi'(r_new) - Phi(r_new)) ]      */
+/* Phi = potential the orbit was drawn in (previous step), Phi' = potential of */
+/* the new configuration.  With the shell potential this makes the total       */
+/* energy T + W exactly invariant: sum_i m_i Phi'(r_old,i) and                 */
+/* sum_i m_i Phi(r_new,i) are the same double sum over pairs.                  */
+/* Arrays are in the NEW radius-sorted order, star k at node k:                */
+/*   r, phi, m_cum  the new table (Phi'(r_new) of star k is phi[k]);            */
+/*   E_old          the star's energy in the old potential (S3's E);            */
+/*   r_old, p_old   its previous radius and Phi(r_old) (the old table at its    */
+/*                  own node), carried through the sort;                        */
+/*   v_r, v_t       the velocities S4 gave it.                                  */
+/* Phi(r_new) is taken from the draw's energy identity, Phi(r_new) = E_old - K, */
+/* K = (v_r^2 + v_t^2)/2; Phi'(r_old) by Eq. 6 (anchored, R3) in the new table. */
+/* New kinetic energy K' = (E_old + dE) - Phi'(r_new); both velocity components */
+/* are scaled by sqrt(K'/K).  K' <= 0 or K <= 0: flag ST_NOKINETIC, unchanged.  */
+/* ------------------------------------------------------------------------ */
+#define ST_NOKINETIC 64u
+
+int hmc_ref_energy_correction(uint64_t n, double G, const double *r, const double *phi, const double *m_cum,
+                              const double *E_old, const double *r_old, const double *p_old,
+                              const double *v_r, const double *v_t,
+                              double *v_r_out, double *v_t_out, uint8_t *status_out)
+{
+    table T = { n, G, r, phi, m_cum };
+    for (uint64_t a = 0; a < n; ++a) {
+        double vr = v_r[a], vt = v_t[a];
+        double K = 0.5 * (vr * vr + vt * vt);
+        double pn = E_old[a] - K;                                /* Phi(r_new) */
+        uint64_t j = shell_of(&T, r_old[a], 0, n);
+        double po2 = phi_in_shell(&T, j, r_old[a]);              /* Phi'(r_old) */
+        double dE = 0.5 * ((po2 - p_old[a]) + (phi[a] - pn));
+        double Kp = (E_old[a] + dE) - phi[a];
+        unsigned st = 0;
+        if (Kp > 0.0 && K > 0.0) {
+            double lam = sqrt(Kp / K);
+            vr = lam * vr; vt = lam * vt;
+        } else st |= ST_NOKINETIC;
+        v_r_out[a] = vr; v_t_out[a] = vt; status_out[a] = (uint8_t)st;
+    }
     return 0;
 }
