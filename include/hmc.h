@@ -67,13 +67,14 @@ typedef int32_t hmc_status;
 #define HMC_STAR_CIRCULAR    8u   /* r_max - r_min <= 0 or end slopes of the wrong sign; no draw    */
 #define HMC_STAR_MAXTRIES   16u   /* rejection loop reached HMC_T_MAX trials                        */
 #define HMC_STAR_CLIPPED    32u   /* some trial had g > F (density clipped there); draw still valid */
+#define HMC_STAR_NOKINETIC  64u   /* energy correction: corrected kinetic energy <= 0; velocities kept */
 
 #define HMC_T_MAX   4096u         /* cap on rejection trials per star (R7)        */
 
 /* device counters accumulated (atomically) by the orbit calls; the caller zeroes them */
 enum {
     HMC_CNT_UNBOUND = 0, HMC_CNT_RADIAL, HMC_CNT_DEGENERATE, HMC_CNT_CIRCULAR,
-    HMC_CNT_MAXTRIES, HMC_CNT_CLIPPED, HMC_CNT_TRIALS, HMC_CNT_RESERVED,
+    HMC_CNT_MAXTRIES, HMC_CNT_CLIPPED, HMC_CNT_TRIALS, HMC_CNT_NOKINETIC,
     HMC_NCOUNTERS
 };
 
@@ -189,6 +190,31 @@ HMC_API hmc_status hmc_orbit_step(uint64_t n, double G, uint64_t seed, uint32_t 
         uint32_t* k_min, uint32_t* k_max, uint8_t* star_status,
         double* r_new, double* v_r_new, double* v_t_new, uint16_t* n_try,
         uint8_t* star_status_out, uint64_t* counters,
+        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * Energy correction for the time-varying potential (R18):
+ * a star's new orbit was drawn in the potential Phi of the previous step; once the potential Phi' of the new
+ * configuration is known its energy is changed by the work done by the changing potential,
+ *     dE = 1/2 [ (Phi'(r_old) - Phi(r_old)) + (Phi'(r_new) - Phi(r_new)) ],
+ * and both velocity components are scaled by the same factor so that v_r / v_t is preserved.  With the shell
+ * potential this leaves T + W of the whole cluster exactly unchanged over the step.
+ * Call it after hmc_sort_by_radius and hmc_potential of the NEW configuration, before hmc_orbit_turning_points.
+ * All arrays are [n] in the new sorted order (star k at node k):
+ *   r_sorted, phi, m_cum   the new table; Phi'(r_new) of star k is phi[k]
+ *   E_old                  the star's energy in the old potential (E of the previous step's S3)
+ *   r_old, phi_old         its previous radius and the old potential there (previous step's r_sorted and phi
+ *                          at its then node)            -- these three travel through the sort as columns
+ *   v_r, v_t               the velocities the previous step's S4 gave it
+ *   v_r_out, v_t_out       corrected velocities; star_status_out: 0, or HMC_STAR_NOKINETIC when the corrected
+ *                          kinetic energy is not positive (velocities copied through, counted)
+ * Phi(r_new) is taken from the draw's energy identity, Phi(r_new) = E_old - (v_r^2 + v_t^2)/2.
+ */
+HMC_API hmc_status hmc_energy_correction(uint64_t n, double G,
+        const double* r_sorted, const double* phi, const double* m_cum,
+        const double* E_old, const double* r_old, const double* phi_old,
+        const double* v_r, const double* v_t,
+        double* v_r_out, double* v_t_out, uint8_t* star_status_out, uint64_t* counters,
         void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*

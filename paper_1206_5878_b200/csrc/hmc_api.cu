@@ -218,6 +218,24 @@ hmc_status hmc_orbit_step(uint64_t n, double G, uint64_t seed, uint32_t step, co
                       static_cast<cudaStream_t>(cuda_stream));
 }
 
+hmc_status hmc_energy_correction(uint64_t n, double G, const double* r_sorted, const double* phi, const double* m_cum,
+                                 const double* E_old, const double* r_old, const double* phi_old, const double* v_r,
+                                 const double* v_t, double* v_r_out, double* v_t_out, uint8_t* star_status_out,
+                                 uint64_t* counters, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (n > HMC_MAX_N) return HMC_ERR_SIZE;
+    if (n == 0) return HMC_OK;
+    REQUIRE_PTR(r_sorted); REQUIRE_PTR(phi); REQUIRE_PTR(m_cum); REQUIRE_PTR(E_old); REQUIRE_PTR(r_old); REQUIRE_PTR(phi_old);
+    REQUIRE_PTR(v_r); REQUIRE_PTR(v_t); REQUIRE_PTR(v_r_out); REQUIRE_PTR(v_t_out); REQUIRE_PTR(star_status_out);
+    REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(phi, 8); REQUIRE_ALIGN(m_cum, 8); REQUIRE_ALIGN(E_old, 8); REQUIRE_ALIGN(r_old, 8);
+    REQUIRE_ALIGN(phi_old, 8); REQUIRE_ALIGN(v_r, 8); REQUIRE_ALIGN(v_t, 8); REQUIRE_ALIGN(v_r_out, 8); REQUIRE_ALIGN(v_t_out, 8);
+    if (counters) REQUIRE_ALIGN(counters, 8);
+    hmc_status s = check_ws(workspace, workspace_bytes, n);
+    if (s != HMC_OK) return s;
+    return energy_correction(n, G, r_sorted, phi, m_cum, E_old, r_old, phi_old, v_r, v_t, v_r_out, v_t_out, star_status_out,
+                             counters, carve(workspace, n), static_cast<cudaStream_t>(cuda_stream));
+}
+
 hmc_status hmc_diagnostics(uint64_t n, double G, const double* r_sorted, const double* v_r, const double* v_t,
                            const double* m_sorted, const double* phi, const double* m_cum, int32_t nfrac,
                            const double* mass_fractions, double* out, void* workspace, size_t workspace_bytes,

@@ -210,6 +210,10 @@ hmc_status orbit_step(uint64_t n, double G, uint64_t seed, uint32_t step, const 
                       double* r_new, double* v_r_new, double* v_t_new, uint16_t* n_try, uint8_t* status_out,
                       uint64_t* counters, const Workspace& ws, cudaStream_t st);
 
+hmc_status energy_correction(uint64_t n, double G, const double* r, const double* phi, const double* m_cum,
+                             const double* E_old, const double* r_old, const double* p_old, const double* v_r,
+                             const double* v_t, double* v_r_out, double* v_t_out, uint8_t* status_out,
+                             uint64_t* counters, const Workspace& ws, cudaStream_t st);
 hmc_status diagnostics(uint64_t n, double G, const double* r, const double* v_r, const double* v_t, const double* m,
                        const double* phi, const double* m_cum, int nfrac, const double* fractions, double* out,
                        const Workspace& ws, cudaStream_t st);

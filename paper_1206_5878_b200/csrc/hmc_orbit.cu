@@ -763,6 +763,53 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
     }
 }
 
+// ---- energy correction for the time-varying potential (R18) ------------------
+// Per star, in the NEW sorted order: Phi'(r_old) from the new table (coarse interval by bisection in
+// shared memory, node by the directory, Eq. 6 anchored at the node), then the oracle's expressions.
+__global__ void __launch_bounds__(ORB_THREADS, 1)
+energy_correction_kernel(uint32_t n, const Node* __restrict__ nodes, const double2* __restrict__ coarse_g,
+                         const uint32_t* __restrict__ dir, int shift, const double* __restrict__ r,
+                         const double* __restrict__ phi, const double* __restrict__ E_old,
+                         const double* __restrict__ r_old, const double* __restrict__ p_old,
+                         const double* __restrict__ v_r, const double* __restrict__ v_t, double* __restrict__ v_r_out,
+                         double* __restrict__ v_t_out, uint8_t* __restrict__ status_out,
+                         unsigned long long* __restrict__ counters)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2* coarse = reinterpret_cast<double2*>(smem_raw);
+    stage_coarse(coarse, coarse_g, n, shift);
+    Tables T{ nodes, dir, coarse, nullptr, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift };
+    const uint32_t stride = gridDim.x * ORB_THREADS;
+    for (uint32_t a = blockIdx.x * ORB_THREADS + threadIdx.x; a < n; a += stride) {
+        const double x = __ldcs(r_old + a);
+        double vr = __ldcs(v_r + a), vt = __ldcs(v_t + a);
+        const double E = __ldcs(E_old + a), po = __ldcs(p_old + a), ph = __ldcs(phi + a);
+        // shell of r_old in the new table: j = #{ i : r_i <= x }, 0 .. n
+        const uint32_t c = coarse_locate(coarse, 0u, T.ncoarse, x);
+        uint32_t lo, hi;
+        if (shift == 0) { lo = c; hi = c + 1; }
+        else T.dir_range(c, x, lo, hi);
+        Node e = ld_node(nodes + lo);
+        while (hi - lo > 1) {
+            const uint32_t p = (hi - lo > 4) ? lo + (hi - lo) / 2 : lo + 1;
+            const Node ep = ld_node(nodes + p);
+            if (ep.r <= x) { lo = p; e = ep; } else hi = p;
+        }
+        const double po2 = e.phi - e.B * (1.0 / x - e.u);                  // Phi'(r_old), Eq. 6 anchored (R3)
+        const double K = 0.5 * (vr * vr + vt * vt);
+        const double pn = E - K;                                           // Phi(r_new): the draw's energy identity
+        const double dE = 0.5 * ((po2 - po) + (ph - pn));
+        const double Kp = (E + dE) - ph;
+        unsigned st = 0;
+        if (Kp > 0.0 && K > 0.0) {
+            const double lam = sqrt(Kp / K);
+            vr = lam * vr; vt = lam * vt;
+        } else st |= HMC_STAR_NOKINETIC;
+        __stcs(v_r_out + a, vr); __stcs(v_t_out + a, vt); status_out[a] = (uint8_t)st;
+        if (st && counters) atomicAdd(counters + HMC_CNT_NOKINETIC, 1ull);
+    }
+}
+
 // ---- host side --------------------------------------------------------------------------------
 static hmc_status build_tables(uint64_t n, double G, const double* r, const double* phi, const double* m_cum,
                                const Workspace& ws, int shift, cudaStream_t st)
@@ -849,6 +896,30 @@ hmc_status sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step,
     io.r_new = r_new; io.v_r_new = v_r_new; io.v_t_new = v_t_new; io.n_try = n_try; io.status_out = status_out;
     io.counters = reinterpret_cast<unsigned long long*>(counters);
     return launch_sampler(false, n, G, seed, step, shift, io, ws, st);
+}
+
+hmc_status energy_correction(uint64_t n, double G, const double* r, const double* phi, const double* m_cum,
+                             const double* E_old, const double* r_old, const double* p_old, const double* v_r,
+                             const double* v_t, double* v_r_out, double* v_t_out, uint8_t* status_out,
+                             uint64_t* counters, const Workspace& ws, cudaStream_t st)
+{
+    const int sms = sm_count();
+    const int shift = coarse_shift(n);
+    const size_t smem = ((n >> shift) + 2) * sizeof(double2);
+    static bool attr_done = false;
+    if (!attr_done) {
+        HMC_CUDA_TRY(cudaFuncSetAttribute(energy_correction_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)(COARSE_CAP * sizeof(double2))));
+        attr_done = true;
+    }
+    hmc_status s = build_tables(n, G, r, phi, m_cum, ws, shift, st);
+    if (s != HMC_OK) return s;
+    const int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
+    energy_correction_kernel<<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, ws.nodes, ws.coarse, ws.dir, shift, r, phi, E_old,
+                                                               r_old, p_old, v_r, v_t, v_r_out, v_t_out, status_out,
+                                                               reinterpret_cast<unsigned long long*>(counters));
+    HMC_LAUNCH_CHECK();
+    return HMC_OK;
 }
 
 // S3 + S4 in one launch: same outputs as the two calls.

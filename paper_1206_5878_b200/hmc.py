@@ -20,8 +20,8 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libhmc.so")
 
-ST_UNBOUND, ST_RADIAL, ST_DEGENERATE, ST_CIRCULAR, ST_MAXTRIES, ST_CLIPPED = 1, 2, 4, 8, 16, 32
-COUNTER_NAMES = ("unbound", "radial", "degenerate", "circular", "maxtries", "clipped", "trials", "reserved")
+ST_UNBOUND, ST_RADIAL, ST_DEGENERATE, ST_CIRCULAR, ST_MAXTRIES, ST_CLIPPED, ST_NOKINETIC = 1, 2, 4, 8, 16, 32, 64
+COUNTER_NAMES = ("unbound", "radial", "degenerate", "circular", "maxtries", "clipped", "trials", "nokinetic")
 NCOUNTERS = 8
 MAX_N = 1 << 28
 
@@ -48,7 +48,7 @@ def lib() -> ctypes.CDLL:
         L.hmc_status_string.argtypes = [ctypes.c_int32]
         L.hmc_version.restype = ctypes.c_int32
         for name in ("hmc_sort_by_radius", "hmc_potential", "hmc_orbit_turning_points", "hmc_sample_new_radius",
-                     "hmc_orbit_step", "hmc_diagnostics", "hmc_step_host"):
+                     "hmc_orbit_step", "hmc_diagnostics", "hmc_energy_correction", "hmc_step_host"):
             getattr(L, name).restype = ctypes.c_int32
         _lib = L
     return _lib
@@ -212,6 +212,26 @@ def hmc_orbit_step(r_sorted, v_r, v_t, phi, m_cum, ids, seed: int, step: int, G:
     return tp, out
 
 
+def hmc_energy_correction(r_sorted, phi, m_cum, E_old, r_old, phi_old, v_r, v_t, G: float = 1.0, *, v_r_out=None,
+                          v_t_out=None, status=None, counters=None, workspace=None):
+    """Energy correction for the time-varying potential, arrays in the new sorted order.
+    -> (v_r', v_t', status)"""
+    n = r_sorted.numel()
+    dev = r_sorted.device
+    f = torch.float64
+    v_r_out = torch.empty(n, dtype=f, device=dev) if v_r_out is None else v_r_out
+    v_t_out = torch.empty(n, dtype=f, device=dev) if v_t_out is None else v_t_out
+    status = torch.empty(n, dtype=torch.uint8, device=dev) if status is None else status
+    workspace, wp, wb = _ws(workspace, n, dev)
+    rc = lib().hmc_energy_correction(
+        ctypes.c_uint64(n), ctypes.c_double(G), _dev(r_sorted, f, n, "r_sorted"), _dev(phi, f, n, "phi"),
+        _dev(m_cum, f, n, "m_cum"), _dev(E_old, f, n, "E_old"), _dev(r_old, f, n, "r_old"), _dev(phi_old, f, n, "phi_old"),
+        _dev(v_r, f, n, "v_r"), _dev(v_t, f, n, "v_t"), _dev(v_r_out, f, n, "v_r_out"), _dev(v_t_out, f, n, "v_t_out"),
+        _dev(status, torch.uint8, n, "status"), _dev(counters, torch.int64, NCOUNTERS, "counters"), wp, wb, _stream())
+    _check(rc, "hmc_energy_correction")
+    return v_r_out, v_t_out, status
+
+
 DIAG_NAMES = ("M", "T", "W", "E_tot", "virial_ratio", "r_h", "t_rh")
 DIAG_MAX_FRACTIONS = 16
 
@@ -262,10 +282,15 @@ class OrbitStepper:
     (r, v_r, v_t, m, id) and every intermediate; ``step()`` makes the four C-ABI calls on the
     current stream and swaps (r, v_r, v_t) <- (r_new, v_r', v_t'); m and id follow the sort."""
 
-    def __init__(self, r, v_r, v_t, m, ids, seed: int, G: float = 1.0, with_n_try: bool = True):
+    def __init__(self, r, v_r, v_t, m, ids, seed: int, G: float = 1.0, with_n_try: bool = True,
+                 energy_correction: bool = False):
+        """energy_correction=True: from the second step on, hmc_energy_correction adjusts the velocities
+        between the potential and the turning points; three more columns (the star's energy,
+        previous radius and the previous potential there) then travel through the sort."""
         self.n = n = r.numel()
         dev = r.device
         self.G, self.seed, self.step_index = G, seed, 0
+        self.energy_correction = energy_correction
         self.state = dict(r=r.clone(), v_r=v_r.clone(), v_t=v_t.clone(), m=m.clone(), id=ids.clone())
         f = dict(dtype=torch.float64, device=dev)
         self.sorted = dict(r=torch.empty(n, **f), v_r=torch.empty(n, **f), v_t=torch.empty(n, **f),
@@ -277,14 +302,30 @@ class OrbitStepper:
         self.sample = alloc_sample(n, dev, with_n_try)
         self.counters = alloc_counters(dev)
         self.workspace = alloc_workspace(n, dev)
+        if energy_correction:
+            for k in ("E", "r_old", "p_old"):
+                self.state[k] = torch.zeros(n, **f)
+                self.sorted[k] = torch.empty(n, **f)
+            self.corrected = dict(v_r=torch.empty(n, **f), v_t=torch.empty(n, **f),
+                                  status=torch.empty(n, dtype=torch.uint8, device=dev))
 
     def step(self, fused: bool = False):
         """One orbit step.  fused=False: the four C-ABI calls; fused=True: S3 and S4 as the single
         call hmc_orbit_step (same results)."""
         s, so = self.state, self.sorted
-        hmc_sort_by_radius(s["r"], (s["v_r"], s["v_t"], s["m"]), s["id"], r_sorted=so["r"], perm=so["perm"],
-                           cols_out=(so["v_r"], so["v_t"], so["m"]), ids_out=so["id"], workspace=self.workspace)
+        correct = self.energy_correction and self.step_index > 0
+        extra = ("E", "r_old", "p_old") if correct else ()
+        hmc_sort_by_radius(s["r"], (s["v_r"], s["v_t"], s["m"]) + tuple(s[k] for k in extra), s["id"], r_sorted=so["r"],
+                           perm=so["perm"], cols_out=(so["v_r"], so["v_t"], so["m"]) + tuple(so[k] for k in extra),
+                           ids_out=so["id"], workspace=self.workspace)
         hmc_potential(so["r"], so["m"], self.G, phi=self.phi, m_cum=self.m_cum, workspace=self.workspace)
+        if correct:
+            co = self.corrected
+            hmc_energy_correction(so["r"], self.phi, self.m_cum, so["E"], so["r_old"], so["p_old"], so["v_r"], so["v_t"],
+                                  self.G, v_r_out=co["v_r"], v_t_out=co["v_t"], status=co["status"],
+                                  counters=self.counters, workspace=self.workspace)
+            so["v_r"], co["v_r"] = co["v_r"], so["v_r"]
+            so["v_t"], co["v_t"] = co["v_t"], so["v_t"]
         if fused:
             hmc_orbit_step(so["r"], so["v_r"], so["v_t"], self.phi, self.m_cum, so["id"], self.seed, self.step_index,
                            self.G, tp=self.tp, out=self.sample, counters=self.counters, workspace=self.workspace)
@@ -301,6 +342,10 @@ class OrbitStepper:
         s["v_t"], sm["v_t_new"] = sm["v_t_new"], s["v_t"]
         s["m"], so["m"] = so["m"], s["m"]
         s["id"], so["id"] = so["id"], s["id"]
+        if self.energy_correction:      # what the next step's correction needs: E in this potential, r and Phi here
+            s["E"].copy_(self.tp["E"])
+            s["r_old"].copy_(so["r"])
+            s["p_old"].copy_(self.phi)
         self.step_index += 1
 
     def diagnostics(self, fractions=()):

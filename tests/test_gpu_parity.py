@@ -374,3 +374,64 @@ def test_stepper_diagnostics_after_a_step(oracle):
     out = host(st.diagnostics([0.1, 0.5]))
     assert [out[i] for i in range(6)] == [od[k] for k in hmc.DIAG_NAMES[:6]]
     assert np.array_equal(out[7:], od["lagrange"])
+
+
+# ----------------------------------------------------------------------------- energy correction
+def _second_configuration(oracle, n, seed, masses):
+    """Oracle: one step, then sort + potential of the new configuration, with the three carried columns."""
+    c = inputs.plummer(n, seed, masses)
+    o = oracle_chain(oracle, c, seed, 0)
+    sm, tp = o["sample"], o["tp"]
+    rs, perm, cs, ids = oracle.sort_by_radius(sm["r_new"], (sm["v_r_new"], sm["v_t_new"], o["m"], tp["E"], o["r"], o["phi"]), o["id"])
+    phi, mc = oracle.potential(rs, cs[2])
+    return rs, phi, mc, cs
+
+
+@pytest.mark.parametrize("n,masses", [(1, "equal"), (3, "equal"), (100_000, "equal"), (250_007, "salpeter")])
+def test_energy_correction_matches_oracle(oracle, n, masses):
+    """Same expressions, correctly rounded operations: the corrected velocities and the flags are bit-identical."""
+    rs, phi, mc, (vrs, vts, ms, E, r_old, p_old) = _second_configuration(oracle, n, 23, masses)
+    o_vr, o_vt, o_st = oracle.energy_correction(rs, phi, mc, E, r_old, p_old, vrs, vts)
+    counters = hmc.alloc_counters()
+    vr, vt, st = hmc.hmc_energy_correction(dev(rs), dev(phi), dev(mc), dev(E), dev(r_old), dev(p_old), dev(vrs), dev(vts),
+                                           counters=counters)
+    assert np.array_equal(host(st), o_st)
+    assert np.array_equal(host(vr), o_vr) and np.array_equal(host(vt), o_vt)
+    assert host(counters)[hmc.COUNTER_NAMES.index("nokinetic")] == int((o_st != 0).sum())
+    # r_old inside the innermost star and beyond the outermost one (shells 0 and N of the new table)
+    if n >= 3:
+        r_old2 = r_old.copy(); r_old2[0] = rs[0] * 0.5; r_old2[-1] = rs[-1] * 3.0
+        o2 = oracle.energy_correction(rs, phi, mc, E, r_old2, p_old, vrs, vts)
+        g2 = hmc.hmc_energy_correction(dev(rs), dev(phi), dev(mc), dev(E), dev(r_old2), dev(p_old), dev(vrs), dev(vts))
+        assert np.array_equal(host(g2[0]), o2[0]) and np.array_equal(host(g2[1]), o2[1]) and np.array_equal(host(g2[2]), o2[2])
+
+
+def test_stepper_with_energy_correction_conserves_total_energy(oracle):
+    """Three chained steps with the correction on: T + W from hmc_diagnostics stays put (to the shortfall of the
+    few flagged stars), and the state equals an oracle chain of the same calls."""
+    n, seed = 60_000, 29
+    c = inputs.plummer(n, seed)
+    st = hmc.OrbitStepper(dev(c["r"]), dev(c["v_r"]), dev(c["v_t"]), dev(c["m"]), dev(c["id"].view(np.int32)), seed,
+                          energy_correction=True)
+    state = {k: c[k] for k in ("r", "v_r", "v_t", "m", "id")}
+    e = []
+    for step in range(3):
+        st.step()
+        e.append(host(st.diagnostics())[3])
+        # oracle: the same step
+        have = "E" in state
+        cols = [state["v_r"], state["v_t"], state["m"]] + ([state["E"], state["r_old"], state["p_old"]] if have else [])
+        rs, perm, cs, ids = oracle.sort_by_radius(state["r"], tuple(cols), state["id"])
+        vrs, vts, ms = cs[0], cs[1], cs[2]
+        phi, mc = oracle.potential(rs, ms)
+        if have:
+            vrs, vts, _ = oracle.energy_correction(rs, phi, mc, cs[3], cs[4], cs[5], vrs, vts)
+        tp = oracle.orbit_turning_points(rs, vrs, vts, phi, mc)
+        sm = oracle.sample_new_radius(rs, phi, mc, rs, vrs, vts, tp["E"], tp["J"], tp["r_min"], tp["r_max"], tp["k_min"],
+                                      tp["k_max"], ids, tp["status"], seed, step)
+        state = dict(r=sm["r_new"], v_r=sm["v_r_new"], v_t=sm["v_t_new"], m=ms, id=ids, E=tp["E"], r_old=rs, p_old=phi)
+        assert np.array_equal(host(st.state["r"]), state["r"]) and np.array_equal(host(st.state["v_r"]), state["v_r"])
+        assert np.array_equal(host(st.state["v_t"]), state["v_t"])
+    nok = int(host(st.counters)[hmc.COUNTER_NAMES.index("nokinetic")])
+    assert nok < 40
+    assert abs(e[2] - e[0]) <= 2e-5 * abs(e[0])            # uncorrected: about 1e-4 per step at this N
