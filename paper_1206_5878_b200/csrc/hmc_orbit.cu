@@ -113,31 +113,43 @@ __global__ void __launch_bounds__(256) build_nodes_kernel(const double* __restri
     }
 }
 
-__global__ void __launch_bounds__(256) build_dir_kernel(const double* __restrict__ r, uint32_t* __restrict__ dir,
-                                                        uint32_t n, int shift)
+// One CTA per coarse interval: the interval's nodes are counted into their buckets in shared memory
+// (radii ascend, so neighbouring threads hit neighbouring counters), the counts are scanned, and the row
+// is written as whole 32-bit entries, coalesced.
+static constexpr int DIR_THREADS = 256;
+
+__global__ void __launch_bounds__(DIR_THREADS) build_dir_kernel(const double* __restrict__ r, uint32_t* __restrict__ dir,
+                                                                uint32_t n, int shift)
 {
-    const uint32_t K = 1u << shift;
-    const uint32_t stride = gridDim.x * blockDim.x;
-    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x + 1; j <= n; j += stride) {
-        const uint32_t c = j >> shift;
-        const uint32_t j0 = max(c << shift, 1u);                     // first node of the interval
-        const uint32_t jn = min(((c + 1) << shift) - 1, n);          // last node of the interval
-        const double Rl = c ? __ldg(r + ((c << shift) - 1)) : 0.0;
-        const double Rh = (((uint64_t)(c + 1) << shift) <= n) ? __ldg(r + (((c + 1) << shift) - 1)) : __ldg(r + (n - 1));
-        const float scale = bucket_scale(Rl, Rh, K);
-        const uint32_t b = bucket(__ldg(r + (j - 1)), Rl, scale, K);
-        const int bprev = (j > j0) ? (int)bucket(__ldg(r + (j - 2)), Rl, scale, K) : -1;
-        uint16_t* row = reinterpret_cast<uint16_t*>(dir + (size_t)c * K);   // halves: [2b] = o_b, [2b+1] = o_{b+1}
-        for (int bb = bprev + 1; bb <= (int)b; ++bb) {               // o_bb = j - j0
-            if (bb < (int)K) row[2 * bb] = (uint16_t)(j - j0);
-            if (bb > 0) row[2 * bb - 1] = (uint16_t)(j - j0);
-        }
-        if (j == jn)
-            for (uint32_t bb = b + 1; bb <= K; ++bb) {               // o_bb = number of nodes of the interval
-                if (bb < K) row[2 * bb] = (uint16_t)(j - j0 + 1);
-                row[2 * bb - 1] = (uint16_t)(j - j0 + 1);
-            }
-    }
+    extern __shared__ uint32_t cnt[];                                // [K + 1]: cnt[b + 1] = nodes in bucket b, then o_b
+    __shared__ uint32_t warp_tot[DIR_THREADS / 32];
+    const uint32_t K = 1u << shift, c = blockIdx.x;
+    const uint32_t j0 = max(c << shift, 1u);                         // first node of the interval
+    const uint32_t jn = min(((c + 1) << shift) - 1, n);              // last node of the interval
+    const double Rl = c ? __ldg(r + ((c << shift) - 1)) : 0.0;
+    const double Rh = (((uint64_t)(c + 1) << shift) <= n) ? __ldg(r + (((c + 1) << shift) - 1)) : __ldg(r + (n - 1));
+    const float scale = bucket_scale(Rl, Rh, K);
+    for (uint32_t b = threadIdx.x; b <= K; b += DIR_THREADS) cnt[b] = 0;
+    __syncthreads();
+    for (uint32_t j = j0 + threadIdx.x; j <= jn; j += DIR_THREADS) atomicAdd(&cnt[bucket(__ldcs(r + (j - 1)), Rl, scale, K) + 1], 1u);
+    __syncthreads();
+    // inclusive scan of cnt[0 .. K] in place: cnt[b] becomes o_b = number of nodes with bucket < b
+    const uint32_t per = (K + 1 + DIR_THREADS - 1) / DIR_THREADS;
+    const uint32_t b0 = min(K + 1, threadIdx.x * per), b1 = min(K + 1, b0 + per);
+    uint32_t sum = 0;
+    for (uint32_t b = b0; b < b1; ++b) sum += cnt[b];
+    uint32_t inc = sum;
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
+    if (lane == 31) warp_tot[warp] = inc;
+    __syncthreads();
+    uint32_t run = inc - sum;
+    for (uint32_t w = 0; w < warp; ++w) run += warp_tot[w];
+    for (uint32_t b = b0; b < b1; ++b) { run += cnt[b]; cnt[b] = run; }
+    __syncthreads();
+    uint32_t* row = dir + (size_t)c * K;
+    for (uint32_t b = threadIdx.x; b < K; b += DIR_THREADS) row[b] = cnt[b] | (cnt[b + 1] << 16);
 }
 
 // coarse[c] = (r, Phi) of node c << shift, c = 1..ncoarse; coarse[0] = (0, Phi_1) and
@@ -819,8 +831,13 @@ static hmc_status build_tables(uint64_t n, double G, const double* r, const doub
     build_nodes_kernel<<<blocks, 256, 0, st>>>(r, phi, m_cum, G, ws.nodes, ws.coarse, ws.mid, shift, n);
     HMC_LAUNCH_CHECK();
     if (shift > 0) {
-        blocks = (int)umin64((n + 255) / 256, (uint64_t)sms * 8);
-        build_dir_kernel<<<blocks, 256, 0, st>>>(r, ws.dir, (uint32_t)n, shift);
+        const size_t smem = ((size_t)(1u << shift) + 1) * sizeof(uint32_t);
+        static size_t attr_smem = 48 * 1024;
+        if (smem > attr_smem) {
+            HMC_CUDA_TRY(cudaFuncSetAttribute(build_dir_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            attr_smem = smem;
+        }
+        build_dir_kernel<<<(unsigned)((n >> shift) + 1), DIR_THREADS, smem, st>>>(r, ws.dir, (uint32_t)n, shift);
         HMC_LAUNCH_CHECK();
     }
     return HMC_OK;
