@@ -36,6 +36,7 @@ namespace hmc {
 
 static constexpr int ORB_THREADS = 1024;
 static constexpr int ORB_WARPS = ORB_THREADS / 32;
+static constexpr int FRONT_ROUNDS = 2;       // S4: trials a lane may run through the squeeze per exact round
 
 __device__ __forceinline__ double pos_inf() { return __longlong_as_double(0x7ff0000000000000ll); }
 
@@ -720,23 +721,35 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
             need = __ballot_sync(0xffffffffu, !have);
         }
         if (!__any_sync(0xffffffffu, have)) break;          // nothing parked, nothing left to prepare
-        // ---- one trial for every lane that holds a star
-        if (have) {
-            const Trial tr = make_trial(o, seed_lo, seed_hi, step, t);
-            const uint32_t c = coarse_locate(coarse, cl, ch, tr.r0);
-            ++t;
-            // squeeze: Phi(r0) lies in [coarse[c].Phi, coarse[c+1].Phi]; everything widened by ~1e-11.
-            // Written multiplied through by r0^2 > 0, so there is no division on this path.
-            const double r2 = tr.r0 * tr.r0;
-            const double top = 2.0 * (o.E - coarse[c].y) * r2;
-            const double tol = 1e-11 * (fabs(top) + o.J2);
-            const double Qh = (top - o.J2) + tol;                       // upper bound of r0^2 Q0
-            bool candidate = Qh > 0.0;
-            if (candidate) {
-                const double Ql = (2.0 * (o.E - coarse[c + 1].y) * r2 - o.J2) - tol;   // lower bound of r0^2 Q0
-                const double fx = o.F * tr.Xp, cc = o.three_q * (1.0 - tr.s * tr.s);
-                if (Ql > 0.0 && (fx * fx) * Ql > ((cc * cc) * r2) * (1.0 + 1e-10)) candidate = false;   // F X' > g for certain
+        // ---- up to FRONT_ROUNDS trials for every lane that holds a star, until one survives the squeeze.
+        // Half the trials are rejected by the squeeze alone; a lane whose trial was, tries its next one at
+        // once instead of idling through the other lanes' exact look-ups (which cost more than a trial's front
+        // part), so fewer of the expensive rounds are needed per star.
+        bool candidate = false;
+        Trial tr{ 0.0, 0.0, 0.0, 0u };
+        uint32_t c = 0;
+#pragma unroll 1
+        for (int round = 0; round < FRONT_ROUNDS; ++round) {
+            if (have && !candidate && t < HMC_T_MAX) {
+                tr = make_trial(o, seed_lo, seed_hi, step, t);
+                c = coarse_locate(coarse, cl, ch, tr.r0);
+                ++t;
+                // squeeze: Phi(r0) lies in [coarse[c].Phi, coarse[c+1].Phi]; everything widened by ~1e-11.
+                // Written multiplied through by r0^2 > 0, so there is no division on this path.
+                const double r2 = tr.r0 * tr.r0;
+                const double top = 2.0 * (o.E - coarse[c].y) * r2;
+                const double tol = 1e-11 * (fabs(top) + o.J2);
+                const double Qh = (top - o.J2) + tol;                       // upper bound of r0^2 Q0
+                candidate = Qh > 0.0;
+                if (candidate) {
+                    const double Ql = (2.0 * (o.E - coarse[c + 1].y) * r2 - o.J2) - tol;   // lower bound of r0^2 Q0
+                    const double fx = o.F * tr.Xp, cc = o.three_q * (1.0 - tr.s * tr.s);
+                    if (Ql > 0.0 && (fx * fx) * Ql > ((cc * cc) * r2) * (1.0 + 1e-10)) candidate = false;   // F X' > g for certain
+                }
             }
+            if (__all_sync(0xffffffffu, !have || candidate || t >= HMC_T_MAX)) break;
+        }
+        if (have) {
             bool done = false, accepted = false, have_good = false;
             double good_r = 0.0, good_Q = 0.0;
             uint32_t good_w3 = 0, used = t;
