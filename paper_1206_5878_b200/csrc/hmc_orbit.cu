@@ -190,15 +190,18 @@ struct Tables {
     }
     // Most likely last node at or below x: the nodes strictly inside dir_range's (lo, hi) share x's
     // bucket, and about the fraction of the bucket that lies below x of them are below x.  A guess only.
-    __device__ __forceinline__ uint32_t dir_guess(uint32_t c, double x) const
+    // In two halves, so that a caller with two radii can have both directory loads in flight at once.
+    __device__ __forceinline__ const uint32_t* dir_guess_slot(uint32_t c, double x, float& frac) const
     {
         const double Rl = coarse[c].x;
         const float scale = bucket_scale(Rl, interval_rh(c), K);
         const uint32_t b = bucket(x, Rl, scale, K);
-        const uint32_t w = ld_u32_na(dir + (size_t)c * K + b);
+        frac = fminf(fmaxf((float)(x - Rl) * scale - (float)b, 0.0f), 1.0f);
+        return dir + (size_t)c * K + b;
+    }
+    __device__ __forceinline__ uint32_t dir_guess_node(uint32_t c, uint32_t w, float frac) const
+    {
         const uint32_t o0 = w & 0xffffu, o1 = w >> 16;
-        float frac = (float)(x - Rl) * scale - (float)b;
-        frac = fminf(fmaxf(frac, 0.0f), 1.0f);
         return max(c << shift, 1u) + o0 - 1 + (uint32_t)(frac * (float)(o1 - o0) + 0.5f);
     }
 };
@@ -251,12 +254,10 @@ struct Side {
 };
 
 // Secant estimate of the root of P(r) = r^2 Q(r) between two nodes with P_lo and P_hi of opposite
-// sign, turned into a node number through the directory.  Only a starting point: any value works.
-__device__ __forceinline__ uint32_t guess_node(const Tables& T, uint32_t lo, uint32_t hi, double r_lo, double P_lo,
-                                               double r_hi, double P_hi)
+// sign; the directory turns it into a node number.  Only a starting point: any value works.
+__device__ __forceinline__ double secant_root(double r_lo, double P_lo, double r_hi, double P_hi)
 {
-    const double x = r_lo + (r_hi - r_lo) * (P_lo / (P_lo - P_hi));
-    return T.dir_guess(lo >> T.shift, x);
+    return r_lo + (r_hi - r_lo) * (P_lo / (P_lo - P_hi));
 }
 
 // One star of S3: brackets, turning points, status, and S4's bound F (0 = no draw).  a = position in the
@@ -331,19 +332,30 @@ __device__ __forceinline__ Solved solve_star(const Tables& T, uint32_t a, double
         // tier 2: secant guess.  The ends are table nodes or the star's own node, where
         // P = r^2 Q = (r_k v_r)^2.  The first and last intervals (a sentinel at one end) bisect.
         const double Pk = (rk * vr) * (rk * vr);
-        if (s1.hi - s1.lo > 2 && s1.lo > 0) {
+        const bool g1 = s1.hi - s1.lo > 2 && s1.lo > 0, g2 = s2.hi - s2.lo > 2 && s2.hi <= n;
+        double x1 = 0.0, x2 = 0.0;
+        if (g1) {
             double2 el = T.aligned_node(s1.lo);
             double r_hi = rk, P_hi = Pk;
             if (s1.hi != k) { double2 eh = T.aligned_node(s1.hi); r_hi = eh.x; P_hi = 2.0 * ((E - eh.y) * (eh.x * eh.x)) - J2; }
-            s1.guess = guess_node(T, s1.lo, s1.hi, el.x, 2.0 * ((E - el.y) * (el.x * el.x)) - J2, r_hi, P_hi);
-            s1.mode = MODE_GUESS;
+            x1 = secant_root(el.x, 2.0 * ((E - el.y) * (el.x * el.x)) - J2, r_hi, P_hi);
         }
-        if (s2.hi - s2.lo > 2 && s2.hi <= n) {
+        if (g2) {
             double2 eh = T.aligned_node(s2.hi);
             double r_lo = rk, P_lo = Pk;
             if (s2.lo != k) { double2 el = T.aligned_node(s2.lo); r_lo = el.x; P_lo = 2.0 * ((E - el.y) * (el.x * el.x)) - J2; }
-            s2.guess = guess_node(T, s2.lo, s2.hi, r_lo, P_lo, eh.x, 2.0 * ((E - eh.y) * (eh.x * eh.x)) - J2);
-            s2.mode = MODE_GUESS;
+            x2 = secant_root(r_lo, P_lo, eh.x, 2.0 * ((E - eh.y) * (eh.x * eh.x)) - J2);
+        }
+        {   // both directory entries in flight together
+            float f1 = 0.0f, f2 = 0.0f;
+            const uint32_t c1 = s1.lo >> shift, c2 = s2.lo >> shift;
+            const uint32_t* a1 = g1 ? T.dir_guess_slot(c1, x1, f1) : nullptr;
+            const uint32_t* a2 = g2 ? T.dir_guess_slot(c2, x2, f2) : nullptr;
+            uint32_t w1 = 0, w2 = 0;
+            if (g1) w1 = ld_u32_na(a1);
+            if (g2) w2 = ld_u32_na(a2);
+            if (g1) { s1.guess = T.dir_guess_node(c1, w1, f1); s1.mode = MODE_GUESS; }
+            if (g2) { s2.guess = T.dir_guess_node(c2, w2, f2); s2.mode = MODE_GUESS; }
         }
         // tier 3: exact probes of adjacent node pairs, the two searches interleaved
         while (true) {
