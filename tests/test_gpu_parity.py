@@ -435,3 +435,27 @@ def test_stepper_with_energy_correction_conserves_total_energy(oracle):
     nok = int(host(st.counters)[hmc.COUNTER_NAMES.index("nokinetic")])
     assert nok < 40
     assert abs(e[2] - e[0]) <= 2e-5 * abs(e[0])            # uncorrected: about 1e-4 per step at this N
+
+
+def test_twenty_step_soak_properties():
+    """Twenty chained steps of a 10^6-star cluster with the energy correction on: properties that hold at any size
+    and step (no oracle): sorted radii, the ids stay a permutation, no star flagged by S3/S4, the cluster stays in
+    virial equilibrium with a stable half-mass radius, and T + W moves only by the flagged stars' shortfall."""
+    n, seed = 1_000_000, 41
+    c = inputs.plummer(n, seed)
+    st = hmc.OrbitStepper(dev(c["r"]), dev(c["v_r"]), dev(c["v_t"]), dev(c["m"]), dev(c["id"].view(np.int32)), seed,
+                          energy_correction=True)
+    e, rh = [], []
+    for step in range(20):
+        st.step()
+        r = st.sorted["r"]
+        assert bool((r[1:] >= r[:-1]).all())
+        dg = host(st.diagnostics())
+        e.append(dg[3]); rh.append(dg[5])
+        assert abs(dg[4] - 1.0) < 0.01
+    assert torch.equal(torch.sort(st.state["id"].long())[0], torch.arange(n, device="cuda"))
+    cnt = dict(zip(hmc.COUNTER_NAMES, host(st.counters).tolist()))
+    assert cnt["unbound"] == cnt["radial"] == cnt["degenerate"] == cnt["circular"] == cnt["maxtries"] == 0
+    assert cnt["nokinetic"] < 20 * n * 1e-4 and 1.5 * 20 * n < cnt["trials"] < 2.5 * 20 * n
+    assert abs(e[-1] - e[0]) <= 2e-6 * abs(e[0])
+    assert max(rh) / min(rh) < 1.01
