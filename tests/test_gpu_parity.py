@@ -64,7 +64,7 @@ def test_sort_matches_oracle(oracle, n):
     assert np.array_equal(host(ids_s, np.uint32), o_ids)
 
 
-@pytest.mark.parametrize("kind", ["ties", "all_equal", "sorted", "reversed", "extreme", "two_values"])
+@pytest.mark.parametrize("kind", ["ties", "all_equal", "sorted", "reversed", "extreme", "two_values", "denormal", "narrow"])
 def test_sort_adversarial_keys(oracle, kind):
     g = np.random.default_rng(5)
     n = 50_001
@@ -75,6 +75,8 @@ def test_sort_adversarial_keys(oracle, kind):
         reversed=np.sort(g.random(n) + 0.5)[::-1].copy(),
         extreme=10.0 ** g.uniform(-300, 300, n),
         two_values=np.where(g.random(n) < 0.5, 1.0, 2.0),
+        denormal=np.where(g.random(n) < 0.5, g.integers(1, 1 << 40, n).astype(np.uint64).view(np.float64), 10.0 ** g.uniform(-310, -300, n)),
+        narrow=1.0 + g.integers(0, 1000, n) * 2.0 ** -52,        # a thousand adjacent doubles: long runs of exact ties
     )[kind]
     rs, perm, _, _ = hmc.hmc_sort_by_radius(dev(r))
     o_rs, o_perm, _, _ = oracle.sort_by_radius(r)
