@@ -461,3 +461,22 @@ def test_twenty_step_soak_properties():
     assert cnt["nokinetic"] < 20 * n * 1e-4 and 1.5 * 20 * n < cnt["trials"] < 2.5 * 20 * n
     assert abs(e[-1] - e[0]) <= 2e-6 * abs(e[0])
     assert max(rh) / min(rh) < 1.01
+
+
+def test_empty_inputs_are_no_ops():
+    """n = 0: every call returns HMC_OK without touching anything (include/hmc.h conventions)."""
+    f = torch.empty(0, dtype=torch.float64, device="cuda")
+    i = torch.empty(0, dtype=torch.int32, device="cuda")
+    ws = hmc.alloc_workspace(0)
+    phi, mc = hmc.hmc_potential(f, f, workspace=ws)
+    assert phi.numel() == 0 and mc.numel() == 0
+    tp = hmc.hmc_orbit_turning_points(f, f, f, f, f, workspace=ws)
+    sm = hmc.hmc_sample_new_radius(f, f, f, f, f, tp, i, 1, 0, workspace=ws)
+    assert sm["r_new"].numel() == 0
+    tp2, sm2 = hmc.hmc_orbit_step(f, f, f, f, f, i, 1, 0, workspace=ws)
+    assert sm2["r_new"].numel() == 0
+    vr, vt, st = hmc.hmc_energy_correction(f, f, f, f, f, f, f, f, workspace=ws)
+    assert vr.numel() == 0
+    with pytest.raises(hmc.HmcError):                      # the diagnostics of nothing are not defined
+        hmc.hmc_diagnostics(f, f, f, f, f, f, workspace=ws)
+    torch.cuda.synchronize()
