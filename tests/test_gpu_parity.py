@@ -480,3 +480,19 @@ def test_empty_inputs_are_no_ops():
     with pytest.raises(hmc.HmcError):                      # the diagnostics of nothing are not defined
         hmc.hmc_diagnostics(f, f, f, f, f, f, workspace=ws)
     torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("n", [10_238, 10_239, 20_476, 20_477, 40_957])
+def test_sizes_around_the_coarse_table_capacity(oracle, n):
+    """The coarse table holds every 2^shift-th node and at most 10 240 entries: n = 10 238 is the last size
+    with the whole table in shared memory (shift 0), 10 239 the first with a directory (shift 1), and so on."""
+    c = inputs.plummer(n, 5)
+    o = oracle_chain(oracle, c, 5, 0)
+    st = hmc.OrbitStepper(dev(c["r"]), dev(c["v_r"]), dev(c["v_t"]), dev(c["m"]), dev(c["id"].view(np.int32)), 5)
+    st.step()
+    assert np.array_equal(host(st.sorted["perm"], np.uint32), o["perm"])
+    assert np.array_equal(host(st.phi), o["phi"])
+    sm = dict(r_new=st.state["r"], v_r_new=st.state["v_r"], v_t_new=st.state["v_t"], n_try=st.sample["n_try"],
+              status=st.sample["status"])                  # step() swapped the new coordinates into the state
+    check_orbit_against(oracle, o, st.tp, sm, report="n=%d" % n)
+    assert np.array_equal(host(st.state["r"]), o["sample"]["r_new"])
