@@ -496,3 +496,24 @@ def test_sizes_around_the_coarse_table_capacity(oracle, n):
               status=st.sample["status"])                  # step() swapped the new coordinates into the state
     check_orbit_against(oracle, o, st.tp, sm, report="n=%d" % n)
     assert np.array_equal(host(st.state["r"]), o["sample"]["r_new"])
+
+
+@pytest.mark.parametrize("copies", [2, 5])
+def test_orbit_stages_with_tied_radii(oracle, copies):
+    """Every radius occurs `copies` times (distinct velocities and masses): nodes of equal radius, zero-width
+    shells, directory buckets holding several identical radii.  Brackets bit-exact, the rest as usual."""
+    g = np.random.default_rng(77)
+    base = inputs.plummer(60_000 // copies, 19)
+    r = np.repeat(base["r"], copies)
+    n = r.shape[0]
+    vr, vt = g.permutation(np.repeat(base["v_r"], copies)), np.abs(g.permutation(np.repeat(base["v_t"], copies))) + 1e-3
+    m = g.uniform(0.5, 1.5, n); m /= m.sum()
+    c = dict(r=r, v_r=vr, v_t=vt, m=m, id=np.arange(n, dtype=np.uint32))
+    o = oracle_chain(oracle, c, 19, 3)
+    rs, vrs, vts, phi, mc = (dev(o[k]) for k in ("r", "v_r", "v_t", "phi", "m_cum"))
+    ws = hmc.alloc_workspace(n)
+    tp = hmc.hmc_orbit_turning_points(rs, vrs, vts, phi, mc, workspace=ws)
+    sm = hmc.hmc_sample_new_radius(rs, phi, mc, vrs, vts, tp, dev(o["id"].view(np.int32)), 19, 3, workspace=ws,
+                                   reuse_tables=True)
+    check_orbit_against(oracle, o, tp, sm, report="ties x%d" % copies)
+    assert np.array_equal(host(hmc.hmc_sort_by_radius(dev(r))[1], np.uint32), o["perm"])
