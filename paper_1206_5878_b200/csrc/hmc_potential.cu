@@ -15,8 +15,8 @@
 
 namespace hmc {
 
-static constexpr int SCAN_THREADS = 256;
-static constexpr int SCAN_ITEMS = SCAN_TILE / SCAN_THREADS;   // 8
+static constexpr int SCAN_THREADS = 128;
+static constexpr int SCAN_ITEMS = SCAN_TILE / SCAN_THREADS;   // 16
 static constexpr int SCAN_WARPS = SCAN_THREADS / 32;
 static constexpr int TOT_THREADS = 1024;
 
