@@ -15,9 +15,10 @@
 // RUN_MAX sets a flag instead, and the general eight-pass sort of hmc_sort.cu, which is launched
 // after this path and returns at once when the flag is clear, redoes the call.
 //
-// Record columns: one random 8-byte read per column per star costs a 64-byte DRAM fetch each.
+// Record columns: one random 8-byte read per column per star costs a whole DRAM line each.
 // The columns are therefore first copied, coalesced, into one 64-byte record per star
-// (r, columns, id), and the final kernel fetches one record per star.
+// (r, columns, id) -- by the histogram kernel, which reads the radii anyway and is bound by
+// shared-memory atomics, not by memory -- and the final kernel fetches one record per star.
 #include "hmc_common.cuh"
 
 namespace hmc {
@@ -102,6 +103,46 @@ __global__ void __launch_bounds__(512) sort_minmax_kernel(const uint64_t* __rest
     }
 }
 
+// ---- 64-byte star records -------------------------------------------------------------------------
+// record i = { r_i, cols[0][i], ..., cols[ncols-1][i], (uint32) id_i, padding }, ncols <= PK_REC_COLS
+static constexpr int PK_REC_COLS = 6;
+
+struct PkCols {
+    const double* in[HMC_MAX_COLS];
+    double* out[HMC_MAX_COLS];
+    const uint32_t* id_in;
+    uint32_t* id_out;
+    int ncols;
+};
+
+// Records of the 32 stars base .. base+31 (< n), written by one warp.  Lane l owns slot l & 7 (its source
+// array is chosen once) and, in each of 8 steps, star 4*step + (l >> 3): every load instruction reads one
+// full sector from each array, every store instruction writes 256 contiguous bytes.
+__device__ __forceinline__ void write_records_32(const double* __restrict__ r, const PkCols& g, double* __restrict__ rec,
+                                                 uint32_t base, uint32_t n, uint32_t lane)
+{
+    const uint32_t slot = lane & 7, sub = lane >> 3;
+    const double* src = nullptr;
+    if (slot == 0) src = r;
+    else if ((int)slot <= g.ncols) src = g.in[slot - 1];
+    const uint32_t* src_id = ((int)slot == g.ncols + 1) ? g.id_in : nullptr;
+    double v[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        const uint32_t i = base + 4 * j + sub;
+        v[j] = 0.0;
+        if (i < n) {
+            if (src) v[j] = __ldcs(src + i);
+            else if (src_id) v[j] = __longlong_as_double((long long)(unsigned long long)__ldcs(src_id + i));
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        const uint32_t i = base + 4 * j + sub;
+        if (i < n) __stcs(rec + (size_t)i * 8 + slot, v[j]);
+    }
+}
+
 // ---- digit histograms of the key part, all passes in one read -------------------------------------
 static constexpr int PKH_THREADS = 512;
 static constexpr int PKH_COPIES = 4;
@@ -109,7 +150,8 @@ static constexpr int PKH_UNROLL = 4;
 
 __global__ void __launch_bounds__(PKH_THREADS) sort_pk_histogram_kernel(const uint64_t* __restrict__ keys, uint32_t n,
                                                                         const uint64_t* __restrict__ ctl,
-                                                                        uint32_t* __restrict__ hist /*[5][256]*/)
+                                                                        uint32_t* __restrict__ hist /*[5][256]*/, PkCols g,
+                                                                        double* __restrict__ rec /* nullptr: no records */)
 {
     __shared__ uint32_t sh[PKH_COPIES][PK_MAXPASS * PK_RADIX];
     for (int i = threadIdx.x; i < PKH_COPIES * PK_MAXPASS * PK_RADIX; i += PKH_THREADS) (&sh[0][0])[i] = 0;
@@ -128,6 +170,15 @@ __global__ void __launch_bounds__(PKH_THREADS) sort_pk_histogram_kernel(const ui
             const uint32_t iu = i + u * stride;
             ok[u] = (it + u < iters) && iu < n;
             kp[u] = ok[u] ? __ldcs(keys + iu) : 0ull;
+        }
+        // the star records of the same stars (this kernel waits on shared-memory atomics and leaves the
+        // memory system idle; a warp's 32 keys of one round are 32 consecutive stars)
+        if (rec) {
+            const uint32_t lane = threadIdx.x & 31;
+            for (int u = 0; u < PKH_UNROLL; ++u) {
+                const uint32_t base = i + u * stride - lane;
+                if (it + u < iters && base < n) write_records_32(reinterpret_cast<const double*>(keys), g, rec, base, n, lane);
+            }
         }
 #pragma unroll
         for (int u = 0; u < PKH_UNROLL; ++u) {
@@ -179,58 +230,6 @@ __global__ void sort_pk_scan_hist_kernel(uint32_t* __restrict__ hist, uint32_t n
     if (d == 0) pass_live[p] = single ? 0u : 1u;
 }
 
-// ---- 64-byte star records -------------------------------------------------------------------------
-// record i = { r_i, cols[0][i], ..., cols[ncols-1][i], (uint32) id_i, padding }, ncols <= PK_REC_COLS
-static constexpr int PK_REC_COLS = 6;
-
-struct PkCols {
-    const double* in[HMC_MAX_COLS];
-    double* out[HMC_MAX_COLS];
-    const uint32_t* id_in;
-    uint32_t* id_out;
-    int ncols;
-};
-
-// Records of the 32 stars base .. base+31 (< n), written by one warp.  Lane l owns slot l & 7 (its source
-// array is chosen once) and, in each of 8 steps, star 4*step + (l >> 3): every load instruction reads one
-// full sector from each array, every store instruction writes 256 contiguous bytes.
-__device__ __forceinline__ void write_records_32(const double* __restrict__ r, const PkCols& g, double* __restrict__ rec,
-                                                 uint32_t base, uint32_t n, uint32_t lane)
-{
-    const uint32_t slot = lane & 7, sub = lane >> 3;
-    const double* src = nullptr;
-    if (slot == 0) src = r;
-    else if ((int)slot <= g.ncols) src = g.in[slot - 1];
-    const uint32_t* src_id = ((int)slot == g.ncols + 1) ? g.id_in : nullptr;
-    double v[8];
-#pragma unroll
-    for (int j = 0; j < 8; ++j) {
-        const uint32_t i = base + 4 * j + sub;
-        v[j] = 0.0;
-        if (i < n) {
-            if (src) v[j] = __ldcs(src + i);
-            else if (src_id) v[j] = __longlong_as_double((long long)(unsigned long long)__ldcs(src_id + i));
-        }
-    }
-#pragma unroll
-    for (int j = 0; j < 8; ++j) {
-        const uint32_t i = base + 4 * j + sub;
-        if (i < n) __stcs(rec + (size_t)i * 8 + slot, v[j]);
-    }
-}
-
-// Stand-alone record pass, needed only when no digit pass is live (all key parts equal): otherwise the
-// first live digit pass, which walks the stars in input order anyway and leaves the memory system idle,
-// writes the records of its tiles.
-__global__ void __launch_bounds__(256) sort_pk_records_kernel(const double* __restrict__ r, PkCols g, uint32_t n,
-                                                              double* __restrict__ rec, const uint32_t* __restrict__ pass_live)
-{
-    for (int p = 0; p < PK_MAXPASS; ++p)
-        if (pass_live[p]) return;
-    const uint32_t warps = (gridDim.x * blockDim.x) >> 5, gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    for (uint32_t base = gw * 32; base < n; base += warps * 32) write_records_32(r, g, rec, base, n, threadIdx.x & 31);
-}
-
 // ---- one digit pass over the packed words -------------------------------------------------------
 // Same scheme as the general sort (tiles in ticket order, stable warp-level ranking, decoupled
 // look-back over per-tile digit counts, scatter through shared memory), but 8 bytes per star.
@@ -250,8 +249,7 @@ struct PkBuffers {
 __global__ void __launch_bounds__(PK_THREADS, 2)
 sort_pk_pass_kernel(PkBuffers b, uint32_t n, const uint64_t* __restrict__ ctl,
                     const uint32_t* __restrict__ bin_offset /*[256] exclusive*/, uint32_t* __restrict__ lookback,
-                    uint32_t* __restrict__ ticket, const uint32_t* __restrict__ pass_live, int pass, PkCols g,
-                    double* __restrict__ rec /* nullptr: no records wanted */)
+                    uint32_t* __restrict__ ticket, const uint32_t* __restrict__ pass_live, int pass)
 {
     if (!pass_live[pass]) return;
     int live_before = 0;
@@ -275,11 +273,6 @@ sort_pk_pass_kernel(PkBuffers b, uint32_t n, const uint64_t* __restrict__ ctl,
     if (tile >= tiles) break;
     const uint32_t tile_base = tile * PK_TILE;
     const uint32_t valid = min((uint32_t)PK_TILE, n - tile_base);
-    if (first && rec) {                                         // the star records of this tile (input order)
-        for (int round = 0; round < PK_ITEMS; ++round)
-            write_records_32(reinterpret_cast<const double*>(b.keys_src), g, rec, tile_base + warp * (32 * PK_ITEMS) + round * 32, n, lane);
-    }
-
     // load, warp-striped: item i of lane l sits at tile position warp*256 + i*32 + l
     uint64_t w[PK_ITEMS];
     const uint32_t wbase = warp * (32 * PK_ITEMS) + lane;
@@ -457,19 +450,19 @@ hmc_status sort_fast(uint64_t n, const double* r_in, double* r_sorted, uint32_t*
     // sortctl, pk_hist and pk_tickets are adjacent in the workspace: one memset
     HMC_CUDA_TRY(cudaMemsetAsync(ws.sortctl, 0, reinterpret_cast<char*>(ws.pk_tickets + 16) - reinterpret_cast<char*>(ws.sortctl), st));
     HMC_CUDA_TRY(cudaMemsetAsync(ws.lookback, 0, (size_t)PK_MAXPASS * tiles * PK_RADIX * 4, st));
-    const int stream_blocks = (int)umin64((n + 511) / 512, (uint64_t)sms * 4);
-    sort_minmax_kernel<<<stream_blocks, 512, 0, st>>>(keys, n, reinterpret_cast<unsigned long long*>(ws.sortctl));
-    HMC_LAUNCH_CHECK();
-    sort_pk_histogram_kernel<<<(int)umin64((n + PKH_THREADS - 1) / PKH_THREADS, (uint64_t)sms * 3), PKH_THREADS, 0, st>>>(
-        keys, (uint32_t)n, ws.sortctl, ws.pk_hist);
-    HMC_LAUNCH_CHECK();
-    sort_pk_scan_hist_kernel<<<PK_MAXPASS, PK_RADIX, 0, st>>>(ws.pk_hist, (uint32_t)n, pass_live);
-    HMC_LAUNCH_CHECK();
     PkCols g{};
     g.ncols = ncols;
     for (int c = 0; c < ncols; ++c) { g.in[c] = cols_in[c]; g.out[c] = cols_out[c]; }
     g.id_in = id_in; g.id_out = id_out;
     const bool use_rec = (ncols > 0 || id_in) && ncols <= PK_REC_COLS;
+    const int stream_blocks = (int)umin64((n + 511) / 512, (uint64_t)sms * 4);
+    sort_minmax_kernel<<<stream_blocks, 512, 0, st>>>(keys, n, reinterpret_cast<unsigned long long*>(ws.sortctl));
+    HMC_LAUNCH_CHECK();
+    sort_pk_histogram_kernel<<<(int)umin64((n + PKH_THREADS - 1) / PKH_THREADS, (uint64_t)sms * 3), PKH_THREADS, 0, st>>>(
+        keys, (uint32_t)n, ws.sortctl, ws.pk_hist, g, use_rec ? reinterpret_cast<double*>(ws.rec) : nullptr);
+    HMC_LAUNCH_CHECK();
+    sort_pk_scan_hist_kernel<<<PK_MAXPASS, PK_RADIX, 0, st>>>(ws.pk_hist, (uint32_t)n, pass_live);
+    HMC_LAUNCH_CHECK();
     const int copy_blocks = (int)umin64((n + 255) / 256, (uint64_t)sms * 8);
     static bool attr_done = false;
     if (!attr_done) {
@@ -487,11 +480,7 @@ hmc_status sort_fast(uint64_t n, const double* r_in, double* r_sorted, uint32_t*
     for (int p = 0; p < npass; ++p) {
         sort_pk_pass_kernel<<<(int)umin64(tiles, (uint64_t)sms * 2), PK_THREADS, sizeof(PkSmem), st>>>(b, (uint32_t)n, ws.sortctl, ws.pk_hist + p * PK_RADIX,
                                                                        ws.lookback + (size_t)p * tiles * PK_RADIX,
-                                                                       ws.pk_tickets + p, pass_live, p, g, use_rec ? reinterpret_cast<double*>(ws.rec) : nullptr);
-        HMC_LAUNCH_CHECK();
-    }
-    if (use_rec) {                                                          // returns at once unless no pass was live
-        sort_pk_records_kernel<<<copy_blocks, 256, 0, st>>>(r_in, g, (uint32_t)n, reinterpret_cast<double*>(ws.rec), pass_live);
+                                                                       ws.pk_tickets + p, pass_live, p);
         HMC_LAUNCH_CHECK();
     }
     if (use_rec)

@@ -264,8 +264,7 @@ def kernel_launches_per_step(n: int, ncols: int = 3, with_id: bool = True, fused
     idx_bits = max(24, ib)
     key_bits = min(((ib + 8 + 7) // 8) * 8, 40, 64 - idx_bits)
     npass = (key_bits + 7) // 8
-    rec = 1 if ((ncols or with_id) and ncols <= 6) else 0
-    fast = 3 + rec + npass + 1                       # range, histogram, bin scan, records, digit passes, finish
+    fast = 3 + npass + 1                             # range, histogram (+ star records), bin scan, digit passes, finish
     general = 1 + 2 + 8 + 1 + (1 if (ncols or with_id) else 0)   # guarded: zero, histogram, bin scan, 8 passes, identity, gather
     shift = 0
     while (n >> shift) + 2 > 10240:
