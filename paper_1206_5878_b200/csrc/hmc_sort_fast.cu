@@ -70,9 +70,9 @@ __device__ __forceinline__ unsigned match_digit(uint32_t d)
     unsigned peers = 0xffffffffu;
 #pragma unroll
     for (int bit = 0; bit < 8; ++bit) {
-        const bool on = (d >> bit) & 1u;
-        const unsigned m = __ballot_sync(0xffffffffu, on);
-        peers &= on ? m : ~m;
+        const unsigned mask = (unsigned)((int)(d << (31 - bit)) >> 31);     // all ones if the bit is set
+        const unsigned m = __ballot_sync(0xffffffffu, mask != 0u);
+        peers &= ~(m ^ mask);                                              // m if set, ~m if not
     }
     return peers;
 }
