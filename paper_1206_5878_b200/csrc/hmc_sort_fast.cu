@@ -308,13 +308,22 @@ sort_pk_pass_kernel(PkBuffers b, uint32_t n, const uint64_t* __restrict__ ctl,
         if (d == PK_RADIX - 1) count -= (PK_TILE - valid);      // padding is not data
         uint32_t* my = lookback + (size_t)tile * PK_RADIX + d;
         st_volatile_u32(my, PK_FLAG_AGG | count);
+        // look back four tiles at a time (their words are loaded together: one L2 round trip for four steps)
         uint32_t excl = 0;
-        for (int64_t t = (int64_t)tile - 1; t >= 0; --t) {
-            const uint32_t* q = lookback + (size_t)t * PK_RADIX + d;
-            uint32_t v;
-            do { v = ld_volatile_u32(q); } while ((v & PK_FLAG_MASK) == 0);
-            excl += v & ~PK_FLAG_MASK;
-            if ((v & PK_FLAG_MASK) == PK_FLAG_INC) break;
+        for (int64_t t = (int64_t)tile - 1; t >= 0; t -= 4) {
+            uint32_t v[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) v[j] = (t - j >= 0) ? ld_volatile_u32(lookback + (size_t)(t - j) * PK_RADIX + d) : PK_FLAG_INC;
+            bool stop = false;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                if (stop) break;
+                uint32_t x = v[j];
+                while ((x & PK_FLAG_MASK) == 0) x = ld_volatile_u32(lookback + (size_t)(t - j) * PK_RADIX + d);
+                excl += x & ~PK_FLAG_MASK;
+                stop = (x & PK_FLAG_MASK) == PK_FLAG_INC;
+            }
+            if (stop) break;
         }
         st_volatile_u32(my, PK_FLAG_INC | (excl + count));
         s.digit_base[d] = run;                                  // padded tile count, scanned below
