@@ -31,6 +31,7 @@ static constexpr int PK_WARPS = PK_THREADS / 32;
 static constexpr int PK_ITEMS = 8;
 static constexpr int PK_TILE = PK_THREADS * PK_ITEMS;          // 4096
 static constexpr int RUN_MAX = 32;
+static constexpr int LB = 4;                                  // look-back words loaded per round trip
 
 static constexpr uint32_t PK_FLAG_AGG = 1u << 30;
 static constexpr uint32_t PK_FLAG_INC = 2u << 30;
@@ -308,15 +309,15 @@ sort_pk_pass_kernel(PkBuffers b, uint32_t n, const uint64_t* __restrict__ ctl,
         if (d == PK_RADIX - 1) count -= (PK_TILE - valid);      // padding is not data
         uint32_t* my = lookback + (size_t)tile * PK_RADIX + d;
         st_volatile_u32(my, PK_FLAG_AGG | count);
-        // look back four tiles at a time (their words are loaded together: one L2 round trip for four steps)
+        // look back LB tiles at a time (their words are loaded together: one L2 round trip for four steps)
         uint32_t excl = 0;
-        for (int64_t t = (int64_t)tile - 1; t >= 0; t -= 4) {
-            uint32_t v[4];
+        for (int64_t t = (int64_t)tile - 1; t >= 0; t -= LB) {
+            uint32_t v[LB];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) v[j] = (t - j >= 0) ? ld_volatile_u32(lookback + (size_t)(t - j) * PK_RADIX + d) : PK_FLAG_INC;
+            for (int j = 0; j < LB; ++j) v[j] = (t - j >= 0) ? ld_volatile_u32(lookback + (size_t)(t - j) * PK_RADIX + d) : PK_FLAG_INC;
             bool stop = false;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
+            for (int j = 0; j < LB; ++j) {
                 if (stop) break;
                 uint32_t x = v[j];
                 while ((x & PK_FLAG_MASK) == 0) x = ld_volatile_u32(lookback + (size_t)(t - j) * PK_RADIX + d);
