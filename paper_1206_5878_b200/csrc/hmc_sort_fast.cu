@@ -300,16 +300,43 @@ sort_pk_pass_kernel(PkBuffers b, uint32_t n, const uint64_t* __restrict__ ctl,
         __syncwarp();
     }
     __syncthreads();
+    // digit d is owned by thread d: its count in the tile is published at once (the later tiles' look-back
+    // needs it), the look-back itself is left until after the scatter so that the earlier tiles have had time
+    // to publish their inclusive sums (shorter chains)
+    uint32_t count = 0;
     if (tid < PK_RADIX) {
         const int d = tid;
         uint32_t run = 0;
 #pragma unroll
         for (int q = 0; q < PK_WARPS; ++q) { const uint32_t c = s.warp_counts[q][d]; s.warp_counts[q][d] = run; run += c; }
-        uint32_t count = run;
+        count = run;
         if (d == PK_RADIX - 1) count -= (PK_TILE - valid);      // padding is not data
+        st_volatile_u32(lookback + (size_t)tile * PK_RADIX + d, PK_FLAG_AGG | count);
+        s.digit_base[d] = run;                                  // padded tile count, scanned below
+    }
+    __syncthreads();
+    // exclusive scan of the 256 tile counts by warp 0 (8 per lane)
+    if (warp == 0) {
+        uint32_t c[8], sum = 0;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { c[i] = s.digit_base[lane * 8 + i]; sum += c[i]; }
+        uint32_t inc = sum;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
+        uint32_t run = inc - sum;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { s.digit_base[lane * 8 + i] = run; run += c[i]; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < PK_ITEMS; ++i) {
+        const uint32_t d = (uint32_t)(w[i] >> shift) & 255u;
+        s.words[s.digit_base[d] + s.warp_counts[warp][d] + rank[i]] = w[i];
+    }
+    if (tid < PK_RADIX) {
+        const int d = tid;
         uint32_t* my = lookback + (size_t)tile * PK_RADIX + d;
-        st_volatile_u32(my, PK_FLAG_AGG | count);
-        // look back LB tiles at a time (their words are loaded together: one L2 round trip for four steps)
+        // look back LB tiles at a time (their words are loaded together: one L2 round trip for LB steps)
         uint32_t excl = 0;
         for (int64_t t = (int64_t)tile - 1; t >= 0; t -= LB) {
             uint32_t v[LB];
@@ -327,31 +354,7 @@ sort_pk_pass_kernel(PkBuffers b, uint32_t n, const uint64_t* __restrict__ ctl,
             if (stop) break;
         }
         st_volatile_u32(my, PK_FLAG_INC | (excl + count));
-        s.digit_base[d] = run;                                  // padded tile count, scanned below
-        s.global_base[d] = bin_offset[d] + excl;
-    }
-    __syncthreads();
-    // exclusive scan of the 256 tile counts by warp 0 (8 per lane)
-    if (warp == 0) {
-        uint32_t c[8], sum = 0;
-#pragma unroll
-        for (int i = 0; i < 8; ++i) { c[i] = s.digit_base[lane * 8 + i]; sum += c[i]; }
-        uint32_t inc = sum;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
-        uint32_t run = inc - sum;
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            s.digit_base[lane * 8 + i] = run;
-            s.global_base[lane * 8 + i] -= run;                 // global position = global_base[d] + tile position
-            run += c[i];
-        }
-    }
-    __syncthreads();
-#pragma unroll
-    for (int i = 0; i < PK_ITEMS; ++i) {
-        const uint32_t d = (uint32_t)(w[i] >> shift) & 255u;
-        s.words[s.digit_base[d] + s.warp_counts[warp][d] + rank[i]] = w[i];
+        s.global_base[d] = bin_offset[d] + excl - s.digit_base[d];   // global position = global_base[d] + tile position
     }
     __syncthreads();
 #pragma unroll
