@@ -60,16 +60,21 @@ def measured_peak_gbs():
 
 
 def ncu_traffic_bytes(kernel: str, n: int):
-    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture (profiles/dram_traffic.csv), if any."""
+    """(DRAM bytes per launch of `kernel`, what the capture was taken from) out of the committed ncu --set full
+    capture, profiles/dram_traffic.csv: a constant of THAT build (the `# capture:` line names its commit), not
+    something this run measured -- it goes stale when the kernel changes, which is why the line prints it."""
     p = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+    capture, found = None, None
     try:
         for line in open(p):
+            if line.startswith("# capture:"):
+                capture = line.split(":", 1)[1].strip()
             f = line.strip().split(",")
             if len(f) == 3 and f[0] == str(n) and f[1].split("<")[0] == kernel:
-                return int(f[2])
+                found = int(f[2])
     except Exception:
         pass
-    return None
+    return found, capture
 
 
 # --------------------------------------------------------------------------- clocks
@@ -178,10 +183,25 @@ def aggregate_throughput(stars_this_rank: float, ms_this_rank: float, device="cp
 
 
 # --------------------------------------------------------------------------- CPU oracle legs
-def oracle_sampled_step(cluster, seed, step, stride):
-    """Time the oracle as it stands on a bounded sample of one step: S1 and S2 on all stars, S3 and
-    S4 on every `stride`-th star of the sorted order; returns (estimated seconds for the full step,
-    per-stage seconds measured, result of the step)."""
+def host_cpu():
+    """(model string, logical cores visible to this process) of the box the oracle is timed on."""
+    model = "unknown"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.lower().startswith("model name"):
+                model = line.split(":", 1)[1].strip()
+                break
+    except Exception:
+        pass
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    return model, cores
+
+
+def oracle_step_timed(cluster, seed, step, stride=1):
+    """One step of the oracle (whichever build oracle.use() selected), timed per stage.  stride = 1: every
+    star, everything measured.  stride > 1 (explicit opt-in): S3 / S4 on every stride-th star of the sorted
+    order only; the caller scales the orbit stages and marks the figure as estimated.
+    -> (per-stage seconds measured, result of the step)"""
     import oracle
     t0 = time.perf_counter()
     rs, perm, (vrs, vts, ms), ids = oracle.sort_by_radius(cluster["r"], (cluster["v_r"], cluster["v_t"], cluster["m"]),
@@ -195,49 +215,88 @@ def oracle_sampled_step(cluster, seed, step, stride):
     sm = oracle.sample_new_radius(rs, phi, mc, rs[sl], vrs[sl], vts[sl], tp["E"], tp["J"], tp["r_min"], tp["r_max"],
                                   tp["k_min"], tp["k_max"], ids[sl], tp["status"], seed, step)
     t4 = time.perf_counter()
-    n = len(rs)
-    scale = n / max(len(tp["E"]), 1)
     meas = dict(sort=t1 - t0, potential=t2 - t1, turning_points=t3 - t2, sampling=t4 - t3)
-    est = meas["sort"] + meas["potential"] + scale * (meas["turning_points"] + meas["sampling"])
-    return est, meas, scale
+    nxt = None
+    if stride == 1:
+        nxt = dict(r=sm["r_new"], v_r=sm["v_r_new"], v_t=sm["v_t_new"], m=ms, id=ids)
+    return meas, nxt
 
 
-def cpu_baseline_leg(cluster, seed, stride=64):
-    est, meas, scale = oracle_sampled_step(cluster, seed, 0, stride)
+def oracle_leg(cluster, seed, variant, stride=1):
+    """One oracle step on `cluster` with the given build -> dict for the JSON line."""
+    import oracle
     n = len(cluster["r"])
-    return dict(value=n / est, unit=UNIT, cores=1, kind="oracle",
-                sample="one step at N=%d: sort and potential on all stars, turning points and sampling on every "
-                       "%d-th star of the sorted order (%.1f s measured), orbit stages scaled x%.0f"
-                       % (n, stride, sum(meas.values()), scale),
-                seconds_measured=round(sum(meas.values()), 2), est_seconds_per_step=round(est, 2),
-                stage_seconds_measured={k: round(v, 3) for k, v in meas.items()})
+    with oracle.use(variant):
+        threads = oracle.threads()
+        meas, _ = oracle_step_timed(cluster, seed, 0, stride)
+    secs = meas["sort"] + meas["potential"] + stride * (meas["turning_points"] + meas["sampling"])
+    d = dict(value=n / secs, unit=UNIT, cores=threads, seconds_per_step=round(secs, 3),
+             stage_seconds={k: round(v * (stride if k in ("turning_points", "sampling") else 1), 3) for k, v in meas.items()})
+    if stride > 1:
+        d["estimated"] = "turning points and sampling timed on every %d-th star and scaled x%d" % (stride, stride)
+    return d
+
+
+def cpu_baseline_leg(cluster, seed, stride=1):
+    """the oracle as it stands on this box's host cores, same input bytes: (ii) the -fopenmp
+    build of the same source on all cores (the top-level figure; `cores` = threads it used) and (i) the
+    single-threaded build (`single_core`).  One whole step each at N <= 2e7: measured, nothing scaled."""
+    n = len(cluster["r"])
+    model, nproc = host_cpu()
+    if stride == 1 and n > 20_000_000:
+        stride = 16                      # about 10 min per step otherwise; marked as estimated
+    allc = oracle_leg(cluster, seed, "omp", stride)
+    one = oracle_leg(cluster, seed, "serial", stride)
+    what = "every star" if stride == 1 else "S1/S2 on every star, S3/S4 on every %d-th star (scaled)" % stride
+    out = dict(value=allc["value"], unit=UNIT, cores=allc["cores"], kind="oracle",
+               sample="one whole orbit step at N=%d (%s): %.1f s with the -fopenmp build on %d threads, %.1f s "
+                      "single-threaded" % (n, what, allc["seconds_per_step"], allc["cores"], one["seconds_per_step"]),
+               cpu_model=model, nproc=nproc, flags="gcc -O2 -ffp-contract=off (-fopenmp: per-star loops of S3/S4 and the gather)",
+               all_cores=allc, single_core=one)
+    if stride > 1:
+        out["estimated"] = allc["estimated"]
+    return out
 
 
 def run_reference(args, cfg):
+    """The reference arm: the oracle, chained over warmup + steps whole steps on this arm's config.  Default build:
+    -fopenmp on all host cores (a step at N = 1e7 takes seconds, so 25 steps end within a few minutes and every
+    reported millisecond was measured); --ref-variant serial is the single-threaded oracle (about 30 s per step)."""
     rank, _, world = dist_env()
     if rank != 0:
         return 0
     from paper_1206_5878_b200 import inputs
     import oracle
-    oracle.build()
+    oracle.build_all()
     c = inputs.config(args.config, args.n)
     cluster = {k: c[k] for k in ("r", "v_r", "v_t", "m", "id")}
     n = c["n"]
-    stride = args.ref_stride
-    ests = []
-    for i in range(args.warmup + args.steps):
-        est, meas, scale = oracle_sampled_step(cluster, c["seed"], i, stride)
-        if i >= args.warmup:
-            ests.append(est)
-    ms = 1e3 * sum(ests) / len(ests)
+    stride = max(1, args.ref_stride)
+    model, nproc = host_cpu()
+    secs, stage = [], []
+    with oracle.use(args.ref_variant):
+        threads = oracle.threads()
+        for i in range(args.warmup + args.steps):
+            meas, nxt = oracle_step_timed(cluster, c["seed"], i, stride)
+            if nxt is not None:
+                cluster = nxt                     # chained, as the GPU arm
+            if i >= args.warmup:
+                secs.append(meas["sort"] + meas["potential"] + stride * (meas["turning_points"] + meas["sampling"]))
+                stage.append(meas)
+    ms = 1e3 * sum(secs) / len(secs)
     value = n / (ms * 1e-3)
+    what = "every star of every step, steps chained" if stride == 1 else \
+        "S1/S2 on every star, S3/S4 on every %d-th star and scaled x%d (ESTIMATED; steps not chained)" % (stride, stride)
+    cpu = dict(value=value, unit=UNIT, cores=threads, kind="oracle", cpu_model=model, nproc=nproc,
+               sample="%d whole orbit steps at N=%d with the %s build of oracle/hmc_oracle.c: %s"
+                      % (args.steps, n, args.ref_variant, what),
+               stage_seconds={k: round(sum(m[k] for m in stage) / len(stage), 3) for k in STAGES})
     line = dict(impl="reference", metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
                 warmup=args.warmup, ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None,
-                dtype="f64", data="synthetic", config=cfg,
-                cpu_baseline=dict(value=value, unit=UNIT, cores=1, kind="oracle",
-                                  sample="each step: sort and potential on all %d stars, turning points and sampling "
-                                         "on every %d-th star of the sorted order, orbit stages scaled x%d" % (n, stride, stride)),
+                dtype="f64", data="synthetic", config=cfg, cpu_baseline=cpu,
                 e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    if stride > 1:
+        line["estimated"] = True
     print(json.dumps(line))
     return 0
 
@@ -306,10 +365,12 @@ def run_gpu(args, cfg):
     sampler.start()
     evs = [mk() for _ in range(args.steps)]
     t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches_before = int(hmc.lib().hmc_launch_count())
     t_start.record(stream)
     for i in range(args.steps):
         staged_step(evs[i])
     t_end.record(stream)
+    gpu_launches = int(hmc.lib().hmc_launch_count()) - launches_before      # counted by the library at each launch
     torch.cuda.synchronize()
     dist_barrier()
     clocks = sampler.stop()
@@ -364,10 +425,19 @@ def run_gpu(args, cfg):
     peak, peak_src = measured_peak_gbs()
     dom, dom_kernel = "sampling", "sample_new_radius_kernel"
     achieved = model[dom] * n / (stage_ms[dom] * 1e-3) / 1e9
+    traffic, capture = ncu_traffic_bytes(dom_kernel, n)
     roofline = dict(bound="hbm", kernel=dom_kernel, stage=dom, achieved=achieved, peak=peak, unit="GB/s",
-                    frac=achieved / peak, traffic=ncu_traffic_bytes(dom_kernel, n), peak_source=peak_src,
+                    frac=achieved / peak, traffic=traffic, peak_source=peak_src,
                     algorithmic_bytes_per_star=model[dom], stars_per_launch=n, launch_ms=stage_ms[dom],
-                    launches_timed=args.steps)
+                    launches_timed=args.steps,
+                    # `achieved` / `frac` are SURVEY.md 8(d)'s ALGORITHMIC bytes over the measured launch time: a model
+                    # fraction (one table entry per probe of the paper's bisection; this kernel serves most probes from
+                    # shared memory).  What the launch physically moved, by ncu, over the same measured time:
+                    model_frac=achieved / peak,
+                    physical=(dict(dram_bytes_per_launch=traffic, achieved=traffic / (stage_ms[dom] * 1e-3) / 1e9,
+                                   frac=traffic / (stage_ms[dom] * 1e-3) / 1e9 / peak, capture=capture,
+                                   limiter="latency of dependent random loads (DRAM lines touched), not streamed bytes; "
+                                           "see profiles/") if traffic else None))
     orbit_ms = stage_ms["potential"] + stage_ms["turning_points"] + stage_ms["sampling"]
     orbit_bytes = model["potential"] + model["turning_points"] + model["sampling"]
     stages = {s: dict(ms=stage_ms[s], stars_per_s=n / (stage_ms[s] * 1e-3), algorithmic_bytes_per_star=model[s],
@@ -382,12 +452,12 @@ def run_gpu(args, cfg):
     if world == 1 or rank == 0:
         if not args.no_cpu_baseline:
             import oracle
-            oracle.build()
-            cpu = cpu_baseline_leg(cluster, c["seed"], args.ref_stride)
+            oracle.build_all()
+            cpu = cpu_baseline_leg(cluster, c["seed"], max(1, args.ref_stride))
 
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
                 ms_per_step=ms_max / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
-                data="synthetic", config=cfg, clocks=clocks, e2e=e2e, gpu_launches=hmc.kernel_launches_per_step(n) * args.steps,
+                data="synthetic", config=cfg, clocks=clocks, e2e=e2e, gpu_launches=gpu_launches,
                 roofline=roofline, cpu_baseline=cpu, stages=stages, potential_plus_orbit=potential_plus_orbit,
                 counters=counters)
     print(json.dumps(line))
@@ -402,7 +472,10 @@ def main(argv=None):
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (default 2: N=1e7, the metric's)")
     ap.add_argument("--n", type=int, default=None, help="override N (same recipe and seed); not a bench line")
-    ap.add_argument("--ref-stride", type=int, default=4, help="oracle legs: orbit stages on every k-th star")
+    ap.add_argument("--ref-stride", type=int, default=1,
+                    help="oracle legs, explicit opt-in: orbit stages on every k-th star, scaled (marks the figure ESTIMATED)")
+    ap.add_argument("--ref-variant", default="omp", choices=["omp", "serial"],
+                    help="--impl reference: which build of the oracle (omp = all host cores, serial = one core)")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--fused", action="store_true", help="S3 and S4 as the single call hmc_orbit_step")
     ap.add_argument("--no-e2e", action="store_true")

@@ -69,7 +69,9 @@ typedef int32_t hmc_status;
 #define HMC_STAR_CLIPPED    32u   /* some trial had g > F (density clipped there); draw still valid */
 #define HMC_STAR_NOKINETIC  64u   /* energy correction: corrected kinetic energy <= 0; velocities kept */
 
+#ifndef HMC_T_MAX                 /* (a test-only build lowers it to reach the exhaustion path) */
 #define HMC_T_MAX   4096u         /* cap on rejection trials per star (R7)        */
+#endif
 
 /* device counters accumulated (atomically) by the orbit calls; the caller zeroes them */
 enum {
@@ -88,6 +90,14 @@ HMC_API const char* hmc_status_string(hmc_status s);
 
 /* Library version as major*10000 + minor*100 + patch. */
 HMC_API int32_t hmc_version(void);
+
+/* The cap on rejection trials this build was compiled with (HMC_T_MAX). */
+HMC_API uint32_t hmc_t_max(void);
+
+/* Number of CUDA kernels this process has launched through the library so far (all threads, all devices;
+ * memsets and copies are not kernels).  A monotone counter for accounting: bench.py reports the difference
+ * over its timed region as `gpu_launches`. */
+HMC_API uint64_t hmc_launch_count(void);
 
 /*
  * S1  "Sort stars by radial distance".

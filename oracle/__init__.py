@@ -5,9 +5,17 @@ this package; only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s
 ``cpu_baseline`` / ``--impl reference`` legs do.  The arithmetic lives in
 ``hmc_oracle.c`` (plain C, one translation unit, written from the paper); this
 file only compiles it with gcc and marshals numpy arrays through ctypes.
+
+Builds of the one source file (``use(name)`` selects which one the functions below call):
+  serial  libhmc_oracle.so       the oracle as defined: single-threaded
+  omp     libhmc_oracle_omp.so   -fopenmp over the per-star loops of S3 / S4 / energy correction and the
+                                 gather; bit-identical results (tests check it)
+  tmax3   libhmc_oracle_tmax3.so -DT_MAX=3u, test-only: reaches the exhaustion branch of S4 (the product's
+                                 counterpart is libhmc_tmax3.so, built with -DHMC_T_MAX=3u)
 """
 from __future__ import annotations
 
+import contextlib
 import ctypes
 import os
 import subprocess
@@ -16,32 +24,69 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "hmc_oracle.c")
-_LIB = os.path.join(_HERE, "libhmc_oracle.so")
 # -ffp-contract=off: no FMA contraction; see the header of hmc_oracle.c.
-CFLAGS = ["-O2", "-ffp-contract=off", "-fPIC", "-shared", "-std=gnu11", "-Wall"]
+CFLAGS = ["-O2", "-ffp-contract=off", "-fPIC", "-shared", "-std=gnu11", "-Wall", "-Wno-unknown-pragmas"]
+VARIANTS = {
+    "serial": ("libhmc_oracle.so", []),
+    "omp": ("libhmc_oracle_omp.so", ["-fopenmp"]),
+    "tmax3": ("libhmc_oracle_tmax3.so", ["-DT_MAX=3u"]),
+}
 
 ST_UNBOUND, ST_RADIAL, ST_DEGENERATE, ST_CIRCULAR, ST_MAXTRIES, ST_CLIPPED = 1, 2, 4, 8, 16, 32
 T_MAX = 4096
 C_F = 1.2
 
-_lib = None
+_libs = {}
+_current = "serial"
 
 
-def build(force: bool = False) -> str:
-    """Compile hmc_oracle.c -> libhmc_oracle.so (in-tree) if missing or stale."""
-    stale = (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC)
+def build(force: bool = False, variant: str = "serial") -> str:
+    """Compile hmc_oracle.c -> the variant's shared library (in-tree) if missing or stale."""
+    name, extra = VARIANTS[variant]
+    out = os.path.join(_HERE, name)
+    stale = (not os.path.exists(out)) or os.path.getmtime(out) < os.path.getmtime(_SRC)
     if force or stale:
-        tmp = _LIB + ".tmp.%d" % os.getpid()
-        subprocess.run(["gcc", *CFLAGS, _SRC, "-o", tmp, "-lm"], check=True)
-        os.replace(tmp, _LIB)
-    return _LIB
+        tmp = out + ".tmp.%d" % os.getpid()
+        subprocess.run(["gcc", *CFLAGS, *extra, _SRC, "-o", tmp, "-lm"], check=True)
+        os.replace(tmp, out)
+    return out
 
 
-def lib() -> ctypes.CDLL:
-    global _lib
-    if _lib is None:
-        _lib = ctypes.CDLL(build())
-    return _lib
+def build_all(force: bool = False):
+    return [build(force, v) for v in VARIANTS]
+
+
+def lib(variant: str | None = None) -> ctypes.CDLL:
+    v = variant or _current
+    if v not in _libs:
+        L = ctypes.CDLL(build(variant=v))
+        L.hmc_ref_t_max.restype = ctypes.c_uint32
+        _libs[v] = L
+    return _libs[v]
+
+
+@contextlib.contextmanager
+def use(variant: str):
+    """``with oracle.use("omp"): ...`` -- the functions of this module call that build inside the block."""
+    global _current
+    prev, _current = _current, variant
+    try:
+        lib()
+        yield
+    finally:
+        _current = prev
+
+
+def t_max(variant: str | None = None) -> int:
+    return int(lib(variant).hmc_ref_t_max())
+
+
+def threads() -> int:
+    """Threads the per-star loops of the current build use (1 for the builds without -fopenmp)."""
+    if not lib().hmc_ref_openmp():
+        return 1
+    n = os.environ.get("OMP_NUM_THREADS")
+    return int(n) if n else (len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else os.cpu_count())
 
 
 def _p(a):

@@ -13,6 +13,11 @@
  * (-ffp-contract=off: no fused multiply-add, every +,-,*,/,sqrt below is one
  *  correctly rounded IEEE-754 binary64 operation, evaluated in the order the
  *  parentheses state -- DESIGN.md "Readings" R2.)
+ * The same source built with -fopenmp (libhmc_oracle_omp.so) runs the per-star loops of S3,
+ * S4 and the energy correction on all host cores: every star is
+ * independent of the others and the random numbers are counter-based, so the results are
+ * bit-identical to the single-threaded build (tests check it); the sort and the running
+ * sums stay serial.  Without -fopenmp the pragmas are ignored.
  *
  * Numbering.  The paper numbers the radius-sorted stars 1..N.
  * Arrays here are 0-based: array element a holds node j = a+1.  Sentinel nodes
@@ -48,7 +53,9 @@
 #define ST_MAXTRIES   16u  /* rejection loop hit T_MAX                               */
 #define ST_CLIPPED    32u  /* some trial had g > F (density clipped; informational)  */
 
+#ifndef T_MAX              /* a test-only build with -DT_MAX=3u exercises the exhaustion branch of S4 */
 #define T_MAX 4096u        /* DESIGN.md R7 */
+#endif
 #define C_F   1.2          /* DESIGN.md R7 */
 
 /* ------------------------------------------------------------------------ */
@@ -94,6 +101,17 @@ static int cmp_key_index(const void *pa, const void *pb)
     return 0;
 }
 
+/* what this build is: T_MAX and whether the per-star loops are threaded */
+uint32_t hmc_ref_t_max(void) { return T_MAX; }
+int hmc_ref_openmp(void)
+{
+#ifdef _OPENMP
+    return 1;
+#else
+    return 0;
+#endif
+}
+
 int hmc_ref_sort_by_radius(uint64_t n, const double *r_in, double *r_sorted, uint32_t *perm,
                            int ncols, const double *const *cols_in, double *const *cols_out,
                            const uint32_t *id_in, uint32_t *id_out)
@@ -107,10 +125,14 @@ int hmc_ref_sort_by_radius(uint64_t n, const double *r_in, double *r_sorted, uin
         perm[k] = a[k].i;
         r_sorted[k] = a[k].r;
     }
-    for (int c = 0; c < ncols; ++c)
+    for (int c = 0; c < ncols; ++c) {
+#pragma omp parallel for schedule(static)
         for (uint64_t k = 0; k < n; ++k) cols_out[c][k] = cols_in[c][perm[k]];
-    if (id_in && id_out)
+    }
+    if (id_in && id_out) {
+#pragma omp parallel for schedule(static)
         for (uint64_t k = 0; k < n; ++k) id_out[k] = id_in[perm[k]];
+    }
     free(a);
     return 0;
 }
@@ -204,6 +226,7 @@ int hmc_ref_orbit_turning_points(uint64_t n, double G,
         uint32_t *k_min_out, uint32_t *k_max_out, uint8_t *status_out)
 {
     table T = { n, G, r, phi, m_cum };
+#pragma omp parallel for schedule(dynamic, 4096)
     for (uint64_t i = 0; i < count; ++i) {
         uint64_t a = first + i * stride;        /* array index           */
         uint64_t k = a + 1;                     /* node number, 1..N     */
@@ -306,6 +329,7 @@ int hmc_ref_sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step
     const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
     const double two_m53 = 1.0 / 9007199254740992.0;
     uint64_t total_trials = 0;
+#pragma omp parallel for schedule(dynamic, 4096) reduction(+ : total_trials)
     for (uint64_t i = 0; i < count; ++i) {
         unsigned st = status_in[i];
         r_new[i] = r_self[i]; v_r_new[i] = v_r_self[i]; v_t_new[i] = v_t_self[i];
@@ -444,6 +468,7 @@ int hmc_ref_energy_correction(uint64_t n, double G, const double *r, const doubl
                               double *v_r_out, double *v_t_out, uint8_t *status_out)
 {
     table T = { n, G, r, phi, m_cum };
+#pragma omp parallel for schedule(dynamic, 4096)
     for (uint64_t a = 0; a < n; ++a) {
         double vr = v_r[a], vt = v_t[a];
         double K = 0.5 * (vr * vr + vt * vt);

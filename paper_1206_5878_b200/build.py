@@ -26,23 +26,40 @@ NVCC_FLAGS = [
 ]
 
 
-def _stale() -> bool:
-    if not os.path.exists(LIB):
+# "product" is the library; "tmax3" is a TEST-ONLY build of the same sources with the cap on rejection trials
+# lowered to 3, so that the GPU tests reach S4's exhaustion path (draw_exhaustive, MAXTRIES) and compare it
+# with the oracle built the same way (oracle/: -DT_MAX=3u).  Nothing but tests loads it.
+VARIANTS = {
+    "product": ("libhmc.so", []),
+    "tmax3": ("libhmc_tmax3.so", ["-DHMC_T_MAX=3u"]),
+}
+
+
+def lib_path(variant: str = "product") -> str:
+    return os.path.join(HERE, VARIANTS[variant][0])
+
+
+def _stale(lib: str) -> bool:
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(ROOT, "include", "hmc.h"), __file__]
+    t = os.path.getmtime(lib)
+    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh"))]
+    deps += [os.path.join(ROOT, "include", "hmc.h"), __file__]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not (force or _stale()):
+def build(force: bool = False, verbose: bool = False, variant: str = "product") -> str:
+    LIB = lib_path(variant)
+    defines = VARIANTS[variant][1]
+    if not (force or _stale(LIB)):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     objs = []
     procs = []
+    suffix = ".o" if variant == "product" else ".%s.o" % variant
     for src in SOURCES:
-        obj = os.path.join(CSRC, src[:-3] + ".o")
-        cmd = [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, src), "-o", obj]
+        obj = os.path.join(CSRC, src[:-3] + suffix)
+        cmd = [nvcc, *NVCC_FLAGS, *defines, "-c", os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
@@ -60,5 +77,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_all(force: bool = False, verbose: bool = False):
+    return [build(force, verbose, v) for v in VARIANTS]
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    for path in build_all(force="--force" in sys.argv, verbose="-v" in sys.argv):
+        print(path)

@@ -1,21 +1,23 @@
 // hmc_api.cu -- extern "C" boundary of libhmc (include/hmc.h): argument checks, workspace
 // carve-up, stream plumbing.  No arithmetic of the method lives here.
+#include <vector>
 #include "hmc_common.cuh"
 
 namespace hmc {
 
+std::atomic<uint64_t> g_launches{ 0 };
+
 int sm_count()
 {
-    static int cached = 0;
-    if (cached == 0) {
-        int dev = 0, sms = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
-            cached = sms;
-        else
-            cached = HMC_SM_COUNT_FALLBACK;
-    }
-    return cached;
+    static std::atomic<int> cached[64];                     // zero-initialised; one slot per device ordinal
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return HMC_SM_COUNT_FALLBACK;
+    const bool slot = dev >= 0 && dev < 64;
+    if (slot && (sms = cached[dev].load(std::memory_order_relaxed)) > 0) return sms;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+        sms = HMC_SM_COUNT_FALLBACK;
+    if (slot) cached[dev].store(sms, std::memory_order_relaxed);
+    return sms;
 }
 
 static hmc_status check_ws(const void* ws, size_t bytes, uint64_t n)
@@ -64,24 +66,30 @@ static Arena carve_arena(void* base, uint64_t n)
 }
 
 // hmc_step_host only: a second stream on which the sorted masses and ids go back to the host while the
-// potential and orbit stages run (the two directions and the kernels then overlap).  One per host thread and
-// device, created at first use, never destroyed.
+// potential and orbit stages run (the two directions and the kernels then overlap).  One per (host thread,
+// device), created at first use and kept for the life of the thread: the only state the library owns.
 struct SideStream {
-    int device = -1;
+    bool made = false;
     cudaStream_t stream = nullptr;
     cudaEvent_t sorted = nullptr, copied = nullptr;
+    cudaEvent_t up[2] = { nullptr, nullptr };
 };
 
 static hmc_status side_stream(SideStream** out)
 {
-    static thread_local SideStream ss;
+    static thread_local std::vector<SideStream> per_device;
     int dev = 0;
     HMC_CUDA_TRY(cudaGetDevice(&dev));
-    if (ss.device != dev) {
+    if (dev < 0) return HMC_ERR_CUDA;
+    if ((size_t)dev >= per_device.size()) per_device.resize((size_t)dev + 1);
+    SideStream& ss = per_device[(size_t)dev];
+    if (!ss.made) {
         HMC_CUDA_TRY(cudaStreamCreateWithFlags(&ss.stream, cudaStreamNonBlocking));
         HMC_CUDA_TRY(cudaEventCreateWithFlags(&ss.sorted, cudaEventDisableTiming));
         HMC_CUDA_TRY(cudaEventCreateWithFlags(&ss.copied, cudaEventDisableTiming));
-        ss.device = dev;
+        HMC_CUDA_TRY(cudaEventCreateWithFlags(&ss.up[0], cudaEventDisableTiming));
+        HMC_CUDA_TRY(cudaEventCreateWithFlags(&ss.up[1], cudaEventDisableTiming));
+        ss.made = true;
     }
     *out = &ss;
     return HMC_OK;
@@ -98,7 +106,11 @@ extern "C" {
 
 size_t hmc_workspace_bytes(uint64_t n) { return carve(nullptr, n).total; }
 
-int32_t hmc_version(void) { return 100; }
+int32_t hmc_version(void) { return 200; }
+
+uint32_t hmc_t_max(void) { return HMC_T_MAX; }
+
+uint64_t hmc_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 const char* hmc_status_string(hmc_status s)
 {

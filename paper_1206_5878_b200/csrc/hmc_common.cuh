@@ -4,6 +4,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <atomic>
 #include "hmc.h"
 
 #define HMC_SM_COUNT_FALLBACK 148
@@ -30,12 +31,30 @@ static inline hmc_status cuda_ok(cudaError_t e) { return e == cudaSuccess ? HMC_
         if (_e != cudaSuccess) return HMC_ERR_CUDA;          \
     } while (0)
 
+// after every kernel launch: counts it (hmc_launch_count) and turns a launch failure into HMC_ERR_CUDA
 #define HMC_LAUNCH_CHECK()                                   \
     do {                                                     \
+        ::hmc::g_launches.fetch_add(1, std::memory_order_relaxed); \
         if (cudaPeekAtLastError() != cudaSuccess) return HMC_ERR_CUDA; \
     } while (0)
 
-int sm_count();   // cached multiprocessor count of the current device
+extern std::atomic<uint64_t> g_launches;   // kernels launched by this process through the library
+
+int sm_count();   // multiprocessor count of the CURRENT device (cached per device)
+
+// Function attributes (the opt-in to more than 48 KB of dynamic shared memory) are per DEVICE: a kernel's
+// attribute is set the first time the kernel is launched on each device.  `mask` has one bit per device
+// ordinal < 64 (beyond that the attribute is simply set every time); setting it twice is harmless, so no lock.
+template <class Kernel>
+static inline hmc_status smem_opt_in(std::atomic<uint64_t>& mask, Kernel kernel, size_t bytes)
+{
+    int dev = 0;
+    HMC_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev >= 0 && dev < 64 && ((mask.load(std::memory_order_acquire) >> dev) & 1ull)) return HMC_OK;
+    HMC_CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    if (dev >= 0 && dev < 64) mask.fetch_or(1ull << dev, std::memory_order_release);
+    return HMC_OK;
+}
 
 // ---- workspace layout (one carve-up used by every call) -------------------------------------
 // All offsets are multiples of 256 bytes.

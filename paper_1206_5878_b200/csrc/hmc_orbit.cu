@@ -857,11 +857,9 @@ static hmc_status build_tables(uint64_t n, double G, const double* r, const doub
     HMC_LAUNCH_CHECK();
     if (shift > 0) {
         const size_t smem = ((size_t)(1u << shift) + 1) * sizeof(uint32_t);
-        static size_t attr_smem = 48 * 1024;
-        if (smem > attr_smem) {
-            HMC_CUDA_TRY(cudaFuncSetAttribute(build_dir_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            attr_smem = smem;
-        }
+        static std::atomic<uint64_t> opted{ 0 };                  // the largest row any n <= HMC_MAX_N needs
+        hmc_status so = smem_opt_in(opted, build_dir_kernel, ((size_t)(1u << coarse_shift(HMC_MAX_N)) + 1) * sizeof(uint32_t));
+        if (so != HMC_OK) return so;
         build_dir_kernel<<<(unsigned)((n >> shift) + 1), DIR_THREADS, smem, st>>>(r, ws.dir, (uint32_t)n, shift);
         HMC_LAUNCH_CHECK();
     }
@@ -876,12 +874,9 @@ hmc_status turning_points(uint64_t n, double G, const double* r, const double* v
     const int sms = sm_count();
     const int shift = coarse_shift(n);
     const size_t smem = ((n >> shift) + 2) * sizeof(double2);
-    static bool attr_done = false;
-    if (!attr_done) {
-        HMC_CUDA_TRY(cudaFuncSetAttribute(turning_points_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)(COARSE_CAP * sizeof(double2))));
-        attr_done = true;
-    }
+    static std::atomic<uint64_t> opted{ 0 };
+    hmc_status so = smem_opt_in(opted, turning_points_kernel, COARSE_CAP * sizeof(double2));
+    if (so != HMC_OK) return so;
     hmc_status s = build_tables(n, G, r, phi, m_cum, ws, shift, st);
     if (s != HMC_OK) return s;
     const int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
@@ -897,13 +892,11 @@ static hmc_status launch_sampler(bool fused, uint64_t n, double G, uint64_t seed
 {
     const int sms = sm_count();
     const size_t smem = ORB_WARPS * sizeof(Park) + ((n >> shift) + 2) * sizeof(double2);
-    static bool attr_done = false;
-    if (!attr_done) {
-        const int cap = (int)(ORB_WARPS * sizeof(Park) + COARSE_CAP * sizeof(double2));
-        HMC_CUDA_TRY(cudaFuncSetAttribute(sample_new_radius_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap));
-        HMC_CUDA_TRY(cudaFuncSetAttribute(sample_new_radius_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap));
-        attr_done = true;
-    }
+    static std::atomic<uint64_t> opted[2];
+    const size_t cap = ORB_WARPS * sizeof(Park) + COARSE_CAP * sizeof(double2);
+    hmc_status so = fused ? smem_opt_in(opted[1], sample_new_radius_kernel<true>, cap)
+                          : smem_opt_in(opted[0], sample_new_radius_kernel<false>, cap);
+    if (so != HMC_OK) return so;
     const int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
     HMC_CUDA_TRY(cudaMemsetAsync(ws.tickets + 16, 0, 4, st));
     SampleIO io = io_in;
@@ -948,12 +941,9 @@ hmc_status energy_correction(uint64_t n, double G, const double* r, const double
     const int sms = sm_count();
     const int shift = coarse_shift(n);
     const size_t smem = ((n >> shift) + 2) * sizeof(double2);
-    static bool attr_done = false;
-    if (!attr_done) {
-        HMC_CUDA_TRY(cudaFuncSetAttribute(energy_correction_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)(COARSE_CAP * sizeof(double2))));
-        attr_done = true;
-    }
+    static std::atomic<uint64_t> opted{ 0 };
+    hmc_status so = smem_opt_in(opted, energy_correction_kernel, COARSE_CAP * sizeof(double2));
+    if (so != HMC_OK) return so;
     hmc_status s = build_tables(n, G, r, phi, m_cum, ws, shift, st);
     if (s != HMC_OK) return s;
     const int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);

@@ -320,12 +320,9 @@ static hmc_status sort_general(uint64_t n, const double* r_in, double* r_sorted,
         sort_scan_hist_kernel<<<NPASS, RADIX, 0, st>>>(ws.digit_hist, n, pass_live, guard);
         HMC_LAUNCH_CHECK();
     }
-    static bool attr_done = false;
-    if (!attr_done) {
-        HMC_CUDA_TRY(cudaFuncSetAttribute(sort_onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)sizeof(SortSmem)));
-        attr_done = true;
-    }
+    static std::atomic<uint64_t> opted{ 0 };
+    hmc_status so = smem_opt_in(opted, sort_onesweep_kernel, sizeof(SortSmem));
+    if (so != HMC_OK) return so;
     SortBuffers buf;
     buf.keys_src = keys0;
     buf.keys[0] = ws.keys_alt; buf.keys[1] = reinterpret_cast<uint64_t*>(r_sorted);

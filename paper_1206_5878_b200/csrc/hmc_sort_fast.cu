@@ -477,11 +477,9 @@ hmc_status sort_fast(uint64_t n, const double* r_in, double* r_sorted, uint32_t*
     sort_pk_scan_hist_kernel<<<PK_MAXPASS, PK_RADIX, 0, st>>>(ws.pk_hist, (uint32_t)n, pass_live);
     HMC_LAUNCH_CHECK();
     const int copy_blocks = (int)umin64((n + 255) / 256, (uint64_t)sms * 8);
-    static bool attr_done = false;
-    if (!attr_done) {
-        HMC_CUDA_TRY(cudaFuncSetAttribute(sort_pk_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PkSmem)));
-        attr_done = true;
-    }
+    static std::atomic<uint64_t> opted{ 0 };
+    hmc_status so = smem_opt_in(opted, sort_pk_pass_kernel, sizeof(PkSmem));
+    if (so != HMC_OK) return so;
     PkBuffers b{ keys, { ws.keys_alt, ws.pk_alt } };
     int ib = 1;
     while ((1ull << ib) < n) ++ib;                                          // as packing_of

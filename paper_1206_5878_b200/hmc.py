@@ -32,25 +32,31 @@ class HmcError(RuntimeError):
     pass
 
 
+def load(path: str) -> ctypes.CDLL:
+    """Open a build of libhmc and declare its entry points.  Raises if absent (there is no CPU fallback)."""
+    if not os.path.exists(path):
+        raise HmcError("%s not found; run `python -m paper_1206_5878_b200.build` (there is no CPU fallback)" % path)
+    L = ctypes.CDLL(path)
+    L.hmc_workspace_bytes.restype = ctypes.c_size_t
+    L.hmc_workspace_bytes.argtypes = [ctypes.c_uint64]
+    L.hmc_step_host_arena_bytes.restype = ctypes.c_size_t
+    L.hmc_step_host_arena_bytes.argtypes = [ctypes.c_uint64]
+    L.hmc_status_string.restype = ctypes.c_char_p
+    L.hmc_status_string.argtypes = [ctypes.c_int32]
+    L.hmc_version.restype = ctypes.c_int32
+    L.hmc_t_max.restype = ctypes.c_uint32
+    L.hmc_launch_count.restype = ctypes.c_uint64
+    for name in ("hmc_sort_by_radius", "hmc_potential", "hmc_orbit_turning_points", "hmc_sample_new_radius",
+                 "hmc_orbit_step", "hmc_diagnostics", "hmc_energy_correction", "hmc_step_host"):
+        getattr(L, name).restype = ctypes.c_int32
+    return L
+
+
 def lib() -> ctypes.CDLL:
-    """Load libhmc.so (built in-tree by paper_1206_5878_b200.build).  Raises if absent."""
+    """The library every binding call goes through: libhmc.so, loaded at first use."""
     global _lib
     if _lib is None:
-        if not os.path.exists(LIB_PATH):
-            raise HmcError("libhmc.so not found at %s; run `python -m paper_1206_5878_b200.build` "
-                           "(there is no CPU fallback)" % LIB_PATH)
-        L = ctypes.CDLL(LIB_PATH)
-        L.hmc_workspace_bytes.restype = ctypes.c_size_t
-        L.hmc_workspace_bytes.argtypes = [ctypes.c_uint64]
-        L.hmc_step_host_arena_bytes.restype = ctypes.c_size_t
-        L.hmc_step_host_arena_bytes.argtypes = [ctypes.c_uint64]
-        L.hmc_status_string.restype = ctypes.c_char_p
-        L.hmc_status_string.argtypes = [ctypes.c_int32]
-        L.hmc_version.restype = ctypes.c_int32
-        for name in ("hmc_sort_by_radius", "hmc_potential", "hmc_orbit_turning_points", "hmc_sample_new_radius",
-                     "hmc_orbit_step", "hmc_diagnostics", "hmc_energy_correction", "hmc_step_host"):
-            getattr(L, name).restype = ctypes.c_int32
-        _lib = L
+        _lib = load(LIB_PATH)
     return _lib
 
 
@@ -255,24 +261,9 @@ def hmc_diagnostics(r_sorted, v_r, v_t, m_sorted, phi, m_cum, fractions: Sequenc
     return out
 
 
-def kernel_launches_per_step(n: int, ncols: int = 3, with_id: bool = True, fused: bool = False) -> int:
-    """How many kernels of libhmc one orbit step (the four calls, S4 with reuse_tables) launches for
-    n stars; mirrors the host code of csrc/*.cu (memsets are not counted)."""
-    if n < 2:
-        return (14 if (ncols or with_id) else 13) + 3 + 3 + 1
-    ib = max(1, (n - 1).bit_length())
-    idx_bits = max(24, ib)
-    key_bits = min(((ib + 8 + 7) // 8) * 8, 40, 64 - idx_bits)
-    npass = (key_bits + 7) // 8
-    fast = 3 + npass + 1                             # range, histogram (+ star records), bin scan, digit passes, finish
-    general = 1 + 2 + 8 + 1 + (1 if (ncols or with_id) else 0)   # guarded: zero, histogram, bin scan, 8 passes, identity, gather
-    shift = 0
-    while (n >> shift) + 2 > 10240:
-        shift += 1
-    tables = 2 if shift > 0 else 1
-    if fused:
-        return fast + general + 3 + (tables + 1)     # + potential (3) + tables and the fused S3/S4 kernel
-    return fast + general + 3 + (tables + 1) + 1     # + potential (3) + S3 (tables, search) + S4 (1)
+def launch_count() -> int:
+    """Kernels this process has launched through libhmc so far (hmc_launch_count)."""
+    return int(lib().hmc_launch_count())
 
 
 class OrbitStepper:

@@ -49,6 +49,21 @@ def test_host_only_entry_points(libhmc):
     assert libhmc.hmc_version() >= 100
 
 
+def test_build_variants_and_launch_counter(libhmc):
+    """The product build caps the rejection loop at 4096 trials; the test-only build (GPU tests of the
+    exhaustion path) at 3.  The launch counter starts at zero and nothing here launches a kernel."""
+    from paper_1206_5878_b200 import build
+    libhmc.hmc_t_max.restype = ctypes.c_uint32
+    libhmc.hmc_launch_count.restype = ctypes.c_uint64
+    assert libhmc.hmc_t_max() == 4096
+    assert libhmc.hmc_launch_count() == 0
+    t3 = ctypes.CDLL(build.build(variant="tmax3"))
+    t3.hmc_t_max.restype = ctypes.c_uint32
+    assert t3.hmc_t_max() == 3
+    for f in declared_functions():
+        assert hasattr(t3, f), f
+
+
 def test_argument_errors_do_not_need_a_gpu(libhmc):
     # call-level validation happens before any CUDA call
     null = ctypes.c_void_p(0)
