@@ -75,6 +75,23 @@ __device__ __forceinline__ uint32_t ld_u32_na(const uint32_t* __restrict__ p)
     return v;
 }
 
+// The radius directory (4 bytes per star) is small enough to live in the 126 MB L2, the node table
+// (32 bytes per star) is not, and every star reads a few random lines of each: directory lines are
+// loaded with an evict-last L2 policy so that the node traffic streaming through L2 does not push them out.
+__device__ __forceinline__ uint64_t l2_keep_policy()
+{
+    uint64_t pol;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+
+__device__ __forceinline__ uint32_t ld_u32_keep(const uint32_t* __restrict__ p, uint64_t pol)
+{
+    uint32_t v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.u32 %0, [%1], %2;" : "=r"(v) : "l"(p), "l"(pol));
+    return v;
+}
+
 // ---- radius directory -------------------------------------------------------------------------
 // Coarse interval c holds the nodes j with j >> shift == c (j >= 1); its radii lie in [Rl, Rh],
 // Rl = r of node c << shift (0 for c = 0), Rh = r of node (c+1) << shift (r_N in the last
@@ -114,13 +131,18 @@ __global__ void __launch_bounds__(256) build_nodes_kernel(const double* __restri
     }
 }
 
-// One CTA per coarse interval: the interval's nodes are counted into their buckets in shared memory
-// (radii ascend, so neighbouring threads hit neighbouring counters), the counts are scanned, and the row
-// is written as whole 32-bit entries, coalesced.
+// The tables of one coarse interval, by one CTA (shift > 0): the interval's nodes are written (r, Phi, M read once,
+// coalesced), counted into their buckets in shared memory (radii ascend, so neighbouring threads hit neighbouring
+// counters), the counts are scanned, and the directory row is written as whole 32-bit entries, coalesced.
+// The CTA of interval 0 also writes the sentinel node 0, the last one node N+1; coarse and mid entries are written
+// by whoever owns the node.
 static constexpr int DIR_THREADS = 256;
 
-__global__ void __launch_bounds__(DIR_THREADS) build_dir_kernel(const double* __restrict__ r, uint32_t* __restrict__ dir,
-                                                                uint32_t n, int shift)
+__global__ void __launch_bounds__(DIR_THREADS) build_tables_kernel(const double* __restrict__ r, const double* __restrict__ phi,
+                                                                   const double* __restrict__ m_cum, double G,
+                                                                   Node* __restrict__ nodes, double2* __restrict__ coarse_g,
+                                                                   double2* __restrict__ mid_g, uint32_t* __restrict__ dir,
+                                                                   uint32_t n, int shift)
 {
     extern __shared__ uint32_t cnt[];                                // [K + 1]: cnt[b + 1] = nodes in bucket b, then o_b
     __shared__ uint32_t warp_tot[DIR_THREADS / 32];
@@ -131,8 +153,29 @@ __global__ void __launch_bounds__(DIR_THREADS) build_dir_kernel(const double* __
     const double Rh = (((uint64_t)(c + 1) << shift) <= n) ? __ldg(r + (((c + 1) << shift) - 1)) : __ldg(r + (n - 1));
     const float scale = bucket_scale(Rl, Rh, K);
     for (uint32_t b = threadIdx.x; b <= K; b += DIR_THREADS) cnt[b] = 0;
+    if (threadIdx.x == 0) {
+        if (c == 0) {
+            Node e; e.r = 0.0; e.phi = __ldg(phi); e.B = 0.0; e.u = 0.0;
+            nodes[0] = e;
+            coarse_g[0] = make_double2(e.r, e.phi);
+            if (shift > MID_SHIFT) mid_g[0] = make_double2(e.r, e.phi);
+        }
+        if (c == gridDim.x - 1) {
+            Node e; e.r = pos_inf(); e.phi = 0.0; e.B = G * __ldg(m_cum + (n - 1)); e.u = 0.0;
+            nodes[(size_t)n + 1] = e;
+        }
+    }
     __syncthreads();
-    for (uint32_t j = j0 + threadIdx.x; j <= jn; j += DIR_THREADS) atomicAdd(&cnt[bucket(__ldcs(r + (j - 1)), Rl, scale, K) + 1], 1u);
+    const uint32_t low_mask = K - 1u;
+    for (uint32_t j = j0 + threadIdx.x; j <= jn; j += DIR_THREADS) {
+        Node e;
+        const double rj = __ldcs(r + (j - 1));
+        e.r = rj; e.phi = __ldcs(phi + (j - 1)); e.B = G * __ldcs(m_cum + (j - 1)); e.u = 1.0 / rj;
+        nodes[j] = e;
+        if ((j & low_mask) == 0) coarse_g[j >> shift] = make_double2(e.r, e.phi);
+        if (shift > MID_SHIFT && (j & ((1u << MID_SHIFT) - 1)) == 0) mid_g[j >> MID_SHIFT] = make_double2(e.r, e.phi);
+        atomicAdd(&cnt[bucket(rj, Rl, scale, K) + 1], 1u);
+    }
     __syncthreads();
     // inclusive scan of cnt[0 .. K] in place: cnt[b] becomes o_b = number of nodes with bucket < b
     const uint32_t per = (K + 1 + DIR_THREADS - 1) / DIR_THREADS;
@@ -171,6 +214,7 @@ struct Tables {
     double r_last;           // r_N
     uint32_t n, ncoarse, K;
     int shift;
+    uint64_t keep;           // L2 evict-last policy for directory loads
     // (r, Phi) of node j, j a multiple of the finest table spacing in use
     __device__ __forceinline__ double2 aligned_node(uint32_t j) const { return mid ? ld_d2_na(mid + (j >> MID_SHIFT)) : coarse[j >> shift]; }
     // upper radius of coarse interval c, as build_dir_kernel defines it
@@ -182,7 +226,7 @@ struct Tables {
     {
         const double Rl = coarse[c].x;
         const uint32_t b = bucket(x, Rl, bucket_scale(Rl, interval_rh(c), K), K);
-        const uint32_t w = ld_u32_na(dir + (size_t)c * K + b);
+        const uint32_t w = ld_u32_keep(dir + (size_t)c * K + b, keep);
         const uint32_t o0 = w & 0xffffu, o1 = w >> 16;
         const uint32_t j0 = max(c << shift, 1u);
         lo = j0 + o0 - 1;
@@ -352,8 +396,8 @@ __device__ __forceinline__ Solved solve_star(const Tables& T, uint32_t a, double
             const uint32_t* a1 = g1 ? T.dir_guess_slot(c1, x1, f1) : nullptr;
             const uint32_t* a2 = g2 ? T.dir_guess_slot(c2, x2, f2) : nullptr;
             uint32_t w1 = 0, w2 = 0;
-            if (g1) w1 = ld_u32_na(a1);
-            if (g2) w2 = ld_u32_na(a2);
+            if (g1) w1 = ld_u32_keep(a1, T.keep);
+            if (g2) w2 = ld_u32_keep(a2, T.keep);
             if (g1) { s1.guess = T.dir_guess_node(c1, w1, f1); s1.mode = MODE_GUESS; }
             if (g2) { s2.guess = T.dir_guess_node(c2, w2, f2); s2.mode = MODE_GUESS; }
         }
@@ -405,7 +449,7 @@ turning_points_kernel(uint32_t n, double G, const double* __restrict__ r, const 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* coarse = reinterpret_cast<double2*>(smem_raw);
     stage_coarse(coarse, coarse_g, n, shift);
-    Tables T{ nodes, dir, coarse, shift > MID_SHIFT ? mid_g : nullptr, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift };
+    Tables T{ nodes, dir, coarse, shift > MID_SHIFT ? mid_g : nullptr, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift, l2_keep_policy() };
 
     const uint32_t stride = gridDim.x * ORB_THREADS;
     for (uint32_t a = blockIdx.x * ORB_THREADS + threadIdx.x; a < n; a += stride) {
@@ -682,7 +726,7 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
     Park& pk = reinterpret_cast<Park*>(smem_raw)[threadIdx.x >> 5];
     double2* coarse = reinterpret_cast<double2*>(smem_raw + ORB_WARPS * sizeof(Park));
     stage_coarse(coarse, coarse_g, n, shift);
-    Tables T{ nodes, dir, coarse, (FUSED && shift > MID_SHIFT) ? mid_g : nullptr, __ldg(io.r + (n - 1)), n, n >> shift, 1u << shift, shift };
+    Tables T{ nodes, dir, coarse, (FUSED && shift > MID_SHIFT) ? mid_g : nullptr, __ldg(io.r + (n - 1)), n, n >> shift, 1u << shift, shift, l2_keep_policy() };
     unsigned long long my_trials = 0;
     const unsigned lane_lt = lanemask_lt();
     const uint32_t lane = threadIdx.x & 31;
@@ -815,7 +859,7 @@ energy_correction_kernel(uint32_t n, const Node* __restrict__ nodes, const doubl
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* coarse = reinterpret_cast<double2*>(smem_raw);
     stage_coarse(coarse, coarse_g, n, shift);
-    Tables T{ nodes, dir, coarse, nullptr, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift };
+    Tables T{ nodes, dir, coarse, nullptr, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift, l2_keep_policy() };
     const uint32_t stride = gridDim.x * ORB_THREADS;
     for (uint32_t a = blockIdx.x * ORB_THREADS + threadIdx.x; a < n; a += stride) {
         const double x = __ldcs(r_old + a);
@@ -851,18 +895,19 @@ energy_correction_kernel(uint32_t n, const Node* __restrict__ nodes, const doubl
 static hmc_status build_tables(uint64_t n, double G, const double* r, const double* phi, const double* m_cum,
                                const Workspace& ws, int shift, cudaStream_t st)
 {
-    const int sms = sm_count();
-    int blocks = (int)umin64((n + 2 + 255) / 256, (uint64_t)sms * 8);
-    build_nodes_kernel<<<blocks, 256, 0, st>>>(r, phi, m_cum, G, ws.nodes, ws.coarse, ws.mid, shift, n);
-    HMC_LAUNCH_CHECK();
-    if (shift > 0) {
-        const size_t smem = ((size_t)(1u << shift) + 1) * sizeof(uint32_t);
-        static std::atomic<uint64_t> opted{ 0 };                  // the largest row any n <= HMC_MAX_N needs
-        hmc_status so = smem_opt_in(opted, build_dir_kernel, ((size_t)(1u << coarse_shift(HMC_MAX_N)) + 1) * sizeof(uint32_t));
-        if (so != HMC_OK) return so;
-        build_dir_kernel<<<(unsigned)((n >> shift) + 1), DIR_THREADS, smem, st>>>(r, ws.dir, (uint32_t)n, shift);
+    if (shift == 0) {                                            // the coarse table is the whole table: no directory
+        const int blocks = (int)umin64((n + 2 + 255) / 256, (uint64_t)sm_count() * 8);
+        build_nodes_kernel<<<blocks, 256, 0, st>>>(r, phi, m_cum, G, ws.nodes, ws.coarse, ws.mid, shift, n);
         HMC_LAUNCH_CHECK();
+        return HMC_OK;
     }
+    const size_t smem = ((size_t)(1u << shift) + 1) * sizeof(uint32_t);
+    static std::atomic<uint64_t> opted{ 0 };                      // the largest row any n <= HMC_MAX_N needs
+    hmc_status so = smem_opt_in(opted, build_tables_kernel, ((size_t)(1u << coarse_shift(HMC_MAX_N)) + 1) * sizeof(uint32_t));
+    if (so != HMC_OK) return so;
+    build_tables_kernel<<<(unsigned)((n >> shift) + 1), DIR_THREADS, smem, st>>>(r, phi, m_cum, G, ws.nodes, ws.coarse, ws.mid,
+                                                                                 ws.dir, (uint32_t)n, shift);
+    HMC_LAUNCH_CHECK();
     return HMC_OK;
 }
 

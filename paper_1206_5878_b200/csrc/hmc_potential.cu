@@ -1,24 +1,49 @@
 // hmc_potential.cu -- S2: Phi_k = -G (M_k / r_k + S_k) on the radius-sorted arrays.
 //
 // The paper computes Phi by the backward recursion Eq. 2-5 and calls it "inherently sequential"
-// (PAPER.md:185).  Here it is a reduce-then-scan over tiles of 2048 stars, three launches:
-//   1. potential_reduce_kernel : per tile, T_m = sum m_i and T_t = sum fl(m_i / r_i)
-//   2. potential_totals_kernel : one CTA; exclusive prefix of T_m (inside out) and exclusive
-//                                suffix of T_t (outside in) over the tiles
-//   3. potential_apply_kernel  : per tile, forward scan of m and backward scan of m/r in
-//                                registers, M_k and S_k rounded once, Phi_k = -(G*(M_k/r_k + S_k)).
-// Every partial sum is double-double (106 bits), so M_k and S_k are the exact sums rounded once
-// and do not depend on the association order (R1p).  There is no inter-CTA waiting.
-// Launch 3 walks the tiles in the opposite order to launch 1, so the part of r, m that is still
-// in the 126 MB L2 is read from there.
+// (PAPER.md:185).  Here the stars are cut into CHUNKS of consecutive tiles (a tile = 2048 stars), one chunk per
+// CTA of a grid that fills the machine once, and the stage is two launches without any inter-CTA waiting:
+//   1. potential_reduce_kernel : every warp sums slices of 1024 consecutive stars, T_m = sum m_i and
+//                                T_t = sum fl(m_i / r_i); per-slice and per-chunk totals go to the workspace.
+//   2. potential_apply_kernel  : the CTA of chunk c adds up the chunk totals before (T_m) and after (T_t) its
+//                                chunk -- a few hundred values, once per CTA -- and the slice totals inside it,
+//                                then walks its tiles from the last to the first: forward scan of m and
+//                                backward scan of m/r in registers, M_k and S_k rounded once,
+//                                Phi_k = -(G*(M_k/r_k + S_k)).
+// (Round 1 had a third, single-CTA launch between the two that scanned ~5000 tile totals while the rest of the
+// GPU idled for 20 us.)  The reduce launch walks each chunk forwards, the apply launch backwards, so the tail of
+// every chunk is still in the 126 MB L2 when it is read the second time.
+//
+// Every partial sum is double-double (106 bits), so M_k and S_k are the exact sums rounded once and do not
+// depend on the association order (R1p).  Adding two double-double PARTIAL SUMS uses the short form of
+// the addition (one two_sum and a renormalisation): its error bound, 2^-104 relative to |a| + |b|, is relative to
+// the result because the summands m_i and m_i / r_i are non-negative (precondition m >= 0, r > 0).
 #include "hmc_common.cuh"
 
 namespace hmc {
 
-static constexpr int SCAN_THREADS = 128;
-static constexpr int SCAN_ITEMS = SCAN_TILE / SCAN_THREADS;   // 16
+static constexpr int SCAN_THREADS = 256;
 static constexpr int SCAN_WARPS = SCAN_THREADS / 32;
-static constexpr int TOT_THREADS = 1024;
+static constexpr int SCAN_ITEMS = SCAN_TILE / SCAN_THREADS;   // 8 consecutive stars per thread in the apply launch
+static constexpr int SLICE = 1024;                            // stars per warp-slice of the reduce launch
+static constexpr int SLICES_PER_TILE = SCAN_TILE / SLICE;     // 2
+#ifndef HMC_S2_CTAS
+#define HMC_S2_CTAS 3
+#endif
+#ifndef HMC_S2_BATCH
+#define HMC_S2_BATCH 4
+#endif
+static constexpr int CHUNK_CTAS_PER_SM = HMC_S2_CTAS;         // chunks = CTAs resident at once: registers allow 3 x 256 threads
+static constexpr int RED_BATCH = HMC_S2_BATCH;                // 16-byte loads in flight per array and lane in the reduce launch
+static_assert(SCAN_ITEMS == 8, "the apply launch loads 2 x 4 consecutive doubles per thread and array");
+
+// double-double sum of two double-double values of the same sign (see the header): 11 operations instead of 20
+__device__ __forceinline__ dd dd_add_pos(dd a, dd b)
+{
+    dd s = two_sum(a.hi, b.hi);
+    s.lo += a.lo + b.lo;
+    return quick_two_sum(s.hi, s.lo);
+}
 
 __device__ __forceinline__ dd dd_shfl_xor(dd v, int mask)
 {
@@ -28,177 +53,205 @@ __device__ __forceinline__ dd dd_shfl_down(dd v, int delta)
 {
     return dd{ __shfl_down_sync(0xffffffffu, v.hi, delta), __shfl_down_sync(0xffffffffu, v.lo, delta) };
 }
+__device__ __forceinline__ dd dd_shfl(dd v, int lane)
+{
+    return dd{ __shfl_sync(0xffffffffu, v.hi, lane), __shfl_sync(0xffffffffu, v.lo, lane) };
+}
 
-// ---- 1. tile totals ---------------------------------------------------------------------------
-// totals[tile] = (T_m.hi, T_m.lo, T_t.hi, T_t.lo).  Element order inside a tile is irrelevant for
-// a sum, so the loads are fully coalesced 16-byte loads.
-__global__ void __launch_bounds__(SCAN_THREADS)
-potential_reduce_kernel(const double* __restrict__ r, const double* __restrict__ m, uint64_t n,
-                        double4* __restrict__ totals)
+__device__ __forceinline__ void ld4(const double* __restrict__ p, double v[4])
+{
+    asm("ld.global.nc.L1::no_allocate.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3]) : "l"(p));
+}
+__device__ __forceinline__ void st4(double* __restrict__ p, const double v[4])
+{
+    asm volatile("st.global.cs.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(v[0]), "d"(v[1]), "d"(v[2]), "d"(v[3]) : "memory");
+}
+
+// How the stars are cut up; the same for both launches.  Chunk c = tiles [c * tpc, min(ntiles, (c+1) * tpc)).
+struct ScanPlan {
+    uint32_t ntiles, nslices, tpc, nchunks;
+};
+
+static inline ScanPlan scan_plan(uint64_t n, int sms)
+{
+    ScanPlan p;
+    p.ntiles = (uint32_t)((n + SCAN_TILE - 1) / SCAN_TILE);
+    p.nslices = (uint32_t)((n + SLICE - 1) / SLICE);
+    const uint32_t want = (uint32_t)sms * CHUNK_CTAS_PER_SM;
+    p.tpc = (p.ntiles + want - 1) / want;
+    if (p.tpc == 0) p.tpc = 1;
+    p.nchunks = (p.ntiles + p.tpc - 1) / p.tpc;
+    return p;
+}
+
+// ---- 1. slice and chunk totals -----------------------------------------------------------------
+// slice_tot[s] = (T_m.hi, T_m.lo, T_t.hi, T_t.lo) of stars [s * 1024, (s+1) * 1024); chunk_tot[c] likewise for
+// the whole chunk.  The order of the elements inside a slice is irrelevant for a sum, so the loads are fully
+// coalesced 16-byte loads; a warp works alone (no barrier inside the loop).
+__global__ void __launch_bounds__(SCAN_THREADS, CHUNK_CTAS_PER_SM)
+potential_reduce_kernel(const double* __restrict__ r, const double* __restrict__ m, uint64_t n, ScanPlan plan,
+                        double4* __restrict__ slice_tot, double4* __restrict__ chunk_tot)
 {
     __shared__ dd sm_m[SCAN_WARPS], sm_t[SCAN_WARPS];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint64_t base = (uint64_t)blockIdx.x * SCAN_TILE;
-    dd am{ 0.0, 0.0 }, at{ 0.0, 0.0 };
-    if (base + SCAN_TILE <= n && ((reinterpret_cast<uintptr_t>(r) | reinterpret_cast<uintptr_t>(m)) & 15) == 0) {
-        const double2* r2 = reinterpret_cast<const double2*>(r + base);
-        const double2* m2 = reinterpret_cast<const double2*>(m + base);
-        double2 rv[SCAN_ITEMS / 2], mv[SCAN_ITEMS / 2];
+    const uint32_t c = blockIdx.x;
+    const uint32_t s0 = c * plan.tpc * SLICES_PER_TILE;
+    const uint32_t s1 = min(plan.nslices, (c + 1) * plan.tpc * SLICES_PER_TILE);
+    const bool aligned = ((reinterpret_cast<uintptr_t>(r) | reinterpret_cast<uintptr_t>(m)) & 15) == 0;
+    dd cm{ 0.0, 0.0 }, ct{ 0.0, 0.0 };                           // this warp's share of the chunk
+    for (uint32_t s = s0 + warp; s < s1; s += SCAN_WARPS) {
+        const uint64_t base = (uint64_t)s * SLICE;
+        dd am{ 0.0, 0.0 }, at{ 0.0, 0.0 }, bm{ 0.0, 0.0 }, bt{ 0.0, 0.0 };   // two chains per sum: the adds are dependent
+        if (base + SLICE <= n && aligned) {
+            const double2* r2 = reinterpret_cast<const double2*>(r + base) + lane;
+            const double2* m2 = reinterpret_cast<const double2*>(m + base) + lane;
 #pragma unroll
-        for (int i = 0; i < SCAN_ITEMS / 2; ++i) { rv[i] = __ldg(r2 + i * SCAN_THREADS + tid); mv[i] = __ldg(m2 + i * SCAN_THREADS + tid); }
+            for (int h = 0; h < 16 / RED_BATCH; ++h) {
+                double2 rv[RED_BATCH], mv[RED_BATCH];
 #pragma unroll
-        for (int i = 0; i < SCAN_ITEMS / 2; ++i) {
-            am = dd_add_d(am, mv[i].x); am = dd_add_d(am, mv[i].y);
-            at = dd_add_d(at, mv[i].x / rv[i].x); at = dd_add_d(at, mv[i].y / rv[i].y);
+                for (int i = 0; i < RED_BATCH; ++i) { rv[i] = __ldg(r2 + (h * RED_BATCH + i) * 32); mv[i] = __ldg(m2 + (h * RED_BATCH + i) * 32); }
+#pragma unroll
+                for (int i = 0; i < RED_BATCH; ++i) {
+                    am = dd_add_d(am, mv[i].x); bm = dd_add_d(bm, mv[i].y);
+                    at = dd_add_d(at, mv[i].x / rv[i].x); bt = dd_add_d(bt, mv[i].y / rv[i].y);
+                }
+            }
+            am = dd_add_pos(am, bm); at = dd_add_pos(at, bt);
+        } else {
+            for (int i = 0; i < SLICE / 32; ++i) {
+                const uint64_t a = base + (uint64_t)i * 32 + lane;
+                if (a < n) { const double mm = m[a]; am = dd_add_d(am, mm); at = dd_add_d(at, mm / r[a]); }
+            }
         }
-    } else {
 #pragma unroll
-        for (int i = 0; i < SCAN_ITEMS; ++i) {
-            uint64_t a = base + (uint64_t)i * SCAN_THREADS + tid;
-            if (a < n) { double mm = m[a]; am = dd_add_d(am, mm); at = dd_add_d(at, mm / r[a]); }
-        }
+        for (int d = 16; d > 0; d >>= 1) { am = dd_add_pos(am, dd_shfl_xor(am, d)); at = dd_add_pos(at, dd_shfl_xor(at, d)); }
+        if (lane == 0) slice_tot[s] = make_double4(am.hi, am.lo, at.hi, at.lo);
+        cm = dd_add_pos(cm, am); ct = dd_add_pos(ct, at);         // the same value in every lane
     }
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) { am = dd_add(am, dd_shfl_xor(am, d)); at = dd_add(at, dd_shfl_xor(at, d)); }
-    if (lane == 0) { sm_m[warp] = am; sm_t[warp] = at; }
+    if (lane == 0) { sm_m[warp] = cm; sm_t[warp] = ct; }
     __syncthreads();
     if (tid == 0) {
 #pragma unroll
-        for (int w = 1; w < SCAN_WARPS; ++w) { am = dd_add(am, sm_m[w]); at = dd_add(at, sm_t[w]); }
-        totals[blockIdx.x] = make_double4(am.hi, am.lo, at.hi, at.lo);
+        for (int w = 1; w < SCAN_WARPS; ++w) { cm = dd_add_pos(cm, sm_m[w]); ct = dd_add_pos(ct, sm_t[w]); }
+        chunk_tot[c] = make_double4(cm.hi, cm.lo, ct.hi, ct.lo);
     }
 }
 
-// ---- 2. scan of the tile totals (single CTA) ---------------------------------------------------
-// in : totals[tile] = (T_m, T_t);  out: totals[tile] = (prefix of T_m over tiles < tile,
-//                                                       suffix of T_t over tiles > tile)
-__global__ void __launch_bounds__(TOT_THREADS)
-potential_totals_kernel(double4* __restrict__ totals, uint32_t ntiles)
-{
-    __shared__ dd sm_m[TOT_THREADS / 32], sm_t[TOT_THREADS / 32];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t per = (ntiles + TOT_THREADS - 1) / TOT_THREADS;
-    const uint32_t lo = min(ntiles, (uint32_t)tid * per), hi = min(ntiles, lo + per);
-    dd tm{ 0.0, 0.0 }, tt{ 0.0, 0.0 };
-    for (uint32_t i = lo; i < hi; ++i) {
-        double4 v = totals[i];
-        tm = dd_add(tm, dd{ v.x, v.y });
-        tt = dd_add(tt, dd{ v.z, v.w });
-    }
-    // inclusive scans over threads: forward for m, backward for t
-    dd im = tm, it = tt;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        dd up = dd_shfl_up(im, d);
-        if (lane >= d) im = dd_add(up, im);
-        dd dn = dd_shfl_down(it, d);
-        if (lane + d < 32) it = dd_add(it, dn);
-    }
-    if (lane == 31) sm_m[warp] = im;
-    if (lane == 0) sm_t[warp] = it;
-    __syncthreads();
-    dd em{ 0.0, 0.0 }, et{ 0.0, 0.0 };
-    for (int w = 0; w < warp; ++w) em = dd_add(em, sm_m[w]);
-    for (int w = TOT_THREADS / 32 - 1; w > warp; --w) et = dd_add(et, sm_t[w]);
-    {
-        dd pm = dd_shfl_up(im, 1), pt = dd_shfl_down(it, 1);
-        if (lane > 0) em = dd_add(em, pm);
-        if (lane < 31) et = dd_add(et, pt);
-    }
-    // em = sum of T_m over all tiles owned by lower threads; et = sum of T_t over higher threads.
-    // suffix inside the thread's own range needs the later tiles first: walk it backwards.
-    dd run_t = et;
-    for (uint32_t i = hi; i-- > lo;) {
-        double4 v = totals[i];
-        totals[i].z = run_t.hi; totals[i].w = run_t.lo;
-        run_t = dd_add(run_t, dd{ v.z, v.w });
-    }
-    dd run_m = em;
-    for (uint32_t i = lo; i < hi; ++i) {
-        double4 v = totals[i];
-        totals[i].x = run_m.hi; totals[i].y = run_m.lo;
-        run_m = dd_add(run_m, dd{ v.x, v.y });
-    }
-}
+// ---- 2. per-tile scans and Phi -----------------------------------------------------------------
+static constexpr int MAX_TPC_SMEM = 256;      // tiles per chunk whose offsets fit the shared array (n <= HMC_MAX_N: 222)
 
-// ---- 3. per-tile scans and Phi -----------------------------------------------------------------
-__global__ void __launch_bounds__(SCAN_THREADS)
+__global__ void __launch_bounds__(SCAN_THREADS, CHUNK_CTAS_PER_SM)
 potential_apply_kernel(const double* __restrict__ r, const double* __restrict__ m, double* __restrict__ phi,
-                       double* __restrict__ m_cum, uint64_t n, double G, const double4* __restrict__ totals,
-                       uint32_t ntiles)
+                       double* __restrict__ m_cum, uint64_t n, double G, ScanPlan plan,
+                       const double4* __restrict__ slice_tot, const double4* __restrict__ chunk_tot)
 {
-    __shared__ dd sm_m[SCAN_WARPS], sm_t[SCAN_WARPS];
+    __shared__ dd sm_m[2][SCAN_WARPS], sm_t[2][SCAN_WARPS];     // per-warp totals of the tile being scanned (by tile parity)
+    __shared__ dd sm_pm[MAX_TPC_SMEM];                          // sum of m over everything before tile k of this chunk
+    __shared__ dd sm_slice[MAX_TPC_SMEM * SLICES_PER_TILE];     // T_m of the chunk's slices (prologue only)
+    __shared__ dd sm_after[2];                                  // sum of m/r over everything after the current tile (by parity)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t tile = ntiles - 1 - blockIdx.x;           // opposite order to the reduce launch
-    const uint64_t p0 = (uint64_t)tile * SCAN_TILE + (uint64_t)tid * SCAN_ITEMS;
-    double rr[SCAN_ITEMS], mm[SCAN_ITEMS], tt[SCAN_ITEMS];
-    const bool full = (uint64_t)tile * SCAN_TILE + SCAN_TILE <= n;
-    const bool al = ((reinterpret_cast<uintptr_t>(r) | reinterpret_cast<uintptr_t>(m)) & 15) == 0;
-    if (full && al) {
-        const double2* r2 = reinterpret_cast<const double2*>(r + p0);
-        const double2* m2 = reinterpret_cast<const double2*>(m + p0);
-#pragma unroll
-        for (int i = 0; i < SCAN_ITEMS / 2; ++i) {
-            double2 a = __ldg(r2 + i), b = __ldg(m2 + i);
-            rr[2 * i] = a.x; rr[2 * i + 1] = a.y; mm[2 * i] = b.x; mm[2 * i + 1] = b.y;
-        }
-    } else {
-#pragma unroll
-        for (int i = 0; i < SCAN_ITEMS; ++i) {
-            uint64_t p = p0 + i;
-            rr[i] = (p < n) ? r[p] : 1.0;
-            mm[i] = (p < n) ? m[p] : 0.0;
-        }
-    }
-    dd tm{ 0.0, 0.0 }, ts{ 0.0, 0.0 };
-#pragma unroll
-    for (int i = 0; i < SCAN_ITEMS; ++i) {
-        tt[i] = mm[i] / rr[i];
-        tm = dd_add_d(tm, mm[i]);
-        ts = dd_add_d(ts, tt[i]);
-    }
-    dd im = tm, it = ts;                                       // inclusive over threads: forward m, backward t
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        dd up = dd_shfl_up(im, d);
-        if (lane >= d) im = dd_add(up, im);
-        dd dn = dd_shfl_down(it, d);
-        if (lane + d < 32) it = dd_add(it, dn);
-    }
-    if (lane == 31) sm_m[warp] = im;
-    if (lane == 0) sm_t[warp] = it;
-    __syncthreads();
-    const double4 tp = totals[tile];
-    dd em{ tp.x, tp.y }, et{ tp.z, tp.w };                     // everything before / after this tile
-    for (int w = 0; w < warp; ++w) em = dd_add(em, sm_m[w]);
-    for (int w = SCAN_WARPS - 1; w > warp; --w) et = dd_add(et, sm_t[w]);
+    const uint32_t c = blockIdx.x;
+    const uint32_t t0 = c * plan.tpc, t1 = min(plan.ntiles, t0 + plan.tpc);
+
+    // ---- prologue: what lies before and after this chunk, from the chunk totals (once per CTA)
     {
-        dd pm = dd_shfl_up(im, 1), pt = dd_shfl_down(it, 1);
-        if (lane > 0) em = dd_add(em, pm);
-        if (lane < 31) et = dd_add(et, pt);
+        dd pm{ 0.0, 0.0 }, st{ 0.0, 0.0 };
+        for (uint32_t j = tid; j < plan.nchunks; j += SCAN_THREADS) {
+            if (j == c) continue;
+            const double4 v = chunk_tot[j];
+            if (j < c) pm = dd_add_pos(pm, dd{ v.x, v.y });
+            else st = dd_add_pos(st, dd{ v.z, v.w });
+        }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) { pm = dd_add_pos(pm, dd_shfl_xor(pm, d)); st = dd_add_pos(st, dd_shfl_xor(st, d)); }
+        if (lane == 0) { sm_m[0][warp] = pm; sm_t[0][warp] = st; }
+        const uint32_t sl0 = t0 * SLICES_PER_TILE, sl1 = min(plan.nslices, t1 * SLICES_PER_TILE);
+        for (uint32_t s = sl0 + tid; s < sl1; s += SCAN_THREADS) { const double4 v = slice_tot[s]; sm_slice[s - sl0] = dd{ v.x, v.y }; }
+        __syncthreads();
+        if (tid == 0) {
+#pragma unroll
+            for (int w = 1; w < SCAN_WARPS; ++w) { pm = dd_add_pos(pm, sm_m[0][w]); st = dd_add_pos(st, sm_t[0][w]); }
+            sm_after[(t1 - 1) & 1] = st;
+            // offsets of the chunk's tiles: the slice totals of the reduce launch, added up in order
+            dd run = pm;
+            for (uint32_t k = 0; k < t1 - t0; ++k) {
+                sm_pm[k] = run;
+                for (uint32_t s = k * SLICES_PER_TILE; s < min(sl1 - sl0, (k + 1) * SLICES_PER_TILE); ++s) run = dd_add_pos(run, sm_slice[s]);
+            }
+        }
+        __syncthreads();
     }
-    double Mk[SCAN_ITEMS], Sk[SCAN_ITEMS];
+
+    const bool al_in = ((reinterpret_cast<uintptr_t>(r) | reinterpret_cast<uintptr_t>(m)) & 31) == 0;
+    const bool al_out = ((reinterpret_cast<uintptr_t>(phi) | reinterpret_cast<uintptr_t>(m_cum)) & 31) == 0;
+    for (uint32_t tile = t1; tile-- > t0;) {                      // last tile of the chunk first
+        const uint64_t p0 = (uint64_t)tile * SCAN_TILE + (uint64_t)tid * SCAN_ITEMS;
+        const bool full = (uint64_t)tile * SCAN_TILE + SCAN_TILE <= n;
+        double rr[SCAN_ITEMS], mm[SCAN_ITEMS], tt[SCAN_ITEMS];
+        if (full && al_in) {
+            ld4(r + p0, rr); ld4(r + p0 + 4, rr + 4);
+            ld4(m + p0, mm); ld4(m + p0 + 4, mm + 4);
+        } else {
 #pragma unroll
-    for (int i = 0; i < SCAN_ITEMS; ++i) { em = dd_add_d(em, mm[i]); Mk[i] = em.hi; }     // inclusive prefix, rounded once
+            for (int i = 0; i < SCAN_ITEMS; ++i) {
+                const uint64_t p = p0 + i;
+                rr[i] = (p < n) ? r[p] : 1.0;
+                mm[i] = (p < n) ? m[p] : 0.0;
+            }
+        }
+        dd tm{ 0.0, 0.0 }, ts{ 0.0, 0.0 }, um{ 0.0, 0.0 }, us{ 0.0, 0.0 };   // two chains per sum: the adds are dependent
 #pragma unroll
-    for (int i = SCAN_ITEMS - 1; i >= 0; --i) { Sk[i] = et.hi; et = dd_add_d(et, tt[i]); }  // exclusive suffix, rounded once
-    double ph[SCAN_ITEMS];
-#pragma unroll
-    for (int i = 0; i < SCAN_ITEMS; ++i) ph[i] = -(G * (Mk[i] / rr[i] + Sk[i]));           // Eq. 1 at r = r_k
-    const bool alo = ((reinterpret_cast<uintptr_t>(phi) | reinterpret_cast<uintptr_t>(m_cum)) & 15) == 0;
-    if (full && alo) {
-        double2* p2 = reinterpret_cast<double2*>(phi + p0);
-        double2* c2 = reinterpret_cast<double2*>(m_cum + p0);
+        for (int i = 0; i < SCAN_ITEMS; ++i) tt[i] = mm[i] / rr[i];
 #pragma unroll
         for (int i = 0; i < SCAN_ITEMS / 2; ++i) {
-            p2[i] = make_double2(ph[2 * i], ph[2 * i + 1]);
-            c2[i] = make_double2(Mk[2 * i], Mk[2 * i + 1]);
+            tm = dd_add_d(tm, mm[i]); um = dd_add_d(um, mm[i + SCAN_ITEMS / 2]);
+            ts = dd_add_d(ts, tt[i]); us = dd_add_d(us, tt[i + SCAN_ITEMS / 2]);
         }
-    } else {
+        tm = dd_add_pos(tm, um); ts = dd_add_pos(ts, us);
+        dd im = tm, it = ts;                                       // inclusive over lanes: forward m, backward t
 #pragma unroll
-        for (int i = 0; i < SCAN_ITEMS; ++i) {
-            uint64_t p = p0 + i;
-            if (p < n) { phi[p] = ph[i]; m_cum[p] = Mk[i]; }
+        for (int d = 1; d < 32; d <<= 1) {
+            const dd up = dd_shfl_up(im, d);
+            if (lane >= d) im = dd_add_pos(up, im);
+            const dd dn = dd_shfl_down(it, d);
+            if (lane + d < 32) it = dd_add_pos(it, dn);
+        }
+        const int par = tile & 1;                                  // shared words alternate between two sets: one barrier per tile
+        if (lane == 31) sm_m[par][warp] = im;
+        if (lane == 0) sm_t[par][warp] = it;
+        __syncthreads();
+        // everything before this thread's stars (m) / after them (m/r): chunk offset, earlier / later warps, lanes
+        dd em = sm_pm[tile - t0], et = sm_after[par];
+        if (tid == 0) {                                            // the tile's m/r lies "after" the next (earlier) tile
+            dd a = et;
+#pragma unroll
+            for (int w = 0; w < SCAN_WARPS; ++w) a = dd_add_pos(a, sm_t[par][w]);
+            sm_after[par ^ 1] = a;
+        }
+        for (int w = 0; w < warp; ++w) em = dd_add_pos(em, sm_m[par][w]);
+        for (int w = SCAN_WARPS - 1; w > warp; --w) et = dd_add_pos(et, sm_t[par][w]);
+        {
+            const dd pm = dd_shfl_up(im, 1), pt = dd_shfl_down(it, 1);
+            if (lane > 0) em = dd_add_pos(em, pm);
+            if (lane < 31) et = dd_add_pos(et, pt);
+        }
+        double Mk[SCAN_ITEMS], ph[SCAN_ITEMS];
+#pragma unroll
+        for (int i = 0; i < SCAN_ITEMS; ++i) { em = dd_add_d(em, mm[i]); Mk[i] = em.hi; }      // inclusive prefix, rounded once
+#pragma unroll
+        for (int i = SCAN_ITEMS - 1; i >= 0; --i) {
+            ph[i] = -(G * (Mk[i] / rr[i] + et.hi));                // Eq. 1 at r = r_k; et.hi = S_k, exclusive suffix rounded once
+            et = dd_add_d(et, tt[i]);
+        }
+        if (full && al_out) {
+            st4(phi + p0, ph); st4(phi + p0 + 4, ph + 4);
+            st4(m_cum + p0, Mk); st4(m_cum + p0 + 4, Mk + 4);
+        } else {
+#pragma unroll
+            for (int i = 0; i < SCAN_ITEMS; ++i) {
+                const uint64_t p = p0 + i;
+                if (p < n) { phi[p] = ph[i]; m_cum[p] = Mk[i]; }
+            }
         }
     }
 }
@@ -206,13 +259,13 @@ potential_apply_kernel(const double* __restrict__ r, const double* __restrict__ 
 hmc_status potential(uint64_t n, double G, const double* r, const double* m, double* phi, double* m_cum,
                      const Workspace& ws, cudaStream_t st)
 {
-    const uint32_t tiles = (uint32_t)((n + SCAN_TILE - 1) / SCAN_TILE);
-    double4* totals = reinterpret_cast<double4*>(ws.scan_status);
-    potential_reduce_kernel<<<tiles, SCAN_THREADS, 0, st>>>(r, m, n, totals);
+    const ScanPlan plan = scan_plan(n, sm_count());
+    if (plan.tpc > MAX_TPC_SMEM) return HMC_ERR_SIZE;             // cannot happen for n <= HMC_MAX_N on >= 4 SMs
+    double4* slice_tot = reinterpret_cast<double4*>(ws.scan_status);
+    double4* chunk_tot = slice_tot + plan.nslices;
+    potential_reduce_kernel<<<plan.nchunks, SCAN_THREADS, 0, st>>>(r, m, n, plan, slice_tot, chunk_tot);
     HMC_LAUNCH_CHECK();
-    potential_totals_kernel<<<1, TOT_THREADS, 0, st>>>(totals, tiles);
-    HMC_LAUNCH_CHECK();
-    potential_apply_kernel<<<tiles, SCAN_THREADS, 0, st>>>(r, m, phi, m_cum, n, G, totals, tiles);
+    potential_apply_kernel<<<plan.nchunks, SCAN_THREADS, 0, st>>>(r, m, phi, m_cum, n, G, plan, slice_tot, chunk_tot);
     HMC_LAUNCH_CHECK();
     return HMC_OK;
 }
