@@ -8,6 +8,14 @@
 // publishes its per-digit counts, obtains the counts of all earlier tiles by decoupled
 // look-back, and scatters through shared memory so that global writes are coalesced runs.
 // A digit whose histogram has a single occupied bin is skipped.
+//
+// This general sort is the FALLBACK of S1: hmc_sort_fast.cu sorts ordinary input, and only when it meets a run
+// of more than 32 stars agreeing in all the key bits it kept does it raise a device-side flag.  The host cannot
+// read that flag without synchronising, so the fallback is always enqueued -- as ONE cooperative launch whose
+// CTAs return at once when the flag is clear (round 1 enqueued its 13 kernels separately: 38 us per step of empty
+// launches).  Its phases (zero, histograms, bin scan, eight digit passes, identity, column gather) are separated
+// by grid-wide barriers.
+#include <cooperative_groups.h>
 #include "hmc_common.cuh"
 
 namespace hmc {
@@ -25,10 +33,9 @@ static_assert(SORT_THREADS == RADIX, "thread d owns digit d");
 __device__ __forceinline__ bool guard_open(const uint64_t* __restrict__ guard) { return guard == nullptr || guard[2] != 0; }
 
 // zero-fill of the look-back words, digit histograms and tickets, under the same guard
-__global__ void sort_zero_kernel(uint32_t* __restrict__ a, uint64_t na, uint32_t* __restrict__ b, uint64_t nb,
-                                 uint32_t* __restrict__ c, uint64_t nc, const uint64_t* __restrict__ guard)
+__device__ __forceinline__ void sort_zero_phase(uint32_t* __restrict__ a, uint64_t na, uint32_t* __restrict__ b, uint64_t nb,
+                                                uint32_t* __restrict__ c, uint64_t nc)
 {
-    if (!guard_open(guard)) return;
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x, t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     for (uint64_t i = t; i < na; i += stride) a[i] = 0;
     for (uint64_t i = t; i < nb; i += stride) b[i] = 0;
@@ -43,16 +50,14 @@ static constexpr uint32_t FLAG_MASK = 3u << 30;
 // Low digits of a radius are uniformly distributed: plain shared-memory atomics on one of
 // HIST_COPIES replicated histograms hardly ever collide.  The two top digits (sign, exponent, top
 // mantissa bits) take only a handful of values, so those are first aggregated across the warp.
-static constexpr int HIST_THREADS = 512;
+static constexpr int HIST_THREADS = 256;
 static constexpr int HIST_COPIES = 4;
 static constexpr int HIST_SKEWED_FROM = 6;      // digits >= this are warp-aggregated
 
-__global__ void __launch_bounds__(HIST_THREADS) sort_histogram_kernel(const uint64_t* __restrict__ keys, uint64_t n,
-                                                                      uint32_t* __restrict__ hist /*[8][256]*/,
-                                                                      const uint64_t* __restrict__ guard)
+__device__ __forceinline__ void sort_histogram_phase(const uint64_t* __restrict__ keys, uint64_t n,
+                                                     uint32_t* __restrict__ hist /*[8][256]*/, unsigned char* smem_raw)
 {
-    if (!guard_open(guard)) return;
-    __shared__ uint32_t sh[HIST_COPIES][NPASS * RADIX];
+    uint32_t (*sh)[NPASS * RADIX] = reinterpret_cast<uint32_t (*)[NPASS * RADIX]>(smem_raw);      // [HIST_COPIES][8 * 256]
     for (int i = threadIdx.x; i < HIST_COPIES * NPASS * RADIX; i += HIST_THREADS) (&sh[0][0])[i] = 0;
     __syncthreads();
     uint32_t* mine = sh[(threadIdx.x >> 5) % HIST_COPIES];
@@ -84,12 +89,12 @@ __global__ void __launch_bounds__(HIST_THREADS) sort_histogram_kernel(const uint
 }
 
 // exclusive scan of each digit's 256 counts; pass_live[p] = 0 when one bin holds every key
-__global__ void sort_scan_hist_kernel(uint32_t* __restrict__ hist, uint64_t n, uint32_t* __restrict__ pass_live,
-                                      const uint64_t* __restrict__ guard)
+__device__ __forceinline__ void sort_scan_hist_phase(uint32_t* __restrict__ hist, uint64_t n, uint32_t* __restrict__ pass_live,
+                                                     int p, unsigned char* smem_raw)
 {
-    if (!guard_open(guard)) return;
-    __shared__ uint32_t sh[RADIX];
-    const int p = blockIdx.x, d = threadIdx.x;
+    uint32_t* sh = reinterpret_cast<uint32_t*>(smem_raw);                                         // [256]
+    const int d = threadIdx.x;
+    __syncthreads();
     uint32_t c = hist[p * RADIX + d];
     sh[d] = c;
     __syncthreads();
@@ -126,13 +131,11 @@ struct SortBuffers {
     uint32_t* vals[2];
 };
 
-__global__ void __launch_bounds__(SORT_THREADS, 2)
-sort_onesweep_kernel(SortBuffers buf, uint32_t n, int shift,
-                     const uint32_t* __restrict__ bin_offset /*[256] exclusive*/, uint32_t* __restrict__ lookback,
-                     uint32_t* __restrict__ ticket, const uint32_t* __restrict__ pass_live, int pass,
-                     const uint64_t* __restrict__ guard)
+__device__ __forceinline__ void sort_onesweep_phase(const SortBuffers& buf, uint32_t n, int shift,
+                                                    const uint32_t* __restrict__ bin_offset /*[256] exclusive*/,
+                                                    uint32_t* __restrict__ lookback, uint32_t* __restrict__ ticket,
+                                                    const uint32_t* __restrict__ pass_live, int pass, unsigned char* smem_raw)
 {
-    if (!guard_open(guard)) return;
     if (!pass_live[pass]) return;
     int live_before = 0, live_total = 0;
 #pragma unroll
@@ -147,12 +150,10 @@ sort_onesweep_kernel(SortBuffers buf, uint32_t n, int shift,
     const uint32_t* __restrict__ vals_in = buf.vals[ob ^ 1];
     uint64_t* __restrict__ keys_out = buf.keys[ob];
     uint32_t* __restrict__ vals_out = buf.vals[ob];
-    extern __shared__ __align__(16) unsigned char smem_raw[];
     SortSmem& s = *reinterpret_cast<SortSmem*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
-    // persistent CTAs: tiles are taken in ticket order until none is left (the grid is a few CTAs
-    // per SM, so that a guarded launch that has nothing to do costs next to nothing)
+    // persistent CTAs: tiles are taken in ticket order until none is left
     const uint32_t tiles = (n + SORT_TILE - 1) / SORT_TILE;
     for (;;) {
     __syncthreads();                                            // previous tile's shared memory is no longer read
@@ -253,12 +254,10 @@ sort_onesweep_kernel(SortBuffers buf, uint32_t n, int shift,
 }
 
 // ---- copy-through for the degenerate case "every pass skipped" and final gather ---------------
-__global__ void sort_iota_copy_kernel(const uint64_t* __restrict__ keys_in, uint64_t* __restrict__ keys_out,
-                                      uint32_t* __restrict__ perm, uint64_t n, const uint32_t* __restrict__ pass_live,
-                                      const uint64_t* __restrict__ guard)
+__device__ __forceinline__ void sort_iota_copy_phase(const uint64_t* __restrict__ keys_in, uint64_t* __restrict__ keys_out,
+                                                     uint32_t* __restrict__ perm, uint64_t n, const uint32_t* __restrict__ pass_live)
 {
-    if (!guard_open(guard)) return;
-    // runs only when no pass was live (all keys equal): identity permutation
+    // does something only when no pass was live (all keys equal): identity permutation
     uint32_t any = 0;
     for (int p = 0; p < NPASS; ++p) any |= pass_live[p];
     if (any) return;
@@ -277,10 +276,9 @@ struct GatherCols {
     int ncols;
 };
 
-__global__ void __launch_bounds__(256) sort_gather_kernel(GatherCols g, const uint32_t* __restrict__ perm, uint64_t n,
-                                                          const uint64_t* __restrict__ guard)
+__device__ __forceinline__ void sort_gather_phase(const GatherCols& g, const uint32_t* __restrict__ perm, uint64_t n)
 {
-    if (!guard_open(guard)) return;
+    if (g.ncols == 0 && !g.id_in) return;
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
     for (uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += stride) {
         uint32_t src = perm[k];
@@ -300,49 +298,88 @@ hmc_status sort_fast(uint64_t n, const double* r_in, double* r_sorted, uint32_t*
                      const double* const* cols_in, double* const* cols_out, const uint32_t* id_in, uint32_t* id_out,
                      const Workspace& ws, cudaStream_t st);
 
+// ---- the whole general sort as one cooperative launch ------------------------------------------------
+struct GeneralSortArgs {
+    SortBuffers buf;
+    GatherCols cols;
+    uint32_t *lookback, *digit_hist, *tickets;   // tickets: [0..7] tile tickets, [8..15] pass_live
+    uint32_t* perm;
+    const uint64_t* guard;                       // sortctl of the fast path, or nullptr: run always
+    uint64_t n;
+    uint32_t tiles;
+};
+
+static constexpr size_t GENERAL_SMEM = sizeof(SortSmem) > HIST_COPIES * NPASS * RADIX * 4 ? sizeof(SortSmem) : HIST_COPIES * NPASS * RADIX * 4;
+
+__global__ void __launch_bounds__(SORT_THREADS, 2) sort_general_kernel(GeneralSortArgs a)
+{
+    if (!guard_open(a.guard)) return;                            // the same answer in every CTA: nobody waits at a barrier
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    uint32_t* pass_live = a.tickets + 8;
+    sort_zero_phase(a.lookback, (uint64_t)NPASS * a.tiles * RADIX, a.digit_hist, NPASS * RADIX, a.tickets, 16);
+    grid.sync();
+    sort_histogram_phase(a.buf.keys_src, a.n, a.digit_hist, smem_raw);
+    grid.sync();
+    for (int p = blockIdx.x; p < NPASS; p += gridDim.x) sort_scan_hist_phase(a.digit_hist, a.n, pass_live, p, smem_raw);
+    grid.sync();
+    for (int p = 0; p < NPASS; ++p) {
+        sort_onesweep_phase(a.buf, (uint32_t)a.n, p * RADIX_BITS, a.digit_hist + p * RADIX, a.lookback + (size_t)p * a.tiles * RADIX,
+                            a.tickets + p, pass_live, p, smem_raw);
+        grid.sync();
+    }
+    sort_iota_copy_phase(a.buf.keys_src, a.buf.keys[1], a.perm, a.n, pass_live);
+    grid.sync();
+    sort_gather_phase(a.cols, a.perm, a.n);
+}
+
+// CTAs that can be resident at once on the current device (a cooperative launch must not exceed it)
+static hmc_status general_grid_limit(int* out)
+{
+    static std::atomic<int> cached[64];
+    int dev = 0;
+    HMC_CUDA_TRY(cudaGetDevice(&dev));
+    const bool slot = dev >= 0 && dev < 64;
+    int v = slot ? cached[dev].load(std::memory_order_relaxed) : 0;
+    if (v <= 0) {
+        int per_sm = 0;
+        HMC_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sort_general_kernel, SORT_THREADS, GENERAL_SMEM));
+        if (per_sm < 1) return HMC_ERR_CUDA;
+        v = (per_sm > 2 ? 2 : per_sm) * sm_count();
+        if (slot) cached[dev].store(v, std::memory_order_relaxed);
+    }
+    *out = v;
+    return HMC_OK;
+}
+
 // the general eight-pass sort; with a guard it is enqueued but does nothing unless the guard is set
 static hmc_status sort_general(uint64_t n, const double* r_in, double* r_sorted, uint32_t* perm, int ncols,
                                const double* const* cols_in, double* const* cols_out, const uint32_t* id_in,
                                uint32_t* id_out, const Workspace& ws, const uint64_t* guard, cudaStream_t st)
 {
-    const uint32_t tiles = (uint32_t)((n + SORT_TILE - 1) / SORT_TILE);
-    uint32_t* pass_live = ws.tickets + 8;    // [8] words after the 8 sort tickets
-    const int sms = sm_count();
-    const int copy_blocks = (int)umin64((n + 255) / 256, (uint64_t)sms * 8);
-    sort_zero_kernel<<<copy_blocks, 256, 0, st>>>(ws.lookback, (uint64_t)NPASS * tiles * RADIX, ws.digit_hist, NPASS * RADIX,
-                                                 ws.tickets, 16, guard);
-    HMC_LAUNCH_CHECK();
-    const uint64_t* keys0 = reinterpret_cast<const uint64_t*>(r_in);
-    {
-        int blocks = (int)umin64((n + HIST_THREADS - 1) / HIST_THREADS, (uint64_t)sms * 3);
-        sort_histogram_kernel<<<blocks, HIST_THREADS, 0, st>>>(keys0, n, ws.digit_hist, guard);
-        HMC_LAUNCH_CHECK();
-        sort_scan_hist_kernel<<<NPASS, RADIX, 0, st>>>(ws.digit_hist, n, pass_live, guard);
-        HMC_LAUNCH_CHECK();
-    }
     static std::atomic<uint64_t> opted{ 0 };
-    hmc_status so = smem_opt_in(opted, sort_onesweep_kernel, sizeof(SortSmem));
+    hmc_status so = smem_opt_in(opted, sort_general_kernel, GENERAL_SMEM);
     if (so != HMC_OK) return so;
-    SortBuffers buf;
-    buf.keys_src = keys0;
-    buf.keys[0] = ws.keys_alt; buf.keys[1] = reinterpret_cast<uint64_t*>(r_sorted);
-    buf.vals[0] = ws.vals_alt; buf.vals[1] = perm;
-    for (int p = 0; p < NPASS; ++p) {
-        sort_onesweep_kernel<<<(int)umin64(tiles, (uint64_t)sms * 2), SORT_THREADS, sizeof(SortSmem), st>>>(
-            buf, (uint32_t)n, p * RADIX_BITS, ws.digit_hist + p * RADIX, ws.lookback + (size_t)p * tiles * RADIX,
-            ws.tickets + p, pass_live, p, guard);
-        HMC_LAUNCH_CHECK();
-    }
-    sort_iota_copy_kernel<<<copy_blocks, 256, 0, st>>>(keys0, buf.keys[1], perm, n, pass_live, guard);
+    int limit = 0;
+    so = general_grid_limit(&limit);
+    if (so != HMC_OK) return so;
+    GeneralSortArgs a{};
+    a.tiles = (uint32_t)((n + SORT_TILE - 1) / SORT_TILE);
+    a.n = n;
+    a.buf.keys_src = reinterpret_cast<const uint64_t*>(r_in);
+    a.buf.keys[0] = ws.keys_alt; a.buf.keys[1] = reinterpret_cast<uint64_t*>(r_sorted);
+    a.buf.vals[0] = ws.vals_alt; a.buf.vals[1] = perm;
+    a.cols.ncols = ncols;
+    for (int c = 0; c < ncols; ++c) { a.cols.in[c] = cols_in[c]; a.cols.out[c] = cols_out[c]; }
+    a.cols.id_in = id_in; a.cols.id_out = id_out;
+    a.lookback = ws.lookback; a.digit_hist = ws.digit_hist; a.tickets = ws.tickets;
+    a.perm = perm;
+    a.guard = guard;
+    const unsigned blocks = (unsigned)umin64(a.tiles > 8 ? a.tiles : 8, (uint64_t)limit);
+    void* args[] = { &a };
+    HMC_CUDA_TRY(cudaLaunchCooperativeKernel(reinterpret_cast<void*>(sort_general_kernel), dim3(blocks), dim3(SORT_THREADS), args,
+                                             GENERAL_SMEM, st));
     HMC_LAUNCH_CHECK();
-    if (ncols > 0 || id_in) {
-        GatherCols g{};
-        g.ncols = ncols;
-        for (int c = 0; c < ncols; ++c) { g.in[c] = cols_in[c]; g.out[c] = cols_out[c]; }
-        g.id_in = id_in; g.id_out = id_out;
-        sort_gather_kernel<<<copy_blocks, 256, 0, st>>>(g, perm, n, guard);
-        HMC_LAUNCH_CHECK();
-    }
     return HMC_OK;
 }
 

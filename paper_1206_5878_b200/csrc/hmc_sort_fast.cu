@@ -283,7 +283,7 @@ sort_pk_pass_kernel(PkBuffers b, uint32_t n, const uint64_t* __restrict__ ctl,
         if (pos < valid) {
             const uint32_t g = tile_base + pos;
             w[i] = first ? ((pk.key_part(__ldcs(b.keys_src + g)) << pk.idx_bits) | g) : __ldcs(in + g);
-        } else w[i] = ~0ull;                                    // padding: digit 255, ranks last in the tile
+        } else w[i] = ~0ull;                                    // padding: the largest digit of the pass, ranks last in the tile
     }
     // stable rank inside the warp, item by item
     uint32_t rank[PK_ITEMS];
@@ -310,7 +310,9 @@ sort_pk_pass_kernel(PkBuffers b, uint32_t n, const uint64_t* __restrict__ ctl,
 #pragma unroll
         for (int q = 0; q < PK_WARPS; ++q) { const uint32_t c = s.warp_counts[q][d]; s.warp_counts[q][d] = run; run += c; }
         count = run;
-        if (d == PK_RADIX - 1) count -= (PK_TILE - valid);      // padding is not data
+        // padding is not data.  Its digit is 255 except in a last pass whose digit reaches beyond bit 63
+        // (n > 2^24: the index takes more than 24 bits), where the bits above the word read as zero.
+        if (d == (int)((uint32_t)(~0ull >> shift) & 255u)) count -= (PK_TILE - valid);
         st_volatile_u32(lookback + (size_t)tile * PK_RADIX + d, PK_FLAG_AGG | count);
         s.digit_base[d] = run;                                  // padded tile count, scanned below
     }
