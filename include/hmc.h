@@ -252,6 +252,53 @@ HMC_API hmc_status hmc_diagnostics(uint64_t n, double G,
         void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*
+ * Sharded step (SURVEY.md 8(e), 8(f) item 5; PAPER.md:196 duplicated arrays, :213-223 parallel flow, :239-243 sample
+ * sort, :259-261 redistribution).  The stars are cut into `nranks` consecutive ranges of the sorted order, one per
+ * GPU (Eq. 17's decomposition; host logic in paper_1206_5878_b200/shard.py).  Each rank sorts its stars
+ * (hmc_sort_by_radius), places the splitters in its sorted radii (hmc_partition_points), exchanges partitions and
+ * sorts what it received (hmc_sort_by_radius again: stable, so ties keep source order); then
+ *   hmc_potential_totals   totals[4] (DEVICE, 32-byte aligned) = the shard's sum of m and of fl(m/r), each as a
+ *                          double-double (hi, lo) pair: what the other shards need from this one
+ *   hmc_potential_shard    as hmc_potential on the shard's stars, with rank_totals[nranks][4] (DEVICE: every shard's
+ *                          totals, all-gathered) giving what lies before (lower ranks) and after (higher ranks):
+ *                          M_k and S_k are the same exact sums rounded once as on one GPU (R1p)
+ *   hmc_orbit_turning_points_range / hmc_sample_new_radius_range
+ *                          S3 / S4 for the stars at positions first .. first+count-1 of the all-gathered table:
+ *                          r_sorted, phi, m_cum are the TABLE's arrays [n]; v_r, v_t, id, every other per-star input
+ *                          and every output are the range's own arrays [count].  first = 0, count = n is exactly
+ *                          hmc_orbit_turning_points / hmc_sample_new_radius.  Workspace: hmc_workspace_bytes(n).
+ * hmc_partition_points: counts[j] = number of radii <= splitters[j], j < nsplit (splitters, counts: DEVICE arrays).
+ * Errors: HMC_ERR_SIZE if rank >= nranks, or first + count > n.
+ */
+HMC_API hmc_status hmc_potential_totals(uint64_t n, const double* r_sorted, const double* m_sorted, double* totals,
+        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+HMC_API hmc_status hmc_potential_shard(uint64_t n, double G, const double* r_sorted, const double* m_sorted,
+        uint32_t nranks, uint32_t rank, const double* rank_totals, double* phi, double* m_cum,
+        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+HMC_API hmc_status hmc_partition_points(uint64_t n, const double* r_sorted, uint32_t nsplit, const double* splitters,
+        uint64_t* counts, void* cuda_stream);
+
+HMC_API hmc_status hmc_orbit_turning_points_range(uint64_t n, uint64_t first, uint64_t count, double G,
+        const double* r_sorted, const double* v_r, const double* v_t,
+        const double* phi, const double* m_cum,
+        double* E, double* J, double* r_min, double* r_max,
+        uint32_t* k_min, uint32_t* k_max, uint8_t* star_status,
+        uint64_t* counters,
+        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+HMC_API hmc_status hmc_sample_new_radius_range(uint64_t n, uint64_t first, uint64_t count, double G, uint64_t seed, uint32_t step,
+        const double* r_sorted, const double* phi, const double* m_cum,
+        const double* v_r, const double* v_t,
+        const double* E, const double* J, const double* r_min, const double* r_max,
+        const uint32_t* k_min, const uint32_t* k_max, const uint32_t* id,
+        const uint8_t* star_status_in,
+        double* r_new, double* v_r_new, double* v_t_new, uint16_t* n_try,
+        uint8_t* star_status_out, uint64_t* counters, int32_t reuse_tables,
+        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
  * Host-buffer variant of one whole orbit step (the four calls above, in order), for callers
  * whose star data lives in HOST memory.  r, v_r, v_t, m, id are HOST arrays [n] (unsorted);
  * r_new, v_r_new, v_t_new, m_out, id_out are HOST arrays [n] receiving the stars in radius-sorted

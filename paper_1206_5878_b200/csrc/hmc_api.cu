@@ -155,7 +155,7 @@ hmc_status hmc_potential(uint64_t n, double G, const double* r_sorted, const dou
     REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(m_sorted, 8); REQUIRE_ALIGN(phi, 8); REQUIRE_ALIGN(m_cum, 8);
     hmc_status s = check_ws(workspace, workspace_bytes, n);
     if (s != HMC_OK) return s;
-    return potential(n, G, r_sorted, m_sorted, phi, m_cum, carve(workspace, n), static_cast<cudaStream_t>(cuda_stream));
+    return potential(n, G, r_sorted, m_sorted, phi, m_cum, nullptr, 0, 0, carve(workspace, n), static_cast<cudaStream_t>(cuda_stream));
 }
 
 hmc_status hmc_orbit_turning_points(uint64_t n, double G, const double* r_sorted, const double* v_r,
@@ -175,7 +175,7 @@ hmc_status hmc_orbit_turning_points(uint64_t n, double G, const double* r_sorted
     if (counters) REQUIRE_ALIGN(counters, 8);
     hmc_status s = check_ws(workspace, workspace_bytes, n);
     if (s != HMC_OK) return s;
-    return turning_points(n, G, r_sorted, v_r, v_t, phi, m_cum, E, J, r_min, r_max, k_min, k_max, star_status,
+    return turning_points(n, 0, n, G, r_sorted, v_r, v_t, phi, m_cum, E, J, r_min, r_max, k_min, k_max, star_status,
                           counters, carve(workspace, n), static_cast<cudaStream_t>(cuda_stream));
 }
 
@@ -201,7 +201,7 @@ hmc_status hmc_sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t s
     if (counters) REQUIRE_ALIGN(counters, 8);
     hmc_status s = check_ws(workspace, workspace_bytes, n);
     if (s != HMC_OK) return s;
-    return sample_new_radius(n, G, seed, step, r_sorted, phi, m_cum, v_r, v_t, E, J, r_min, r_max, k_min, k_max, id,
+    return sample_new_radius(n, 0, n, G, seed, step, r_sorted, phi, m_cum, v_r, v_t, E, J, r_min, r_max, k_min, k_max, id,
                              star_status_in, r_new, v_r_new, v_t_new, n_try, star_status_out, counters, reuse_tables != 0,
                              carve(workspace, n), static_cast<cudaStream_t>(cuda_stream));
 }
@@ -225,7 +225,7 @@ hmc_status hmc_orbit_step(uint64_t n, double G, uint64_t seed, uint32_t step, co
     if (counters) REQUIRE_ALIGN(counters, 8);
     hmc_status s = check_ws(workspace, workspace_bytes, n);
     if (s != HMC_OK) return s;
-    return orbit_step(n, G, seed, step, r_sorted, v_r, v_t, phi, m_cum, id, E, J, r_min, r_max, k_min, k_max, star_status,
+    return orbit_step(n, 0, n, G, seed, step, r_sorted, v_r, v_t, phi, m_cum, id, E, J, r_min, r_max, k_min, k_max, star_status,
                       r_new, v_r_new, v_t_new, n_try, star_status_out, counters, carve(workspace, n),
                       static_cast<cudaStream_t>(cuda_stream));
 }
@@ -265,6 +265,93 @@ hmc_status hmc_diagnostics(uint64_t n, double G, const double* r_sorted, const d
                        static_cast<cudaStream_t>(cuda_stream));
 }
 
+/* ---- sharded step (include/hmc.h "Sharded step") ------------------------------------------------------------- */
+
+hmc_status hmc_potential_totals(uint64_t n, const double* r_sorted, const double* m_sorted, double* totals,
+                                void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (n > HMC_MAX_N) return HMC_ERR_SIZE;
+    REQUIRE_PTR(totals); REQUIRE_ALIGN(totals, 32);
+    if (n > 0) { REQUIRE_PTR(r_sorted); REQUIRE_PTR(m_sorted); REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(m_sorted, 8); }
+    hmc_status s = check_ws(workspace, workspace_bytes, n);
+    if (s != HMC_OK) return s;
+    return potential_totals(n, r_sorted, m_sorted, totals, carve(workspace, n), static_cast<cudaStream_t>(cuda_stream));
+}
+
+hmc_status hmc_potential_shard(uint64_t n, double G, const double* r_sorted, const double* m_sorted, uint32_t nranks,
+                               uint32_t rank, const double* rank_totals, double* phi, double* m_cum, void* workspace,
+                               size_t workspace_bytes, void* cuda_stream)
+{
+    if (n > HMC_MAX_N || nranks == 0 || rank >= nranks) return HMC_ERR_SIZE;
+    if (n == 0) return HMC_OK;
+    REQUIRE_PTR(r_sorted); REQUIRE_PTR(m_sorted); REQUIRE_PTR(phi); REQUIRE_PTR(m_cum); REQUIRE_PTR(rank_totals);
+    REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(m_sorted, 8); REQUIRE_ALIGN(phi, 8); REQUIRE_ALIGN(m_cum, 8);
+    REQUIRE_ALIGN(rank_totals, 32);
+    hmc_status s = check_ws(workspace, workspace_bytes, n);
+    if (s != HMC_OK) return s;
+    return potential(n, G, r_sorted, m_sorted, phi, m_cum, rank_totals, nranks, rank, carve(workspace, n),
+                     static_cast<cudaStream_t>(cuda_stream));
+}
+
+hmc_status hmc_partition_points(uint64_t n, const double* r_sorted, uint32_t nsplit, const double* splitters,
+                                uint64_t* counts, void* cuda_stream)
+{
+    if (n > HMC_MAX_N) return HMC_ERR_SIZE;
+    if (nsplit == 0) return HMC_OK;
+    REQUIRE_PTR(splitters); REQUIRE_PTR(counts);
+    if (n > 0) REQUIRE_PTR(r_sorted);
+    REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(splitters, 8); REQUIRE_ALIGN(counts, 8);
+    return partition_points(n, r_sorted, nsplit, splitters, counts, static_cast<cudaStream_t>(cuda_stream));
+}
+
+hmc_status hmc_orbit_turning_points_range(uint64_t n, uint64_t first, uint64_t count, double G, const double* r_sorted,
+                                          const double* v_r, const double* v_t, const double* phi, const double* m_cum,
+                                          double* E, double* J, double* r_min, double* r_max, uint32_t* k_min,
+                                          uint32_t* k_max, uint8_t* star_status, uint64_t* counters, void* workspace,
+                                          size_t workspace_bytes, void* cuda_stream)
+{
+    if (n > HMC_MAX_N || first > n || count > n - first) return HMC_ERR_SIZE;
+    if (n == 0 || count == 0) return HMC_OK;
+    REQUIRE_PTR(r_sorted); REQUIRE_PTR(v_r); REQUIRE_PTR(v_t); REQUIRE_PTR(phi); REQUIRE_PTR(m_cum);
+    REQUIRE_PTR(E); REQUIRE_PTR(J); REQUIRE_PTR(r_min); REQUIRE_PTR(r_max); REQUIRE_PTR(k_min); REQUIRE_PTR(k_max);
+    REQUIRE_PTR(star_status);
+    REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(v_r, 8); REQUIRE_ALIGN(v_t, 8); REQUIRE_ALIGN(phi, 8);
+    REQUIRE_ALIGN(m_cum, 8); REQUIRE_ALIGN(E, 8); REQUIRE_ALIGN(J, 8); REQUIRE_ALIGN(r_min, 8);
+    REQUIRE_ALIGN(r_max, 8); REQUIRE_ALIGN(k_min, 4); REQUIRE_ALIGN(k_max, 4);
+    if (counters) REQUIRE_ALIGN(counters, 8);
+    hmc_status s = check_ws(workspace, workspace_bytes, n);
+    if (s != HMC_OK) return s;
+    return turning_points(n, first, count, G, r_sorted, v_r, v_t, phi, m_cum, E, J, r_min, r_max, k_min, k_max, star_status,
+                          counters, carve(workspace, n), static_cast<cudaStream_t>(cuda_stream));
+}
+
+hmc_status hmc_sample_new_radius_range(uint64_t n, uint64_t first, uint64_t count, double G, uint64_t seed, uint32_t step,
+                                       const double* r_sorted, const double* phi, const double* m_cum, const double* v_r,
+                                       const double* v_t, const double* E, const double* J, const double* r_min,
+                                       const double* r_max, const uint32_t* k_min, const uint32_t* k_max,
+                                       const uint32_t* id, const uint8_t* star_status_in, double* r_new, double* v_r_new,
+                                       double* v_t_new, uint16_t* n_try, uint8_t* star_status_out, uint64_t* counters,
+                                       int32_t reuse_tables, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (n > HMC_MAX_N || first > n || count > n - first) return HMC_ERR_SIZE;
+    if (n == 0 || count == 0) return HMC_OK;
+    REQUIRE_PTR(r_sorted); REQUIRE_PTR(phi); REQUIRE_PTR(m_cum); REQUIRE_PTR(v_r); REQUIRE_PTR(v_t);
+    REQUIRE_PTR(E); REQUIRE_PTR(J); REQUIRE_PTR(r_min); REQUIRE_PTR(r_max); REQUIRE_PTR(k_min); REQUIRE_PTR(k_max);
+    REQUIRE_PTR(id); REQUIRE_PTR(star_status_in); REQUIRE_PTR(r_new); REQUIRE_PTR(v_r_new); REQUIRE_PTR(v_t_new);
+    REQUIRE_PTR(star_status_out);
+    REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(phi, 8); REQUIRE_ALIGN(m_cum, 8); REQUIRE_ALIGN(v_r, 8);
+    REQUIRE_ALIGN(v_t, 8); REQUIRE_ALIGN(E, 8); REQUIRE_ALIGN(J, 8); REQUIRE_ALIGN(r_min, 8); REQUIRE_ALIGN(r_max, 8);
+    REQUIRE_ALIGN(k_min, 4); REQUIRE_ALIGN(k_max, 4); REQUIRE_ALIGN(id, 4); REQUIRE_ALIGN(r_new, 8);
+    REQUIRE_ALIGN(v_r_new, 8); REQUIRE_ALIGN(v_t_new, 8);
+    if (n_try) REQUIRE_ALIGN(n_try, 2);
+    if (counters) REQUIRE_ALIGN(counters, 8);
+    hmc_status s = check_ws(workspace, workspace_bytes, n);
+    if (s != HMC_OK) return s;
+    return sample_new_radius(n, first, count, G, seed, step, r_sorted, phi, m_cum, v_r, v_t, E, J, r_min, r_max, k_min, k_max,
+                             id, star_status_in, r_new, v_r_new, v_t_new, n_try, star_status_out, counters, reuse_tables != 0,
+                             carve(workspace, n), static_cast<cudaStream_t>(cuda_stream));
+}
+
 size_t hmc_step_host_arena_bytes(uint64_t n) { return carve_arena(nullptr, n).total; }
 
 hmc_status hmc_step_host(uint64_t n, double G, uint64_t seed, uint32_t step, const double* r, const double* v_r,
@@ -299,12 +386,12 @@ hmc_status hmc_step_host(uint64_t n, double G, uint64_t seed, uint32_t step, con
     HMC_CUDA_TRY(cudaMemcpyAsync(m_out, a.ms, n * 8, cudaMemcpyDeviceToHost, side->stream));
     HMC_CUDA_TRY(cudaMemcpyAsync(id_out, a.ids, n * 4, cudaMemcpyDeviceToHost, side->stream));
     HMC_CUDA_TRY(cudaEventRecord(side->copied, side->stream));
-    s = potential(n, G, a.rs, a.ms, a.phi, a.mcum, ws, st);
+    s = potential(n, G, a.rs, a.ms, a.phi, a.mcum, nullptr, 0, 0, ws, st);
     if (s != HMC_OK) return s;
-    s = turning_points(n, G, a.rs, a.vrs, a.vts, a.phi, a.mcum, a.E, a.J, a.rmin, a.rmax, a.kmin, a.kmax, a.st0,
+    s = turning_points(n, 0, n, G, a.rs, a.vrs, a.vts, a.phi, a.mcum, a.E, a.J, a.rmin, a.rmax, a.kmin, a.kmax, a.st0,
                        a.counters, ws, st);
     if (s != HMC_OK) return s;
-    s = sample_new_radius(n, G, seed, step, a.rs, a.phi, a.mcum, a.vrs, a.vts, a.E, a.J, a.rmin, a.rmax, a.kmin,
+    s = sample_new_radius(n, 0, n, G, seed, step, a.rs, a.phi, a.mcum, a.vrs, a.vts, a.E, a.J, a.rmin, a.rmax, a.kmin,
                           a.kmax, a.ids, a.st0, a.rn, a.vrn, a.vtn, nullptr, a.st1, a.counters, true, ws, st);
     if (s != HMC_OK) return s;
     HMC_CUDA_TRY(cudaMemcpyAsync(r_new, a.rn, n * 8, cudaMemcpyDeviceToHost, st));

@@ -209,13 +209,20 @@ __device__ __forceinline__ unsigned lanemask_lt()
 hmc_status sort_by_radius(uint64_t n, const double* r_in, double* r_sorted, uint32_t* perm, int ncols,
                           const double* const* cols_in, double* const* cols_out, const uint32_t* id_in,
                           uint32_t* id_out, const Workspace& ws, cudaStream_t st);
+// ext_tot == nullptr: the whole cluster.  Else (sharded step): r, m are shard `rank` of `nranks` consecutive shards of
+// the sorted cluster and ext_tot[nranks][4] (device) holds every shard's totals as potential_totals() writes them.
 hmc_status potential(uint64_t n, double G, const double* r, const double* m, double* phi, double* m_cum,
-                     const Workspace& ws, cudaStream_t st);
-hmc_status turning_points(uint64_t n, double G, const double* r, const double* v_r, const double* v_t,
+                     const double* ext_tot, uint32_t nranks, uint32_t rank, const Workspace& ws, cudaStream_t st);
+hmc_status potential_totals(uint64_t n, const double* r, const double* m, double* totals4, const Workspace& ws, cudaStream_t st);
+hmc_status partition_points(uint64_t n, const double* r_sorted, uint32_t nsplit, const double* splitters, uint64_t* counts,
+                            cudaStream_t st);
+// orbit stages: the table arrays (r, phi, m_cum) are [n]; the stars treated are positions first .. first+count-1 of
+// the table and every per-star array is [count] (the single-GPU calls pass first = 0, count = n)
+hmc_status turning_points(uint64_t n, uint64_t first, uint64_t count, double G, const double* r, const double* v_r, const double* v_t,
                           const double* phi, const double* m_cum, double* E, double* J, double* r_min,
                           double* r_max, uint32_t* k_min, uint32_t* k_max, uint8_t* status, uint64_t* counters,
                           const Workspace& ws, cudaStream_t st);
-hmc_status sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step, const double* r,
+hmc_status sample_new_radius(uint64_t n, uint64_t first, uint64_t count, double G, uint64_t seed, uint32_t step, const double* r,
                              const double* phi, const double* m_cum, const double* v_r, const double* v_t,
                              const double* E, const double* J, const double* r_min, const double* r_max,
                              const uint32_t* k_min, const uint32_t* k_max, const uint32_t* id,
@@ -223,7 +230,7 @@ hmc_status sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step,
                              uint16_t* n_try, uint8_t* status_out, uint64_t* counters, bool reuse_tables,
                              const Workspace& ws, cudaStream_t st);
 
-hmc_status orbit_step(uint64_t n, double G, uint64_t seed, uint32_t step, const double* r, const double* v_r,
+hmc_status orbit_step(uint64_t n, uint64_t first, uint64_t count, double G, uint64_t seed, uint32_t step, const double* r, const double* v_r,
                       const double* v_t, const double* phi, const double* m_cum, const uint32_t* id, double* E,
                       double* J, double* r_min, double* r_max, uint32_t* k_min, uint32_t* k_max, uint8_t* status,
                       double* r_new, double* v_r_new, double* v_t_new, uint16_t* n_try, uint8_t* status_out,

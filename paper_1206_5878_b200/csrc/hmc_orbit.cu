@@ -437,8 +437,10 @@ __device__ __forceinline__ Solved solve_star(const Tables& T, uint32_t a, double
     return Solved{ E, J, rmin, rmax, Fv, kmin, kmax, st };
 }
 
+// Stars first .. first+count-1 of the table (0-based positions; star at position p is node p + 1).  r and phi
+// are the table's arrays [n]; v_r, v_t and every output are the range's own arrays [count].
 __global__ void __launch_bounds__(ORB_THREADS, 1)
-turning_points_kernel(uint32_t n, double G, const double* __restrict__ r, const double* __restrict__ v_r,
+turning_points_kernel(uint32_t n, uint32_t first, uint32_t count, double G, const double* __restrict__ r, const double* __restrict__ v_r,
                       const double* __restrict__ v_t, const double* __restrict__ phi,
                       const Node* __restrict__ nodes, const double2* __restrict__ coarse_g,
                       const double2* __restrict__ mid_g, const uint32_t* __restrict__ dir, int shift, double* __restrict__ E_out, double* __restrict__ J_out, double* __restrict__ rmin_out,
@@ -452,8 +454,8 @@ turning_points_kernel(uint32_t n, double G, const double* __restrict__ r, const 
     Tables T{ nodes, dir, coarse, shift > MID_SHIFT ? mid_g : nullptr, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift, l2_keep_policy() };
 
     const uint32_t stride = gridDim.x * ORB_THREADS;
-    for (uint32_t a = blockIdx.x * ORB_THREADS + threadIdx.x; a < n; a += stride) {
-        const Solved v = solve_star(T, a, __ldcs(r + a), __ldcs(v_r + a), __ldcs(v_t + a), __ldcs(phi + a));
+    for (uint32_t a = blockIdx.x * ORB_THREADS + threadIdx.x; a < count; a += stride) {
+        const Solved v = solve_star(T, first + a, __ldcs(r + first + a), __ldcs(v_r + a), __ldcs(v_t + a), __ldcs(phi + first + a));
         const double E = v.E, J = v.J, rmin = v.rmin, rmax = v.rmax, Fv = v.Fv;
         const uint32_t kmin = v.kmin, kmax = v.kmax;
         const unsigned st = v.st;
@@ -583,7 +585,8 @@ __device__ __noinline__ Exhaustive draw_exhaustive(Tables T, Orbit o, uint32_t s
 }
 
 struct SampleIO {
-    const double *r, *v_r, *v_t, *E, *J, *rmin, *rmax;
+    uint32_t first, count;   // the stars drawn are positions first .. first+count-1 of the table; per-star arrays are [count]
+    const double *r, *v_r, *v_t, *E, *J, *rmin, *rmax;     // r: the table's radii [n]
     const uint32_t *kmin, *kmax, *id;
     const uint8_t* status_in;
     const double* F_ws;      // S3's bound F per star (workspace), or nullptr: compute it here
@@ -656,7 +659,7 @@ __device__ __forceinline__ uint32_t park_from_arrays(const Node* __restrict__ no
         }
         if (!ok) st |= HMC_STAR_CIRCULAR;
     }
-    if (in && !ok) finish_star(io, a, __ldg(io.r + a), __ldcs(io.v_r + a), __ldcs(io.v_t + a), 0u, st);
+    if (in && !ok) finish_star(io, a, __ldg(io.r + io.first + a), __ldcs(io.v_r + a), __ldcs(io.v_t + a), 0u, st);
     const unsigned valid = __ballot_sync(0xffffffffu, ok);
     if (ok) {
         const uint32_t slot = __popc(valid & lane_lt);
@@ -678,9 +681,9 @@ __device__ __forceinline__ uint32_t park_by_solving(const Tables& T, const Sampl
     Solved v{ 0.0, 0.0, 0.0, 0.0, 0.0, 0u, 0u, 0u };
     uint32_t sid = 0;
     if (in) {
-        const double rk = __ldcs(io.r + a), vr = __ldcs(io.v_r + a), vt = __ldcs(io.v_t + a), phik = __ldcs(io.phi + a);
+        const double rk = __ldcs(io.r + io.first + a), vr = __ldcs(io.v_r + a), vt = __ldcs(io.v_t + a), phik = __ldcs(io.phi + io.first + a);
         sid = __ldcs(io.id + a);
-        v = solve_star(T, a, rk, vr, vt, phik);
+        v = solve_star(T, io.first + a, rk, vr, vt, phik);
         __stcs(io.E_w + a, v.E); __stcs(io.J_w + a, v.J); __stcs(io.rmin_w + a, v.rmin); __stcs(io.rmax_w + a, v.rmax);
         __stcs(io.kmin_w + a, v.kmin); __stcs(io.kmax_w + a, v.kmax); io.status_w[a] = (uint8_t)v.st;
         if (v.st && io.counters) {
@@ -708,7 +711,7 @@ __device__ __forceinline__ uint32_t park_by_solving(const Tables& T, const Sampl
 template <bool FUSED>
 __device__ __forceinline__ void prefetch_inputs(const SampleIO& io, uint32_t a)
 {
-    if (FUSED) { prefetch_l2(io.r + a); prefetch_l2(io.v_r + a); prefetch_l2(io.v_t + a); prefetch_l2(io.phi + a); prefetch_l2(io.id + a); }
+    if (FUSED) { prefetch_l2(io.r + io.first + a); prefetch_l2(io.v_r + a); prefetch_l2(io.v_t + a); prefetch_l2(io.phi + io.first + a); prefetch_l2(io.id + a); }
     else {
         prefetch_l2(io.E + a); prefetch_l2(io.J + a); prefetch_l2(io.rmin + a); prefetch_l2(io.rmax + a);
         prefetch_l2(io.kmin + a); prefetch_l2(io.kmax + a); prefetch_l2(io.id + a); prefetch_l2(io.status_in + a);
@@ -752,12 +755,12 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
                 // the batch claimed one round ago is prepared now; the next one is claimed here and its
                 // per-star inputs are pulled into L2 meanwhile
                 const uint32_t base = next_base;
-                if (base >= n) { exhausted = true; break; }
+                if (base >= io.count) { exhausted = true; break; }
                 if (lane == 0) next_base = atomicAdd(io.batch_counter, 32u);
                 next_base = __shfl_sync(0xffffffffu, next_base, 0);
-                if (next_base + lane < n) prefetch_inputs<FUSED>(io, next_base + lane);
-                parked = FUSED ? park_by_solving(T, io, pk, base, n, lane, lane_lt)
-                               : park_from_arrays(nodes, io, pk, base, n, lane, lane_lt);
+                if (next_base + lane < io.count) prefetch_inputs<FUSED>(io, next_base + lane);
+                parked = FUSED ? park_by_solving(T, io, pk, base, io.count, lane, lane_lt)
+                               : park_from_arrays(nodes, io, pk, base, io.count, lane, lane_lt);
                 head = 0;
                 continue;
             }
@@ -832,7 +835,7 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
                     out_vt = o.J / good_r;
                     const double vrn = sqrt(good_Q);                    // v_r = Q^(1/2)
                     out_vr = (good_w3 & 1u) ? -vrn : vrn;
-                } else { out_r = __ldg(io.r + a); out_vr = __ldcs(io.v_r + a); out_vt = __ldcs(io.v_t + a); }
+                } else { out_r = __ldg(io.r + io.first + a); out_vr = __ldcs(io.v_r + a); out_vt = __ldcs(io.v_t + a); }
                 finish_star(io, a, out_r, out_vr, out_vt, used, st);
                 have = false;
             }
@@ -911,7 +914,7 @@ static hmc_status build_tables(uint64_t n, double G, const double* r, const doub
     return HMC_OK;
 }
 
-hmc_status turning_points(uint64_t n, double G, const double* r, const double* v_r, const double* v_t,
+hmc_status turning_points(uint64_t n, uint64_t first, uint64_t count, double G, const double* r, const double* v_r, const double* v_t,
                           const double* phi, const double* m_cum, double* E, double* J, double* r_min,
                           double* r_max, uint32_t* k_min, uint32_t* k_max, uint8_t* status, uint64_t* counters,
                           const Workspace& ws, cudaStream_t st)
@@ -924,8 +927,9 @@ hmc_status turning_points(uint64_t n, double G, const double* r, const double* v
     if (so != HMC_OK) return so;
     hmc_status s = build_tables(n, G, r, phi, m_cum, ws, shift, st);
     if (s != HMC_OK) return s;
-    const int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
-    turning_points_kernel<<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, G, r, v_r, v_t, phi, ws.nodes, ws.coarse, ws.mid, ws.dir, shift,
+    if (count == 0) return HMC_OK;
+    const int blocks = (int)umin64((count + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
+    turning_points_kernel<<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, (uint32_t)first, (uint32_t)count, G, r, v_r, v_t, phi, ws.nodes, ws.coarse, ws.mid, ws.dir, shift,
                                                             E, J, r_min, r_max, k_min, k_max, status, ws.orbitF,
                                                             reinterpret_cast<unsigned long long*>(counters));
     HMC_LAUNCH_CHECK();
@@ -942,7 +946,8 @@ static hmc_status launch_sampler(bool fused, uint64_t n, double G, uint64_t seed
     hmc_status so = fused ? smem_opt_in(opted[1], sample_new_radius_kernel<true>, cap)
                           : smem_opt_in(opted[0], sample_new_radius_kernel<false>, cap);
     if (so != HMC_OK) return so;
-    const int blocks = (int)umin64((n + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
+    if (io_in.count == 0) return HMC_OK;
+    const int blocks = (int)umin64(((uint64_t)io_in.count + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
     HMC_CUDA_TRY(cudaMemsetAsync(ws.tickets + 16, 0, 4, st));
     SampleIO io = io_in;
     io.batch_counter = ws.tickets + 16;
@@ -956,7 +961,7 @@ static hmc_status launch_sampler(bool fused, uint64_t n, double G, uint64_t seed
     return HMC_OK;
 }
 
-hmc_status sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step, const double* r,
+hmc_status sample_new_radius(uint64_t n, uint64_t first, uint64_t count, double G, uint64_t seed, uint32_t step, const double* r,
                              const double* phi, const double* m_cum, const double* v_r, const double* v_t,
                              const double* E, const double* J, const double* r_min, const double* r_max,
                              const uint32_t* k_min, const uint32_t* k_max, const uint32_t* id,
@@ -970,6 +975,7 @@ hmc_status sample_new_radius(uint64_t n, double G, uint64_t seed, uint32_t step,
         if (s != HMC_OK) return s;
     }
     SampleIO io{};
+    io.first = (uint32_t)first; io.count = (uint32_t)count;
     io.r = r; io.v_r = v_r; io.v_t = v_t; io.E = E; io.J = J; io.rmin = r_min; io.rmax = r_max;
     io.kmin = k_min; io.kmax = k_max; io.id = id; io.status_in = status_in;
     io.F_ws = reuse_tables ? ws.orbitF : nullptr;
@@ -1000,7 +1006,7 @@ hmc_status energy_correction(uint64_t n, double G, const double* r, const double
 }
 
 // S3 + S4 in one launch: same outputs as the two calls.
-hmc_status orbit_step(uint64_t n, double G, uint64_t seed, uint32_t step, const double* r, const double* v_r,
+hmc_status orbit_step(uint64_t n, uint64_t first, uint64_t count, double G, uint64_t seed, uint32_t step, const double* r, const double* v_r,
                       const double* v_t, const double* phi, const double* m_cum, const uint32_t* id, double* E,
                       double* J, double* r_min, double* r_max, uint32_t* k_min, uint32_t* k_max, uint8_t* status,
                       double* r_new, double* v_r_new, double* v_t_new, uint16_t* n_try, uint8_t* status_out,
@@ -1010,6 +1016,7 @@ hmc_status orbit_step(uint64_t n, double G, uint64_t seed, uint32_t step, const 
     hmc_status s = build_tables(n, G, r, phi, m_cum, ws, shift, st);
     if (s != HMC_OK) return s;
     SampleIO io{};
+    io.first = (uint32_t)first; io.count = (uint32_t)count;
     io.r = r; io.v_r = v_r; io.v_t = v_t; io.id = id; io.phi = phi;
     io.E_w = E; io.J_w = J; io.rmin_w = r_min; io.rmax_w = r_max; io.kmin_w = k_min; io.kmax_w = k_max; io.status_w = status;
     io.r_new = r_new; io.v_r_new = v_r_new; io.v_t_new = v_t_new; io.n_try = n_try; io.status_out = status_out;

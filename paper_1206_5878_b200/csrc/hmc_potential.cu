@@ -143,7 +143,8 @@ static constexpr int MAX_TPC_SMEM = 256;      // tiles per chunk whose offsets f
 __global__ void __launch_bounds__(SCAN_THREADS, CHUNK_CTAS_PER_SM)
 potential_apply_kernel(const double* __restrict__ r, const double* __restrict__ m, double* __restrict__ phi,
                        double* __restrict__ m_cum, uint64_t n, double G, ScanPlan plan,
-                       const double4* __restrict__ slice_tot, const double4* __restrict__ chunk_tot)
+                       const double4* __restrict__ slice_tot, const double4* __restrict__ chunk_tot,
+                       const double4* __restrict__ ext_tot, uint32_t nranks, uint32_t rank)
 {
     __shared__ dd sm_m[2][SCAN_WARPS], sm_t[2][SCAN_WARPS];     // per-warp totals of the tile being scanned (by tile parity)
     __shared__ dd sm_pm[MAX_TPC_SMEM];                          // sum of m over everything before tile k of this chunk
@@ -160,6 +161,13 @@ potential_apply_kernel(const double* __restrict__ r, const double* __restrict__ 
             if (j == c) continue;
             const double4 v = chunk_tot[j];
             if (j < c) pm = dd_add_pos(pm, dd{ v.x, v.y });
+            else st = dd_add_pos(st, dd{ v.z, v.w });
+        }
+        // sharded step: the other shards of the cluster lie wholly before (lower rank) or after (higher rank) this one
+        for (uint32_t j = tid; ext_tot != nullptr && j < nranks; j += SCAN_THREADS) {
+            if (j == rank) continue;
+            const double4 v = ext_tot[j];
+            if (j < rank) pm = dd_add_pos(pm, dd{ v.x, v.y });
             else st = dd_add_pos(st, dd{ v.z, v.w });
         }
 #pragma unroll
@@ -256,8 +264,70 @@ potential_apply_kernel(const double* __restrict__ r, const double* __restrict__ 
     }
 }
 
+// totals of a whole array (sharded step): the chunk totals of the reduce launch added up by one CTA
+__global__ void __launch_bounds__(SCAN_THREADS) potential_sum_chunks_kernel(const double4* __restrict__ chunk_tot, uint32_t nchunks,
+                                                                            double4* __restrict__ out)
+{
+    __shared__ dd sm_m[SCAN_WARPS], sm_t[SCAN_WARPS];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    dd am{ 0.0, 0.0 }, at{ 0.0, 0.0 };
+    for (uint32_t j = tid; j < nchunks; j += SCAN_THREADS) {
+        const double4 v = chunk_tot[j];
+        am = dd_add_pos(am, dd{ v.x, v.y }); at = dd_add_pos(at, dd{ v.z, v.w });
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) { am = dd_add_pos(am, dd_shfl_xor(am, d)); at = dd_add_pos(at, dd_shfl_xor(at, d)); }
+    if (lane == 0) { sm_m[warp] = am; sm_t[warp] = at; }
+    __syncthreads();
+    if (tid == 0) {
+#pragma unroll
+        for (int w = 1; w < SCAN_WARPS; ++w) { am = dd_add_pos(am, sm_m[w]); at = dd_add_pos(at, sm_t[w]); }
+        *out = make_double4(am.hi, am.lo, at.hi, at.lo);
+    }
+}
+
+// number of radii <= splitter j, j = 0 .. nsplit-1 (sample sort, phase 4: "the positions of the splitter points in the
+// local array are determined by binary search"); one thread per splitter
+__global__ void partition_points_kernel(const double* __restrict__ r, uint64_t n, const double* __restrict__ splitters,
+                                        uint32_t nsplit, unsigned long long* __restrict__ counts)
+{
+    const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= nsplit) return;
+    const double x = splitters[j];
+    uint64_t lo = 0, hi = n;                                     // first position whose radius is > x
+    while (lo < hi) {
+        const uint64_t mid = lo + (hi - lo) / 2;
+        if (r[mid] <= x) lo = mid + 1; else hi = mid;
+    }
+    counts[j] = lo;
+}
+
+hmc_status partition_points(uint64_t n, const double* r_sorted, uint32_t nsplit, const double* splitters, uint64_t* counts,
+                            cudaStream_t st)
+{
+    if (nsplit == 0) return HMC_OK;
+    partition_points_kernel<<<(nsplit + 127) / 128, 128, 0, st>>>(r_sorted, n, splitters, nsplit,
+                                                                   reinterpret_cast<unsigned long long*>(counts));
+    HMC_LAUNCH_CHECK();
+    return HMC_OK;
+}
+
+hmc_status potential_totals(uint64_t n, const double* r, const double* m, double* totals4, const Workspace& ws, cudaStream_t st)
+{
+    const ScanPlan plan = scan_plan(n, sm_count());
+    double4* slice_tot = reinterpret_cast<double4*>(ws.scan_status);
+    double4* chunk_tot = slice_tot + plan.nslices;
+    if (n > 0) {
+        potential_reduce_kernel<<<plan.nchunks, SCAN_THREADS, 0, st>>>(r, m, n, plan, slice_tot, chunk_tot);
+        HMC_LAUNCH_CHECK();
+    }
+    potential_sum_chunks_kernel<<<1, SCAN_THREADS, 0, st>>>(chunk_tot, n > 0 ? plan.nchunks : 0u, reinterpret_cast<double4*>(totals4));
+    HMC_LAUNCH_CHECK();
+    return HMC_OK;
+}
+
 hmc_status potential(uint64_t n, double G, const double* r, const double* m, double* phi, double* m_cum,
-                     const Workspace& ws, cudaStream_t st)
+                     const double* ext_tot, uint32_t nranks, uint32_t rank, const Workspace& ws, cudaStream_t st)
 {
     const ScanPlan plan = scan_plan(n, sm_count());
     if (plan.tpc > MAX_TPC_SMEM) return HMC_ERR_SIZE;             // cannot happen for n <= HMC_MAX_N on >= 4 SMs
@@ -265,7 +335,8 @@ hmc_status potential(uint64_t n, double G, const double* r, const double* m, dou
     double4* chunk_tot = slice_tot + plan.nslices;
     potential_reduce_kernel<<<plan.nchunks, SCAN_THREADS, 0, st>>>(r, m, n, plan, slice_tot, chunk_tot);
     HMC_LAUNCH_CHECK();
-    potential_apply_kernel<<<plan.nchunks, SCAN_THREADS, 0, st>>>(r, m, phi, m_cum, n, G, plan, slice_tot, chunk_tot);
+    potential_apply_kernel<<<plan.nchunks, SCAN_THREADS, 0, st>>>(r, m, phi, m_cum, n, G, plan, slice_tot, chunk_tot,
+                                                                  reinterpret_cast<const double4*>(ext_tot), nranks, rank);
     HMC_LAUNCH_CHECK();
     return HMC_OK;
 }

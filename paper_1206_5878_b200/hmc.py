@@ -47,7 +47,9 @@ def load(path: str) -> ctypes.CDLL:
     L.hmc_t_max.restype = ctypes.c_uint32
     L.hmc_launch_count.restype = ctypes.c_uint64
     for name in ("hmc_sort_by_radius", "hmc_potential", "hmc_orbit_turning_points", "hmc_sample_new_radius",
-                 "hmc_orbit_step", "hmc_diagnostics", "hmc_energy_correction", "hmc_step_host"):
+                 "hmc_orbit_step", "hmc_diagnostics", "hmc_energy_correction", "hmc_step_host", "hmc_potential_totals",
+                 "hmc_potential_shard", "hmc_partition_points", "hmc_orbit_turning_points_range",
+                 "hmc_sample_new_radius_range"):
         getattr(L, name).restype = ctypes.c_int32
     return L
 
@@ -137,21 +139,25 @@ def hmc_potential(r_sorted: torch.Tensor, m_sorted: torch.Tensor, G: float = 1.0
 
 
 def hmc_orbit_turning_points(r_sorted, v_r, v_t, phi, m_cum, G: float = 1.0, *, out=None, counters=None,
-                             workspace=None):
-    """S3 (PAPER.md:117-124).  -> dict(E, J, r_min, r_max, k_min, k_max, status)"""
+                             workspace=None, first: Optional[int] = None):
+    """S3 (PAPER.md:117-124).  -> dict(E, J, r_min, r_max, k_min, k_max, status)
+    ``first`` given (sharded step): hmc_orbit_turning_points_range -- r_sorted, phi, m_cum are the table [n], v_r and
+    v_t the stars at positions first .. first + len(v_r) - 1 of it; outputs have that length."""
     n = r_sorted.numel()
+    c = n if first is None else v_r.numel()
     dev = r_sorted.device
     if out is None:
-        out = alloc_turning_points(n, dev)
+        out = alloc_turning_points(c, dev)
     workspace, wp, wb = _ws(workspace, n, dev)
     f = torch.float64
-    rc = lib().hmc_orbit_turning_points(
-        ctypes.c_uint64(n), ctypes.c_double(G), _dev(r_sorted, f, n, "r_sorted"), _dev(v_r, f, n, "v_r"),
-        _dev(v_t, f, n, "v_t"), _dev(phi, f, n, "phi"), _dev(m_cum, f, n, "m_cum"), _dev(out["E"], f, n, "E"),
-        _dev(out["J"], f, n, "J"), _dev(out["r_min"], f, n, "r_min"), _dev(out["r_max"], f, n, "r_max"),
-        _dev(out["k_min"], torch.int32, n, "k_min"), _dev(out["k_max"], torch.int32, n, "k_max"),
-        _dev(out["status"], torch.uint8, n, "status"), _dev(counters, torch.int64, NCOUNTERS, "counters"), wp, wb,
-        _stream())
+    head = (ctypes.c_uint64(n),) if first is None else (ctypes.c_uint64(n), ctypes.c_uint64(first), ctypes.c_uint64(c))
+    fn = lib().hmc_orbit_turning_points if first is None else lib().hmc_orbit_turning_points_range
+    rc = fn(*head, ctypes.c_double(G), _dev(r_sorted, f, n, "r_sorted"), _dev(v_r, f, c, "v_r"),
+            _dev(v_t, f, c, "v_t"), _dev(phi, f, n, "phi"), _dev(m_cum, f, n, "m_cum"), _dev(out["E"], f, c, "E"),
+            _dev(out["J"], f, c, "J"), _dev(out["r_min"], f, c, "r_min"), _dev(out["r_max"], f, c, "r_max"),
+            _dev(out["k_min"], torch.int32, c, "k_min"), _dev(out["k_max"], torch.int32, c, "k_max"),
+            _dev(out["status"], torch.uint8, c, "status"), _dev(counters, torch.int64, NCOUNTERS, "counters"), wp, wb,
+            _stream())
     _check(rc, "hmc_orbit_turning_points")
     return out
 
@@ -172,28 +178,74 @@ def alloc_sample(n: int, device="cuda", with_n_try: bool = True):
 
 
 def hmc_sample_new_radius(r_sorted, phi, m_cum, v_r, v_t, tp, ids, seed: int, step: int, G: float = 1.0, *,
-                          out=None, counters=None, workspace=None, reuse_tables: bool = False):
+                          out=None, counters=None, workspace=None, reuse_tables: bool = False,
+                          first: Optional[int] = None):
     """S4.  ``tp`` is the dict returned by hmc_orbit_turning_points.
-    -> dict(r_new, v_r_new, v_t_new, n_try, status)"""
+    -> dict(r_new, v_r_new, v_t_new, n_try, status)
+    ``first`` given (sharded step): hmc_sample_new_radius_range, per-star arrays of the range's length."""
     n = r_sorted.numel()
+    c = n if first is None else v_r.numel()
     dev = r_sorted.device
     if out is None:
-        out = alloc_sample(n, dev)
+        out = alloc_sample(c, dev)
     workspace, wp, wb = _ws(workspace, n, dev)
     f = torch.float64
-    rc = lib().hmc_sample_new_radius(
-        ctypes.c_uint64(n), ctypes.c_double(G), ctypes.c_uint64(seed), ctypes.c_uint32(step),
-        _dev(r_sorted, f, n, "r_sorted"), _dev(phi, f, n, "phi"), _dev(m_cum, f, n, "m_cum"), _dev(v_r, f, n, "v_r"),
-        _dev(v_t, f, n, "v_t"), _dev(tp["E"], f, n, "E"), _dev(tp["J"], f, n, "J"), _dev(tp["r_min"], f, n, "r_min"),
-        _dev(tp["r_max"], f, n, "r_max"), _dev(tp["k_min"], torch.int32, n, "k_min"),
-        _dev(tp["k_max"], torch.int32, n, "k_max"), _dev(ids, torch.int32, n, "ids"),
-        _dev(tp["status"], torch.uint8, n, "status_in"), _dev(out["r_new"], f, n, "r_new"),
-        _dev(out["v_r_new"], f, n, "v_r_new"), _dev(out["v_t_new"], f, n, "v_t_new"),
-        _dev(out.get("n_try"), torch.int16, n, "n_try"), _dev(out["status"], torch.uint8, n, "status_out"),
-        _dev(counters, torch.int64, NCOUNTERS, "counters"), ctypes.c_int32(1 if reuse_tables else 0), wp, wb,
-        _stream())
+    head = (ctypes.c_uint64(n),) if first is None else (ctypes.c_uint64(n), ctypes.c_uint64(first), ctypes.c_uint64(c))
+    fn = lib().hmc_sample_new_radius if first is None else lib().hmc_sample_new_radius_range
+    rc = fn(*head, ctypes.c_double(G), ctypes.c_uint64(seed), ctypes.c_uint32(step),
+            _dev(r_sorted, f, n, "r_sorted"), _dev(phi, f, n, "phi"), _dev(m_cum, f, n, "m_cum"), _dev(v_r, f, c, "v_r"),
+            _dev(v_t, f, c, "v_t"), _dev(tp["E"], f, c, "E"), _dev(tp["J"], f, c, "J"), _dev(tp["r_min"], f, c, "r_min"),
+            _dev(tp["r_max"], f, c, "r_max"), _dev(tp["k_min"], torch.int32, c, "k_min"),
+            _dev(tp["k_max"], torch.int32, c, "k_max"), _dev(ids, torch.int32, c, "ids"),
+            _dev(tp["status"], torch.uint8, c, "status_in"), _dev(out["r_new"], f, c, "r_new"),
+            _dev(out["v_r_new"], f, c, "v_r_new"), _dev(out["v_t_new"], f, c, "v_t_new"),
+            _dev(out.get("n_try"), torch.int16, c, "n_try"), _dev(out["status"], torch.uint8, c, "status_out"),
+            _dev(counters, torch.int64, NCOUNTERS, "counters"), ctypes.c_int32(1 if reuse_tables else 0), wp, wb,
+            _stream())
     _check(rc, "hmc_sample_new_radius")
     return out
+
+
+def hmc_potential_totals(r_sorted, m_sorted, *, totals=None, workspace=None):
+    """Sharded step: a shard's (sum m, sum m/r) as two double-double pairs -> device float64[4]."""
+    n = r_sorted.numel()
+    dev = r_sorted.device
+    totals = torch.empty(4, dtype=torch.float64, device=dev) if totals is None else totals
+    workspace, wp, wb = _ws(workspace, n, dev)
+    f = torch.float64
+    rc = lib().hmc_potential_totals(ctypes.c_uint64(n), _dev(r_sorted, f, n, "r_sorted"), _dev(m_sorted, f, n, "m_sorted"),
+                                    _dev(totals, f, 4, "totals"), wp, wb, _stream())
+    _check(rc, "hmc_potential_totals")
+    return totals
+
+
+def hmc_potential_shard(r_sorted, m_sorted, rank: int, rank_totals, G: float = 1.0, *, phi=None, m_cum=None,
+                        workspace=None):
+    """Sharded step: S2 on shard ``rank``; rank_totals is the device float64[nranks, 4] of every shard's totals."""
+    n = r_sorted.numel()
+    dev = r_sorted.device
+    nranks = rank_totals.numel() // 4
+    f = torch.float64
+    phi = torch.empty(n, dtype=f, device=dev) if phi is None else phi
+    m_cum = torch.empty(n, dtype=f, device=dev) if m_cum is None else m_cum
+    workspace, wp, wb = _ws(workspace, n, dev)
+    rc = lib().hmc_potential_shard(ctypes.c_uint64(n), ctypes.c_double(G), _dev(r_sorted, f, n, "r_sorted"),
+                                   _dev(m_sorted, f, n, "m_sorted"), ctypes.c_uint32(nranks), ctypes.c_uint32(rank),
+                                   _dev(rank_totals, f, 4 * nranks, "rank_totals"), _dev(phi, f, n, "phi"),
+                                   _dev(m_cum, f, n, "m_cum"), wp, wb, _stream())
+    _check(rc, "hmc_potential_shard")
+    return phi, m_cum
+
+
+def hmc_partition_points(r_sorted, splitters, *, counts=None):
+    """Sample sort, phase 4: counts[j] = number of radii <= splitters[j] (device int64)."""
+    n, k = r_sorted.numel(), splitters.numel()
+    counts = torch.empty(k, dtype=torch.int64, device=r_sorted.device) if counts is None else counts
+    f = torch.float64
+    rc = lib().hmc_partition_points(ctypes.c_uint64(n), _dev(r_sorted, f, n, "r_sorted"), ctypes.c_uint32(k),
+                                    _dev(splitters, f, k, "splitters"), _dev(counts, torch.int64, k, "counts"), _stream())
+    _check(rc, "hmc_partition_points")
+    return counts
 
 
 def hmc_orbit_step(r_sorted, v_r, v_t, phi, m_cum, ids, seed: int, step: int, G: float = 1.0, *, tp=None, out=None,

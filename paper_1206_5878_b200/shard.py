@@ -1,0 +1,294 @@
+"""The orbit step sharded over G GPUs, in the paper's own shape:
+
+* the stars are cut into G consecutive ranges of the radius-sorted order, every range but the last a multiple of
+  n_m = 20 stars (Eq. 17);
+* S1 is the paper's Sample Sort: sort the local stars, sample s keys per rank, gather the
+  samples, pick the splitters, exchange partitions (all-to-all), sort what was received; then the redistribution
+  phase (exclusive scan of the counts + all-to-all) restores the exact decomposition;
+* S2 needs one all-gather of G x 4 doubles: every shard's (sum m, sum m/r) in double-double, from which each rank's
+  launch adds up what lies before and after its range (the MPI_Exscan idea of PAPER.md:259 applied to the potential
+  the paper calls "inherently sequential", :185);
+* r, Phi and M are replicated by an all-gather ("we maintain a copy of it on all nodes"), after which S3
+  and S4 of a rank's own stars need no communication.
+
+This file holds HOST LOGIC ONLY: integer bookkeeping of the decomposition, which slices go where, and two
+communication back-ends with the same five collectives.  Every sort, sum, search and draw is a libhmc kernel called
+through ``hmc`` (there is no CPU path: the kernels need a GPU).  The random numbers are keyed by the persistent star id
+(R9) and M_k, S_k are exact sums rounded once (R1p), so the sharded step reproduces the single-GPU step bit
+for bit whatever G is (tests/test_gpu_shard.py).
+
+Back-ends:
+  InProcessComm(G)   G shards held by ONE process on one device; a collective is a hand-over of device tensors.
+                     This is what one GPU can test, and what the tests use.
+  DistComm()         one shard per process over torch.distributed (NCCL between GPUs; gloo on CPU tensors in the
+                     world-size-2 host-logic tests).  UNMEASURED ON HARDWARE: no multi-GPU node was available.
+"""
+from __future__ import annotations
+
+from typing import Callable, List, Optional, Sequence
+
+import torch
+
+N_M = 20   # "we choose a bin size of 20 ... the number of stars per processor is a multiple of 20"
+
+
+# ------------------------------------------------------------------------------------------------ decomposition
+def partition_counts(n_stars: int, p: int, n_m: int = N_M) -> List[int]:
+    """Stars per processor: multiples of n_m for the first p - 1 processors, the rest to the last;
+    the block counts are those Eq. 17 implies: with B = floor(N / n_m) blocks, processors id < B mod p hold
+    floor(B / p) + 1 blocks, the others floor(B / p)."""
+    blocks = n_stars // n_m
+    q, rem = divmod(blocks, p)
+    counts = [(q + 1) * n_m if rank < rem else q * n_m for rank in range(p)]
+    counts[-1] += n_stars - blocks * n_m
+    return counts
+
+
+def global_index(i: int, rank: int, n_stars: int, p: int, n_m: int = N_M) -> int:
+    """Eq. 17: global index of local star i on processor `rank`."""
+    blocks = n_stars // n_m
+    q, rem = divmod(blocks, p)
+    if rank < rem:
+        return i + rank * q * n_m + rank * n_m
+    return i + rank * q * n_m + rem * n_m
+
+
+def exclusive_scan(counts: Sequence[int]) -> List[int]:
+    out, run = [], 0
+    for c in counts:
+        out.append(run)
+        run += c
+    return out
+
+
+def redistribution_plan(have: Sequence[int], want: Sequence[int]) -> List[List[int]]:
+    """PAPER.md:259-261.  After the sort processor s holds have[s] consecutive stars of the global order; the
+    decomposition wants want[d] on processor d.  -> send[s][d] = how many of its stars s passes to d; a processor's
+    stars go out in order, lowest destination first, and arrive in source order, which is the global order."""
+    if sum(have) != sum(want):
+        raise ValueError("redistribution_plan: %d stars held, %d wanted" % (sum(have), sum(want)))
+    h0, w0 = exclusive_scan(have), exclusive_scan(want)      # the parallel prefix reduction (MPI_Exscan)
+    p = len(have)
+    send = [[0] * p for _ in range(p)]
+    for s in range(p):
+        for d in range(p):
+            lo, hi = max(h0[s], w0[d]), min(h0[s] + have[s], w0[d] + want[d])
+            send[s][d] = max(0, hi - lo)
+    return send
+
+
+def sample_positions(n_local: int, s: int) -> List[int]:
+    """Phase 2: "uniformly sample s keys" of the locally sorted block."""
+    return [min(n_local - 1, ((2 * k + 1) * n_local) // (2 * s)) for k in range(s)] if n_local > 0 else []
+
+
+def splitter_positions(s: int, p: int) -> List[int]:
+    """Phase 3: "keys at indices s, 2s, 3s, ..., (p-1)s" of the sorted combined sample."""
+    return [j * s for j in range(1, p)]
+
+
+# ------------------------------------------------------------------------------------------------ communication
+class InProcessComm:
+    """G ranks in one process.  Arguments and results are lists with one entry per rank."""
+
+    def __init__(self, world: int):
+        self.world = world
+        self.local_ranks = list(range(world))
+
+    def all_gather(self, xs: List[torch.Tensor]) -> List[List[torch.Tensor]]:
+        """out[rank] = [x of rank 0, ..., x of rank G-1]."""
+        return [list(xs) for _ in self.local_ranks]
+
+    def all_to_all(self, send: List[List[torch.Tensor]]) -> List[List[torch.Tensor]]:
+        """send[src][dst] -> recv[dst][src]."""
+        return [[send[src][dst] for src in range(self.world)] for dst in range(self.world)]
+
+    def all_gather_ints(self, xs: List[List[int]]) -> List[List[List[int]]]:
+        return [list(xs) for _ in self.local_ranks]
+
+
+class DistComm:
+    """One rank per process over torch.distributed.  Lists have ONE entry (this process's rank); the nested lists
+    of the results run over all ranks.  Works with the tensors' own backend: NCCL for CUDA tensors, gloo for CPU."""
+
+    def __init__(self, group=None):
+        import torch.distributed as dist
+        self.dist = dist
+        self.group = group
+        self.world = dist.get_world_size(group)
+        self.rank = dist.get_rank(group)
+        self.local_ranks = [self.rank]
+
+    def all_gather_ints(self, xs: List[List[int]]) -> List[List[List[int]]]:
+        out = [None] * self.world
+        self.dist.all_gather_object(out, list(xs[0]), group=self.group)
+        return [out]
+
+    def all_gather(self, xs: List[torch.Tensor]) -> List[List[torch.Tensor]]:
+        x = xs[0].contiguous()
+        sizes = [v[0] for v in self.all_gather_ints([[x.numel()]])[0]]
+        biggest = max(sizes)
+        pad = x if x.numel() == biggest else torch.cat([x.reshape(-1), x.new_zeros(biggest - x.numel())])
+        bufs = [torch.empty(biggest, dtype=x.dtype, device=x.device) for _ in range(self.world)]
+        self.dist.all_gather(bufs, pad.reshape(-1), group=self.group)
+        return [[b[:k] for b, k in zip(bufs, sizes)]]
+
+    def all_to_all(self, send: List[List[torch.Tensor]]) -> List[List[torch.Tensor]]:
+        mine = [t.contiguous() for t in send[0]]
+        counts = self.all_gather_ints([[t.numel() for t in mine]])[0]            # counts[src][dst]
+        recv = [torch.empty(counts[src][self.rank], dtype=mine[0].dtype, device=mine[0].device) for src in range(self.world)]
+        recv[self.rank] = mine[self.rank]
+        ops = []
+        for other in range(self.world):                                            # point-to-point: gloo has no all_to_all
+            if other == self.rank:
+                continue
+            if mine[other].numel():
+                ops.append(self.dist.P2POp(self.dist.isend, mine[other], other, self.group))
+            if recv[other].numel():
+                ops.append(self.dist.P2POp(self.dist.irecv, recv[other], other, self.group))
+        if ops:
+            for w in self.dist.batch_isend_irecv(ops):
+                w.wait()
+        return [recv]
+
+
+# ------------------------------------------------------------------------------------------------ sample sort
+def _cat(parts):
+    parts = [p for p in parts if p.numel()]
+    return torch.cat(parts) if len(parts) > 1 else (parts[0] if parts else None)
+
+
+def sample_sort(comm, cols: List[List[torch.Tensor]], sample_size: int, want: Sequence[int],
+                local_sort: Callable, partition_points: Callable) -> List[List[torch.Tensor]]:
+    """The paper's Sample Sort + redistribution over the ranks of `comm`.
+
+    cols[lr] = the columns of local rank lr, the KEY (radius) first; every column of a rank has the same length.
+    local_sort(columns) -> columns sorted by the first one, stably; partition_points(sorted_keys, splitters) ->
+    list of ints, the number of keys <= each splitter.  Both are libhmc kernels in the product
+    (ShardedStepper); the host-logic tests pass CPU stand-ins.  -> the columns of each local rank after the sort:
+    rank d holds stars exclusive_scan(want)[d] ... of the global order, want[d] of them."""
+    world, L = comm.world, len(comm.local_ranks)
+    ncol = len(cols[0])
+    # phase 1: sort local data
+    cols = [local_sort(c) if c[0].numel() > 1 else c for c in cols]
+    if world > 1:
+        # phase 2: sampling (a rank without stars contributes +inf samples, which sort last)
+        samples = []
+        for c in cols:
+            key = c[0]
+            pos = sample_positions(key.numel(), sample_size)
+            samples.append(key[torch.tensor(pos, dtype=torch.long, device=key.device)] if pos
+                           else torch.full((sample_size,), float("inf"), dtype=key.dtype, device=key.device))
+        gathered = comm.all_gather(samples)
+        # phase 3: splitter selection (every rank does what the designated processor would broadcast)
+        sent = []
+        for i, c in enumerate(cols):
+            combined = local_sort([torch.cat(gathered[i])])[0]
+            spl = combined[torch.tensor(splitter_positions(sample_size, world), dtype=torch.long, device=combined.device)]
+            # phase 4: place the splitters, cut the local array into `world` partitions
+            cut = [0] + [int(x) for x in partition_points(c[0], spl)] + [c[0].numel()]
+            sent.append([[col[cut[d]:cut[d + 1]] for d in range(world)] for col in c])
+        received = [comm.all_to_all([sent[i][k] for i in range(L)]) for k in range(ncol)]     # received[k][lr][src]
+        # phase 5: merge = concatenate in source order and sort again (stable: ties keep source order)
+        merged = []
+        for i in range(L):
+            c = [_cat(received[k][i]) for k in range(ncol)]
+            if c[0] is None:
+                c = [cols[i][k][:0] for k in range(ncol)]
+            merged.append(local_sort(c) if c[0].numel() > 1 else c)
+        cols = merged
+        # redistribution: exclusive scan of the counts, all-to-all of the chunks that belong elsewhere
+        have = [v[0] for v in comm.all_gather_ints([[c[0].numel()] for c in cols])[0]]
+        plan = redistribution_plan(have, want)
+        sent = []
+        for i, rank in enumerate(comm.local_ranks):
+            off = exclusive_scan(plan[rank])
+            sent.append([[col[off[d]:off[d] + plan[rank][d]] for d in range(world)] for col in cols[i]])
+        received = [comm.all_to_all([sent[i][k] for i in range(L)]) for k in range(ncol)]
+        out = []
+        for i in range(L):
+            c = [_cat(received[k][i]) for k in range(ncol)]       # chunks arrive in source order = global order
+            if c[0] is None:
+                c = [cols[i][k][:0] for k in range(ncol)]
+            out.append(c)
+        cols = out
+    return cols
+
+
+# ------------------------------------------------------------------------------------------------ the stepper
+class ShardedStepper:
+    """hmc.OrbitStepper over the ranks of a communicator.  ``shards`` = one dict(r, v_r, v_t, m, id) of CUDA tensors
+    per local rank: the rank's range of the (unsorted) cluster, the ranges in rank order making up the whole cluster
+    in the order a single-GPU stepper would be given it.  After step() the state of rank d is the stars of its range
+    of the sorted order with their new coordinates, exactly as hmc.OrbitStepper's state cut at the same places."""
+
+    def __init__(self, comm, shards: List[dict], seed: int, G: float = 1.0, sample_size: int = 256,
+                 n_total: Optional[int] = None):
+        from . import hmc
+        self.hmc = hmc
+        self.comm, self.seed, self.G, self.sample_size, self.step_index = comm, seed, G, sample_size, 0
+        self.state = [dict(s) for s in shards]
+        if n_total is None:
+            sizes = comm.all_gather_ints([[s["r"].numel()] for s in shards])[0]
+            n_total = sum(v[0] for v in sizes)
+        self.n = n_total
+        self.want = partition_counts(self.n, comm.world)
+        self.offsets = exclusive_scan(self.want)
+        self.counters = [hmc.alloc_counters(s["r"].device) for s in shards]
+        self.workspace = [hmc.alloc_workspace(self.n, s["r"].device) for s in shards]
+        self.last = None
+
+    def _local_sort(self, ws):
+        hmc = self.hmc
+
+        def sort(columns):
+            key, rest = columns[0], list(columns[1:])
+            ids = next((c for c in rest if c.dtype == torch.int32), None)
+            f64 = [c for c in rest if c.dtype == torch.float64]
+            rs, _, cs, ids_s = hmc.hmc_sort_by_radius(key, f64, ids, workspace=ws)
+            it = iter(cs)
+            return [rs] + [ids_s if c.dtype == torch.int32 else next(it) for c in rest]
+        return sort
+
+    def step(self):
+        hmc, comm = self.hmc, self.comm
+        L = len(comm.local_ranks)
+        cols = [[s["r"], s["v_r"], s["v_t"], s["m"], s["id"]] for s in self.state]
+        # S1: sample sort + redistribution.  One workspace serves all local ranks' sorts (they run one after another).
+        sort = self._local_sort(self.workspace[0])
+        cols = sample_sort(comm, cols, self.sample_size, self.want, sort,
+                           lambda keys, spl: hmc.hmc_partition_points(keys, spl).cpu().tolist())
+        # S2: shard totals -> all-gather -> local scan with what lies before and after
+        totals = [hmc.hmc_potential_totals(c[0], c[3], workspace=self.workspace[i]) for i, c in enumerate(cols)]
+        all_totals = [torch.cat(t) for t in comm.all_gather(totals)]
+        pots = [hmc.hmc_potential_shard(c[0], c[3], rank, all_totals[i], self.G, workspace=self.workspace[i])
+                for i, (c, rank) in enumerate(zip(cols, comm.local_ranks))]
+        # the replicated table
+        table_r = [torch.cat(t) for t in comm.all_gather([c[0] for c in cols])]
+        table_phi = [torch.cat(t) for t in comm.all_gather([p[0] for p in pots])]
+        table_m = [torch.cat(t) for t in comm.all_gather([p[1] for p in pots])]
+        # S3 / S4 on the rank's own range: no communication
+        new_state, last = [], []
+        for i, rank in enumerate(comm.local_ranks):
+            r, vr, vt, m, ids = cols[i]
+            first = self.offsets[rank]
+            if r.numel():
+                tp = hmc.hmc_orbit_turning_points(table_r[i], vr, vt, table_phi[i], table_m[i], self.G, first=first,
+                                                  counters=self.counters[i], workspace=self.workspace[i])
+                sm = hmc.hmc_sample_new_radius(table_r[i], table_phi[i], table_m[i], vr, vt, tp, ids, self.seed,
+                                               self.step_index, self.G, first=first, counters=self.counters[i],
+                                               workspace=self.workspace[i], reuse_tables=True)
+            else:
+                tp, sm = hmc.alloc_turning_points(0, r.device), hmc.alloc_sample(0, r.device)
+            new_state.append(dict(r=sm["r_new"], v_r=sm["v_r_new"], v_t=sm["v_t_new"], m=m, id=ids))
+            last.append(dict(r=r, v_r=vr, v_t=vt, phi=pots[i][0], m_cum=pots[i][1], tp=tp, sample=sm))
+        self.state, self.last = new_state, last
+        self.step_index += 1
+
+
+def split_cluster(cluster: dict, world: int) -> List[dict]:
+    """Cut the arrays of a cluster (any indexable columns of equal length) into the decomposition's ranges."""
+    n = len(cluster["r"])
+    counts = partition_counts(n, world)
+    offs = exclusive_scan(counts)
+    return [{k: v[o:o + c] for k, v in cluster.items()} for o, c in zip(offs, counts)]
