@@ -252,6 +252,39 @@ HMC_API hmc_status hmc_diagnostics(uint64_t n, double G,
         void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*
+ * Relaxation: the two steps of the paper's loop between the potential and the new orbits.
+ *
+ * hmc_relaxation_timestep -- Eq. 7 on radial bins of HMC_BIN = 20 consecutive sorted stars
+ * (the n mod 20 stars left over join the last bin), and "the minimum is taken as the value of the
+ * global relaxation timestep" (:108):
+ *     T_b = (theta_max / (pi/2)) (pi/32) <v_rel>^3 / ( ln(gamma n) G^2 n_b <(M_1 + M_2)^2> )
+ * over the bin's neighbour pairs (2j, 2j+1): v_rel = ((v_r1 - v_r2)^2 + v_t1^2 + v_t2^2)^(1/2) (rms over the unknown
+ * angle between the transverse velocities), n_b = stars of the bin / volume of the shell from the previous bin's last
+ * star to this bin's last star (R19).  t_rel_bin: DEVICE [max(1, n / 20)] or NULL; t_rel_min: DEVICE [1]
+ * (+inf when there is no pair).  gamma: the Coulomb logarithm's factor (the paper uses 0.1, :348).
+ *
+ * hmc_two_body_relaxation -- "an analytic expression for a representative encounter between two nearest-neighbor
+ * stars" (the expression is in Joshi et al. 2000, not in the paper: DESIGN.md R20 is Henon's scheme).
+ * Each pair (2j, 2j+1) undergoes one elastic encounter in its centre-of-mass frame by the deflection angle beta with
+ * sin^2(beta/2) = 2 pi G^2 (m_1+m_2)^2 n_b ln(gamma n) dt / w^3 (capped at 1), about a uniformly random axis; the
+ * pair's momentum and kinetic energy are conserved.  The angles are Philox4x32-10(counter = (id of the pair's first
+ * star, 1, step, t), key = seed), turned into unit vectors without trigonometric functions.  v_r_out / v_t_out [n]
+ * receive the new velocities (an odd last star is copied).  Needs no workspace.  The step is dt, or, when dt_device
+ * (DEVICE [1], e.g. t_rel_min of hmc_relaxation_timestep) is not NULL, dt * (*dt_device): no host round trip.
+ */
+#define HMC_BIN 20
+
+HMC_API hmc_status hmc_relaxation_timestep(uint64_t n, double G, double gamma, double theta_max,
+        const double* r_sorted, const double* v_r, const double* v_t, const double* m_sorted,
+        double* t_rel_bin, double* t_rel_min,
+        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+HMC_API hmc_status hmc_two_body_relaxation(uint64_t n, double G, double gamma, double dt, const double* dt_device,
+        uint64_t seed, uint32_t step,
+        const double* r_sorted, const double* v_r, const double* v_t, const double* m_sorted, const uint32_t* id,
+        double* v_r_out, double* v_t_out, void* cuda_stream);
+
+/*
  * Sharded step (SURVEY.md 8(e), 8(f) item 5; PAPER.md:196 duplicated arrays, :213-223 parallel flow, :239-243 sample
  * sort, :259-261 redistribution).  The stars are cut into `nranks` consecutive ranges of the sorted order, one per
  * GPU (Eq. 17's decomposition; host logic in paper_1206_5878_b200/shard.py).  Each rank sorts its stars

@@ -17,6 +17,7 @@ from __future__ import annotations
 
 import contextlib
 import ctypes
+import math
 import os
 import subprocess
 
@@ -207,6 +208,40 @@ def energy_correction(r, phi, m_cum, E_old, r_old, p_old, v_r, v_t, G=1.0):
                                          _p(r_old), _p(p_old), _p(v_r), _p(v_t), _p(vro), _p(vto), _p(st))
     assert rc == 0
     return vro, vto, st
+
+
+BIN = 20
+
+
+def n_bins(n):
+    return (1 if n else 0) if n < BIN else n // BIN
+
+
+def relaxation_timestep(r, v_r, v_t, m, gamma=0.1, theta_max=1.0, G=1.0, ln_gamma_n=None):
+    """Eq. 7 per bin of 20 sorted stars and its minimum.  -> (t_rel_bin, t_rel_min)"""
+    r, v_r, v_t, m = map(_f64, (r, v_r, v_t, m))
+    n = r.shape[0]
+    lg = math.log(gamma * n) if ln_gamma_n is None else float(ln_gamma_n)   # libm's log, as libhmc's host code
+    tb = np.empty(n_bins(n), np.float64)
+    tmin = np.empty(1, np.float64)
+    rc = lib().hmc_ref_relaxation_timestep(ctypes.c_uint64(n), ctypes.c_double(G), ctypes.c_double(lg),
+                                           ctypes.c_double(theta_max), _p(r), _p(v_r), _p(v_t), _p(m), _p(tb), _p(tmin))
+    assert rc == 0
+    return tb, float(tmin[0])
+
+
+def two_body_relaxation(r, v_r, v_t, m, ids, dt, seed, step, gamma=0.1, G=1.0, ln_gamma_n=None):
+    """Representative two-body encounter of every neighbour pair (R20).  -> (v_r', v_t')"""
+    r, v_r, v_t, m = map(_f64, (r, v_r, v_t, m))
+    ids = np.ascontiguousarray(ids, np.uint32)
+    n = r.shape[0]
+    lg = math.log(gamma * n) if ln_gamma_n is None else float(ln_gamma_n)   # libm's log, as libhmc's host code
+    vro, vto = np.empty(n), np.empty(n)
+    rc = lib().hmc_ref_two_body_relaxation(ctypes.c_uint64(n), ctypes.c_double(G), ctypes.c_double(lg), ctypes.c_double(dt),
+                                           ctypes.c_uint64(seed), ctypes.c_uint32(step), _p(r), _p(v_r), _p(v_t), _p(m),
+                                           _p(ids), _p(vro), _p(vto))
+    assert rc == 0
+    return vro, vto
 
 
 def orbit_step(r, v_r, v_t, m, ids, seed, step, G=1.0, sample=None):

@@ -486,3 +486,171 @@ int hmc_ref_energy_correction(uint64_t n, double G, const double *r, const doubl
     }
     return 0;
 }
+
+/* ------------------------------------------------------------------------ */
+/* Relaxation timestep and two-body relaxation on neighbour pairs           */
+/* (Eq. 7 at :87; bins of 20 at :194).  SURVEY.md 8(f) 3.  */
+/*                                                                          */
+/* Eq. 7:  T_rel = (theta_max / (pi/2)) (pi/32) <v_rel>^3                   */
+/*                 / ( ln(gamma N) G^2 n <(M_1 + M_2)^2> ).                 */
+/* "Instead of using sliding averages for each star, we choose radial bins  */
+/* containing a fixed number of stars ... a bin size of 20"; */
+/* "the minimum is taken as the value of the global relaxation timestep"    */
+/* (:108).  Readings (R19):                                       */
+/*  - bin b = sorted stars 20b .. 20b+19; the n mod 20 stars left over join */
+/*    the last bin; n < 20: one bin.                                        */
+/*  - pairs are the neighbours (2j, 2j+1) of the sorted order ("pairs of    */
+/*    neighboring stars", :177), which never straddle a bin; an odd last    */
+/*    star has no partner.                                                  */
+/*  - v_rel of a pair: its transverse velocities make an unknown angle,     */
+/*    uniform in [0, 2 pi); the timestep takes the rms over that angle,     */
+/*    v_rel = sqrt((v_r1 - v_r2)^2 + v_t1^2 + v_t2^2); < > is the mean over */
+/*    the bin's pairs, summed in pair order.                                */
+/*  - n: the shell between the last star of the previous bin (r = 0 for the */
+/*    first bin) and the last star of this bin holds exactly the bin's      */
+/*    stars: n = count / ((4 pi / 3) (r_out^3 - r_in^3)).                   */
+/*  - ln(gamma N) is passed in (the caller evaluates the logarithm once).   */
+/*  - a bin without a pair, with zero volume, or with zero mass: no         */
+/*    constraint, T = +inf (zero volume: n = inf gives T = 0, kept).        */
+/* ------------------------------------------------------------------------ */
+#define BIN 20u
+#define FOUR_PI_3 4.1887902047863909846   /* 4 pi / 3 */
+#define PI_OVER_2 1.5707963267948966192
+#define PI_OVER_32 0.098174770424681038702
+#define TWO_PI 6.2831853071795864769
+
+static uint64_t n_bins(uint64_t n) { return n < BIN ? (n ? 1 : 0) : n / BIN; }
+
+/* number density of bin b (count / volume of its shell) */
+static double bin_density(uint64_t n, const double *r, uint64_t b)
+{
+    uint64_t nb = n_bins(n);
+    uint64_t first = b * BIN, last = (b + 1 == nb) ? n - 1 : first + BIN - 1;
+    double r_in = b ? r[first - 1] : 0.0, r_out = r[last];
+    double vol = FOUR_PI_3 * ((r_out * r_out) * r_out - (r_in * r_in) * r_in);
+    return (double)(last - first + 1) / vol;
+}
+
+int hmc_ref_relaxation_timestep(uint64_t n, double G, double ln_gamma_n, double theta_max,
+                                const double *r, const double *v_r, const double *v_t, const double *m,
+                                double *t_rel_bin, double *t_rel_min)
+{
+    uint64_t nb = n_bins(n);
+    double tmin = INFINITY;
+    for (uint64_t b = 0; b < nb; ++b) {
+        uint64_t first = b * BIN, last = (b + 1 == nb) ? n - 1 : first + BIN - 1;
+        double sv = 0.0, sm = 0.0;
+        uint64_t pairs = 0;
+        for (uint64_t a = first; a + 1 <= last; a += 2) {
+            double dvr = v_r[a] - v_r[a + 1];
+            double w = sqrt(dvr * dvr + v_t[a] * v_t[a] + v_t[a + 1] * v_t[a + 1]);
+            double M = m[a] + m[a + 1];
+            sv += w; sm += M * M;
+            ++pairs;
+        }
+        double T = INFINITY;
+        if (pairs) {
+            double vmean = sv / (double)pairs, m2mean = sm / (double)pairs;
+            double dens = bin_density(n, r, b);
+            double den = ((ln_gamma_n * (G * G)) * dens) * m2mean;
+            if (den > 0.0) T = (((theta_max / PI_OVER_2) * PI_OVER_32) * ((vmean * vmean) * vmean)) / den;
+        }
+        if (t_rel_bin) t_rel_bin[b] = T;
+        if (T < tmin) tmin = T;
+    }
+    *t_rel_min = tmin;
+    return 0;
+}
+
+/* ------------------------------------------------------------------------ */
+/* "Two-body relaxation is applied based on an analytic expression for a    */
+/* representative encounter between two nearest-neighbor stars"             */
+/* (PAPER.md:110); the expression is deferred to Joshi et al. (2000) and is  */
+/* not in the text.  Reading DESIGN.md R20 (Henon's scheme):                */
+/*  - the pair (1, 2) = sorted stars (2j, 2j+1); in a local frame with z    */
+/*    radial, v_1 = (v_t1, 0, v_r1), v_2 = (v_t2 cos phi, v_t2 sin phi,     */
+/*    v_r2), phi uniform;  w = v_1 - v_2,  V = (m_1 v_1 + m_2 v_2) / M,     */
+/*    M = m_1 + m_2;                                                        */
+/*  - one encounter deflects w by the angle beta that the many distant      */
+/*    encounters of the step dt add up to: the mean square deflection       */
+/*    behind Eq. 7, <beta^2> = 8 pi G^2 n M^2 ln(gamma N) dt / w^3 (Eq. 7   */
+/*    is this set to (pi/2) theta_max), carried by sin^2(beta/2) =          */
+/*    2 pi G^2 M^2 n ln(gamma N) dt / w^3, capped at 1;                     */
+/*  - w' = w cos beta + |w| sin beta (e_1 cos psi + e_2 sin psi), psi       */
+/*    uniform, e_1 = (w_y, -w_x, 0)/w_p, e_2 = (w_x w_z, w_y w_z, -w_p^2) /  */
+/*    (w_p |w|), w_p = (w_x^2 + w_y^2)^(1/2) (w along z: e_1 = x, e_2 = y); */
+/*  - v_1' = V + (m_2/M) w',  v_2' = V - (m_1/M) w': the pair's momentum    */
+/*    and kinetic energy are conserved;  v_r' = z,  v_t' = (x^2+y^2)^(1/2). */
+/*  - unit vectors (cos, sin) without trigonometric functions (which are    */
+/*    not correctly rounded): (a, b) uniform in the unit disc by rejection, */
+/*    then (cos, sin) = ((a^2 - b^2)/s, 2ab/s), s = a^2 + b^2 -- the        */
+/*    doubled angle of a uniform point is uniform.  Draw t of the pair      */
+/*    uses Philox4x32-10(counter = (id of star 1, 1, step, t)); phi takes   */
+/*    the first accepted draw, psi the next accepted one (at most 64 draws, */
+/*    then (1, 0)).                                                         */
+/*  n is the pair's bin density as in the timestep.                          */
+/* ------------------------------------------------------------------------ */
+static void unit_vector(uint32_t id, uint32_t step, const uint32_t key[2], uint32_t *t, double *c, double *s_out)
+{
+    const double two_m53 = 1.0 / 9007199254740992.0;
+    while (*t < 64u) {
+        uint32_t ctr[4] = { id, 1u, step, *t }, w[4];
+        ++*t;
+        hmc_ref_philox4x32_10(ctr, key, w);
+        double a = 2.0 * ((double)((((uint64_t)w[0] << 32) | w[1]) >> 11) * two_m53) - 1.0;
+        double b = 2.0 * ((double)((((uint64_t)w[2] << 32) | w[3]) >> 11) * two_m53) - 1.0;
+        double s = a * a + b * b;
+        if (s > 0.0 && s < 1.0) { *c = (a * a - b * b) / s; *s_out = (2.0 * (a * b)) / s; return; }
+    }
+    *c = 1.0; *s_out = 0.0;
+}
+
+int hmc_ref_two_body_relaxation(uint64_t n, double G, double ln_gamma_n, double dt, uint64_t seed, uint32_t step,
+                                const double *r, const double *v_r, const double *v_t, const double *m,
+                                const uint32_t *id, double *v_r_out, double *v_t_out)
+{
+    const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    uint64_t nb = n_bins(n);
+#pragma omp parallel for schedule(dynamic, 4096)
+    for (uint64_t j = 0; j < (n + 1) / 2; ++j) {
+        uint64_t a = 2 * j, b = a + 1;
+        if (b >= n) { v_r_out[a] = v_r[a]; v_t_out[a] = v_t[a]; continue; }      /* odd star out */
+        uint64_t bin = a / BIN; if (bin >= nb) bin = nb - 1;
+        double dens = bin_density(n, r, bin);
+        double m1 = m[a], m2 = m[b], M = m1 + m2;
+        uint32_t t = 0;
+        double cphi, sphi, cpsi, spsi;
+        unit_vector(id[a], step, key, &t, &cphi, &sphi);
+        unit_vector(id[a], step, key, &t, &cpsi, &spsi);
+        double x1 = v_t[a], z1 = v_r[a];
+        double x2 = v_t[b] * cphi, y2 = v_t[b] * sphi, z2 = v_r[b];
+        double wx = x1 - x2, wy = 0.0 - y2, wz = z1 - z2;
+        double wp2 = wx * wx + wy * wy, w2 = wp2 + wz * wz, wn = sqrt(w2);
+        if (!(wn > 0.0) || !(M > 0.0)) {
+            v_r_out[a] = v_r[a]; v_t_out[a] = v_t[a]; v_r_out[b] = v_r[b]; v_t_out[b] = v_t[b];
+            continue;
+        }
+        double S = (((((TWO_PI * (G * G)) * (M * M)) * dens) * ln_gamma_n) * dt) / (w2 * wn);
+        if (!(S < 1.0)) S = 1.0;
+        if (!(S > 0.0)) S = 0.0;
+        double cb = 1.0 - 2.0 * S, sb = 2.0 * sqrt(S * (1.0 - S));
+        double wp = sqrt(wp2);
+        double e1x, e1y, e1z, e2x, e2y, e2z;
+        if (wp > 0.0) {
+            e1x = wy / wp; e1y = (0.0 - wx) / wp; e1z = 0.0;
+            double q = wp * wn;
+            e2x = (wx * wz) / q; e2y = (wy * wz) / q; e2z = (0.0 - wp2) / q;
+        } else { e1x = 1.0; e1y = 0.0; e1z = 0.0; e2x = 0.0; e2y = 1.0; e2z = 0.0; }
+        double k = wn * sb;
+        double nx = wx * cb + k * (e1x * cpsi + e2x * spsi);
+        double ny = wy * cb + k * (e1y * cpsi + e2y * spsi);
+        double nz = wz * cb + k * (e1z * cpsi + e2z * spsi);
+        double Vx = (m1 * x1 + m2 * x2) / M, Vy = (m2 * y2) / M, Vz = (m1 * z1 + m2 * z2) / M;
+        double f1 = m2 / M, f2 = m1 / M;
+        double ax = Vx + f1 * nx, ay = Vy + f1 * ny, az = Vz + f1 * nz;
+        double bx = Vx - f2 * nx, by = Vy - f2 * ny, bz = Vz - f2 * nz;
+        v_r_out[a] = az; v_t_out[a] = sqrt(ax * ax + ay * ay);
+        v_r_out[b] = bz; v_t_out[b] = sqrt(bx * bx + by * by);
+    }
+    return 0;
+}

@@ -18,7 +18,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhmc.so")
-SOURCES = ["hmc_api.cu", "hmc_sort.cu", "hmc_sort_fast.cu", "hmc_potential.cu", "hmc_orbit.cu", "hmc_diag.cu"]
+SOURCES = ["hmc_api.cu", "hmc_sort.cu", "hmc_sort_fast.cu", "hmc_potential.cu", "hmc_orbit.cu", "hmc_diag.cu", "hmc_relax.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-fmad=false",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-cudart", "static",

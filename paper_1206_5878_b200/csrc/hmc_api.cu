@@ -1,5 +1,6 @@
 // hmc_api.cu -- extern "C" boundary of libhmc (include/hmc.h): argument checks, workspace
 // carve-up, stream plumbing.  No arithmetic of the method lives here.
+#include <cmath>
 #include <vector>
 #include "hmc_common.cuh"
 
@@ -263,6 +264,39 @@ hmc_status hmc_diagnostics(uint64_t n, double G, const double* r_sorted, const d
     if (s != HMC_OK) return s;
     return diagnostics(n, G, r_sorted, v_r, v_t, m_sorted, phi, m_cum, nfrac, mass_fractions, out, carve(workspace, n),
                        static_cast<cudaStream_t>(cuda_stream));
+}
+
+/* ---- relaxation (include/hmc.h "Relaxation") -------------------------------------------------------------------- */
+
+hmc_status hmc_relaxation_timestep(uint64_t n, double G, double gamma, double theta_max, const double* r_sorted,
+                                   const double* v_r, const double* v_t, const double* m_sorted, double* t_rel_bin,
+                                   double* t_rel_min, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (n > HMC_MAX_N) return HMC_ERR_SIZE;
+    REQUIRE_PTR(t_rel_min); REQUIRE_ALIGN(t_rel_min, 8);
+    if (n > 0) { REQUIRE_PTR(r_sorted); REQUIRE_PTR(v_r); REQUIRE_PTR(v_t); REQUIRE_PTR(m_sorted); }
+    REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(v_r, 8); REQUIRE_ALIGN(v_t, 8); REQUIRE_ALIGN(m_sorted, 8);
+    if (t_rel_bin) REQUIRE_ALIGN(t_rel_bin, 8);
+    hmc_status s = check_ws(workspace, workspace_bytes, n);
+    if (s != HMC_OK) return s;
+    const double lg = std::log(gamma * (double)n);               // the Coulomb logarithm ln(gamma N), once, on the host
+    return relaxation_timestep(n, G, lg, theta_max, r_sorted, v_r, v_t, m_sorted, t_rel_bin, t_rel_min, carve(workspace, n),
+                               static_cast<cudaStream_t>(cuda_stream));
+}
+
+hmc_status hmc_two_body_relaxation(uint64_t n, double G, double gamma, double dt, const double* dt_device, uint64_t seed, uint32_t step,
+                                   const double* r_sorted, const double* v_r, const double* v_t, const double* m_sorted,
+                                   const uint32_t* id, double* v_r_out, double* v_t_out, void* cuda_stream)
+{
+    if (n > HMC_MAX_N) return HMC_ERR_SIZE;
+    if (n == 0) return HMC_OK;
+    REQUIRE_PTR(r_sorted); REQUIRE_PTR(v_r); REQUIRE_PTR(v_t); REQUIRE_PTR(m_sorted); REQUIRE_PTR(id);
+    REQUIRE_PTR(v_r_out); REQUIRE_PTR(v_t_out);
+    REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(v_r, 8); REQUIRE_ALIGN(v_t, 8); REQUIRE_ALIGN(m_sorted, 8); REQUIRE_ALIGN(id, 4);
+    REQUIRE_ALIGN(v_r_out, 8); REQUIRE_ALIGN(v_t_out, 8); REQUIRE_ALIGN(dt_device, 8);
+    const double lg = std::log(gamma * (double)n);
+    return two_body_relaxation(n, G, lg, dt, dt_device, seed, step, r_sorted, v_r, v_t, m_sorted, id, v_r_out, v_t_out,
+                               static_cast<cudaStream_t>(cuda_stream));
 }
 
 /* ---- sharded step (include/hmc.h "Sharded step") ------------------------------------------------------------- */

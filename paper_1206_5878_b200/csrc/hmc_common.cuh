@@ -203,6 +203,29 @@ __device__ __forceinline__ unsigned lanemask_lt()
     asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
     return m;
 }
+// ---- Philox4x32-10 (Salmon et al. 2011) ---------------------------------------------------------
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                              uint32_t k1, uint32_t w[4])
+{
+#pragma unroll
+    for (int round = 0; round < 10; ++round) {
+        uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    w[0] = c0; w[1] = c1; w[2] = c2; w[3] = c3;
+}
+
+// ((hi * 2^32 + lo) >> 11) * 2^-53, a double in [0, 1) (R9).  The 53-bit integer is split into its top 21 and
+// low 32 bits, converted separately (both exact) and added (exact: 53 bits): the same value as converting the 64-bit
+// integer, without the slow 64-bit integer-to-double conversion.
+__device__ __forceinline__ double u53_to_unit(uint32_t hi, uint32_t lo)
+{
+    const double two_m21 = 1.0 / 2097152.0, two_m53 = 1.0 / 9007199254740992.0;
+    return __uint2double_rn(hi >> 11) * two_m21 + __uint2double_rn((hi << 21) | (lo >> 11)) * two_m53;
+}
 #endif  // __CUDACC__
 
 // stage entry points implemented in the .cu files (same signatures as hmc.h, Workspace carved)
@@ -240,6 +263,12 @@ hmc_status energy_correction(uint64_t n, double G, const double* r, const double
                              const double* E_old, const double* r_old, const double* p_old, const double* v_r,
                              const double* v_t, double* v_r_out, double* v_t_out, uint8_t* status_out,
                              uint64_t* counters, const Workspace& ws, cudaStream_t st);
+hmc_status relaxation_timestep(uint64_t n, double G, double ln_gamma_n, double theta_max, const double* r, const double* v_r,
+                               const double* v_t, const double* m, double* t_rel_bin, double* t_rel_min, const Workspace& ws,
+                               cudaStream_t st);
+hmc_status two_body_relaxation(uint64_t n, double G, double ln_gamma_n, double dt, const double* dt_dev, uint64_t seed, uint32_t step, const double* r,
+                               const double* v_r, const double* v_t, const double* m, const uint32_t* id, double* v_r_out,
+                               double* v_t_out, cudaStream_t st);
 hmc_status diagnostics(uint64_t n, double G, const double* r, const double* v_r, const double* v_t, const double* m,
                        const double* phi, const double* m_cum, int nfrac, const double* fractions, double* out,
                        const Workspace& ws, cudaStream_t st);

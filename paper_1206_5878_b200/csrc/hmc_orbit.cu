@@ -470,21 +470,6 @@ turning_points_kernel(uint32_t n, uint32_t first, uint32_t count, double G, cons
     }
 }
 
-// ---- Philox4x32-10 (Salmon et al. 2011) ---------------------------------------------------------
-__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
-                                              uint32_t k1, uint32_t w[4])
-{
-#pragma unroll
-    for (int round = 0; round < 10; ++round) {
-        uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-        uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-        uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
-        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
-        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
-    }
-    w[0] = c0; w[1] = c1; w[2] = c2; w[3] = c3;
-}
-
 // ---- S4 ---------------------------------------------------------------------------------------
 struct Orbit {          // per-star constants of the draw
     double E, J, J2, mid, quarter, three_q, F;
@@ -503,10 +488,9 @@ __device__ __forceinline__ Trial make_trial(const Orbit& o, uint32_t seed_lo, ui
     // X = ((w0 * 2^32 + w1) >> 11) * 2^-53 (R9).  The 53-bit integer is split into its top 21 and low 32
     // bits, converted separately (both exact) and added (exact: 53 bits): the same value as converting the
     // 64-bit integer, without the slow 64-bit integer-to-double conversion.
-    const double two_m21 = 1.0 / 2097152.0, two_m53 = 1.0 / 9007199254740992.0;
-    const double X = __uint2double_rn(w[0] >> 11) * two_m21 + __uint2double_rn((w[0] << 21) | (w[1] >> 11)) * two_m53;
+    const double X = u53_to_unit(w[0], w[1]);
     Trial tr;
-    tr.Xp = __uint2double_rn(w[2] >> 11) * two_m21 + __uint2double_rn((w[2] << 21) | (w[3] >> 11)) * two_m53;
+    tr.Xp = u53_to_unit(w[2], w[3]);
     tr.s = 2.0 * X - 1.0;
     tr.r0 = o.mid + o.quarter * (3.0 * tr.s - (tr.s * tr.s) * tr.s);     // replaces Eq. 14 (R7)
     tr.w3 = w[3];

@@ -49,7 +49,7 @@ def load(path: str) -> ctypes.CDLL:
     for name in ("hmc_sort_by_radius", "hmc_potential", "hmc_orbit_turning_points", "hmc_sample_new_radius",
                  "hmc_orbit_step", "hmc_diagnostics", "hmc_energy_correction", "hmc_step_host", "hmc_potential_totals",
                  "hmc_potential_shard", "hmc_partition_points", "hmc_orbit_turning_points_range",
-                 "hmc_sample_new_radius_range"):
+                 "hmc_sample_new_radius_range", "hmc_relaxation_timestep", "hmc_two_body_relaxation"):
         getattr(L, name).restype = ctypes.c_int32
     return L
 
@@ -313,6 +313,47 @@ def hmc_diagnostics(r_sorted, v_r, v_t, m_sorted, phi, m_cum, fractions: Sequenc
     return out
 
 
+BIN = 20
+
+
+def hmc_relaxation_timestep(r_sorted, v_r, v_t, m_sorted, gamma: float = 0.1, theta_max: float = 1.0, G: float = 1.0, *,
+                            t_rel_bin=None, t_rel_min=None, workspace=None):
+    """Eq. 7 per bin of 20 sorted stars and its minimum.
+    -> (t_rel_bin: device float64[max(1, n // 20)], t_rel_min: device float64[1])"""
+    n = r_sorted.numel()
+    dev = r_sorted.device
+    f = torch.float64
+    nb = (1 if n else 0) if n < BIN else n // BIN
+    t_rel_bin = torch.empty(nb, dtype=f, device=dev) if t_rel_bin is None else t_rel_bin
+    t_rel_min = torch.empty(1, dtype=f, device=dev) if t_rel_min is None else t_rel_min
+    workspace, wp, wb = _ws(workspace, n, dev)
+    rc = lib().hmc_relaxation_timestep(ctypes.c_uint64(n), ctypes.c_double(G), ctypes.c_double(gamma),
+                                       ctypes.c_double(theta_max), _dev(r_sorted, f, n, "r_sorted"), _dev(v_r, f, n, "v_r"),
+                                       _dev(v_t, f, n, "v_t"), _dev(m_sorted, f, n, "m_sorted"),
+                                       _dev(t_rel_bin, f, nb, "t_rel_bin"), _dev(t_rel_min, f, 1, "t_rel_min"), wp, wb, _stream())
+    _check(rc, "hmc_relaxation_timestep")
+    return t_rel_bin, t_rel_min
+
+
+def hmc_two_body_relaxation(r_sorted, v_r, v_t, m_sorted, ids, dt: float, seed: int, step: int, gamma: float = 0.1,
+                            G: float = 1.0, *, v_r_out=None, v_t_out=None, dt_device=None):
+    """Representative two-body encounter of every neighbour pair.  -> (v_r', v_t')
+    dt_device (device float64[1]) given: the step is dt * dt_device[0], read on the device."""
+    n = r_sorted.numel()
+    dev = r_sorted.device
+    f = torch.float64
+    v_r_out = torch.empty(n, dtype=f, device=dev) if v_r_out is None else v_r_out
+    v_t_out = torch.empty(n, dtype=f, device=dev) if v_t_out is None else v_t_out
+    rc = lib().hmc_two_body_relaxation(ctypes.c_uint64(n), ctypes.c_double(G), ctypes.c_double(gamma), ctypes.c_double(dt),
+                                       _dev(dt_device, f, 1, "dt_device"), ctypes.c_uint64(seed), ctypes.c_uint32(step),
+                                       _dev(r_sorted, f, n, "r_sorted"),
+                                       _dev(v_r, f, n, "v_r"), _dev(v_t, f, n, "v_t"), _dev(m_sorted, f, n, "m_sorted"),
+                                       _dev(ids, torch.int32, n, "ids"), _dev(v_r_out, f, n, "v_r_out"),
+                                       _dev(v_t_out, f, n, "v_t_out"), _stream())
+    _check(rc, "hmc_two_body_relaxation")
+    return v_r_out, v_t_out
+
+
 def launch_count() -> int:
     """Kernels this process has launched through libhmc so far (hmc_launch_count)."""
     return int(lib().hmc_launch_count())
@@ -325,7 +366,7 @@ class OrbitStepper:
     current stream and swaps (r, v_r, v_t) <- (r_new, v_r', v_t'); m and id follow the sort."""
 
     def __init__(self, r, v_r, v_t, m, ids, seed: int, G: float = 1.0, with_n_try: bool = True,
-                 energy_correction: bool = False):
+                 energy_correction: bool = False, relaxation: bool = False, gamma: float = 0.1, theta_max: float = 1.0):
         """energy_correction=True: from the second step on, hmc_energy_correction adjusts the velocities
         between the potential and the turning points; three more columns (the star's energy,
         previous radius and the previous potential there) then travel through the sort."""
@@ -333,6 +374,14 @@ class OrbitStepper:
         dev = r.device
         self.G, self.seed, self.step_index = G, seed, 0
         self.energy_correction = energy_correction
+        # relaxation=True: between the potential and the turning points, the relaxation timestep of Eq. 7 and one
+        # representative encounter per neighbour pair over that timestep, all on the device
+        self.relaxation, self.gamma, self.theta_max = relaxation, gamma, theta_max
+        if relaxation:
+            self.t_rel_bin = torch.empty(max(1, n // BIN), dtype=torch.float64, device=r.device)
+            self.t_rel_min = torch.empty(1, dtype=torch.float64, device=r.device)
+            self.relaxed = dict(v_r=torch.empty(n, dtype=torch.float64, device=r.device),
+                                v_t=torch.empty(n, dtype=torch.float64, device=r.device))
         self.state = dict(r=r.clone(), v_r=v_r.clone(), v_t=v_t.clone(), m=m.clone(), id=ids.clone())
         f = dict(dtype=torch.float64, device=dev)
         self.sorted = dict(r=torch.empty(n, **f), v_r=torch.empty(n, **f), v_t=torch.empty(n, **f),
@@ -368,6 +417,15 @@ class OrbitStepper:
                                   counters=self.counters, workspace=self.workspace)
             so["v_r"], co["v_r"] = co["v_r"], so["v_r"]
             so["v_t"], co["v_t"] = co["v_t"], so["v_t"]
+        if self.relaxation:
+            rx = self.relaxed
+            hmc_relaxation_timestep(so["r"], so["v_r"], so["v_t"], so["m"], self.gamma, self.theta_max, self.G,
+                                    t_rel_bin=self.t_rel_bin[: (1 if self.n < BIN else self.n // BIN)], t_rel_min=self.t_rel_min,
+                                    workspace=self.workspace)
+            hmc_two_body_relaxation(so["r"], so["v_r"], so["v_t"], so["m"], so["id"], 1.0, self.seed, self.step_index,
+                                    self.gamma, self.G, v_r_out=rx["v_r"], v_t_out=rx["v_t"], dt_device=self.t_rel_min)
+            so["v_r"], rx["v_r"] = rx["v_r"], so["v_r"]
+            so["v_t"], rx["v_t"] = rx["v_t"], so["v_t"]
         if fused:
             hmc_orbit_step(so["r"], so["v_r"], so["v_t"], self.phi, self.m_cum, so["id"], self.seed, self.step_index,
                            self.G, tp=self.tp, out=self.sample, counters=self.counters, workspace=self.workspace)
