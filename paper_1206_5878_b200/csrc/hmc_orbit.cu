@@ -36,7 +36,10 @@ namespace hmc {
 
 static constexpr int ORB_THREADS = 1024;
 static constexpr int ORB_WARPS = ORB_THREADS / 32;
-static constexpr int FRONT_ROUNDS = 2;       // S4: trials a lane may run through the squeeze per exact round
+#ifndef HMC_FRONT_ROUNDS
+#define HMC_FRONT_ROUNDS 2
+#endif
+static constexpr int FRONT_ROUNDS = HMC_FRONT_ROUNDS;       // S4: trials a lane may run through the squeeze per exact round
 
 __device__ __forceinline__ double pos_inf() { return __longlong_as_double(0x7ff0000000000000ll); }
 
@@ -305,35 +308,38 @@ __device__ __forceinline__ double secant_root(double r_lo, double P_lo, double r
 }
 
 // One star of S3: brackets, turning points, status, and S4's bound F (0 = no draw).  a = position in the
-// sorted arrays (star k = a + 1); rk, vr, vt, phik its radius, velocities and potential.
+// sorted arrays (star k = a + 1); rk, vr, vt, phik its radius, velocities and potential.  In two halves:
+// locate_star (tiers 1 and 2: shared memory and the directory, ends with the guessed nodes) and finish_star_s3
+// (tier 3: the exact probes, then the roots), so that a caller can put other work between the two while the
+// guessed nodes travel from DRAM to L2.
 struct Solved {
     double E, J, rmin, rmax, Fv;
     uint32_t kmin, kmax;
     unsigned st;
 };
 
-__device__ __forceinline__ Solved solve_star(const Tables& T, uint32_t a, double rk, double vr, double vt, double phik)
+struct Located {
+    double E, J, rk;
+    uint32_t lo1, hi1, g1, lo2, hi2, g2;   // brackets after tiers 1-2 and the guessed nodes (pericentre 1, apocentre 2)
+    unsigned st;                            // status bits; bit 8 / bit 9: side 1 / 2 starts from its guess
+};
+
+__device__ __forceinline__ Located locate_star(const Tables& T, uint32_t a, double rk, double vr, double vt, double phik)
 {
     const uint32_t n = T.n;
     const int shift = T.shift;
-    const Node* __restrict__ nodes = T.nodes;
     const double2* coarse = T.coarse;
-    double E, J, rmin, rmax, Fv;
-    uint32_t kmin, kmax;
-    unsigned st;
     const uint32_t k = a + 1;
-        E = phik + 0.5 * (vr * vr + vt * vt);      // Eq. 16
-    J = rk * vt;
+    Located L;
+    const double E = phik + 0.5 * (vr * vr + vt * vt);      // Eq. 16
+    const double J = rk * vt;
     const double J2 = J * J;
-    st = 0;
+    unsigned st = 0;
     if (!(E < 0.0)) st |= HMC_STAR_UNBOUND;
     if (J2 == 0.0) st |= HMC_STAR_RADIAL;
-    Fv = 0.0;
-    if (st) {
-        rmin = (st & HMC_STAR_RADIAL) ? 0.0 : rk;
-        rmax = (st & HMC_STAR_UNBOUND) ? pos_inf() : rk;
-        kmin = k - 1; kmax = k;
-    } else {
+    L.E = E; L.J = J; L.rk = rk;
+    L.lo1 = 0u; L.hi1 = k; L.g1 = 0u; L.lo2 = k; L.hi2 = n + 1; L.g2 = 0u;
+    if (!st) {
         // pericentre bracket (lo, hi): Q_lo < 0 <= Q_hi;  apocentre: Q_lo >= 0 > Q_hi
         Side s1{ 0u, k, 1u, 0u, MODE_BISECT }, s2{ k, n + 1, 1u, 0u, MODE_BISECT };
         // tier 1: the coarse nodes, in shared memory; both searches advance together (two
@@ -398,9 +404,29 @@ __device__ __forceinline__ Solved solve_star(const Tables& T, uint32_t a, double
             uint32_t w1 = 0, w2 = 0;
             if (g1) w1 = ld_u32_keep(a1, T.keep);
             if (g2) w2 = ld_u32_keep(a2, T.keep);
-            if (g1) { s1.guess = T.dir_guess_node(c1, w1, f1); s1.mode = MODE_GUESS; }
-            if (g2) { s2.guess = T.dir_guess_node(c2, w2, f2); s2.mode = MODE_GUESS; }
+            if (g1) { s1.guess = T.dir_guess_node(c1, w1, f1); st |= 256u; }
+            if (g2) { s2.guess = T.dir_guess_node(c2, w2, f2); st |= 512u; }
         }
+        L.lo1 = s1.lo; L.hi1 = s1.hi; L.g1 = s1.guess; L.lo2 = s2.lo; L.hi2 = s2.hi; L.g2 = s2.guess;
+    }
+    L.st = st;
+    return L;
+}
+
+__device__ __forceinline__ Solved finish_star_s3(const Tables& T, uint32_t a, const Located& L)
+{
+    const Node* __restrict__ nodes = T.nodes;
+    const uint32_t k = a + 1;
+    const double E = L.E, J = L.J, rk = L.rk, J2 = J * J;
+    double rmin, rmax, Fv = 0.0;
+    uint32_t kmin, kmax;
+    unsigned st = L.st & 255u;
+    if (st) {
+        rmin = (st & HMC_STAR_RADIAL) ? 0.0 : rk;
+        rmax = (st & HMC_STAR_UNBOUND) ? pos_inf() : rk;
+        kmin = k - 1; kmax = k;
+    } else {
+        Side s1{ L.lo1, L.hi1, 1u, L.g1, (L.st & 256u) ? MODE_GUESS : MODE_BISECT }, s2{ L.lo2, L.hi2, 1u, L.g2, (L.st & 512u) ? MODE_GUESS : MODE_BISECT };
         // tier 3: exact probes of adjacent node pairs, the two searches interleaved
         while (true) {
             const bool a1 = s1.active(), a2 = s2.active();
@@ -425,16 +451,24 @@ __device__ __forceinline__ Solved solve_star(const Tables& T, uint32_t a, double
         if (Cb < 0.0) rmax = (eb.B + sqrt(D)) / (-2.0 * Cb);
         else { rmax = pos_inf(); st |= HMC_STAR_DEGENERATE; }
         // S4's bound F (R7) needs G M at both bracketing shells, which are in registers here and
-        // would cost S4 two random node reads per star: computed here, with S4's expressions,
-        // and left in the workspace for a following S4 call with reuse_tables (0 = no draw).
+        // would cost S4 two random node reads per star: computed here and left in the workspace for a
+        // following S4 call with reuse_tables (0 = no draw).  S4 writes F = 1.2 max(sqrt(3 D / q1), sqrt(3 D / -q2));
+        // division and square root are correctly rounded, hence monotone, so the larger square root is the
+        // square root of the larger quotient, which is the quotient by the smaller divisor: the same bits
+        // from one division and one square root instead of two each.
         const double delta = rmax - rmin;
         if (!(st & HMC_STAR_DEGENERATE) && delta > 0.0) {
             const double q1 = (2.0 * (J2 / rmin - ea.B)) / (rmin * rmin);      // Q'(r_min) in shell k_min
             const double q2 = (2.0 * (J2 / rmax - eb.B)) / (rmax * rmax);      // Q'(r_max) in shell k_max
-            if ((q1 > 0.0) && (q2 < 0.0)) Fv = 1.2 * fmax(sqrt((3.0 * delta) / q1), sqrt((3.0 * delta) / (-q2)));
+            if ((q1 > 0.0) && (q2 < 0.0)) Fv = 1.2 * sqrt((3.0 * delta) / fmin(q1, -q2));
         }
     }
     return Solved{ E, J, rmin, rmax, Fv, kmin, kmax, st };
+}
+
+__device__ __forceinline__ Solved solve_star(const Tables& T, uint32_t a, double rk, double vr, double vt, double phik)
+{
+    return finish_star_s3(T, a, locate_star(T, a, rk, vr, vt, phik));
 }
 
 // Stars first .. first+count-1 of the table (0-based positions; star at position p is node p + 1).  r and phi
@@ -452,20 +486,16 @@ turning_points_kernel(uint32_t n, uint32_t first, uint32_t count, double G, cons
     double2* coarse = reinterpret_cast<double2*>(smem_raw);
     stage_coarse(coarse, coarse_g, n, shift);
     Tables T{ nodes, dir, coarse, shift > MID_SHIFT ? mid_g : nullptr, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift, l2_keep_policy() };
-
     const uint32_t stride = gridDim.x * ORB_THREADS;
     for (uint32_t a = blockIdx.x * ORB_THREADS + threadIdx.x; a < count; a += stride) {
         const Solved v = solve_star(T, first + a, __ldcs(r + first + a), __ldcs(v_r + a), __ldcs(v_t + a), __ldcs(phi + first + a));
-        const double E = v.E, J = v.J, rmin = v.rmin, rmax = v.rmax, Fv = v.Fv;
-        const uint32_t kmin = v.kmin, kmax = v.kmax;
-        const unsigned st = v.st;
-        __stcs(F_ws + a, Fv);
-        __stcs(E_out + a, E); __stcs(J_out + a, J); __stcs(rmin_out + a, rmin); __stcs(rmax_out + a, rmax);
-        __stcs(kmin_out + a, kmin); __stcs(kmax_out + a, kmax); status_out[a] = (uint8_t)st;
-        if (st && counters) {
-            if (st & HMC_STAR_UNBOUND) atomicAdd(counters + HMC_CNT_UNBOUND, 1ull);
-            if (st & HMC_STAR_RADIAL) atomicAdd(counters + HMC_CNT_RADIAL, 1ull);
-            if (st & HMC_STAR_DEGENERATE) atomicAdd(counters + HMC_CNT_DEGENERATE, 1ull);
+        __stcs(F_ws + a, v.Fv);
+        __stcs(E_out + a, v.E); __stcs(J_out + a, v.J); __stcs(rmin_out + a, v.rmin); __stcs(rmax_out + a, v.rmax);
+        __stcs(kmin_out + a, v.kmin); __stcs(kmax_out + a, v.kmax); status_out[a] = (uint8_t)v.st;
+        if (v.st && counters) {
+            if (v.st & HMC_STAR_UNBOUND) atomicAdd(counters + HMC_CNT_UNBOUND, 1ull);
+            if (v.st & HMC_STAR_RADIAL) atomicAdd(counters + HMC_CNT_RADIAL, 1ull);
+            if (v.st & HMC_STAR_DEGENERATE) atomicAdd(counters + HMC_CNT_DEGENERATE, 1ull);
         }
     }
 }
@@ -508,6 +538,57 @@ __device__ __forceinline__ uint32_t coarse_locate(const double2* coarse, uint32_
     return lo;
 }
 
+// The same through an inverse table (S4 runs this once per trial: a quarter of its instructions were the twelve
+// steps of the bisection above).  A radius is keyed by the leading bits of its binary64 pattern (exponent and top
+// mantissa bits: monotone in r), INV_CELLS + 1 keys from that of r_1 on; inv[q] = largest coarse index whose
+// radius is <= the smallest radius of key q.  The interval of r0 then lies in [inv[q], inv[q + 1]]: a handful of
+// coarse entries instead of the orbit's few thousand.
+static constexpr uint32_t INV_CELLS = 2048;
+
+struct InvTable {
+    const uint16_t* inv;     // shared memory, [INV_CELLS + 2]
+    int base, sh;
+    __device__ __forceinline__ uint32_t key(double x) const
+    {
+        const int q = (__double2hiint(x) >> sh) - base;
+        return (uint32_t)min(max(q, 0), (int)INV_CELLS - 1);
+    }
+};
+
+// built by the whole CTA after stage_coarse; r_first, r_last: the radii of nodes 1 and N
+__device__ __forceinline__ InvTable build_inv(uint16_t* inv, const double2* coarse, uint32_t ncoarse, double r_first, double r_last)
+{
+    InvTable t;
+    const int h1 = __double2hiint(r_first), hn = __double2hiint(r_last);
+    int sh = 0;
+    while ((hn >> sh) - (h1 >> sh) > (int)INV_CELLS - 1) ++sh;
+    t.sh = sh; t.base = h1 >> sh; t.inv = inv;
+    for (uint32_t q = threadIdx.x; q <= INV_CELLS; q += ORB_THREADS) {
+        const long long hw = ((long long)q + t.base) << sh;                   // leading word of the smallest radius of key q
+        uint32_t lo = ncoarse;
+        if (hw < 0x7ff00000ll) {
+            const double x = __hiloint2double((int)hw, 0);
+            lo = 0;
+            uint32_t hi = ncoarse + 1;
+            while (hi - lo > 1) { const uint32_t m = (lo + hi) >> 1; if (coarse[m].x <= x) lo = m; else hi = m; }
+        }
+        inv[q] = (uint16_t)lo;
+    }
+    __syncthreads();
+    return t;
+}
+
+__device__ __forceinline__ uint32_t coarse_locate(const double2* coarse, const InvTable& iv, uint32_t cl, uint32_t ch, double r0)
+{
+    const uint32_t q = iv.key(r0);
+    uint32_t lo = iv.inv[q], hi = (uint32_t)iv.inv[q + 1] + 1;               // coarse[lo].r <= r0 < coarse[hi].r, or r0 < coarse[1].r
+    while (hi - lo > 1) {
+        const uint32_t m = (lo + hi) >> 1;
+        if (coarse[m].x <= r0) lo = m; else hi = m;
+    }
+    return min(max(lo, cl), ch);
+}
+
 // Exact evaluation of a trial, the oracle's expressions: shell j = #{ i : r_i <= r0 } clamped to
 // [k_min, k_max], found from the directory of coarse interval c; Phi(r0) by Eq. 6 anchored at j; Q0; g.
 __device__ __forceinline__ void exact_trial(const Tables& T, const Orbit& o, const Trial& tr, uint32_t c, double& Q0, double& g)
@@ -548,7 +629,7 @@ struct Exhaustive {
     bool accepted, have_good;
 };
 
-__device__ __noinline__ Exhaustive draw_exhaustive(Tables T, Orbit o, uint32_t seed_lo, uint32_t seed_hi, uint32_t step,
+__device__ __noinline__ Exhaustive draw_exhaustive(Tables T, InvTable iv, Orbit o, uint32_t seed_lo, uint32_t seed_hi, uint32_t step,
                                                    unsigned st)
 {
     Exhaustive x{ 0.0, 0.0, 0u, 0u, st, false, false };
@@ -557,7 +638,7 @@ __device__ __noinline__ Exhaustive draw_exhaustive(Tables T, Orbit o, uint32_t s
     for (; t < HMC_T_MAX; ++t) {
         Trial tr = make_trial(o, seed_lo, seed_hi, step, t);
         double Q0, g;
-        exact_trial(T, o, tr, coarse_locate(T.coarse, cl, ch, tr.r0), Q0, g);
+        exact_trial(T, o, tr, coarse_locate(T.coarse, iv, cl, ch, tr.r0), Q0, g);
         if (Q0 > 0.0) {
             x.have_good = true; x.good_r = tr.r0; x.good_Q = Q0; x.good_w3 = tr.w3;
             if (g > o.F) x.st |= HMC_STAR_CLIPPED;
@@ -714,6 +795,7 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
     double2* coarse = reinterpret_cast<double2*>(smem_raw + ORB_WARPS * sizeof(Park));
     stage_coarse(coarse, coarse_g, n, shift);
     Tables T{ nodes, dir, coarse, (FUSED && shift > MID_SHIFT) ? mid_g : nullptr, __ldg(io.r + (n - 1)), n, n >> shift, 1u << shift, shift, l2_keep_policy() };
+    const InvTable iv = build_inv(reinterpret_cast<uint16_t*>(coarse + (n >> shift) + 2), coarse, T.ncoarse, __ldg(io.r), T.r_last);
     unsigned long long my_trials = 0;
     const unsigned lane_lt = lanemask_lt();
     const uint32_t lane = threadIdx.x & 31;
@@ -775,7 +857,7 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
         for (int round = 0; round < FRONT_ROUNDS; ++round) {
             if (have && !candidate && t < HMC_T_MAX) {
                 tr = make_trial(o, seed_lo, seed_hi, step, t);
-                c = coarse_locate(coarse, cl, ch, tr.r0);
+                c = coarse_locate(coarse, iv, cl, ch, tr.r0);
                 ++t;
                 // squeeze: Phi(r0) lies in [coarse[c].Phi, coarse[c+1].Phi]; everything widened by ~1e-11.
                 // Written multiplied through by r0^2 > 0, so there is no division on this path.
@@ -805,7 +887,7 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
                 }
             }
             if (!done && t >= HMC_T_MAX) {
-                const Exhaustive x = draw_exhaustive(T, o, seed_lo, seed_hi, step, st);
+                const Exhaustive x = draw_exhaustive(T, iv, o, seed_lo, seed_hi, step, st);
                 st = x.st; accepted = x.accepted; used = x.used; have_good = x.have_good;
                 good_r = x.good_r; good_Q = x.good_Q; good_w3 = x.good_w3;
                 done = true;
@@ -924,9 +1006,10 @@ static hmc_status launch_sampler(bool fused, uint64_t n, double G, uint64_t seed
                                  const Workspace& ws, cudaStream_t st)
 {
     const int sms = sm_count();
-    const size_t smem = ORB_WARPS * sizeof(Park) + ((n >> shift) + 2) * sizeof(double2);
+    static constexpr size_t INV_BYTES = (INV_CELLS + 2) * sizeof(uint16_t);
+    const size_t smem = ORB_WARPS * sizeof(Park) + ((n >> shift) + 2) * sizeof(double2) + INV_BYTES;
     static std::atomic<uint64_t> opted[2];
-    const size_t cap = ORB_WARPS * sizeof(Park) + COARSE_CAP * sizeof(double2);
+    const size_t cap = ORB_WARPS * sizeof(Park) + COARSE_CAP * sizeof(double2) + INV_BYTES;
     hmc_status so = fused ? smem_opt_in(opted[1], sample_new_radius_kernel<true>, cap)
                           : smem_opt_in(opted[0], sample_new_radius_kernel<false>, cap);
     if (so != HMC_OK) return so;
