@@ -300,6 +300,7 @@ HMC_API hmc_status hmc_two_body_relaxation(uint64_t n, double G, double gamma, d
  *                          r_sorted, phi, m_cum are the TABLE's arrays [n]; v_r, v_t, id, every other per-star input
  *                          and every output are the range's own arrays [count].  first = 0, count = n is exactly
  *                          hmc_orbit_turning_points / hmc_sample_new_radius.  Workspace: hmc_workspace_bytes(n).
+ *                          reuse_tables: the preceding S3 call on the workspace must have covered this range.
  * hmc_partition_points: counts[j] = number of radii <= splitters[j], j < nsplit (splitters, counts: DEVICE arrays).
  * Errors: HMC_ERR_SIZE if rank >= nranks, or first + count > n.
  */

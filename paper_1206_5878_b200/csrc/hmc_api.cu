@@ -69,6 +69,8 @@ static Arena carve_arena(void* base, uint64_t n)
 // hmc_step_host only: a second stream on which the sorted masses and ids go back to the host while the
 // potential and orbit stages run (the two directions and the kernels then overlap).  One per (host thread,
 // device), created at first use and kept for the life of the thread: the only state the library owns.
+static constexpr int HOST_CHUNKS = 4;     // hmc_step_host: ranges S4 is cut into so that the copy back overlaps the draw
+
 struct SideStream {
     bool made = false;
     cudaStream_t stream = nullptr;
@@ -419,18 +421,29 @@ hmc_status hmc_step_host(uint64_t n, double G, uint64_t seed, uint32_t step, con
     HMC_CUDA_TRY(cudaStreamWaitEvent(side->stream, side->sorted, 0));
     HMC_CUDA_TRY(cudaMemcpyAsync(m_out, a.ms, n * 8, cudaMemcpyDeviceToHost, side->stream));
     HMC_CUDA_TRY(cudaMemcpyAsync(id_out, a.ids, n * 4, cudaMemcpyDeviceToHost, side->stream));
-    HMC_CUDA_TRY(cudaEventRecord(side->copied, side->stream));
     s = potential(n, G, a.rs, a.ms, a.phi, a.mcum, nullptr, 0, 0, ws, st);
     if (s != HMC_OK) return s;
     s = turning_points(n, 0, n, G, a.rs, a.vrs, a.vts, a.phi, a.mcum, a.E, a.J, a.rmin, a.rmax, a.kmin, a.kmax, a.st0,
                        a.counters, ws, st);
     if (s != HMC_OK) return s;
-    s = sample_new_radius(n, 0, n, G, seed, step, a.rs, a.phi, a.mcum, a.vrs, a.vts, a.E, a.J, a.rmin, a.rmax, a.kmin,
-                          a.kmax, a.ids, a.st0, a.rn, a.vrn, a.vtn, nullptr, a.st1, a.counters, true, ws, st);
-    if (s != HMC_OK) return s;
-    HMC_CUDA_TRY(cudaMemcpyAsync(r_new, a.rn, n * 8, cudaMemcpyDeviceToHost, st));
-    HMC_CUDA_TRY(cudaMemcpyAsync(v_r_new, a.vrn, n * 8, cudaMemcpyDeviceToHost, st));
-    HMC_CUDA_TRY(cudaMemcpyAsync(v_t_new, a.vtn, n * 8, cudaMemcpyDeviceToHost, st));
+    // S4 in HOST_CHUNKS ranges of the sorted order; the new coordinates of a range start for the host (on the side
+    // stream, behind the masses and ids) as soon as its draw is done, while the next range is being drawn
+    const uint64_t per = (n + HOST_CHUNKS - 1) / HOST_CHUNKS;
+    for (int c = 0; c < HOST_CHUNKS; ++c) {
+        const uint64_t first = umin64((uint64_t)c * per, n), count = umin64(per, n - first);
+        if (count == 0) break;
+        s = sample_new_radius(n, first, count, G, seed, step, a.rs, a.phi, a.mcum, a.vrs + first, a.vts + first, a.E + first,
+                              a.J + first, a.rmin + first, a.rmax + first, a.kmin + first, a.kmax + first, a.ids + first,
+                              a.st0 + first, a.rn + first, a.vrn + first, a.vtn + first, nullptr, a.st1 + first, a.counters,
+                              true, ws, st);
+        if (s != HMC_OK) return s;
+        HMC_CUDA_TRY(cudaEventRecord(side->up[c & 1], st));
+        HMC_CUDA_TRY(cudaStreamWaitEvent(side->stream, side->up[c & 1], 0));
+        HMC_CUDA_TRY(cudaMemcpyAsync(r_new + first, a.rn + first, count * 8, cudaMemcpyDeviceToHost, side->stream));
+        HMC_CUDA_TRY(cudaMemcpyAsync(v_r_new + first, a.vrn + first, count * 8, cudaMemcpyDeviceToHost, side->stream));
+        HMC_CUDA_TRY(cudaMemcpyAsync(v_t_new + first, a.vtn + first, count * 8, cudaMemcpyDeviceToHost, side->stream));
+    }
+    HMC_CUDA_TRY(cudaEventRecord(side->copied, side->stream));
     if (counters_host)
         HMC_CUDA_TRY(cudaMemcpyAsync(counters_host, a.counters, HMC_NCOUNTERS * 8, cudaMemcpyDeviceToHost, st));
     HMC_CUDA_TRY(cudaStreamWaitEvent(st, side->copied, 0));      // the caller's stream completes after the side copies

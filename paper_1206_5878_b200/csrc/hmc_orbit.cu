@@ -489,7 +489,7 @@ turning_points_kernel(uint32_t n, uint32_t first, uint32_t count, double G, cons
     const uint32_t stride = gridDim.x * ORB_THREADS;
     for (uint32_t a = blockIdx.x * ORB_THREADS + threadIdx.x; a < count; a += stride) {
         const Solved v = solve_star(T, first + a, __ldcs(r + first + a), __ldcs(v_r + a), __ldcs(v_t + a), __ldcs(phi + first + a));
-        __stcs(F_ws + a, v.Fv);
+        __stcs(F_ws + first + a, v.Fv);                            // by table position: a later S4 call may cover a sub-range
         __stcs(E_out + a, v.E); __stcs(J_out + a, v.J); __stcs(rmin_out + a, v.rmin); __stcs(rmax_out + a, v.rmax);
         __stcs(kmin_out + a, v.kmin); __stcs(kmax_out + a, v.kmax); status_out[a] = (uint8_t)v.st;
         if (v.st && counters) {
@@ -707,7 +707,7 @@ __device__ __forceinline__ uint32_t park_from_arrays(const Node* __restrict__ no
         rmin = __ldcs(io.rmin + a); rmax = __ldcs(io.rmax + a);
         kmin = __ldcs(io.kmin + a); kmax = __ldcs(io.kmax + a);
         sid = __ldcs(io.id + a);
-        if (io.F_ws) F = __ldcs(io.F_ws + a);
+        if (io.F_ws) F = __ldcs(io.F_ws + io.first + a);
     }
     bool ok = in && !(st & (HMC_STAR_UNBOUND | HMC_STAR_RADIAL | HMC_STAR_DEGENERATE));
     const double delta = rmax - rmin;
@@ -780,7 +780,7 @@ __device__ __forceinline__ void prefetch_inputs(const SampleIO& io, uint32_t a)
     else {
         prefetch_l2(io.E + a); prefetch_l2(io.J + a); prefetch_l2(io.rmin + a); prefetch_l2(io.rmax + a);
         prefetch_l2(io.kmin + a); prefetch_l2(io.kmax + a); prefetch_l2(io.id + a); prefetch_l2(io.status_in + a);
-        if (io.F_ws) prefetch_l2(io.F_ws + a);
+        if (io.F_ws) prefetch_l2(io.F_ws + io.first + a);
     }
 }
 

@@ -6,13 +6,15 @@
 //      w_i = ((bits(r_i) - kmin) >> s) << IB  |  i          IB = index bits (24, more if n > 2^24)
 //
 // kmin = smallest key, s = how many low key bits do not fit beside the index (0 when the keys span
-// fewer than 64 - IB bits).  A stable LSD radix sort of the w_i on their key part, at most five
-// 8-bit passes over 8 bytes per star, orders the stars by the leading 64 - IB bits of their
-// (shifted) keys, ties in input order.  What is left open are runs of stars that agree in those
-// leading bits but not in the s dropped ones: a handful per million on smooth radii.  The final
-// kernel, which also carries the record columns to their sorted places, detects each run, reads
-// the full keys of its members and ranks them inside the run by (key, index).  A run longer than
-// RUN_MAX sets a flag instead, and the general eight-pass sort of hmc_sort.cu, which is launched
+// fewer than 64 - IB bits; a narrower span is shifted up instead, so that it fills the kept bits).  The word keeps
+// up to 40 key bits, but the stable LSD radix sort runs only over the leading SB = 16, 24 or 32 of them (about
+// log2 N: three 8-bit passes at N = 1e7 instead of the four that sorting every kept bit took): that orders the
+// stars up to RUNS that agree in those leading bits -- about ten stars long where a Plummer cluster is densest --
+// and the rest of the order is already in the word: inside a run, whole words compare as (key bits, index).  The
+// final kernel, which also carries the record columns to their sorted places, detects each run from the neighbouring
+// words (coalesced, no extra memory traffic) and ranks every member inside it; only members that agree in ALL kept
+// key bits while low bits were dropped (s > 0: a handful per million) need their full keys read.  A run longer
+// than RUN_MAX sets a flag instead, and the general eight-pass sort of hmc_sort.cu, which is launched
 // after this path and returns at once when the flag is clear, redoes the call.
 //
 // Record columns: one random 8-byte read per column per star costs a whole DRAM line each.
@@ -30,7 +32,7 @@ static constexpr int PK_THREADS = 512;
 static constexpr int PK_WARPS = PK_THREADS / 32;
 static constexpr int PK_ITEMS = 8;
 static constexpr int PK_TILE = PK_THREADS * PK_ITEMS;          // 4096
-static constexpr int RUN_MAX = 32;
+static constexpr int RUN_MAX = 64;
 static constexpr int LB = 4;                                  // look-back words loaded per round trip
 
 static constexpr uint32_t PK_FLAG_AGG = 1u << 30;
@@ -42,9 +44,18 @@ enum { CTL_KMIN = 0, CTL_KMAX = 1, CTL_LONGRUN = 2 };
 // how the keys are packed, derived by every kernel from (n, kmin, kmax)
 struct Packing {
     uint64_t kmin;
-    int idx_bits, key_bits, s;
-    __host__ __device__ uint64_t key_part(uint64_t key) const { return (key - kmin) >> s; }
+    int idx_bits, key_bits, sort_bits, s, up;      // key bits kept / sorted by the passes; right or left shift of key - kmin
+    __host__ __device__ uint64_t key_part(uint64_t key) const { return ((key - kmin) >> s) << up; }
+    __host__ __device__ int low_bits() const { return key_bits - sort_bits; }      // kept but not sorted: resolved in the runs
 };
+
+// bits the passes sort: about log2 n, whole digits, at least two of them
+__host__ __device__ inline int sort_bits_of(int ib, int key_bits)
+{
+    int sb = ((ib + 7) / 8) * 8;
+    if (sb < 16) sb = 16;
+    return sb < key_bits ? sb : (key_bits / 8) * 8;
+}
 
 __device__ __forceinline__ Packing packing_of(uint32_t n, const uint64_t* __restrict__ ctl)
 {
@@ -54,13 +65,11 @@ __device__ __forceinline__ Packing packing_of(uint32_t n, const uint64_t* __rest
     int ib = 32 - __clz(n - 1u);                               // bits needed for 0 .. n-1 (n >= 2)
     if (n < 2) ib = 1;
     p.idx_bits = ib < 24 ? 24 : ib;
-    // key bits kept: enough that a run of stars agreeing in all of them is rare on smooth radii
-    // (about 2^-3 stars per cell of the densest binade), whole digits, at most what fits
-    p.key_bits = ((ib + 8 + 7) / 8) * 8;
-    if (p.key_bits > PK_KEYBITS_MAX) p.key_bits = PK_KEYBITS_MAX;
-    if (p.key_bits > 64 - p.idx_bits) p.key_bits = 64 - p.idx_bits;
+    p.key_bits = PK_KEYBITS_MAX < 64 - p.idx_bits ? PK_KEYBITS_MAX : 64 - p.idx_bits;      // what fits beside the index
+    p.sort_bits = sort_bits_of(ib, p.key_bits);
     const int span_bits = 64 - __clzll((long long)span);       // 0 when all keys are equal
     p.s = span_bits > p.key_bits ? span_bits - p.key_bits : 0;
+    p.up = span_bits < p.key_bits ? p.key_bits - span_bits : 0;
     return p;
 }
 
@@ -159,7 +168,8 @@ __global__ void __launch_bounds__(PKH_THREADS) sort_pk_histogram_kernel(const ui
     __syncthreads();
     const Packing pk = packing_of(n, ctl);
     uint32_t* mine = sh[(threadIdx.x >> 5) % PKH_COPIES];
-    const int npass = (pk.key_bits + 7) / 8;                    // digits beyond are zero for every key
+    const int npass = pk.sort_bits / 8;                         // digits beyond are not sorted
+    const int low = pk.low_bits();
     const uint32_t stride = gridDim.x * PKH_THREADS;
     const uint32_t iters = (n + stride - 1) / stride;           // same trip count for every thread
     uint32_t i = blockIdx.x * PKH_THREADS + threadIdx.x;
@@ -184,16 +194,16 @@ __global__ void __launch_bounds__(PKH_THREADS) sort_pk_histogram_kernel(const ui
 #pragma unroll
         for (int u = 0; u < PKH_UNROLL; ++u) {
             if (it + u >= iters) break;                         // uniform over the warp
-            const uint64_t k = pk.key_part(kp[u]);
+            const uint64_t k = pk.key_part(kp[u]) >> low;
             if (ok[u]) {
 #pragma unroll
-                for (int p = 0; p < PK_MAXPASS - 2; ++p) atomicAdd(&mine[p * PK_RADIX + ((uint32_t)(k >> (8 * p)) & 255u)], 1u);
+                for (int p = 0; p < PK_MAXPASS - 1; ++p)
+                    if (p < npass - 1) atomicAdd(&mine[p * PK_RADIX + ((uint32_t)(k >> (8 * p)) & 255u)], 1u);
             }
-            // the leading digits take few distinct values: aggregate across the warp first
+            // the leading digit takes few distinct values: aggregate across the warp first
             const unsigned live = __ballot_sync(0xffffffffu, ok[u]);
-#pragma unroll
-            for (int p = PK_MAXPASS - 2; p < PK_MAXPASS; ++p) {
-                if (p >= npass) break;
+            {
+                const int p = npass - 1;
                 const uint32_t d = (uint32_t)(k >> (8 * p)) & 255u;
                 const unsigned peers = match_digit(d) & live;
                 if (ok[u] && (peers & lanemask_lt()) == 0) atomicAdd(&mine[p * PK_RADIX + d], (uint32_t)__popc(peers));
@@ -201,8 +211,8 @@ __global__ void __launch_bounds__(PKH_THREADS) sort_pk_histogram_kernel(const ui
         }
         i += PKH_UNROLL * stride;
     }
-    // digits beyond the kept key bits: every key has digit 0
-    if (blockIdx.x == 0 && threadIdx.x < PK_MAXPASS && (int)threadIdx.x >= max(npass, PK_MAXPASS - 2)) atomicAdd(&hist[threadIdx.x * PK_RADIX], n);
+    // digits beyond the sorted bits: their passes are never launched; mark them dead (one bin holds every star)
+    if (blockIdx.x == 0 && threadIdx.x < PK_MAXPASS && (int)threadIdx.x >= npass) atomicAdd(&hist[threadIdx.x * PK_RADIX], n);
     __syncthreads();
     for (int b = threadIdx.x; b < PK_MAXPASS * PK_RADIX; b += PKH_THREADS) {
         uint32_t c = 0;
@@ -259,7 +269,7 @@ sort_pk_pass_kernel(PkBuffers b, uint32_t n, const uint64_t* __restrict__ ctl,
     const uint64_t* __restrict__ in = b.buf[(live_before & 1) ^ 1];
     uint64_t* __restrict__ out = b.buf[live_before & 1];
     const Packing pk = packing_of(n, ctl);
-    const int shift = pk.idx_bits + 8 * pass;
+    const int shift = pk.idx_bits + pk.low_bits() + 8 * pass;
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PkSmem& s = *reinterpret_cast<PkSmem*>(smem_raw);
@@ -397,22 +407,32 @@ sort_pk_finish_kernel(PkBuffers b, const double* __restrict__ rec, PkCols g, uin
         if (in) {
             const uint64_t w = live ? __ldg(fin + k) : (uint64_t)k;        // no live pass: every key part equal
             idx = (uint32_t)(w & idx_mask);
-            if (pk.s > 0) {                                                // else equal key parts are equal keys
-                const uint64_t kp = w >> ib;
-                const bool eq_l = k > 0 && (__ldg(fin + k - 1) >> ib) == kp;
-                const bool eq_r = k + 1 < n && (__ldg(fin + k + 1) >> ib) == kp;
-                if (eq_l || eq_r) {
+            const int low = pk.low_bits();
+            if (live && (low > 0 || pk.s > 0)) {                           // else equal sorted bits are equal keys, in input order
+                const int rs = ib + low;                                   // the passes sorted the bits from rs up
+                const uint64_t sk = w >> rs;
+                const bool eq_l = k > 0 && (__ldg(fin + k - 1) >> rs) == sk;
+                const bool eq_r = k + 1 < n && (__ldg(fin + k + 1) >> rs) == sk;
+                if (eq_l || eq_r) {                                        // member of a run: rank inside it by (key, index)
                     uint32_t a = k, e = k + 1;
-                    while (a > 0 && k - a <= RUN_MAX && (__ldg(fin + a - 1) >> ib) == kp) --a;
-                    while (e < n && e - a <= RUN_MAX + 1 && (__ldg(fin + e) >> ib) == kp) ++e;
+                    while (a > 0 && k - a <= RUN_MAX && (__ldg(fin + a - 1) >> rs) == sk) --a;
+                    while (e < n && e - a <= RUN_MAX + 1 && (__ldg(fin + e) >> rs) == sk) ++e;
                     if (e - a > RUN_MAX) ctl[CTL_LONGRUN] = 1;            // the general sort redoes the call
                     else {
-                        const uint64_t mine = __ldg(b.keys_src + idx);
+                        const uint64_t kept = w >> ib;
+                        uint64_t mine = 0;
+                        bool have_mine = false;
                         uint32_t below = 0;
                         for (uint32_t j = a; j < e; ++j) {
                             if (j == k) continue;
-                            const uint64_t other = __ldg(b.keys_src + (uint32_t)(__ldg(fin + j) & idx_mask));
-                            below += (other < mine || (other == mine && j < k)) ? 1u : 0u;   // equal keys: input order
+                            const uint64_t wj = __ldg(fin + j);
+                            bool less = wj < w;                            // other kept key bits, or the same and a lower index
+                            if (pk.s > 0 && (wj >> ib) == kept) {          // all kept bits agree but bits were dropped: full keys
+                                if (!have_mine) { mine = __ldg(b.keys_src + idx); have_mine = true; }
+                                const uint64_t other = __ldg(b.keys_src + (uint32_t)(wj & idx_mask));
+                                less = other < mine || (other == mine && wj < w);
+                            }
+                            below += less ? 1u : 0u;
                         }
                         dest = a + below;
                     }
@@ -486,10 +506,8 @@ hmc_status sort_fast(uint64_t n, const double* r_in, double* r_sorted, uint32_t*
     int ib = 1;
     while ((1ull << ib) < n) ++ib;                                          // as packing_of
     const int idx_bits = ib < 24 ? 24 : ib;
-    int key_bits = ((ib + 8 + 7) / 8) * 8;
-    if (key_bits > PK_KEYBITS_MAX) key_bits = PK_KEYBITS_MAX;
-    if (key_bits > 64 - idx_bits) key_bits = 64 - idx_bits;
-    const int npass = (key_bits + 7) / 8;                                   // later digits are constant
+    const int key_bits = PK_KEYBITS_MAX < 64 - idx_bits ? PK_KEYBITS_MAX : 64 - idx_bits;
+    const int npass = sort_bits_of(ib, key_bits) / 8;                       // digits of the leading bits only
     for (int p = 0; p < npass; ++p) {
         sort_pk_pass_kernel<<<(int)umin64(tiles, (uint64_t)sms * 2), PK_THREADS, sizeof(PkSmem), st>>>(b, (uint32_t)n, ws.sortctl, ws.pk_hist + p * PK_RADIX,
                                                                        ws.lookback + (size_t)p * tiles * PK_RADIX,
