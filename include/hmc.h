@@ -15,6 +15,7 @@
  *  - Unless a parameter says "host", every array pointer is a DEVICE pointer owned by the
  *    caller.  The library never allocates, frees or keeps device memory between calls; scratch
  *    space is the caller's `workspace` of at least hmc_workspace_bytes(n) bytes, 256-byte aligned.
+ *    (The one thing it keeps: hmc_step_host's two streams and their events, see there; and a launch counter.)
  *  - Every call is asynchronous on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
  *    legacy default stream) and never synchronises the host.
  *  - Inputs are never modified; outputs must not alias inputs or each other.
@@ -339,10 +340,12 @@ HMC_API hmc_status hmc_sample_new_radius_range(uint64_t n, uint64_t first, uint6
  * order of the INPUT radii.  Host buffers should be page-locked for the copies to be asynchronous.
  * `device_arena` is a DEVICE buffer of at least hmc_step_host_arena_bytes(n) bytes (256-byte
  * aligned) holding the staged columns, every intermediate and the workspace.
- * The call enqueues H2D copies, the four stages and D2H copies on `cuda_stream`; the host arrays
- * are valid after the caller synchronises the stream (m_out and id_out travel on a second, library-owned
- * stream, created at first use per host thread, which `cuda_stream` waits for before the call's work ends).  counters_host (HOST uint64[HMC_NCOUNTERS],
- * may be NULL) receives the step's counters.
+ * The call enqueues the copies in on `cuda_stream`, the four stages on a library-owned stream and the copies out on
+ * another (the only state the library keeps: two streams and a few events per host thread and device, created at
+ * first use), chained by events so that the three overlap: the sort starts when the radii have arrived, the sorted
+ * masses and ids go back while the velocities are still coming in, and the new coordinates go back range by range
+ * behind the draw.  `cuda_stream` waits for all of it: the host arrays are valid after the caller synchronises that
+ * stream.  counters_host (HOST uint64[HMC_NCOUNTERS], may be NULL) receives the step's counters.
  */
 HMC_API size_t hmc_step_host_arena_bytes(uint64_t n);
 

@@ -66,35 +66,36 @@ static Arena carve_arena(void* base, uint64_t n)
     return a;
 }
 
-// hmc_step_host only: a second stream on which the sorted masses and ids go back to the host while the
-// potential and orbit stages run (the two directions and the kernels then overlap).  One per (host thread,
-// device), created at first use and kept for the life of the thread: the only state the library owns.
-static constexpr int HOST_CHUNKS = 4;     // hmc_step_host: ranges S4 is cut into so that the copy back overlaps the draw
+// hmc_step_host only: two library-owned streams and a few events, so that the three things a host-buffer step does --
+// copy in (on the caller's stream), compute (on `kern`) and copy out (on `copy`) -- overlap: PCIe is full duplex and
+// the step is bound by it.  One set per (host thread, device), created at first use and kept for the life of the
+// thread: the only state the library owns.
+static constexpr int HOST_CHUNKS = 4;     // ranges S4 is cut into so that the copy back starts behind the first of them
 
-struct SideStream {
+struct HostStepStreams {
     bool made = false;
-    cudaStream_t stream = nullptr;
-    cudaEvent_t sorted = nullptr, copied = nullptr;
-    cudaEvent_t up[2] = { nullptr, nullptr };
+    cudaStream_t kern = nullptr, copy = nullptr;
+    cudaEvent_t r_up = nullptr, id_up = nullptr, vt_up = nullptr, mid_sorted = nullptr, done = nullptr;
+    cudaEvent_t drawn[HOST_CHUNKS] = {};
 };
 
-static hmc_status side_stream(SideStream** out)
+static hmc_status host_step_streams(HostStepStreams** out)
 {
-    static thread_local std::vector<SideStream> per_device;
+    static thread_local std::vector<HostStepStreams> per_device;
     int dev = 0;
     HMC_CUDA_TRY(cudaGetDevice(&dev));
     if (dev < 0) return HMC_ERR_CUDA;
     if ((size_t)dev >= per_device.size()) per_device.resize((size_t)dev + 1);
-    SideStream& ss = per_device[(size_t)dev];
-    if (!ss.made) {
-        HMC_CUDA_TRY(cudaStreamCreateWithFlags(&ss.stream, cudaStreamNonBlocking));
-        HMC_CUDA_TRY(cudaEventCreateWithFlags(&ss.sorted, cudaEventDisableTiming));
-        HMC_CUDA_TRY(cudaEventCreateWithFlags(&ss.copied, cudaEventDisableTiming));
-        HMC_CUDA_TRY(cudaEventCreateWithFlags(&ss.up[0], cudaEventDisableTiming));
-        HMC_CUDA_TRY(cudaEventCreateWithFlags(&ss.up[1], cudaEventDisableTiming));
-        ss.made = true;
+    HostStepStreams& hs = per_device[(size_t)dev];
+    if (!hs.made) {
+        HMC_CUDA_TRY(cudaStreamCreateWithFlags(&hs.kern, cudaStreamNonBlocking));
+        HMC_CUDA_TRY(cudaStreamCreateWithFlags(&hs.copy, cudaStreamNonBlocking));
+        cudaEvent_t* evs[] = { &hs.r_up, &hs.id_up, &hs.vt_up, &hs.mid_sorted, &hs.done };
+        for (cudaEvent_t* e : evs) HMC_CUDA_TRY(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
+        for (int c = 0; c < HOST_CHUNKS; ++c) HMC_CUDA_TRY(cudaEventCreateWithFlags(&hs.drawn[c], cudaEventDisableTiming));
+        hs.made = true;
     }
-    *out = &ss;
+    *out = &hs;
     return HMC_OK;
 }
 
@@ -403,31 +404,52 @@ hmc_status hmc_step_host(uint64_t n, double G, uint64_t seed, uint32_t step, con
     Arena a = carve_arena(device_arena, n);
     if (arena_bytes < a.total) return HMC_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    HostStepStreams* hs = nullptr;
+    hmc_status s = host_step_streams(&hs);
+    if (s != HMC_OK) return s;
+    cudaStream_t K = hs->kern, D = hs->copy;
+    // copy in, on the caller's stream, in the order the stages need the columns: r (the sort), m and id (they go
+    // back to the host sorted, and S2 needs m), then the velocities (S3)
     HMC_CUDA_TRY(cudaMemcpyAsync(a.r, r, n * 8, cudaMemcpyHostToDevice, st));
-    HMC_CUDA_TRY(cudaMemcpyAsync(a.vr, v_r, n * 8, cudaMemcpyHostToDevice, st));
-    HMC_CUDA_TRY(cudaMemcpyAsync(a.vt, v_t, n * 8, cudaMemcpyHostToDevice, st));
+    HMC_CUDA_TRY(cudaEventRecord(hs->r_up, st));
     HMC_CUDA_TRY(cudaMemcpyAsync(a.m, m, n * 8, cudaMemcpyHostToDevice, st));
     HMC_CUDA_TRY(cudaMemcpyAsync(a.id, id, n * 4, cudaMemcpyHostToDevice, st));
-    HMC_CUDA_TRY(cudaMemsetAsync(a.counters, 0, HMC_NCOUNTERS * 8, st));
+    HMC_CUDA_TRY(cudaEventRecord(hs->id_up, st));
+    HMC_CUDA_TRY(cudaMemcpyAsync(a.vr, v_r, n * 8, cudaMemcpyHostToDevice, st));
+    HMC_CUDA_TRY(cudaMemcpyAsync(a.vt, v_t, n * 8, cudaMemcpyHostToDevice, st));
+    HMC_CUDA_TRY(cudaEventRecord(hs->vt_up, st));
     Workspace ws = carve(a.ws, n);
-    const double* cin[3] = { a.vr, a.vt, a.m };
-    double* cout[3] = { a.vrs, a.vts, a.ms };
-    hmc_status s = sort_by_radius(n, a.r, a.rs, a.perm, 3, cin, cout, a.id, a.ids, ws, st);
+    // S1 as soon as the radii are there: the permutation and the sorted radii (no columns yet)
+    HMC_CUDA_TRY(cudaStreamWaitEvent(K, hs->r_up, 0));
+    HMC_CUDA_TRY(cudaMemsetAsync(a.counters, 0, HMC_NCOUNTERS * 8, K));
+    s = sort_by_radius(n, a.r, a.rs, a.perm, 0, nullptr, nullptr, nullptr, nullptr, ws, K);
     if (s != HMC_OK) return s;
-    SideStream* side = nullptr;
-    s = side_stream(&side);
+    // masses and ids follow the permutation and start back to the host while the velocities are still coming in
+    HMC_CUDA_TRY(cudaStreamWaitEvent(K, hs->id_up, 0));
+    {
+        const double* cin[1] = { a.m };
+        double* cout[1] = { a.ms };
+        s = gather_by_perm(n, a.perm, 1, cin, cout, a.id, a.ids, K);
+        if (s != HMC_OK) return s;
+    }
+    HMC_CUDA_TRY(cudaEventRecord(hs->mid_sorted, K));
+    HMC_CUDA_TRY(cudaStreamWaitEvent(D, hs->mid_sorted, 0));
+    HMC_CUDA_TRY(cudaMemcpyAsync(m_out, a.ms, n * 8, cudaMemcpyDeviceToHost, D));
+    HMC_CUDA_TRY(cudaMemcpyAsync(id_out, a.ids, n * 4, cudaMemcpyDeviceToHost, D));
+    s = potential(n, G, a.rs, a.ms, a.phi, a.mcum, nullptr, 0, 0, ws, K);
     if (s != HMC_OK) return s;
-    HMC_CUDA_TRY(cudaEventRecord(side->sorted, st));
-    HMC_CUDA_TRY(cudaStreamWaitEvent(side->stream, side->sorted, 0));
-    HMC_CUDA_TRY(cudaMemcpyAsync(m_out, a.ms, n * 8, cudaMemcpyDeviceToHost, side->stream));
-    HMC_CUDA_TRY(cudaMemcpyAsync(id_out, a.ids, n * 4, cudaMemcpyDeviceToHost, side->stream));
-    s = potential(n, G, a.rs, a.ms, a.phi, a.mcum, nullptr, 0, 0, ws, st);
-    if (s != HMC_OK) return s;
+    HMC_CUDA_TRY(cudaStreamWaitEvent(K, hs->vt_up, 0));
+    {
+        const double* cin[2] = { a.vr, a.vt };
+        double* cout[2] = { a.vrs, a.vts };
+        s = gather_by_perm(n, a.perm, 2, cin, cout, nullptr, nullptr, K);
+        if (s != HMC_OK) return s;
+    }
     s = turning_points(n, 0, n, G, a.rs, a.vrs, a.vts, a.phi, a.mcum, a.E, a.J, a.rmin, a.rmax, a.kmin, a.kmax, a.st0,
-                       a.counters, ws, st);
+                       a.counters, ws, K);
     if (s != HMC_OK) return s;
-    // S4 in HOST_CHUNKS ranges of the sorted order; the new coordinates of a range start for the host (on the side
-    // stream, behind the masses and ids) as soon as its draw is done, while the next range is being drawn
+    // S4 in HOST_CHUNKS ranges of the sorted order; the new coordinates of a range start back to the host as soon as
+    // its draw is done, while the next range is being drawn
     const uint64_t per = (n + HOST_CHUNKS - 1) / HOST_CHUNKS;
     for (int c = 0; c < HOST_CHUNKS; ++c) {
         const uint64_t first = umin64((uint64_t)c * per, n), count = umin64(per, n - first);
@@ -435,18 +457,18 @@ hmc_status hmc_step_host(uint64_t n, double G, uint64_t seed, uint32_t step, con
         s = sample_new_radius(n, first, count, G, seed, step, a.rs, a.phi, a.mcum, a.vrs + first, a.vts + first, a.E + first,
                               a.J + first, a.rmin + first, a.rmax + first, a.kmin + first, a.kmax + first, a.ids + first,
                               a.st0 + first, a.rn + first, a.vrn + first, a.vtn + first, nullptr, a.st1 + first, a.counters,
-                              true, ws, st);
+                              true, ws, K);
         if (s != HMC_OK) return s;
-        HMC_CUDA_TRY(cudaEventRecord(side->up[c & 1], st));
-        HMC_CUDA_TRY(cudaStreamWaitEvent(side->stream, side->up[c & 1], 0));
-        HMC_CUDA_TRY(cudaMemcpyAsync(r_new + first, a.rn + first, count * 8, cudaMemcpyDeviceToHost, side->stream));
-        HMC_CUDA_TRY(cudaMemcpyAsync(v_r_new + first, a.vrn + first, count * 8, cudaMemcpyDeviceToHost, side->stream));
-        HMC_CUDA_TRY(cudaMemcpyAsync(v_t_new + first, a.vtn + first, count * 8, cudaMemcpyDeviceToHost, side->stream));
+        HMC_CUDA_TRY(cudaEventRecord(hs->drawn[c], K));
+        HMC_CUDA_TRY(cudaStreamWaitEvent(D, hs->drawn[c], 0));
+        HMC_CUDA_TRY(cudaMemcpyAsync(r_new + first, a.rn + first, count * 8, cudaMemcpyDeviceToHost, D));
+        HMC_CUDA_TRY(cudaMemcpyAsync(v_r_new + first, a.vrn + first, count * 8, cudaMemcpyDeviceToHost, D));
+        HMC_CUDA_TRY(cudaMemcpyAsync(v_t_new + first, a.vtn + first, count * 8, cudaMemcpyDeviceToHost, D));
     }
-    HMC_CUDA_TRY(cudaEventRecord(side->copied, side->stream));
     if (counters_host)
-        HMC_CUDA_TRY(cudaMemcpyAsync(counters_host, a.counters, HMC_NCOUNTERS * 8, cudaMemcpyDeviceToHost, st));
-    HMC_CUDA_TRY(cudaStreamWaitEvent(st, side->copied, 0));      // the caller's stream completes after the side copies
+        HMC_CUDA_TRY(cudaMemcpyAsync(counters_host, a.counters, HMC_NCOUNTERS * 8, cudaMemcpyDeviceToHost, D));
+    HMC_CUDA_TRY(cudaEventRecord(hs->done, D));
+    HMC_CUDA_TRY(cudaStreamWaitEvent(st, hs->done, 0));          // the caller's stream completes when everything is back
     return HMC_OK;
 }
 

@@ -234,6 +234,9 @@ hmc_status sort_by_radius(uint64_t n, const double* r_in, double* r_sorted, uint
                           uint32_t* id_out, const Workspace& ws, cudaStream_t st);
 // ext_tot == nullptr: the whole cluster.  Else (sharded step): r, m are shard `rank` of `nranks` consecutive shards of
 // the sorted cluster and ext_tot[nranks][4] (device) holds every shard's totals as potential_totals() writes them.
+// cols_out[c][k] = cols_in[c][perm[k]] (and the ids likewise): the record columns when they arrive after the sort
+hmc_status gather_by_perm(uint64_t n, const uint32_t* perm, int ncols, const double* const* cols_in, double* const* cols_out,
+                          const uint32_t* id_in, uint32_t* id_out, cudaStream_t st);
 hmc_status potential(uint64_t n, double G, const double* r, const double* m, double* phi, double* m_cum,
                      const double* ext_tot, uint32_t nranks, uint32_t rank, const Workspace& ws, cudaStream_t st);
 hmc_status potential_totals(uint64_t n, const double* r, const double* m, double* totals4, const Workspace& ws, cudaStream_t st);

@@ -383,6 +383,24 @@ static hmc_status sort_general(uint64_t n, const double* r_in, double* r_sorted,
     return HMC_OK;
 }
 
+__global__ void __launch_bounds__(256) sort_gather_kernel(GatherCols g, const uint32_t* __restrict__ perm, uint64_t n)
+{
+    sort_gather_phase(g, perm, n);
+}
+
+hmc_status gather_by_perm(uint64_t n, const uint32_t* perm, int ncols, const double* const* cols_in, double* const* cols_out,
+                          const uint32_t* id_in, uint32_t* id_out, cudaStream_t st)
+{
+    if (n == 0 || (ncols == 0 && !id_in)) return HMC_OK;
+    GatherCols g{};
+    g.ncols = ncols;
+    for (int c = 0; c < ncols; ++c) { g.in[c] = cols_in[c]; g.out[c] = cols_out[c]; }
+    g.id_in = id_in; g.id_out = id_out;
+    sort_gather_kernel<<<(int)umin64((n + 255) / 256, (uint64_t)sm_count() * 8), 256, 0, st>>>(g, perm, n);
+    HMC_LAUNCH_CHECK();
+    return HMC_OK;
+}
+
 hmc_status sort_by_radius(uint64_t n, const double* r_in, double* r_sorted, uint32_t* perm, int ncols,
                           const double* const* cols_in, double* const* cols_out, const uint32_t* id_in,
                           uint32_t* id_out, const Workspace& ws, cudaStream_t st)
