@@ -31,6 +31,9 @@ VARIANTS = {
     "serial": ("libhmc_oracle.so", []),
     "omp": ("libhmc_oracle_omp.so", ["-fopenmp"]),
     "tmax3": ("libhmc_oracle_tmax3.so", ["-DT_MAX=3u"]),
+    # AddressSanitizer + UndefinedBehaviorSanitizer build, selected for a whole test run with HMC_ORACLE_VARIANT=asan
+    # and libasan preloaded into the interpreter (profiles/r2.md has the command and its result)
+    "asan": ("libhmc_oracle_asan.so", ["-fsanitize=address,undefined", "-fno-omit-frame-pointer", "-g"]),
 }
 
 ST_UNBOUND, ST_RADIAL, ST_DEGENERATE, ST_CIRCULAR, ST_MAXTRIES, ST_CLIPPED = 1, 2, 4, 8, 16, 32
@@ -38,7 +41,7 @@ T_MAX = 4096
 C_F = 1.2
 
 _libs = {}
-_current = "serial"
+_current = os.environ.get("HMC_ORACLE_VARIANT", "serial")
 
 
 def build(force: bool = False, variant: str = "serial") -> str:
@@ -54,7 +57,7 @@ def build(force: bool = False, variant: str = "serial") -> str:
 
 
 def build_all(force: bool = False):
-    return [build(force, v) for v in VARIANTS]
+    return [build(force, v) for v in VARIANTS if v != "asan"]
 
 
 def lib(variant: str | None = None) -> ctypes.CDLL:

@@ -517,3 +517,29 @@ def test_orbit_stages_with_tied_radii(oracle, copies):
                                    reuse_tables=True)
     check_orbit_against(oracle, o, tp, sm, report="ties x%d" % copies)
     assert np.array_equal(host(hmc.hmc_sort_by_radius(dev(r))[1], np.uint32), o["perm"])
+
+
+def test_repeated_steps_are_bit_reproducible():
+    """The same step run ten times from the same state writes the same bits every time, every array.  The sort's
+    decoupled look-back, the sampler's dynamic batches and the shared-memory parking all order their work
+    differently from run to run; a data race would show as a difference (compute-sanitizer is closed on this pool:
+    profiles/r2.md).  Covers the fast sort path, the fallback sort (runs of 200 near-equal keys) and the fused call."""
+    n, seed = 400_003, 61
+    c = inputs.plummer(n, seed, "salpeter")
+    r = c["r"].copy()
+    r[:60_000] = _clustered_keys(60_000, 200, np.random.default_rng(2))       # long runs: the guarded general sort runs
+    d = [dev(r), dev(c["v_r"]), dev(c["v_t"]), dev(c["m"]), dev(c["id"].view(np.int32))]
+    first = None
+    for rep in range(10):
+        st = hmc.OrbitStepper(*d, seed)
+        st.step()
+        st.step(fused=(rep % 2 == 1))
+        got = dict(perm=st.sorted["perm"], phi=st.phi, m_cum=st.m_cum, r=st.state["r"], v_r=st.state["v_r"], v_t=st.state["v_t"],
+                   id=st.state["id"], n_try=st.sample["n_try"], status=st.sample["status"], counters=st.counters,
+                   **{"tp_" + k: v for k, v in st.tp.items()})
+        got = {k: v.clone() for k, v in got.items()}
+        if first is None:
+            first = got
+        else:
+            for k in first:
+                assert torch.equal(first[k], got[k]), (rep, k)
