@@ -116,8 +116,10 @@ __device__ __forceinline__ uint32_t bucket(double x, double Rl, float scale, uin
 __global__ void __launch_bounds__(256) build_nodes_kernel(const double* __restrict__ r, const double* __restrict__ phi,
                                                           const double* __restrict__ m_cum, double G,
                                                           Node* __restrict__ nodes, double2* __restrict__ coarse_g,
-                                                          double2* __restrict__ mid_g, int shift, uint64_t n)
+                                                          double2* __restrict__ mid_g, int shift, uint64_t n,
+                                                          uint32_t* __restrict__ s4_words)
 {
+    if (blockIdx.x == 0 && threadIdx.x == 0) { s4_words[0] = 0; s4_words[1] = 0; }      // S4's batch and exit counters
     const uint64_t low_mask = (1ull << shift) - 1;
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
     for (uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; j <= n + 1; j += stride) {
@@ -145,8 +147,9 @@ __global__ void __launch_bounds__(DIR_THREADS) build_tables_kernel(const double*
                                                                    const double* __restrict__ m_cum, double G,
                                                                    Node* __restrict__ nodes, double2* __restrict__ coarse_g,
                                                                    double2* __restrict__ mid_g, uint32_t* __restrict__ dir,
-                                                                   uint32_t n, int shift)
+                                                                   uint32_t n, int shift, uint32_t* __restrict__ s4_words)
 {
+    if (blockIdx.x == 0 && threadIdx.x == 0) { s4_words[0] = 0; s4_words[1] = 0; }      // S4's batch and exit counters
     extern __shared__ uint32_t cnt[];                                // [K + 1]: cnt[b + 1] = nodes in bucket b, then o_b
     __shared__ uint32_t warp_tot[DIR_THREADS / 32];
     const uint32_t K = 1u << shift, c = blockIdx.x;
@@ -197,6 +200,64 @@ __global__ void __launch_bounds__(DIR_THREADS) build_tables_kernel(const double*
     __syncthreads();
     uint32_t* row = dir + (size_t)c * K;
     for (uint32_t b = threadIdx.x; b < K; b += DIR_THREADS) row[b] = cnt[b] | (cnt[b + 1] << 16);
+}
+
+// The same for narrow intervals (K = 2^shift <= 256 nodes: N below about 2.6e6): one WARP per interval, eight
+// intervals per CTA, no block-wide barrier.  (One CTA per interval left most of its 256 threads without a node:
+// 27 us at N = 1e6, where the whole turning-point stage takes 100 us.)
+static constexpr int DIR_SMALL_MAX_K = 256;
+
+__global__ void __launch_bounds__(DIR_THREADS) build_tables_small_kernel(const double* __restrict__ r, const double* __restrict__ phi,
+                                                                         const double* __restrict__ m_cum, double G,
+                                                                         Node* __restrict__ nodes, double2* __restrict__ coarse_g,
+                                                                         uint32_t* __restrict__ dir, uint32_t n, int shift,
+                                                                         uint32_t nintervals, uint32_t* __restrict__ s4_words)
+{
+    __shared__ uint32_t cnt_all[DIR_THREADS / 32][DIR_SMALL_MAX_K + 1];
+    if (blockIdx.x == 0 && threadIdx.x == 0) { s4_words[0] = 0; s4_words[1] = 0; }      // S4's batch and exit counters
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t K = 1u << shift, c = blockIdx.x * (DIR_THREADS / 32) + warp;
+    if (c >= nintervals) return;
+    uint32_t* cnt = cnt_all[warp];
+    const uint32_t j0 = max(c << shift, 1u), jn = min(((c + 1) << shift) - 1, n);
+    const double Rl = c ? __ldg(r + ((c << shift) - 1)) : 0.0;
+    const double Rh = (((uint64_t)(c + 1) << shift) <= n) ? __ldg(r + (((c + 1) << shift) - 1)) : __ldg(r + (n - 1));
+    const float scale = bucket_scale(Rl, Rh, K);
+    for (uint32_t b = lane; b <= K; b += 32) cnt[b] = 0;
+    if (lane == 0) {
+        if (c == 0) {
+            Node e; e.r = 0.0; e.phi = __ldg(phi); e.B = 0.0; e.u = 0.0;
+            nodes[0] = e;
+            coarse_g[0] = make_double2(e.r, e.phi);
+        }
+        if (c == nintervals - 1) {
+            Node e; e.r = pos_inf(); e.phi = 0.0; e.B = G * __ldg(m_cum + (n - 1)); e.u = 0.0;
+            nodes[(size_t)n + 1] = e;
+        }
+    }
+    __syncwarp();
+    for (uint32_t j = j0 + lane; j <= jn; j += 32) {
+        Node e;
+        const double rj = __ldcs(r + (j - 1));
+        e.r = rj; e.phi = __ldcs(phi + (j - 1)); e.B = G * __ldcs(m_cum + (j - 1)); e.u = 1.0 / rj;
+        nodes[j] = e;
+        if ((j & (K - 1u)) == 0) coarse_g[j >> shift] = make_double2(e.r, e.phi);
+        atomicAdd(&cnt[bucket(rj, Rl, scale, K) + 1], 1u);
+    }
+    __syncwarp();
+    // inclusive scan of cnt[0 .. K] in place: cnt[b] becomes o_b = number of nodes with bucket < b
+    const uint32_t per = (K + 1 + 31) / 32;
+    const uint32_t b0 = min(K + 1, lane * per), b1 = min(K + 1, b0 + per);
+    uint32_t sum = 0;
+    for (uint32_t b = b0; b < b1; ++b) sum += cnt[b];
+    uint32_t inc = sum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
+    uint32_t run = inc - sum;
+    for (uint32_t b = b0; b < b1; ++b) { run += cnt[b]; cnt[b] = run; }
+    __syncwarp();
+    uint32_t* row = dir + (size_t)c * K;
+    for (uint32_t b = lane; b < K; b += 32) row[b] = cnt[b] | (cnt[b + 1] << 16);
 }
 
 // coarse[c] = (r, Phi) of node c << shift, c = 1..ncoarse; coarse[0] = (0, Phi_1) and
@@ -655,7 +716,8 @@ struct SampleIO {
     const uint32_t *kmin, *kmax, *id;
     const uint8_t* status_in;
     const double* F_ws;      // S3's bound F per star (workspace), or nullptr: compute it here
-    uint32_t* batch_counter; // workspace word, zero at launch: next unclaimed star
+    uint32_t* batch_counter; // two workspace words, zero at launch (the table build zeroes them, this kernel's last CTA
+                             // zeroes them again on its way out): [0] next unclaimed star, [1] CTAs that are done
     // fused S3 + S4 only: S3's table input and where its outputs go
     const double* phi;
     double *E_w, *J_w, *rmin_w, *rmax_w;
@@ -911,6 +973,12 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
         for (int off = 16; off > 0; off >>= 1) my_trials += __shfl_down_sync(0xffffffffu, my_trials, off);
         if ((threadIdx.x & 31) == 0 && my_trials) atomicAdd(io.counters + HMC_CNT_TRIALS, my_trials);
     }
+    // leave the two counter words as they were found, for a next S4 launch on the same tables (ranges of one table)
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(io.batch_counter + 1, 1u) == gridDim.x - 1) { io.batch_counter[0] = 0; io.batch_counter[1] = 0; __threadfence(); }
+    }
 }
 
 // ---- energy correction for the time-varying potential (R18) ------------------
@@ -966,7 +1034,14 @@ static hmc_status build_tables(uint64_t n, double G, const double* r, const doub
 {
     if (shift == 0) {                                            // the coarse table is the whole table: no directory
         const int blocks = (int)umin64((n + 2 + 255) / 256, (uint64_t)sm_count() * 8);
-        build_nodes_kernel<<<blocks, 256, 0, st>>>(r, phi, m_cum, G, ws.nodes, ws.coarse, ws.mid, shift, n);
+        build_nodes_kernel<<<blocks, 256, 0, st>>>(r, phi, m_cum, G, ws.nodes, ws.coarse, ws.mid, shift, n, ws.tickets + 16);
+        HMC_LAUNCH_CHECK();
+        return HMC_OK;
+    }
+    if ((1 << shift) <= DIR_SMALL_MAX_K) {                        // shift <= MID_SHIFT here: no mid table
+        const uint32_t nintervals = (uint32_t)((n >> shift) + 1);
+        build_tables_small_kernel<<<(nintervals + DIR_THREADS / 32 - 1) / (DIR_THREADS / 32), DIR_THREADS, 0, st>>>(
+            r, phi, m_cum, G, ws.nodes, ws.coarse, ws.dir, (uint32_t)n, shift, nintervals, ws.tickets + 16);
         HMC_LAUNCH_CHECK();
         return HMC_OK;
     }
@@ -975,7 +1050,7 @@ static hmc_status build_tables(uint64_t n, double G, const double* r, const doub
     hmc_status so = smem_opt_in(opted, build_tables_kernel, ((size_t)(1u << coarse_shift(HMC_MAX_N)) + 1) * sizeof(uint32_t));
     if (so != HMC_OK) return so;
     build_tables_kernel<<<(unsigned)((n >> shift) + 1), DIR_THREADS, smem, st>>>(r, phi, m_cum, G, ws.nodes, ws.coarse, ws.mid,
-                                                                                 ws.dir, (uint32_t)n, shift);
+                                                                                 ws.dir, (uint32_t)n, shift, ws.tickets + 16);
     HMC_LAUNCH_CHECK();
     return HMC_OK;
 }
@@ -1015,7 +1090,6 @@ static hmc_status launch_sampler(bool fused, uint64_t n, double G, uint64_t seed
     if (so != HMC_OK) return so;
     if (io_in.count == 0) return HMC_OK;
     const int blocks = (int)umin64(((uint64_t)io_in.count + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
-    HMC_CUDA_TRY(cudaMemsetAsync(ws.tickets + 16, 0, 4, st));
     SampleIO io = io_in;
     io.batch_counter = ws.tickets + 16;
     if (fused)
