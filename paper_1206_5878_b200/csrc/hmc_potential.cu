@@ -27,14 +27,8 @@ static constexpr int SCAN_WARPS = SCAN_THREADS / 32;
 static constexpr int SCAN_ITEMS = SCAN_TILE / SCAN_THREADS;   // 8 consecutive stars per thread in the apply launch
 static constexpr int SLICE = 1024;                            // stars per warp-slice of the reduce launch
 static constexpr int SLICES_PER_TILE = SCAN_TILE / SLICE;     // 2
-#ifndef HMC_S2_CTAS
-#define HMC_S2_CTAS 3
-#endif
-#ifndef HMC_S2_BATCH
-#define HMC_S2_BATCH 4
-#endif
-static constexpr int CHUNK_CTAS_PER_SM = HMC_S2_CTAS;         // chunks = CTAs resident at once: registers allow 3 x 256 threads
-static constexpr int RED_BATCH = HMC_S2_BATCH;                // 16-byte loads in flight per array and lane in the reduce launch
+static constexpr int CHUNK_CTAS_PER_SM = 3;                   // chunks = CTAs resident at once: 80 registers x 256 threads (2 and 4 measured slower)
+static constexpr int RED_BATCH = 4;                           // 16-byte loads in flight per array and lane in the reduce launch (2, 8, 16: no better)
 static_assert(SCAN_ITEMS == 8, "the apply launch loads 2 x 4 consecutive doubles per thread and array");
 
 // double-double sum of two double-double values of the same sign (see the header): 11 operations instead of 20

@@ -30,10 +30,7 @@ static constexpr int PK_MAXPASS = 5;
 static constexpr int PK_KEYBITS_MAX = 40;
 static constexpr int PK_THREADS = 512;
 static constexpr int PK_WARPS = PK_THREADS / 32;
-#ifndef HMC_PK_ITEMS
-#define HMC_PK_ITEMS 8
-#endif
-static constexpr int PK_ITEMS = HMC_PK_ITEMS;
+static constexpr int PK_ITEMS = 8;                             // words per thread and tile (6: 3 % slower, 12 / 16: 1.5 % / 0.3 % faster)
 static constexpr int PK_TILE = PK_THREADS * PK_ITEMS;          // 4096
 static constexpr int RUN_MAX = 64;
 static constexpr int LB = 4;                                  // look-back words loaded per round trip

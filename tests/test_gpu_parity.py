@@ -64,7 +64,8 @@ def test_sort_matches_oracle(oracle, n):
     assert np.array_equal(host(ids_s, np.uint32), o_ids)
 
 
-@pytest.mark.parametrize("kind", ["ties", "all_equal", "sorted", "reversed", "extreme", "two_values", "denormal", "narrow"])
+@pytest.mark.parametrize("kind", ["ties", "all_equal", "sorted", "reversed", "extreme", "two_values", "denormal", "narrow",
+                                  "narrow_span", "wide_runs"])
 def test_sort_adversarial_keys(oracle, kind):
     g = np.random.default_rng(5)
     n = 50_001
@@ -77,6 +78,8 @@ def test_sort_adversarial_keys(oracle, kind):
         two_values=np.where(g.random(n) < 0.5, 1.0, 2.0),
         denormal=np.where(g.random(n) < 0.5, g.integers(1, 1 << 40, n).astype(np.uint64).view(np.float64), 10.0 ** g.uniform(-310, -300, n)),
         narrow=1.0 + g.integers(0, 1000, n) * 2.0 ** -52,        # a thousand adjacent doubles: long runs of exact ties
+        narrow_span=1.0 + g.integers(0, 1 << 30, n) * 2.0 ** -52,  # keys spanning 30 bits: shifted up to fill the kept key bits
+        wide_runs=np.repeat(10.0 ** g.uniform(-200, 200, n // 40 + 1), 40)[:n] * (1.0 + g.integers(0, 8, n) * 2.0 ** -52),
     )[kind]
     rs, perm, _, _ = hmc.hmc_sort_by_radius(dev(r))
     o_rs, o_perm, _, _ = oracle.sort_by_radius(r)
@@ -96,9 +99,11 @@ def _clustered_keys(n, cluster, g):
     return r
 
 
-@pytest.mark.parametrize("cluster", [2, 7, 32, 33, 200])
+@pytest.mark.parametrize("cluster", [2, 7, 32, 33, 63, 64, 65, 66, 200])
 def test_sort_runs_of_near_equal_keys(oracle, cluster):
-    """cluster <= 32: runs resolved inside the fast path; > 32: the guarded general sort redoes the call."""
+    """Runs of up to 64 stars that agree in the bits the passes sorted are ranked inside the fast path (from the
+    packed words, or from the full keys where even the kept bits agree); longer ones make the guarded general sort
+    redo the call."""
     g = np.random.default_rng(11 + cluster)
     n = 300_017
     r = _clustered_keys(n, cluster, g)
