@@ -29,9 +29,12 @@ NVCC_FLAGS = [
 # "product" is the library; "tmax3" is a TEST-ONLY build of the same sources with the cap on rejection trials
 # lowered to 3, so that the GPU tests reach S4's exhaustion path (draw_exhaustive, MAXTRIES) and compare it
 # with the oracle built the same way (oracle/: -DT_MAX=3u).  Nothing but tests loads it.
+# "pairs" is a TEST-ONLY build in which S3's exact search runs by lane pairs at every N (the product takes that
+# path from N = 2^25 on, where the node table is far beyond the TLB's reach), so that small parity cases reach it.
 VARIANTS = {
     "product": ("libhmc.so", []),
     "tmax3": ("libhmc_tmax3.so", ["-DHMC_T_MAX=3u"]),
+    "pairs": ("libhmc_pairs.so", ["-DHMC_S3_PAIRS_MIN_N=1"]),
 }
 
 

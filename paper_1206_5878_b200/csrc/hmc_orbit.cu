@@ -471,6 +471,67 @@ __device__ __forceinline__ Located locate_star(const Tables& T, uint32_t a, doub
     return L;
 }
 
+// Tier 3 by lane pairs (warp-collective: all 32 lanes call it together; a lane without a search passes closed
+// sides).  What a random access to a table of gigabytes costs is the REQUEST -- one per load instruction and
+// 128-byte line, about 37 per ns on the whole chip once the table is far beyond the reach of the TLB -- not the
+// bytes (profiles/r2_tlb.md).  A lane that loads nodes p and p+1 itself issues two instructions, hence two requests,
+// and a third to fetch the bracketing node again for the roots.  Here lanes 2i and 2i+1 serve their two stars one
+// after the other: for the star whose turn it is, the even lane loads node p and the odd lane node p+1 in the SAME
+// instruction (one request when both lie in one line, 3 times in 4), each evaluates the sign of Q at its node for
+// that star, the answers come back in a ballot, and when a side closes the lane that holds the bracketing node
+// hands it over through shuffles.  Same probes, same brackets as the one-lane search.
+__device__ __forceinline__ Node shfl_node(const Node& e, int src)
+{
+    Node t;
+    t.r = __shfl_sync(0xffffffffu, e.r, src); t.phi = __shfl_sync(0xffffffffu, e.phi, src);
+    t.B = __shfl_sync(0xffffffffu, e.B, src); t.u = __shfl_sync(0xffffffffu, e.u, src);
+    return t;
+}
+
+// `mine`: the warp's hand-over area in shared memory, one Node per lane and side ([side][lane]).
+__device__ __forceinline__ void probe_pairs(const Node* __restrict__ nodes, Side& s1, Side& s2, double E, double J2,
+                                            Node* __restrict__ mine, bool& have1, bool& have2, uint32_t lane)
+{
+    have1 = have2 = false;
+    const uint32_t odd = lane & 1u, even_lane = lane & ~1u;
+    while (true) {
+        const bool a1 = s1.active(), a2 = s2.active();
+        if (!__any_sync(0xffffffffu, a1 || a2)) break;
+        const uint32_t p1 = a1 ? s1.probe() : 0u, p2 = a2 ? s2.probe() : 0u;
+        const uint32_t act = (a1 ? 1u : 0u) | (a2 ? 2u : 0u);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {                          // h: whose star the pair serves
+            const int owner = (int)(even_lane | (uint32_t)h);
+            const bool own = odd == (uint32_t)h;
+            const uint32_t P1 = __shfl_sync(0xffffffffu, p1, owner), P2 = __shfl_sync(0xffffffffu, p2, owner);
+            const uint32_t A = __shfl_sync(0xffffffffu, act, owner);
+            const double Eo = __shfl_sync(0xffffffffu, E, owner), J2o = __shfl_sync(0xffffffffu, J2, owner);
+            Node n1{ 0.0, 0.0, 0.0, 0.0 }, n2{ 0.0, 0.0, 0.0, 0.0 };
+            bool neg1 = false, neg2 = false;
+            if (A & 1u) { n1 = ld_node(nodes + P1 + odd); neg1 = q_negative(n1.r, n1.phi, Eo, J2o); }
+            if (A & 2u) { n2 = ld_node(nodes + P2 + odd); neg2 = q_negative(n2.r, n2.phi, Eo, J2o); }
+            const unsigned b1 = __ballot_sync(0xffffffffu, neg1), b2 = __ballot_sync(0xffffffffu, neg2);
+            // the owner moves its brackets; a side that closes on a node of this probe names the lane holding it
+            uint32_t want = 0;                                  // bits 0-1 side 1, bits 2-3 side 2: 1 = even lane, 2 = odd lane
+            if (own) {
+                if (a1) {
+                    s1.update(p1, ((b1 >> even_lane) & 1u) != 0u, ((b1 >> (even_lane + 1u)) & 1u) != 0u);
+                    if (!s1.active()) want |= (s1.lo == p1) ? 1u : ((s1.lo == p1 + 1u) ? 2u : 0u);
+                }
+                if (a2) {
+                    s2.update(p2, ((b2 >> even_lane) & 1u) == 0u, ((b2 >> (even_lane + 1u)) & 1u) == 0u);
+                    if (!s2.active()) want |= (s2.lo == p2) ? 4u : ((s2.lo == p2 + 1u) ? 8u : 0u);
+                }
+                have1 = have1 || (want & 3u); have2 = have2 || (want & 12u);
+            }
+            const uint32_t W = __shfl_sync(0xffffffffu, want, owner);
+            if (W & (1u << odd)) mine[owner] = n1;             // this lane holds the node side 1 closed on
+            if (W & (4u << odd)) mine[32 + owner] = n2;
+        }
+    }
+    __syncwarp();
+}
+
 __device__ __forceinline__ Solved finish_star_s3(const Tables& T, uint32_t a, const Located& L)
 {
     const Node* __restrict__ nodes = T.nodes;
@@ -524,6 +585,53 @@ __device__ __forceinline__ Solved finish_star_s3(const Tables& T, uint32_t a, co
     return Solved{ E, J, rmin, rmax, Fv, kmin, kmax, st };
 }
 
+// The same with tier 3 by lane pairs: the whole warp must call this together, `valid` false for a lane without a star.
+__device__ __forceinline__ Solved finish_star_s3_pairs(const Tables& T, uint32_t a, const Located& L, bool valid, uint32_t lane,
+                                                       Node* __restrict__ handover)
+{
+    const Node* __restrict__ nodes = T.nodes;
+    const uint32_t k = a + 1;
+    const double E = L.E, J = L.J, rk = L.rk, J2 = J * J;
+    double rmin = rk, rmax = rk, Fv = 0.0;
+    uint32_t kmin = k - 1, kmax = k;
+    unsigned st = L.st & 255u;
+    const bool search = valid && !st;
+    Side s1{ L.lo1, L.hi1, 1u, L.g1, (L.st & 256u) ? MODE_GUESS : MODE_BISECT }, s2{ L.lo2, L.hi2, 1u, L.g2, (L.st & 512u) ? MODE_GUESS : MODE_BISECT };
+    if (!search) { s1.lo = 0u; s1.hi = 1u; s2.lo = 0u; s2.hi = 1u; }           // closed
+    bool have_a = false, have_b = false;
+    probe_pairs(nodes, s1, s2, E, J2, handover, have_a, have_b, lane);
+    if (st) {
+        rmin = (st & HMC_STAR_RADIAL) ? 0.0 : rk;
+        rmax = (st & HMC_STAR_UNBOUND) ? pos_inf() : rk;
+    } else if (valid) {
+        kmin = s1.lo; kmax = s2.lo;
+        // closed-form roots of Q(u) = 2C + 2Bu - J^2 u^2 in the bracketing shells (R3)
+        const Node ea = have_a ? handover[lane] : ld_node(nodes + kmin), eb = have_b ? handover[32 + lane] : ld_node(nodes + kmax);
+        const double Ca = (E - ea.phi) - ea.B * ea.u;
+        const double Cb = (E - eb.phi) - eb.B * eb.u;
+        double D = ea.B * ea.B + 2.0 * (J2 * Ca);
+        if (D < 0.0) D = 0.0;
+        rmin = J2 / (ea.B + sqrt(D));
+        D = eb.B * eb.B + 2.0 * (J2 * Cb);
+        if (D < 0.0) D = 0.0;
+        if (Cb < 0.0) rmax = (eb.B + sqrt(D)) / (-2.0 * Cb);
+        else { rmax = pos_inf(); st |= HMC_STAR_DEGENERATE; }
+        // S4's bound F (R7) needs G M at both bracketing shells, which are in registers here and
+        // would cost S4 two random node reads per star: computed here and left in the workspace for a
+        // following S4 call with reuse_tables (0 = no draw).  S4 writes F = 1.2 max(sqrt(3 D / q1), sqrt(3 D / -q2));
+        // division and square root are correctly rounded, hence monotone, so the larger square root is the
+        // square root of the larger quotient, which is the quotient by the smaller divisor: the same bits
+        // from one division and one square root instead of two each.
+        const double delta = rmax - rmin;
+        if (!(st & HMC_STAR_DEGENERATE) && delta > 0.0) {
+            const double q1 = (2.0 * (J2 / rmin - ea.B)) / (rmin * rmin);      // Q'(r_min) in shell k_min
+            const double q2 = (2.0 * (J2 / rmax - eb.B)) / (rmax * rmax);      // Q'(r_max) in shell k_max
+            if ((q1 > 0.0) && (q2 < 0.0)) Fv = 1.2 * sqrt((3.0 * delta) / fmin(q1, -q2));
+        }
+    }
+    return Solved{ E, J, rmin, rmax, Fv, kmin, kmax, st };
+}
+
 __device__ __forceinline__ Solved solve_star(const Tables& T, uint32_t a, double rk, double vr, double vt, double phik)
 {
     return finish_star_s3(T, a, locate_star(T, a, rk, vr, vt, phik));
@@ -531,6 +639,7 @@ __device__ __forceinline__ Solved solve_star(const Tables& T, uint32_t a, double
 
 // Stars first .. first+count-1 of the table (0-based positions; star at position p is node p + 1).  r and phi
 // are the table's arrays [n]; v_r, v_t and every output are the range's own arrays [count].
+template <bool PAIRS>
 __global__ void __launch_bounds__(ORB_THREADS, 1)
 turning_points_kernel(uint32_t n, uint32_t first, uint32_t count, double G, const double* __restrict__ r, const double* __restrict__ v_r,
                       const double* __restrict__ v_t, const double* __restrict__ phi,
@@ -545,8 +654,16 @@ turning_points_kernel(uint32_t n, uint32_t first, uint32_t count, double G, cons
     stage_coarse(coarse, coarse_g, n, shift);
     Tables T{ nodes, dir, coarse, shift > MID_SHIFT ? mid_g : nullptr, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift, l2_keep_policy() };
     const uint32_t stride = gridDim.x * ORB_THREADS;
-    for (uint32_t a = blockIdx.x * ORB_THREADS + threadIdx.x; a < count; a += stride) {
-        const Solved v = solve_star(T, first + a, __ldcs(r + first + a), __ldcs(v_r + a), __ldcs(v_t + a), __ldcs(phi + first + a));
+    const uint32_t lane = threadIdx.x & 31u;
+    // pair search: the warp's hand-over area, behind the coarse table
+    Node* handover = reinterpret_cast<Node*>(smem_raw + (((size_t)(n >> shift) + 2) * sizeof(double2) + 31) / 32 * 32) + (threadIdx.x >> 5) * 64;
+    // whole warps stay in the loop together (the pair search is warp-collective); a lane beyond the end has no star
+    for (uint32_t a = blockIdx.x * ORB_THREADS + threadIdx.x; PAIRS ? (a - lane < count) : (a < count); a += stride) {
+        const bool valid = !PAIRS || a < count;
+        const uint32_t b = valid ? a : count - 1;
+        const Located L = locate_star(T, first + b, __ldcs(r + first + b), __ldcs(v_r + b), __ldcs(v_t + b), __ldcs(phi + first + b));
+        const Solved v = PAIRS ? finish_star_s3_pairs(T, first + b, L, valid, lane, handover) : finish_star_s3(T, first + b, L);
+        if (!valid) continue;
         __stcs(F_ws + first + a, v.Fv);                            // by table position: a later S4 call may cover a sub-range
         __stcs(E_out + a, v.E); __stcs(J_out + a, v.J); __stcs(rmin_out + a, v.rmin); __stcs(rmax_out + a, v.rmax);
         __stcs(kmin_out + a, v.kmin); __stcs(kmax_out + a, v.kmax); status_out[a] = (uint8_t)v.st;
@@ -1026,6 +1143,14 @@ energy_correction_kernel(uint32_t n, const Node* __restrict__ nodes, const doubl
 }
 
 // ---- host side --------------------------------------------------------------------------------
+// S3's exact search by lane pairs pays when the node table is far beyond the TLB's reach (see probe_pairs).
+// Turning-point stage, one lane / lane pairs, ms: N = 1e7 0.90 / 1.40, 3e7 4.4 / 4.4, 5e7 8.8 / 7.2, 1e8 20.6 / 15.8.
+// (A test-only build sets the threshold to 1 so that small cases run the pair search: build.py "pairs".)
+#ifndef HMC_S3_PAIRS_MIN_N
+#define HMC_S3_PAIRS_MIN_N (1ull << 25)
+#endif
+static inline bool s3_pairs(uint64_t n) { return n >= HMC_S3_PAIRS_MIN_N; }
+
 static hmc_status build_tables(uint64_t n, double G, const double* r, const double* phi, const double* m_cum,
                                const Workspace& ws, int shift, cudaStream_t st)
 {
@@ -1059,17 +1184,25 @@ hmc_status turning_points(uint64_t n, uint64_t first, uint64_t count, double G, 
 {
     const int sms = sm_count();
     const int shift = coarse_shift(n);
-    const size_t smem = ((n >> shift) + 2) * sizeof(double2);
-    static std::atomic<uint64_t> opted{ 0 };
-    hmc_status so = smem_opt_in(opted, turning_points_kernel, COARSE_CAP * sizeof(double2));
+    const bool pairs = s3_pairs(n);
+    static constexpr size_t HANDOVER_BYTES = (size_t)ORB_WARPS * 64 * sizeof(Node) + 32;
+    const size_t smem = ((n >> shift) + 2) * sizeof(double2) + (pairs ? HANDOVER_BYTES : 0);
+    static std::atomic<uint64_t> opted[2];
+    hmc_status so = pairs ? smem_opt_in(opted[1], turning_points_kernel<true>, COARSE_CAP * sizeof(double2) + HANDOVER_BYTES)
+                          : smem_opt_in(opted[0], turning_points_kernel<false>, COARSE_CAP * sizeof(double2));
     if (so != HMC_OK) return so;
     hmc_status s = build_tables(n, G, r, phi, m_cum, ws, shift, st);
     if (s != HMC_OK) return s;
     if (count == 0) return HMC_OK;
     const int blocks = (int)umin64((count + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
-    turning_points_kernel<<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, (uint32_t)first, (uint32_t)count, G, r, v_r, v_t, phi, ws.nodes, ws.coarse, ws.mid, ws.dir, shift,
-                                                            E, J, r_min, r_max, k_min, k_max, status, ws.orbitF,
-                                                            reinterpret_cast<unsigned long long*>(counters));
+    if (pairs)
+        turning_points_kernel<true><<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, (uint32_t)first, (uint32_t)count, G, r, v_r, v_t, phi, ws.nodes, ws.coarse, ws.mid, ws.dir, shift,
+                                                                      E, J, r_min, r_max, k_min, k_max, status, ws.orbitF,
+                                                                      reinterpret_cast<unsigned long long*>(counters));
+    else
+        turning_points_kernel<false><<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, (uint32_t)first, (uint32_t)count, G, r, v_r, v_t, phi, ws.nodes, ws.coarse, ws.mid, ws.dir, shift,
+                                                                       E, J, r_min, r_max, k_min, k_max, status, ws.orbitF,
+                                                                       reinterpret_cast<unsigned long long*>(counters));
     HMC_LAUNCH_CHECK();
     return HMC_OK;
 }

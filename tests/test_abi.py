@@ -62,6 +62,11 @@ def test_build_variants_and_launch_counter(libhmc):
     assert t3.hmc_t_max() == 3
     for f in declared_functions():
         assert hasattr(t3, f), f
+    pairs = ctypes.CDLL(build.build(variant="pairs"))       # test-only: S3's pair search at every N
+    pairs.hmc_t_max.restype = ctypes.c_uint32
+    assert pairs.hmc_t_max() == 4096
+    for f in declared_functions():
+        assert hasattr(pairs, f), f
 
 
 def test_argument_errors_do_not_need_a_gpu(libhmc):

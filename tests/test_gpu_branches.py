@@ -7,6 +7,8 @@
 * exactly circular orbits (CIRCULAR, or a bracket of a few ulps), stars whose outer quadratic has C >= 0
   (DEGENERATE), unbound and radial stars: flags and outputs bit for bit.
 * the fused entry point hmc_orbit_step against the ORACLE (not against the two GPU calls).
+* S3's exact search by lane pairs (the product's path from N = 2^25 on): the TEST-ONLY build libhmc_pairs.so
+  (-DHMC_S3_PAIRS_MIN_N=1) takes it at every N.
 """
 import numpy as np
 import pytest
@@ -195,3 +197,51 @@ def test_fused_orbit_step_against_the_oracle(oracle, n, masses):
     tp, sm = hmc.hmc_orbit_step(dev(rs), dev(vrs), dev(vts), dev(phi), dev(mc), dev(ids), seed, step, counters=counters)
     assert_bitwise(tp, sm, otp, osm)
     assert host(counters)[hmc.COUNTER_NAMES.index("trials")] == osm["trials"]
+
+
+@pytest.fixture
+def pairs_build(monkeypatch):
+    """S3's exact search by lane pairs at every N; every hmc.* call inside the test goes to that library."""
+    monkeypatch.setattr(hmc, "_lib", hmc.load(hmc_build.build(variant="pairs")))
+
+
+@pytest.mark.parametrize("n,masses", [(1, "equal"), (2, "equal"), (31, "equal"), (33, "equal"), (1025, "equal"),
+                                      (10_239, "equal"), (100_000, "equal"), (300_001, "salpeter"), (1_200_000, "equal")])
+def test_pair_search_matches_oracle(pairs_build, oracle, n, masses):
+    """Lanes 2i and 2i+1 probe nodes p and p+1 of one star in one load instruction and hand the bracketing node
+    over through shared memory: same brackets, roots and flags as the oracle, ragged last warp included; S4
+    on S3's output as usual."""
+    seed, step = 58, 2
+    rs, vrs, vts, ms, ids, phi, mc = sorted_tables(oracle, n, seed, masses)
+    with oracle.use("omp"):
+        otp = oracle.orbit_turning_points(rs, vrs, vts, phi, mc)
+        osm = oracle.sample_new_radius(rs, phi, mc, rs, vrs, vts, otp["E"], otp["J"], otp["r_min"], otp["r_max"],
+                                       otp["k_min"], otp["k_max"], ids, otp["status"], seed, step)
+    tp, sm = gpu_s3_s4(rs, vrs, vts, phi, mc, ids, seed, step)
+    assert_bitwise(tp, sm, otp, osm)
+
+
+def test_pair_search_flagged_stars_and_ranges(pairs_build, oracle):
+    """Unbound and radial stars take no search (their lanes pass closed brackets to the pair search); a range
+    call whose count is not a multiple of 32 leaves lanes without a star in the last warp."""
+    n, seed = 50_003, 61
+    rs, vrs, vts, ms, ids, phi, mc = sorted_tables(oracle, n, seed)
+    vrs, vts = vrs.copy(), vts.copy()
+    vrs[5::40] = 9.0                                         # unbound
+    vts[6::40] = 0.0                                         # radial
+    otp = oracle.orbit_turning_points(rs, vrs, vts, phi, mc)
+    d = [dev(x) for x in (rs, vrs, vts, phi, mc)]
+    ws = hmc.alloc_workspace(n)
+    tp = hmc.hmc_orbit_turning_points(d[0], d[1], d[2], d[3], d[4], 1.0, workspace=ws)
+    for k in ("E", "J", "r_min", "r_max", "status"):
+        assert np.array_equal(host(tp[k]), otp[k]), k
+    for k in ("k_min", "k_max"):
+        assert np.array_equal(host(tp[k], np.uint32), otp[k]), k
+    assert int((otp["status"] != 0).sum()) >= 2 * (n // 40)
+    first, count = 12_345, 7_777
+    tpr = hmc.hmc_orbit_turning_points(d[0], d[1][first:first + count].contiguous(), d[2][first:first + count].contiguous(),
+                                       d[3], d[4], 1.0, workspace=ws, first=first)
+    for k in ("E", "J", "r_min", "r_max", "status"):
+        assert np.array_equal(host(tpr[k]), otp[k][first:first + count]), k
+    for k in ("k_min", "k_max"):
+        assert np.array_equal(host(tpr[k], np.uint32), otp[k][first:first + count]), k

@@ -172,6 +172,15 @@ def test_second_search_table_just_above_the_coarse_capacity(oracle):
     run_self_chained(oracle, 2, n_override=12_000_000, steps=1)
 
 
+def test_second_search_table_with_the_pair_search(oracle, monkeypatch):
+    """The same case in the test-only build whose S3 searches by lane pairs at every N: the second table and the
+    pair search together, on every star (the product build combines them from N = 2^25 on, where the oracle
+    follows on every 16th star only)."""
+    from paper_1206_5878_b200 import build as hmc_build
+    monkeypatch.setattr(hmc, "_lib", hmc.load(hmc_build.build(variant="pairs")))
+    run_self_chained(oracle, 2, n_override=12_000_000, steps=1)
+
+
 STRIDE_1E8 = 16
 
 
