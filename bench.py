@@ -35,6 +35,7 @@ if ROOT not in sys.path:
 METRIC = "stars/sec per orbit step (sort+potential+turning points+sampling), fp64, N=1e7"
 UNIT = "stars/s"
 STAGES = ("sort", "potential", "turning_points", "sampling")
+GRAPH_AUTO_MAX_N = 2_000_000      # below this a step is bound by launching its kernels (0.147 -> 0.122 ms at N = 1e5)
 
 
 # --------------------------------------------------------------------------- roofline model
@@ -365,13 +366,34 @@ def run_gpu(args, cfg):
     sampler.start()
     evs = [mk() for _ in range(args.steps)]
     t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    launches_before = int(hmc.lib().hmc_launch_count())
-    t_start.record(stream)
-    for i in range(args.steps):
-        staged_step(evs[i])
-    t_end.record(stream)
-    gpu_launches = int(hmc.lib().hmc_launch_count()) - launches_before      # counted by the library at each launch
-    torch.cuda.synchronize()
+    use_graph = args.graph == "on" or (args.graph == "auto" and n <= GRAPH_AUTO_MAX_N and args.steps % 2 == 0 and not args.fused)
+    if use_graph:
+        # small N: a step is bound by launching its kernels one by one.  The timed steps are replays of a CUDA graph of
+        # two steps (OrbitStepper.run_graph); the per-stage times below come from eager steps taken after the timed region.
+        while stepper.step_index < 2:                                         # first launches are not captured
+            staged_step(mk())
+        before = int(hmc.lib().hmc_launch_count())
+        stepper.run_graph(2)                                                  # captures two steps, replays them once
+        per_two_steps = int(hmc.lib().hmc_launch_count()) - before            # the library counts a launch when it is captured
+        torch.cuda.synchronize()
+        dist_barrier()
+        t_start.record(stream)
+        stepper.run_graph(args.steps)
+        t_end.record(stream)
+        gpu_launches = per_two_steps * (args.steps // 2)                      # kernel nodes replayed in the timed region
+        cfg = dict(cfg, launch="timed steps replayed from a CUDA graph of two steps (OrbitStepper.run_graph)")
+        torch.cuda.synchronize()
+        for i in range(args.steps):
+            staged_step(evs[i])
+        torch.cuda.synchronize()
+    else:
+        launches_before = int(hmc.lib().hmc_launch_count())
+        t_start.record(stream)
+        for i in range(args.steps):
+            staged_step(evs[i])
+        t_end.record(stream)
+        gpu_launches = int(hmc.lib().hmc_launch_count()) - launches_before      # counted by the library at each launch
+        torch.cuda.synchronize()
     dist_barrier()
     clocks = sampler.stop()
     ms_total = t_start.elapsed_time(t_end)
@@ -478,6 +500,8 @@ def main(argv=None):
                     help="--impl reference: which build of the oracle (omp = all host cores, serial = one core)")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--fused", action="store_true", help="S3 and S4 as the single call hmc_orbit_step")
+    ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
+                    help="timed steps as replays of a CUDA graph of two steps (auto: N <= %d and an even --steps)" % GRAPH_AUTO_MAX_N)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args(argv)

@@ -187,6 +187,26 @@ HMC_API hmc_status hmc_sample_new_radius(uint64_t n, double G, uint64_t seed, ui
         void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*
+ * hmc_sample_new_radius with the step number completed on the DEVICE: the Philox counter's step word (R9)
+ * is step + step_dev[0], step_dev[0] read when the kernel runs.  This is what lets a CUDA graph captured from the
+ * four calls of one orbit step be replayed: every other argument of a step is the same from one step to the next
+ * (or alternates between two buffers), only the step number advances -- hmc_add_u32 enqueues word[0] += increment
+ * on the stream, so a captured step can end by advancing its own counter.  Everything else as hmc_sample_new_radius
+ * (PAPER.md:126-137); step_dev NULL: HMC_ERR_NULL.
+ */
+HMC_API hmc_status hmc_sample_new_radius_dstep(uint64_t n, double G, uint64_t seed, uint32_t step, const uint32_t* step_dev,
+        const double* r_sorted, const double* phi, const double* m_cum,
+        const double* v_r, const double* v_t,
+        const double* E, const double* J, const double* r_min, const double* r_max,
+        const uint32_t* k_min, const uint32_t* k_max, const uint32_t* id,
+        const uint8_t* star_status_in,
+        double* r_new, double* v_r_new, double* v_t_new, uint16_t* n_try,
+        uint8_t* star_status_out, uint64_t* counters, int32_t reuse_tables,
+        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+HMC_API hmc_status hmc_add_u32(uint32_t* word, uint32_t increment, void* cuda_stream);
+
+/*
  * S3 + S4 in one launch (the two calls above fused).  Computes exactly what
  * hmc_orbit_turning_points followed by hmc_sample_new_radius compute, bit for bit, and writes every
  * output of both (E .. star_status are S3's, r_new .. star_status_out S4's): each warp solves 32 stars,

@@ -389,6 +389,40 @@ hmc_status hmc_sample_new_radius_range(uint64_t n, uint64_t first, uint64_t coun
                              carve(workspace, n), static_cast<cudaStream_t>(cuda_stream));
 }
 
+hmc_status hmc_sample_new_radius_dstep(uint64_t n, double G, uint64_t seed, uint32_t step, const uint32_t* step_dev,
+                                       const double* r_sorted, const double* phi, const double* m_cum, const double* v_r,
+                                       const double* v_t, const double* E, const double* J, const double* r_min,
+                                       const double* r_max, const uint32_t* k_min, const uint32_t* k_max,
+                                       const uint32_t* id, const uint8_t* star_status_in, double* r_new, double* v_r_new,
+                                       double* v_t_new, uint16_t* n_try, uint8_t* star_status_out, uint64_t* counters,
+                                       int32_t reuse_tables, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (n > HMC_MAX_N) return HMC_ERR_SIZE;
+    if (n == 0) return HMC_OK;
+    REQUIRE_PTR(step_dev); REQUIRE_ALIGN(step_dev, 4);
+    REQUIRE_PTR(r_sorted); REQUIRE_PTR(phi); REQUIRE_PTR(m_cum); REQUIRE_PTR(v_r); REQUIRE_PTR(v_t);
+    REQUIRE_PTR(E); REQUIRE_PTR(J); REQUIRE_PTR(r_min); REQUIRE_PTR(r_max); REQUIRE_PTR(k_min); REQUIRE_PTR(k_max);
+    REQUIRE_PTR(id); REQUIRE_PTR(star_status_in); REQUIRE_PTR(r_new); REQUIRE_PTR(v_r_new); REQUIRE_PTR(v_t_new);
+    REQUIRE_PTR(star_status_out);
+    REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(phi, 8); REQUIRE_ALIGN(m_cum, 8); REQUIRE_ALIGN(v_r, 8);
+    REQUIRE_ALIGN(v_t, 8); REQUIRE_ALIGN(E, 8); REQUIRE_ALIGN(J, 8); REQUIRE_ALIGN(r_min, 8); REQUIRE_ALIGN(r_max, 8);
+    REQUIRE_ALIGN(k_min, 4); REQUIRE_ALIGN(k_max, 4); REQUIRE_ALIGN(id, 4); REQUIRE_ALIGN(r_new, 8);
+    REQUIRE_ALIGN(v_r_new, 8); REQUIRE_ALIGN(v_t_new, 8);
+    if (n_try) REQUIRE_ALIGN(n_try, 2);
+    if (counters) REQUIRE_ALIGN(counters, 8);
+    hmc_status s = check_ws(workspace, workspace_bytes, n);
+    if (s != HMC_OK) return s;
+    return sample_new_radius(n, 0, n, G, seed, step, r_sorted, phi, m_cum, v_r, v_t, E, J, r_min, r_max, k_min, k_max,
+                             id, star_status_in, r_new, v_r_new, v_t_new, n_try, star_status_out, counters, reuse_tables != 0,
+                             carve(workspace, n), static_cast<cudaStream_t>(cuda_stream), step_dev);
+}
+
+hmc_status hmc_add_u32(uint32_t* word, uint32_t increment, void* cuda_stream)
+{
+    REQUIRE_PTR(word); REQUIRE_ALIGN(word, 4);
+    return add_u32(word, increment, static_cast<cudaStream_t>(cuda_stream));
+}
+
 size_t hmc_step_host_arena_bytes(uint64_t n) { return carve_arena(nullptr, n).total; }
 
 hmc_status hmc_step_host(uint64_t n, double G, uint64_t seed, uint32_t step, const double* r, const double* v_r,

@@ -254,7 +254,8 @@ hmc_status sample_new_radius(uint64_t n, uint64_t first, uint64_t count, double 
                              const uint32_t* k_min, const uint32_t* k_max, const uint32_t* id,
                              const uint8_t* status_in, double* r_new, double* v_r_new, double* v_t_new,
                              uint16_t* n_try, uint8_t* status_out, uint64_t* counters, bool reuse_tables,
-                             const Workspace& ws, cudaStream_t st);
+                             const Workspace& ws, cudaStream_t st, const uint32_t* step_dev = nullptr);
+hmc_status add_u32(uint32_t* p, uint32_t inc, cudaStream_t st);
 
 hmc_status orbit_step(uint64_t n, uint64_t first, uint64_t count, double G, uint64_t seed, uint32_t step, const double* r, const double* v_r,
                       const double* v_t, const double* phi, const double* m_cum, const uint32_t* id, double* E,

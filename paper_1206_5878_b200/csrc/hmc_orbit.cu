@@ -830,6 +830,7 @@ struct SampleIO {
     const uint32_t *kmin, *kmax, *id;
     const uint8_t* status_in;
     const double* F_ws;      // S3's bound F per star (workspace), or nullptr: compute it here
+    const uint32_t* step_dev; // nullptr, or a device word added to the step number when the kernel runs (graph replay)
     uint32_t* batch_counter; // two workspace words, zero at launch (the table build zeroes them, this kernel's last CTA
                              // zeroes them again on its way out): [0] next unclaimed star, [1] CTAs that are done
     // fused S3 + S4 only: S3's table input and where its outputs go
@@ -967,6 +968,7 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
                          const double2* __restrict__ mid_g, const uint32_t* __restrict__ dir, int shift, SampleIO io)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (io.step_dev) step += __ldg(io.step_dev);
     Park& pk = reinterpret_cast<Park*>(smem_raw)[threadIdx.x >> 5];
     double2* coarse = reinterpret_cast<double2*>(smem_raw + ORB_WARPS * sizeof(Park));
     stage_coarse(coarse, coarse_g, n, shift);
@@ -1238,7 +1240,7 @@ hmc_status sample_new_radius(uint64_t n, uint64_t first, uint64_t count, double 
                              const uint32_t* k_min, const uint32_t* k_max, const uint32_t* id,
                              const uint8_t* status_in, double* r_new, double* v_r_new, double* v_t_new,
                              uint16_t* n_try, uint8_t* status_out, uint64_t* counters, bool reuse_tables,
-                             const Workspace& ws, cudaStream_t st)
+                             const Workspace& ws, cudaStream_t st, const uint32_t* step_dev)
 {
     const int shift = coarse_shift(n);
     if (!reuse_tables) {
@@ -1250,6 +1252,7 @@ hmc_status sample_new_radius(uint64_t n, uint64_t first, uint64_t count, double 
     io.r = r; io.v_r = v_r; io.v_t = v_t; io.E = E; io.J = J; io.rmin = r_min; io.rmax = r_max;
     io.kmin = k_min; io.kmax = k_max; io.id = id; io.status_in = status_in;
     io.F_ws = reuse_tables ? ws.orbitF : nullptr;
+    io.step_dev = step_dev;
     io.r_new = r_new; io.v_r_new = v_r_new; io.v_t_new = v_t_new; io.n_try = n_try; io.status_out = status_out;
     io.counters = reinterpret_cast<unsigned long long*>(counters);
     return launch_sampler(false, n, G, seed, step, shift, io, ws, st);
@@ -1272,6 +1275,15 @@ hmc_status energy_correction(uint64_t n, double G, const double* r, const double
     energy_correction_kernel<<<blocks, ORB_THREADS, smem, st>>>((uint32_t)n, ws.nodes, ws.coarse, ws.dir, shift, r, phi, E_old,
                                                                r_old, p_old, v_r, v_t, v_r_out, v_t_out, status_out,
                                                                reinterpret_cast<unsigned long long*>(counters));
+    HMC_LAUNCH_CHECK();
+    return HMC_OK;
+}
+
+__global__ void add_u32_kernel(uint32_t* p, uint32_t inc) { *p += inc; }
+
+hmc_status add_u32(uint32_t* p, uint32_t inc, cudaStream_t st)
+{
+    add_u32_kernel<<<1, 1, 0, st>>>(p, inc);
     HMC_LAUNCH_CHECK();
     return HMC_OK;
 }

@@ -49,7 +49,8 @@ def load(path: str) -> ctypes.CDLL:
     for name in ("hmc_sort_by_radius", "hmc_potential", "hmc_orbit_turning_points", "hmc_sample_new_radius",
                  "hmc_orbit_step", "hmc_diagnostics", "hmc_energy_correction", "hmc_step_host", "hmc_potential_totals",
                  "hmc_potential_shard", "hmc_partition_points", "hmc_orbit_turning_points_range",
-                 "hmc_sample_new_radius_range", "hmc_relaxation_timestep", "hmc_two_body_relaxation"):
+                 "hmc_sample_new_radius_range", "hmc_relaxation_timestep", "hmc_two_body_relaxation",
+                 "hmc_sample_new_radius_dstep", "hmc_add_u32"):
         getattr(L, name).restype = ctypes.c_int32
     return L
 
@@ -179,10 +180,12 @@ def alloc_sample(n: int, device="cuda", with_n_try: bool = True):
 
 def hmc_sample_new_radius(r_sorted, phi, m_cum, v_r, v_t, tp, ids, seed: int, step: int, G: float = 1.0, *,
                           out=None, counters=None, workspace=None, reuse_tables: bool = False,
-                          first: Optional[int] = None):
+                          first: Optional[int] = None, step_dev: Optional[torch.Tensor] = None):
     """S4.  ``tp`` is the dict returned by hmc_orbit_turning_points.
     -> dict(r_new, v_r_new, v_t_new, n_try, status)
-    ``first`` given (sharded step): hmc_sample_new_radius_range, per-star arrays of the range's length."""
+    ``first`` given (sharded step): hmc_sample_new_radius_range, per-star arrays of the range's length.
+    ``step_dev`` given (int32[1] on the device): hmc_sample_new_radius_dstep, the step number is step + step_dev[0],
+    read when the kernel runs (CUDA-graph replay)."""
     n = r_sorted.numel()
     c = n if first is None else v_r.numel()
     dev = r_sorted.device
@@ -192,7 +195,13 @@ def hmc_sample_new_radius(r_sorted, phi, m_cum, v_r, v_t, tp, ids, seed: int, st
     f = torch.float64
     head = (ctypes.c_uint64(n),) if first is None else (ctypes.c_uint64(n), ctypes.c_uint64(first), ctypes.c_uint64(c))
     fn = lib().hmc_sample_new_radius if first is None else lib().hmc_sample_new_radius_range
-    rc = fn(*head, ctypes.c_double(G), ctypes.c_uint64(seed), ctypes.c_uint32(step),
+    stepargs = (ctypes.c_uint32(step),)
+    if step_dev is not None:
+        if first is not None:
+            raise HmcError("step_dev and first cannot be combined")
+        fn = lib().hmc_sample_new_radius_dstep
+        stepargs = (ctypes.c_uint32(step), _dev(step_dev, torch.int32, 1, "step_dev"))
+    rc = fn(*head, ctypes.c_double(G), ctypes.c_uint64(seed), *stepargs,
             _dev(r_sorted, f, n, "r_sorted"), _dev(phi, f, n, "phi"), _dev(m_cum, f, n, "m_cum"), _dev(v_r, f, c, "v_r"),
             _dev(v_t, f, c, "v_t"), _dev(tp["E"], f, c, "E"), _dev(tp["J"], f, c, "J"), _dev(tp["r_min"], f, c, "r_min"),
             _dev(tp["r_max"], f, c, "r_max"), _dev(tp["k_min"], torch.int32, c, "k_min"),
@@ -204,6 +213,11 @@ def hmc_sample_new_radius(r_sorted, phi, m_cum, v_r, v_t, tp, ids, seed: int, st
             _stream())
     _check(rc, "hmc_sample_new_radius")
     return out
+
+
+def hmc_add_u32(word: torch.Tensor, increment: int = 1):
+    """word[0] += increment, enqueued on the current stream (the step counter of hmc_sample_new_radius_dstep)."""
+    _check(lib().hmc_add_u32(_dev(word, torch.int32, 1, "word"), ctypes.c_uint32(increment), _stream()), "hmc_add_u32")
 
 
 def hmc_potential_totals(r_sorted, m_sorted, *, totals=None, workspace=None):
@@ -399,10 +413,44 @@ class OrbitStepper:
                 self.sorted[k] = torch.empty(n, **f)
             self.corrected = dict(v_r=torch.empty(n, **f), v_t=torch.empty(n, **f),
                                   status=torch.empty(n, dtype=torch.uint8, device=dev))
+        self._graph = None
+        self._step_dev = None
+
+    def run_graph(self, steps: int):
+        """``steps`` orbit steps (an even number), replayed from a CUDA graph of TWO steps captured at the first
+        call (the carried arrays alternate between two sets of buffers with period two).  What changes from step to
+        step, the Philox step number, is kept on the device: hmc_sample_new_radius_dstep reads it, hmc_add_u32
+        advances it inside the graph.  For small N, where a step is bound by launching its 13 kernels one
+        by one rather than by the GPU.  Plain steps only (no energy correction, no relaxation stage)."""
+        if self.energy_correction or self.relaxation:
+            raise HmcError("run_graph supports the plain step only")
+        if steps % 2:
+            raise HmcError("run_graph takes an even number of steps (the buffers alternate with period two)")
+        if self._graph is None:
+            if self.step_index == 0:                 # first launches set function attributes: not inside a capture
+                self.step()
+                self.step()
+                steps -= 2
+            self._step_dev = torch.full((1,), self.step_index, dtype=torch.int32, device=self.state["r"].device)
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                self._step_body(False, self._step_dev)
+                self._step_body(False, self._step_dev)
+            self._graph = g
+            self.step_index -= 2                     # the capture ran nothing
+        else:
+            self._step_dev.fill_(self.step_index)    # eager steps may have been taken in between
+        for _ in range(steps // 2):
+            self._graph.replay()
+            self.step_index += 2
 
     def step(self, fused: bool = False):
         """One orbit step.  fused=False: the four C-ABI calls; fused=True: S3 and S4 as the single
         call hmc_orbit_step (same results)."""
+        self._step_body(fused, None)
+
+    def _step_body(self, fused: bool, step_dev):
         s, so = self.state, self.sorted
         correct = self.energy_correction and self.step_index > 0
         extra = ("E", "r_old", "p_old") if correct else ()
@@ -433,8 +481,10 @@ class OrbitStepper:
             hmc_orbit_turning_points(so["r"], so["v_r"], so["v_t"], self.phi, self.m_cum, self.G, out=self.tp,
                                      counters=self.counters, workspace=self.workspace)
             hmc_sample_new_radius(so["r"], self.phi, self.m_cum, so["v_r"], so["v_t"], self.tp, so["id"], self.seed,
-                                  self.step_index, self.G, out=self.sample, counters=self.counters,
-                                  workspace=self.workspace, reuse_tables=True)
+                                  0 if step_dev is not None else self.step_index, self.G, out=self.sample,
+                                  counters=self.counters, workspace=self.workspace, reuse_tables=True, step_dev=step_dev)
+            if step_dev is not None:
+                hmc_add_u32(step_dev, 1)
         # carried state for the next step: new phase-space coordinates, masses and ids in sorted order
         sm = self.sample
         s["r"], sm["r_new"] = sm["r_new"], s["r"]

@@ -548,3 +548,35 @@ def test_repeated_steps_are_bit_reproducible():
         else:
             for k in first:
                 assert torch.equal(first[k], got[k]), (rep, k)
+
+
+@pytest.mark.parametrize("n", [1, 5_000, 100_000, 400_003])
+def test_graph_replay_equals_eager_steps(oracle, n):
+    """OrbitStepper.run_graph: a CUDA graph of two steps, the Philox step number kept on the device
+    (hmc_sample_new_radius_dstep / hmc_add_u32).  Eight steps by replay leave the same bits as eight eager steps,
+    and the last one is compared with the oracle (so the step numbers really advanced); eager steps and replays
+    can be mixed."""
+    seed = 77
+    c = inputs.plummer(n, seed)
+    d = [dev(c["r"]), dev(c["v_r"]), dev(c["v_t"]), dev(c["m"]), dev(c["id"].view(np.int32))]
+    eager = hmc.OrbitStepper(*d, seed)
+    for _ in range(7):
+        eager.step()
+    before = {k: host(eager.state[k]) for k in ("r", "v_r", "v_t", "m")}
+    before["id"] = host(eager.state["id"], np.uint32)
+    eager.step()
+    g = hmc.OrbitStepper(*d, seed)
+    g.run_graph(4)                        # two eager steps (first launches), capture, one replay
+    g.step()
+    g.step()
+    g.run_graph(2)
+    torch.cuda.synchronize()
+    assert g.step_index == eager.step_index == 8
+    for k in ("r", "v_r", "v_t", "m", "id"):
+        assert torch.equal(g.state[k], eager.state[k]), k
+    for k in ("n_try", "status"):
+        assert torch.equal(g.sample[k], eager.sample[k]), k
+    assert torch.equal(g.counters, eager.counters)
+    o = oracle.orbit_step(before["r"], before["v_r"], before["v_t"], before["m"], before["id"], seed, 7)
+    assert np.array_equal(host(g.state["r"]), o["sample"]["r_new"])
+    assert np.array_equal(host(g.sample["n_try"], np.uint16), o["sample"]["n_try"])
