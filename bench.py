@@ -458,8 +458,11 @@ def run_gpu(args, cfg):
                     model_frac=achieved / peak,
                     physical=(dict(dram_bytes_per_launch=traffic, achieved=traffic / (stage_ms[dom] * 1e-3) / 1e9,
                                    frac=traffic / (stage_ms[dom] * 1e-3) / 1e9 / peak, capture=capture,
-                                   limiter="latency of dependent random loads (DRAM lines touched), not streamed bytes; "
-                                           "see profiles/") if traffic else None))
+                                   limiter="not streamed bytes: 8 warps per scheduler of dependent fp64 chains and loads "
+                                           "(ncu: issue slots 50 % used, DRAM 34 % busy; profiles/r2b.md, DESIGN.md 5 and 5a)")
+                              if traffic else None),
+                    # what ncu shows the kernel waits for, as opposed to the roofline the metric is quoted against
+                    bound_observed="issue / dependent-instruction latency at 32 warps per SM")
     orbit_ms = stage_ms["potential"] + stage_ms["turning_points"] + stage_ms["sampling"]
     orbit_bytes = model["potential"] + model["turning_points"] + model["sampling"]
     stages = {s: dict(ms=stage_ms[s], stars_per_s=n / (stage_ms[s] * 1e-3), algorithmic_bytes_per_star=model[s],
