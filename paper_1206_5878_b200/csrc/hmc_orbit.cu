@@ -8,14 +8,15 @@
 //  * The bracket predicate "Q(r_j) < 0" is monotone on either side of the star (Q is concave in
 //    1/r) and "r_j <= r0" is monotone, so ANY probe order finds the same index.  The searches
 //    therefore do not bisect.  They run in three tiers:
-//      1. coarse: the nodes that are multiples of S = 2^shift ((r, Phi) pairs, <= 216 KB) are staged
+//      1. coarse: the nodes that are multiples of S = 2^shift ((r, Phi) pairs, <= 160 KB) are staged
 //         once per CTA in shared memory; a bisection over them costs no global traffic and leaves
 //         an interval of at most S nodes.
 //      2. guess: inside that interval r^2 Q(r) is very nearly linear (the interval spans ~1e-4 of
 //         the cluster), so one secant step gives the root radius to a fraction of the node
 //         spacing (S3); S4 knows the radius it looks for.  A "radius directory" -- for every coarse
 //         interval, S equal-width radius buckets with the offset of the first node of each
-//         bucket, 2 bytes per star, L2 resident -- turns that radius into a node index.
+//         bucket and of the next, 4 bytes per star, L2 resident up to N = 1e7 -- turns that radius into a
+//         node index.
 //      3. exact: the node table proper (r_j, Phi_j, G M_j, 1/r_j in one 32-byte sector) is
 //         probed at the guess and its neighbour; if the sign change is not there the search
 //         gallops away from the guess and bisects what is left.  Typical cost: one directory read
