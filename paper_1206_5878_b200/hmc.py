@@ -438,8 +438,12 @@ class OrbitStepper:
                 self._step_body(False, self._step_dev)
                 self._step_body(False, self._step_dev)
             self._graph = g
+            self._graph_parity = self.step_index % 2          # which of the two buffer arrangements the graph starts from
             self.step_index -= 2                     # the capture ran nothing
         else:
+            if self.step_index % 2 != self._graph_parity:
+                raise HmcError("run_graph: the graph starts from the buffer arrangement it was captured in; take an "
+                               "even number of eager steps between replays")
             self._step_dev.fill_(self.step_index)    # eager steps may have been taken in between
         for _ in range(steps // 2):
             self._graph.replay()
