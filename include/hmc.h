@@ -60,6 +60,7 @@ typedef int32_t hmc_status;
 
 #define HMC_MAX_N      (1ull << 28)   /* stars per call                                     */
 #define HMC_MAX_COLS   8              /* fp64 record columns carried by the sort            */
+#define HMC_MAX_PEERS  16             /* further copies of the table hmc_potential_shard_push writes to */
 
 /* star_status bits */
 #define HMC_STAR_UNBOUND     1u   /* E >= 0 (or NaN): no apocentre; r_max = +inf, no draw           */
@@ -331,6 +332,20 @@ HMC_API hmc_status hmc_potential_totals(uint64_t n, const double* r_sorted, cons
 
 HMC_API hmc_status hmc_potential_shard(uint64_t n, double G, const double* r_sorted, const double* m_sorted,
         uint32_t nranks, uint32_t rank, const double* rank_totals, double* phi, double* m_cum,
+        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * hmc_potential_shard fused with the all-gather of the replicated table ("we maintain a copy of it on
+ * all nodes"): besides phi and m_cum of its own shard, the launch stores the shard's r, phi and m_cum to npeers
+ * further destinations, tile by tile as the scan produces them, so the exchange overlaps the arithmetic instead of
+ * following it.  peer_r, peer_phi, peer_m_cum: HOST arrays of npeers DEVICE pointers, each pointing at this shard's
+ * place (element `first` of that copy of the table); the memory may belong to another GPU (peer access over NVLink:
+ * plain stores) or to this one.  A copy is complete when every rank's call has finished: the caller orders that
+ * (a barrier across ranks, or stream order when the shards share a device).  npeers <= HMC_MAX_PEERS, else HMC_ERR_SIZE.
+ */
+HMC_API hmc_status hmc_potential_shard_push(uint64_t n, double G, const double* r_sorted, const double* m_sorted,
+        uint32_t nranks, uint32_t rank, const double* rank_totals, double* phi, double* m_cum,
+        int32_t npeers, double* const* peer_r, double* const* peer_phi, double* const* peer_m_cum,
         void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 HMC_API hmc_status hmc_partition_points(uint64_t n, const double* r_sorted, uint32_t nsplit, const double* splitters,

@@ -330,6 +330,27 @@ hmc_status hmc_potential_shard(uint64_t n, double G, const double* r_sorted, con
                      static_cast<cudaStream_t>(cuda_stream));
 }
 
+hmc_status hmc_potential_shard_push(uint64_t n, double G, const double* r_sorted, const double* m_sorted, uint32_t nranks,
+                                    uint32_t rank, const double* rank_totals, double* phi, double* m_cum, int32_t npeers,
+                                    double* const* peer_r, double* const* peer_phi, double* const* peer_m_cum,
+                                    void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (n > HMC_MAX_N || nranks == 0 || rank >= nranks || npeers < 0 || npeers > HMC_MAX_PEERS) return HMC_ERR_SIZE;
+    if (n == 0) return HMC_OK;
+    REQUIRE_PTR(r_sorted); REQUIRE_PTR(m_sorted); REQUIRE_PTR(phi); REQUIRE_PTR(m_cum); REQUIRE_PTR(rank_totals);
+    REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(m_sorted, 8); REQUIRE_ALIGN(phi, 8); REQUIRE_ALIGN(m_cum, 8);
+    REQUIRE_ALIGN(rank_totals, 32);
+    if (npeers > 0) { REQUIRE_PTR(peer_r); REQUIRE_PTR(peer_phi); REQUIRE_PTR(peer_m_cum); }
+    for (int g = 0; g < npeers; ++g) {
+        REQUIRE_PTR(peer_r[g]); REQUIRE_PTR(peer_phi[g]); REQUIRE_PTR(peer_m_cum[g]);
+        REQUIRE_ALIGN(peer_r[g], 8); REQUIRE_ALIGN(peer_phi[g], 8); REQUIRE_ALIGN(peer_m_cum[g], 8);
+    }
+    hmc_status s = check_ws(workspace, workspace_bytes, n);
+    if (s != HMC_OK) return s;
+    return potential(n, G, r_sorted, m_sorted, phi, m_cum, rank_totals, nranks, rank, carve(workspace, n),
+                     static_cast<cudaStream_t>(cuda_stream), npeers, peer_r, peer_phi, peer_m_cum);
+}
+
 hmc_status hmc_partition_points(uint64_t n, const double* r_sorted, uint32_t nsplit, const double* splitters,
                                 uint64_t* counts, void* cuda_stream)
 {

@@ -237,8 +237,11 @@ hmc_status sort_by_radius(uint64_t n, const double* r_in, double* r_sorted, uint
 // cols_out[c][k] = cols_in[c][perm[k]] (and the ids likewise): the record columns when they arrive after the sort
 hmc_status gather_by_perm(uint64_t n, const uint32_t* perm, int ncols, const double* const* cols_in, double* const* cols_out,
                           const uint32_t* id_in, uint32_t* id_out, cudaStream_t st);
+// npeers > 0: the shard's r, phi and m_cum are also stored to peer_*[g] (each already offset to the shard's place)
 hmc_status potential(uint64_t n, double G, const double* r, const double* m, double* phi, double* m_cum,
-                     const double* ext_tot, uint32_t nranks, uint32_t rank, const Workspace& ws, cudaStream_t st);
+                     const double* ext_tot, uint32_t nranks, uint32_t rank, const Workspace& ws, cudaStream_t st,
+                     int npeers = 0, double* const* peer_r = nullptr, double* const* peer_phi = nullptr,
+                     double* const* peer_m_cum = nullptr);
 hmc_status potential_totals(uint64_t n, const double* r, const double* m, double* totals4, const Workspace& ws, cudaStream_t st);
 hmc_status partition_points(uint64_t n, const double* r_sorted, uint32_t nsplit, const double* splitters, uint64_t* counts,
                             cudaStream_t st);

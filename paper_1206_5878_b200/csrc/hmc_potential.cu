@@ -134,11 +134,21 @@ potential_reduce_kernel(const double* __restrict__ r, const double* __restrict__
 // ---- 2. per-tile scans and Phi -----------------------------------------------------------------
 static constexpr int MAX_TPC_SMEM = 256;      // tiles per chunk whose offsets fit the shared array (n <= HMC_MAX_N: 222)
 
+// Sharded step: further destinations of the shard's slice of the replicated table, e.g. the other
+// GPUs' copies at this shard's offset, reached by peer access over NVLink.  The launch that produces Phi and M stores
+// them (and the radii it has in registers) there tile by tile, so the table's all-gather is done when the scan is.
+struct PushTargets {
+    int npeers;
+    double* r[HMC_MAX_PEERS];
+    double* phi[HMC_MAX_PEERS];
+    double* m_cum[HMC_MAX_PEERS];
+};
+
 __global__ void __launch_bounds__(SCAN_THREADS, CHUNK_CTAS_PER_SM)
 potential_apply_kernel(const double* __restrict__ r, const double* __restrict__ m, double* __restrict__ phi,
                        double* __restrict__ m_cum, uint64_t n, double G, ScanPlan plan,
                        const double4* __restrict__ slice_tot, const double4* __restrict__ chunk_tot,
-                       const double4* __restrict__ ext_tot, uint32_t nranks, uint32_t rank)
+                       const double4* __restrict__ ext_tot, uint32_t nranks, uint32_t rank, PushTargets push)
 {
     __shared__ dd sm_m[2][SCAN_WARPS], sm_t[2][SCAN_WARPS];     // per-warp totals of the tile being scanned (by tile parity)
     __shared__ dd sm_pm[MAX_TPC_SMEM];                          // sum of m over everything before tile k of this chunk
@@ -255,6 +265,21 @@ potential_apply_kernel(const double* __restrict__ r, const double* __restrict__ 
                 if (p < n) { phi[p] = ph[i]; m_cum[p] = Mk[i]; }
             }
         }
+        for (int g = 0; g < push.npeers; ++g) {                    // the same slice of every peer's table
+            double *pr = push.r[g], *pp = push.phi[g], *pc = push.m_cum[g];
+            const bool al = ((reinterpret_cast<uintptr_t>(pr) | reinterpret_cast<uintptr_t>(pp) | reinterpret_cast<uintptr_t>(pc)) & 31) == 0;
+            if (full && al) {
+                st4(pr + p0, rr); st4(pr + p0 + 4, rr + 4);
+                st4(pp + p0, ph); st4(pp + p0 + 4, ph + 4);
+                st4(pc + p0, Mk); st4(pc + p0 + 4, Mk + 4);
+            } else {
+#pragma unroll
+                for (int i = 0; i < SCAN_ITEMS; ++i) {
+                    const uint64_t p = p0 + i;
+                    if (p < n) { pr[p] = rr[i]; pp[p] = ph[i]; pc[p] = Mk[i]; }
+                }
+            }
+        }
     }
 }
 
@@ -321,8 +346,12 @@ hmc_status potential_totals(uint64_t n, const double* r, const double* m, double
 }
 
 hmc_status potential(uint64_t n, double G, const double* r, const double* m, double* phi, double* m_cum,
-                     const double* ext_tot, uint32_t nranks, uint32_t rank, const Workspace& ws, cudaStream_t st)
+                     const double* ext_tot, uint32_t nranks, uint32_t rank, const Workspace& ws, cudaStream_t st,
+                     int npeers, double* const* peer_r, double* const* peer_phi, double* const* peer_m_cum)
 {
+    PushTargets push{};
+    push.npeers = npeers;
+    for (int g = 0; g < npeers; ++g) { push.r[g] = peer_r[g]; push.phi[g] = peer_phi[g]; push.m_cum[g] = peer_m_cum[g]; }
     const ScanPlan plan = scan_plan(n, sm_count());
     if (plan.tpc > MAX_TPC_SMEM) return HMC_ERR_SIZE;             // cannot happen for n <= HMC_MAX_N on >= 4 SMs
     double4* slice_tot = reinterpret_cast<double4*>(ws.scan_status);
@@ -330,7 +359,7 @@ hmc_status potential(uint64_t n, double G, const double* r, const double* m, dou
     potential_reduce_kernel<<<plan.nchunks, SCAN_THREADS, 0, st>>>(r, m, n, plan, slice_tot, chunk_tot);
     HMC_LAUNCH_CHECK();
     potential_apply_kernel<<<plan.nchunks, SCAN_THREADS, 0, st>>>(r, m, phi, m_cum, n, G, plan, slice_tot, chunk_tot,
-                                                                  reinterpret_cast<const double4*>(ext_tot), nranks, rank);
+                                                                  reinterpret_cast<const double4*>(ext_tot), nranks, rank, push);
     HMC_LAUNCH_CHECK();
     return HMC_OK;
 }

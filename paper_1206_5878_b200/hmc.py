@@ -50,7 +50,7 @@ def load(path: str) -> ctypes.CDLL:
                  "hmc_orbit_step", "hmc_diagnostics", "hmc_energy_correction", "hmc_step_host", "hmc_potential_totals",
                  "hmc_potential_shard", "hmc_partition_points", "hmc_orbit_turning_points_range",
                  "hmc_sample_new_radius_range", "hmc_relaxation_timestep", "hmc_two_body_relaxation",
-                 "hmc_sample_new_radius_dstep", "hmc_add_u32"):
+                 "hmc_sample_new_radius_dstep", "hmc_add_u32", "hmc_potential_shard_push"):
         getattr(L, name).restype = ctypes.c_int32
     return L
 
@@ -234,8 +234,11 @@ def hmc_potential_totals(r_sorted, m_sorted, *, totals=None, workspace=None):
 
 
 def hmc_potential_shard(r_sorted, m_sorted, rank: int, rank_totals, G: float = 1.0, *, phi=None, m_cum=None,
-                        workspace=None):
-    """Sharded step: S2 on shard ``rank``; rank_totals is the device float64[nranks, 4] of every shard's totals."""
+                        workspace=None, push=None):
+    """Sharded step: S2 on shard ``rank``; rank_totals is the device float64[nranks, 4] of every shard's totals.
+    ``push``: a list of (r, phi, m_cum) tensor triples of the shard's length -- views into the other ranks' copies of
+    the replicated table at this shard's place; hmc_potential_shard_push stores the shard's slice there as it is
+    produced (the table's all-gather fused into the scan)."""
     n = r_sorted.numel()
     dev = r_sorted.device
     nranks = rank_totals.numel() // 4
@@ -243,6 +246,17 @@ def hmc_potential_shard(r_sorted, m_sorted, rank: int, rank_totals, G: float = 1
     phi = torch.empty(n, dtype=f, device=dev) if phi is None else phi
     m_cum = torch.empty(n, dtype=f, device=dev) if m_cum is None else m_cum
     workspace, wp, wb = _ws(workspace, n, dev)
+    if push:
+        Arr = ctypes.c_void_p * len(push)
+        pr = Arr(*[_dev(t[0], f, n, "push r").value or 0 for t in push])
+        pp = Arr(*[_dev(t[1], f, n, "push phi").value or 0 for t in push])
+        pc = Arr(*[_dev(t[2], f, n, "push m_cum").value or 0 for t in push])
+        rc = lib().hmc_potential_shard_push(ctypes.c_uint64(n), ctypes.c_double(G), _dev(r_sorted, f, n, "r_sorted"),
+                                            _dev(m_sorted, f, n, "m_sorted"), ctypes.c_uint32(nranks), ctypes.c_uint32(rank),
+                                            _dev(rank_totals, f, 4 * nranks, "rank_totals"), _dev(phi, f, n, "phi"),
+                                            _dev(m_cum, f, n, "m_cum"), ctypes.c_int32(len(push)), pr, pp, pc, wp, wb, _stream())
+        _check(rc, "hmc_potential_shard_push")
+        return phi, m_cum
     rc = lib().hmc_potential_shard(ctypes.c_uint64(n), ctypes.c_double(G), _dev(r_sorted, f, n, "r_sorted"),
                                    _dev(m_sorted, f, n, "m_sorted"), ctypes.c_uint32(nranks), ctypes.c_uint32(rank),
                                    _dev(rank_totals, f, 4 * nranks, "rank_totals"), _dev(phi, f, n, "phi"),

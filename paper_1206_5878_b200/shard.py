@@ -88,6 +88,13 @@ def splitter_positions(s: int, p: int) -> List[int]:
 
 
 # ------------------------------------------------------------------------------------------------ communication
+# A communicator may offer ``table_views(n)``: for every local rank, the (r, phi, m_cum) arrays [n] of EVERY rank's
+# copy of the replicated table, as tensors this process can hand to a kernel (its own memory, or peer memory mapped
+# into this process).  ShardedStepper then fuses the table's all-gather into the potential scan
+# (hmc_potential_shard_push: each rank's launch stores its slice into every copy) and only has to order "all ranks
+# done" before S3.  InProcessComm offers it (all copies live on one device; stream order is the barrier).  DistComm
+# does not: mapping peer GPUs' memory into the process (CUDA IPC handles or torch's symmetric memory) could not be
+# exercised on the one-GPU boxes this was built on, so it takes the three all-gathers.
 class InProcessComm:
     """G ranks in one process.  Arguments and results are lists with one entry per rank."""
 
@@ -105,6 +112,17 @@ class InProcessComm:
 
     def all_gather_ints(self, xs: List[List[int]]) -> List[List[List[int]]]:
         return [list(xs) for _ in self.local_ranks]
+
+    def table_views(self, n: int, device) -> List[dict]:
+        """One copy of the replicated table per rank, every copy reachable by every rank (same device)."""
+        if getattr(self, "_tables_n", None) != (n, str(device)):
+            f = dict(dtype=torch.float64, device=device)
+            self._tables = [dict(r=torch.empty(n, **f), phi=torch.empty(n, **f), m_cum=torch.empty(n, **f)) for _ in self.local_ranks]
+            self._tables_n = (n, str(device))
+        return self._tables
+
+    def tables_complete(self):
+        """Every rank's pushes have landed in every copy: the shards share a device and a stream, so stream order says so."""
 
 
 class DistComm:
@@ -223,8 +241,11 @@ class ShardedStepper:
     of the sorted order with their new coordinates, exactly as hmc.OrbitStepper's state cut at the same places."""
 
     def __init__(self, comm, shards: List[dict], seed: int, G: float = 1.0, sample_size: int = 256,
-                 n_total: Optional[int] = None):
+                 n_total: Optional[int] = None, push_tables: Optional[bool] = None):
+        """push_tables: fuse the replicated table's all-gather into the potential scan (needs a communicator with
+        table_views; default: whenever it has one)."""
         from . import hmc
+        self.push_tables = hasattr(comm, "table_views") if push_tables is None else push_tables
         self.hmc = hmc
         self.comm, self.seed, self.G, self.sample_size, self.step_index = comm, seed, G, sample_size, 0
         self.state = [dict(s) for s in shards]
@@ -261,12 +282,27 @@ class ShardedStepper:
         # S2: shard totals -> all-gather -> local scan with what lies before and after
         totals = [hmc.hmc_potential_totals(c[0], c[3], workspace=self.workspace[i]) for i, c in enumerate(cols)]
         all_totals = [torch.cat(t) for t in comm.all_gather(totals)]
-        pots = [hmc.hmc_potential_shard(c[0], c[3], rank, all_totals[i], self.G, workspace=self.workspace[i])
-                for i, (c, rank) in enumerate(zip(cols, comm.local_ranks))]
-        # the replicated table
-        table_r = [torch.cat(t) for t in comm.all_gather([c[0] for c in cols])]
-        table_phi = [torch.cat(t) for t in comm.all_gather([p[0] for p in pots])]
-        table_m = [torch.cat(t) for t in comm.all_gather([p[1] for p in pots])]
+        if self.push_tables:
+            # the replicated table filled by the scans themselves: rank d's launch stores its slice of
+            # (r, Phi, M) into every rank's copy as it produces it (hmc_potential_shard_push)
+            tabs = comm.table_views(self.n, cols[0][0].device)
+            pots = []
+            for i, (c, rank) in enumerate(zip(cols, comm.local_ranks)):
+                lo, hi = self.offsets[rank], self.offsets[rank] + self.want[rank]
+                mine = tabs[i]
+                others = [(t["r"][lo:hi], t["phi"][lo:hi], t["m_cum"][lo:hi]) for j, t in enumerate(tabs) if j != i]
+                mine["r"][lo:hi].copy_(c[0])
+                pots.append(hmc.hmc_potential_shard(c[0], c[3], rank, all_totals[i], self.G, phi=mine["phi"][lo:hi],
+                                                    m_cum=mine["m_cum"][lo:hi], workspace=self.workspace[i], push=others))
+            comm.tables_complete()
+            table_r, table_phi, table_m = [t["r"] for t in tabs], [t["phi"] for t in tabs], [t["m_cum"] for t in tabs]
+        else:
+            pots = [hmc.hmc_potential_shard(c[0], c[3], rank, all_totals[i], self.G, workspace=self.workspace[i])
+                    for i, (c, rank) in enumerate(zip(cols, comm.local_ranks))]
+            # the replicated table
+            table_r = [torch.cat(t) for t in comm.all_gather([c[0] for c in cols])]
+            table_phi = [torch.cat(t) for t in comm.all_gather([p[0] for p in pots])]
+            table_m = [torch.cat(t) for t in comm.all_gather([p[1] for p in pots])]
         # S3 / S4 on the rank's own range: no communication
         new_state, last = [], []
         for i, rank in enumerate(comm.local_ranks):

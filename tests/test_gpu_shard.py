@@ -26,13 +26,17 @@ def device_cluster(n, seed, masses="equal"):
     return {k: dev(c[k]) for k in ("r", "v_r", "v_t", "m", "id")}, c
 
 
+@pytest.mark.parametrize("push", [True, False])
 @pytest.mark.parametrize("world", [2, 4, 8])
-def test_sharded_step_equals_single_gpu_step(world):
-    """N = 1e6, three chained steps: after every step the shards, put end to end, ARE the single-GPU state."""
+def test_sharded_step_equals_single_gpu_step(world, push):
+    """N = 1e6, three chained steps: after every step the shards, put end to end, ARE the single-GPU state.
+    push=True: every rank's potential scan stores its slice of (r, Phi, M) into every rank's copy of the replicated
+    table (hmc_potential_shard_push); push=False: three all-gathers after the scans."""
     n, seed = 1_000_000, 2
     d, _ = device_cluster(n, seed)
     single = hmc.OrbitStepper(d["r"], d["v_r"], d["v_t"], d["m"], d["id"], seed)
-    sharded = shard.ShardedStepper(shard.InProcessComm(world), shard.split_cluster(d, world), seed)
+    sharded = shard.ShardedStepper(shard.InProcessComm(world), shard.split_cluster(d, world), seed, push_tables=push)
+    assert sharded.push_tables == push
     assert sharded.want == shard.partition_counts(n, world)
     for step in range(3):
         single.step()
