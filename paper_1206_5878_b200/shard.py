@@ -21,7 +21,9 @@ Back-ends:
   InProcessComm(G)   G shards held by ONE process on one device; a collective is a hand-over of device tensors.
                      This is what one GPU can test, and what the tests use.
   DistComm()         one shard per process over torch.distributed (NCCL between GPUs; gloo on CPU tensors in the
-                     world-size-2 host-logic tests).  UNMEASURED ON HARDWARE: no multi-GPU node was available.
+                     world-size-2 host-logic tests); the replicated table in torch's symmetric memory, filled by
+                     the ranks' own stores (see table_views below).  UNMEASURED ON HARDWARE: no multi-GPU node was
+                     available.
 """
 from __future__ import annotations
 
@@ -88,13 +90,16 @@ def splitter_positions(s: int, p: int) -> List[int]:
 
 
 # ------------------------------------------------------------------------------------------------ communication
-# A communicator may offer ``table_views(n)``: for every local rank, the (r, phi, m_cum) arrays [n] of EVERY rank's
-# copy of the replicated table, as tensors this process can hand to a kernel (its own memory, or peer memory mapped
-# into this process).  ShardedStepper then fuses the table's all-gather into the potential scan
-# (hmc_potential_shard_push: each rank's launch stores its slice into every copy) and only has to order "all ranks
-# done" before S3.  InProcessComm offers it (all copies live on one device; stream order is the barrier).  DistComm
-# does not: mapping peer GPUs' memory into the process (CUDA IPC handles or torch's symmetric memory) could not be
-# exercised on the one-GPU boxes this was built on, so it takes the three all-gathers.
+# A communicator may offer ``table_views(n, device)``: for every local rank, (its own copy of the replicated table,
+# the other ranks' copies) as dicts of (r, phi, m_cum) tensors [n] that this process can hand to a kernel -- its own
+# memory, or peer GPUs' memory mapped into this process.  ShardedStepper then fuses the table's all-gather into the
+# potential scan (hmc_potential_shard_push: each rank's launch stores its slice into every copy) and calls
+# ``tables_complete()`` ("every rank's stores have landed") before S3.  ``table_views`` returns None when the
+# communicator cannot offer that (CPU tensors, no peer mapping): the stepper then takes three all-gathers.
+#   InProcessComm: all copies live on one device; stream order is the barrier.
+#   DistComm:      torch's symmetric memory (one allocation per rank, every rank's mapped into every process over
+#                  NVLink peer access; the handle's barrier orders the stores).  Exercised with a world of ONE on the
+#                  one-GPU boxes this was built on; with more ranks it is correct by construction only.
 class InProcessComm:
     """G ranks in one process.  Arguments and results are lists with one entry per rank."""
 
@@ -113,13 +118,13 @@ class InProcessComm:
     def all_gather_ints(self, xs: List[List[int]]) -> List[List[List[int]]]:
         return [list(xs) for _ in self.local_ranks]
 
-    def table_views(self, n: int, device) -> List[dict]:
+    def table_views(self, n: int, device):
         """One copy of the replicated table per rank, every copy reachable by every rank (same device)."""
         if getattr(self, "_tables_n", None) != (n, str(device)):
             f = dict(dtype=torch.float64, device=device)
             self._tables = [dict(r=torch.empty(n, **f), phi=torch.empty(n, **f), m_cum=torch.empty(n, **f)) for _ in self.local_ranks]
             self._tables_n = (n, str(device))
-        return self._tables
+        return [(t, [u for j, u in enumerate(self._tables) if j != i]) for i, t in enumerate(self._tables)]
 
     def tables_complete(self):
         """Every rank's pushes have landed in every copy: the shards share a device and a stream, so stream order says so."""
@@ -141,6 +146,34 @@ class DistComm:
         out = [None] * self.world
         self.dist.all_gather_object(out, list(xs[0]), group=self.group)
         return [out]
+
+    def table_views(self, n: int, device):
+        """This rank's copy of the replicated table in symmetric memory and the other ranks' copies mapped into this
+        process; None when that is not available (CPU tensors, no symmetric-memory support)."""
+        if torch.device(device).type != "cuda":
+            return None
+        if getattr(self, "_tables_n", None) != n:
+            try:
+                import torch.distributed._symmetric_memory as symm
+                group = self.group if self.group is not None else self.dist.group.WORLD
+                buf = symm.empty(3 * n, dtype=torch.float64, device=device)
+                handle = symm.rendezvous(buf, group.group_name)
+                views = [handle.get_buffer(p, (3 * n,), torch.float64) for p in range(self.world)]
+            except Exception:
+                self._tables, self._tables_n = None, n
+                return None
+            cut = lambda v: dict(r=v[:n], phi=v[n:2 * n], m_cum=v[2 * n:])
+            self._symm, self._symm_buf = handle, buf
+            self._tables = (cut(views[self.rank]), [cut(v) for p, v in enumerate(views) if p != self.rank])
+            self._tables_n = n
+        if self._tables is None:
+            return None
+        self._symm.barrier()          # nobody still reads the table of the step before while it is overwritten
+        return [self._tables]
+
+    def tables_complete(self):
+        """Every rank's stores into every copy are done (device-side barrier across the ranks, on the current stream)."""
+        self._symm.barrier()
 
     def all_gather(self, xs: List[torch.Tensor]) -> List[List[torch.Tensor]]:
         x = xs[0].contiguous()
@@ -245,7 +278,7 @@ class ShardedStepper:
         """push_tables: fuse the replicated table's all-gather into the potential scan (needs a communicator with
         table_views; default: whenever it has one)."""
         from . import hmc
-        self.push_tables = hasattr(comm, "table_views") if push_tables is None else push_tables
+        self.push_tables = push_tables            # None: whenever the communicator can hand out the copies
         self.hmc = hmc
         self.comm, self.seed, self.G, self.sample_size, self.step_index = comm, seed, G, sample_size, 0
         self.state = [dict(s) for s in shards]
@@ -282,21 +315,27 @@ class ShardedStepper:
         # S2: shard totals -> all-gather -> local scan with what lies before and after
         totals = [hmc.hmc_potential_totals(c[0], c[3], workspace=self.workspace[i]) for i, c in enumerate(cols)]
         all_totals = [torch.cat(t) for t in comm.all_gather(totals)]
-        if self.push_tables:
+        tabs = None
+        if self.push_tables is not False and hasattr(comm, "table_views"):
+            tabs = comm.table_views(self.n, cols[0][0].device)
+        if self.push_tables and tabs is None:
+            raise RuntimeError("push_tables=True, but the communicator cannot hand out the copies of the table")
+        if tabs is not None:
             # the replicated table filled by the scans themselves: rank d's launch stores its slice of
             # (r, Phi, M) into every rank's copy as it produces it (hmc_potential_shard_push)
-            tabs = comm.table_views(self.n, cols[0][0].device)
             pots = []
             for i, (c, rank) in enumerate(zip(cols, comm.local_ranks)):
                 lo, hi = self.offsets[rank], self.offsets[rank] + self.want[rank]
-                mine = tabs[i]
-                others = [(t["r"][lo:hi], t["phi"][lo:hi], t["m_cum"][lo:hi]) for j, t in enumerate(tabs) if j != i]
+                mine, peers = tabs[i]
+                others = [(t["r"][lo:hi], t["phi"][lo:hi], t["m_cum"][lo:hi]) for t in peers]
                 mine["r"][lo:hi].copy_(c[0])
                 pots.append(hmc.hmc_potential_shard(c[0], c[3], rank, all_totals[i], self.G, phi=mine["phi"][lo:hi],
                                                     m_cum=mine["m_cum"][lo:hi], workspace=self.workspace[i], push=others))
             comm.tables_complete()
-            table_r, table_phi, table_m = [t["r"] for t in tabs], [t["phi"] for t in tabs], [t["m_cum"] for t in tabs]
+            table_r, table_phi, table_m = [t[0]["r"] for t in tabs], [t[0]["phi"] for t in tabs], [t[0]["m_cum"] for t in tabs]
+            self.pushed = True
         else:
+            self.pushed = False
             pots = [hmc.hmc_potential_shard(c[0], c[3], rank, all_totals[i], self.G, workspace=self.workspace[i])
                     for i, (c, rank) in enumerate(zip(cols, comm.local_ranks))]
             # the replicated table
