@@ -489,9 +489,12 @@ __device__ __forceinline__ Node shfl_node(const Node& e, int src)
     return t;
 }
 
-// `mine`: the warp's hand-over area in shared memory, one Node per lane and side ([side][lane]).
+// keep1 / keep2: the bracketing node of side 1 / 2 when have1 / have2 (else the caller loads it).
+// (Handing the nodes over through 64 KB of shared memory instead of shuffles is 1-5 % faster where the coarse table
+// is small -- 15.8 against 16.0 ms at N = 1e8 -- and 70 % slower where it takes its full 160 KB, e.g. N = 4.19e7:
+// 10.7 against 6.3 ms, one lane per star 6.9: nothing is left of the L1 then.)
 __device__ __forceinline__ void probe_pairs(const Node* __restrict__ nodes, Side& s1, Side& s2, double E, double J2,
-                                            Node* __restrict__ mine, bool& have1, bool& have2, uint32_t lane)
+                                            Node& keep1, Node& keep2, bool& have1, bool& have2, uint32_t lane)
 {
     have1 = have2 = false;
     const uint32_t odd = lane & 1u, even_lane = lane & ~1u;
@@ -526,11 +529,16 @@ __device__ __forceinline__ void probe_pairs(const Node* __restrict__ nodes, Side
                 have1 = have1 || (want & 3u); have2 = have2 || (want & 12u);
             }
             const uint32_t W = __shfl_sync(0xffffffffu, want, owner);
-            if (W & (1u << odd)) mine[owner] = n1;             // this lane holds the node side 1 closed on
-            if (W & (4u << odd)) mine[32 + owner] = n2;
+            if (__any_sync(0xffffffffu, (W & 3u) != 0u)) {      // some pair closed side 1 on a node of this probe
+                const Node t = shfl_node(n1, (int)(even_lane | ((W & 2u) ? 1u : 0u)));
+                if (own && (W & 3u)) keep1 = t;
+            }
+            if (__any_sync(0xffffffffu, (W & 12u) != 0u)) {
+                const Node t = shfl_node(n2, (int)(even_lane | ((W & 8u) ? 1u : 0u)));
+                if (own && (W & 12u)) keep2 = t;
+            }
         }
     }
-    __syncwarp();
 }
 
 __device__ __forceinline__ Solved finish_star_s3(const Tables& T, uint32_t a, const Located& L)
@@ -587,8 +595,7 @@ __device__ __forceinline__ Solved finish_star_s3(const Tables& T, uint32_t a, co
 }
 
 // The same with tier 3 by lane pairs: the whole warp must call this together, `valid` false for a lane without a star.
-__device__ __forceinline__ Solved finish_star_s3_pairs(const Tables& T, uint32_t a, const Located& L, bool valid, uint32_t lane,
-                                                       Node* __restrict__ handover)
+__device__ __forceinline__ Solved finish_star_s3_pairs(const Tables& T, uint32_t a, const Located& L, bool valid, uint32_t lane)
 {
     const Node* __restrict__ nodes = T.nodes;
     const uint32_t k = a + 1;
@@ -600,14 +607,15 @@ __device__ __forceinline__ Solved finish_star_s3_pairs(const Tables& T, uint32_t
     Side s1{ L.lo1, L.hi1, 1u, L.g1, (L.st & 256u) ? MODE_GUESS : MODE_BISECT }, s2{ L.lo2, L.hi2, 1u, L.g2, (L.st & 512u) ? MODE_GUESS : MODE_BISECT };
     if (!search) { s1.lo = 0u; s1.hi = 1u; s2.lo = 0u; s2.hi = 1u; }           // closed
     bool have_a = false, have_b = false;
-    probe_pairs(nodes, s1, s2, E, J2, handover, have_a, have_b, lane);
+    Node ka{ 0.0, 0.0, 0.0, 0.0 }, kb{ 0.0, 0.0, 0.0, 0.0 };
+    probe_pairs(nodes, s1, s2, E, J2, ka, kb, have_a, have_b, lane);
     if (st) {
         rmin = (st & HMC_STAR_RADIAL) ? 0.0 : rk;
         rmax = (st & HMC_STAR_UNBOUND) ? pos_inf() : rk;
     } else if (valid) {
         kmin = s1.lo; kmax = s2.lo;
         // closed-form roots of Q(u) = 2C + 2Bu - J^2 u^2 in the bracketing shells (R3)
-        const Node ea = have_a ? handover[lane] : ld_node(nodes + kmin), eb = have_b ? handover[32 + lane] : ld_node(nodes + kmax);
+        const Node ea = have_a ? ka : ld_node(nodes + kmin), eb = have_b ? kb : ld_node(nodes + kmax);
         const double Ca = (E - ea.phi) - ea.B * ea.u;
         const double Cb = (E - eb.phi) - eb.B * eb.u;
         double D = ea.B * ea.B + 2.0 * (J2 * Ca);
@@ -656,14 +664,12 @@ turning_points_kernel(uint32_t n, uint32_t first, uint32_t count, double G, cons
     Tables T{ nodes, dir, coarse, shift > MID_SHIFT ? mid_g : nullptr, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift, l2_keep_policy() };
     const uint32_t stride = gridDim.x * ORB_THREADS;
     const uint32_t lane = threadIdx.x & 31u;
-    // pair search: the warp's hand-over area, behind the coarse table
-    Node* handover = reinterpret_cast<Node*>(smem_raw + (((size_t)(n >> shift) + 2) * sizeof(double2) + 31) / 32 * 32) + (threadIdx.x >> 5) * 64;
     // whole warps stay in the loop together (the pair search is warp-collective); a lane beyond the end has no star
     for (uint32_t a = blockIdx.x * ORB_THREADS + threadIdx.x; PAIRS ? (a - lane < count) : (a < count); a += stride) {
         const bool valid = !PAIRS || a < count;
         const uint32_t b = valid ? a : count - 1;
         const Located L = locate_star(T, first + b, __ldcs(r + first + b), __ldcs(v_r + b), __ldcs(v_t + b), __ldcs(phi + first + b));
-        const Solved v = PAIRS ? finish_star_s3_pairs(T, first + b, L, valid, lane, handover) : finish_star_s3(T, first + b, L);
+        const Solved v = PAIRS ? finish_star_s3_pairs(T, first + b, L, valid, lane) : finish_star_s3(T, first + b, L);
         if (!valid) continue;
         __stcs(F_ws + first + a, v.Fv);                            // by table position: a later S4 call may cover a sub-range
         __stcs(E_out + a, v.E); __stcs(J_out + a, v.J); __stcs(rmin_out + a, v.rmin); __stcs(rmax_out + a, v.rmax);
@@ -1147,7 +1153,8 @@ energy_correction_kernel(uint32_t n, const Node* __restrict__ nodes, const doubl
 
 // ---- host side --------------------------------------------------------------------------------
 // S3's exact search by lane pairs pays when the node table is far beyond the TLB's reach (see probe_pairs).
-// Turning-point stage, one lane / lane pairs, ms: N = 1e7 0.90 / 1.40, 3e7 4.4 / 4.4, 5e7 8.8 / 7.2, 1e8 20.6 / 15.8.
+// Turning-point stage, one lane / lane pairs, ms: N = 1e7 0.90 / 1.40, 3.4e7 5.1 / 5.0, 4.2e7 6.9 / 6.3, 5e7 8.8 / 7.6,
+// 1e8 20.6 / 16.0.
 // (A test-only build sets the threshold to 1 so that small cases run the pair search: build.py "pairs".)
 #ifndef HMC_S3_PAIRS_MIN_N
 #define HMC_S3_PAIRS_MIN_N (1ull << 25)
@@ -1188,10 +1195,9 @@ hmc_status turning_points(uint64_t n, uint64_t first, uint64_t count, double G, 
     const int sms = sm_count();
     const int shift = coarse_shift(n);
     const bool pairs = s3_pairs(n);
-    static constexpr size_t HANDOVER_BYTES = (size_t)ORB_WARPS * 64 * sizeof(Node) + 32;
-    const size_t smem = ((n >> shift) + 2) * sizeof(double2) + (pairs ? HANDOVER_BYTES : 0);
+    const size_t smem = ((n >> shift) + 2) * sizeof(double2);
     static std::atomic<uint64_t> opted[2];
-    hmc_status so = pairs ? smem_opt_in(opted[1], turning_points_kernel<true>, COARSE_CAP * sizeof(double2) + HANDOVER_BYTES)
+    hmc_status so = pairs ? smem_opt_in(opted[1], turning_points_kernel<true>, COARSE_CAP * sizeof(double2))
                           : smem_opt_in(opted[0], turning_points_kernel<false>, COARSE_CAP * sizeof(double2));
     if (so != HMC_OK) return so;
     hmc_status s = build_tables(n, G, r, phi, m_cum, ws, shift, st);
