@@ -268,25 +268,34 @@ __device__ __forceinline__ void stage_coarse(double2* coarse, const double2* __r
     __syncthreads();
 }
 
+// Radii of the coarse nodes in shared memory: either the x components of the (r, Phi) pairs (step 2 doubles) or, in
+// the sampler, an array of their own (step 1; Phi is kept beside it as binary32, see sample_new_radius_kernel).
+struct CoarseR {
+    const double* p;
+    int sh;                  // log2 of the step in doubles
+    __device__ __forceinline__ double operator[](uint32_t c) const { return p[(size_t)c << sh]; }
+};
+
 struct Tables {
     const Node* nodes;       // [n + 2]
     const uint32_t* dir;
-    const double2* coarse;   // shared memory
+    const double2* coarse;   // shared memory: (r, Phi) pairs, or nullptr when only the radii are there (cr)
     const double2* mid;      // global (L2): (r, Phi) of every 2^MID_SHIFT-th node when shift > MID_SHIFT, else nullptr
     double r_last;           // r_N
     uint32_t n, ncoarse, K;
     int shift;
     uint64_t keep;           // L2 evict-last policy for directory loads
+    CoarseR cr;              // radii of the coarse nodes
     // (r, Phi) of node j, j a multiple of the finest table spacing in use
     __device__ __forceinline__ double2 aligned_node(uint32_t j) const { return mid ? ld_d2_na(mid + (j >> MID_SHIFT)) : coarse[j >> shift]; }
     // upper radius of coarse interval c, as build_dir_kernel defines it
-    __device__ __forceinline__ double interval_rh(uint32_t c) const { return c < ncoarse ? coarse[c + 1].x : r_last; }
+    __device__ __forceinline__ double interval_rh(uint32_t c) const { return c < ncoarse ? cr[c + 1] : r_last; }
     // nodes lo < hi with  r_lo <= x < r_hi  as far as the directory knows: every node of interval c
     // outside (lo, hi) is on the side stated.  x must lie in the radius range of interval c for the
     // result to be tight; for any x it is a valid starting point of an exact search.
     __device__ __forceinline__ void dir_range(uint32_t c, double x, uint32_t& lo, uint32_t& hi) const
     {
-        const double Rl = coarse[c].x;
+        const double Rl = cr[c];
         const uint32_t b = bucket(x, Rl, bucket_scale(Rl, interval_rh(c), K), K);
         const uint32_t w = ld_u32_keep(dir + (size_t)c * K + b, keep);
         const uint32_t o0 = w & 0xffffu, o1 = w >> 16;
@@ -299,7 +308,7 @@ struct Tables {
     // In two halves, so that a caller with two radii can have both directory loads in flight at once.
     __device__ __forceinline__ const uint32_t* dir_guess_slot(uint32_t c, double x, float& frac) const
     {
-        const double Rl = coarse[c].x;
+        const double Rl = cr[c];
         const float scale = bucket_scale(Rl, interval_rh(c), K);
         const uint32_t b = bucket(x, Rl, scale, K);
         frac = fminf(fmaxf((float)(x - Rl) * scale - (float)b, 0.0f), 1.0f);
@@ -661,7 +670,7 @@ turning_points_kernel(uint32_t n, uint32_t first, uint32_t count, double G, cons
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* coarse = reinterpret_cast<double2*>(smem_raw);
     stage_coarse(coarse, coarse_g, n, shift);
-    Tables T{ nodes, dir, coarse, shift > MID_SHIFT ? mid_g : nullptr, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift, l2_keep_policy() };
+    Tables T{ nodes, dir, coarse, shift > MID_SHIFT ? mid_g : nullptr, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift, l2_keep_policy(), CoarseR{ reinterpret_cast<const double*>(coarse), 1 } };
     const uint32_t stride = gridDim.x * ORB_THREADS;
     const uint32_t lane = threadIdx.x & 31u;
     // whole warps stay in the loop together (the pair search is warp-collective); a lane beyond the end has no star
@@ -710,12 +719,12 @@ __device__ __forceinline__ Trial make_trial(const Orbit& o, uint32_t seed_lo, ui
 }
 
 // coarse interval of r0, clamped to the orbit's own: largest c in [cl, ch] with coarse[c].r <= r0
-__device__ __forceinline__ uint32_t coarse_locate(const double2* coarse, uint32_t cl, uint32_t ch, double r0)
+__device__ __forceinline__ uint32_t coarse_locate(const CoarseR coarse, uint32_t cl, uint32_t ch, double r0)
 {
     uint32_t lo = cl, hi = ch + 1;
     while (hi - lo > 1) {
         uint32_t m = (lo + hi) >> 1;
-        if (coarse[m].x <= r0) lo = m; else hi = m;
+        if (coarse[m] <= r0) lo = m; else hi = m;
     }
     return lo;
 }
@@ -738,7 +747,7 @@ struct InvTable {
 };
 
 // built by the whole CTA after stage_coarse; r_first, r_last: the radii of nodes 1 and N
-__device__ __forceinline__ InvTable build_inv(uint16_t* inv, const double2* coarse, uint32_t ncoarse, double r_first, double r_last)
+__device__ __forceinline__ InvTable build_inv(uint16_t* inv, const CoarseR coarse, uint32_t ncoarse, double r_first, double r_last)
 {
     InvTable t;
     const int h1 = __double2hiint(r_first), hn = __double2hiint(r_last);
@@ -752,7 +761,7 @@ __device__ __forceinline__ InvTable build_inv(uint16_t* inv, const double2* coar
             const double x = __hiloint2double((int)hw, 0);
             lo = 0;
             uint32_t hi = ncoarse + 1;
-            while (hi - lo > 1) { const uint32_t m = (lo + hi) >> 1; if (coarse[m].x <= x) lo = m; else hi = m; }
+            while (hi - lo > 1) { const uint32_t m = (lo + hi) >> 1; if (coarse[m] <= x) lo = m; else hi = m; }
         }
         inv[q] = (uint16_t)lo;
     }
@@ -760,13 +769,13 @@ __device__ __forceinline__ InvTable build_inv(uint16_t* inv, const double2* coar
     return t;
 }
 
-__device__ __forceinline__ uint32_t coarse_locate(const double2* coarse, const InvTable& iv, uint32_t cl, uint32_t ch, double r0)
+__device__ __forceinline__ uint32_t coarse_locate(const CoarseR coarse, const InvTable& iv, uint32_t cl, uint32_t ch, double r0)
 {
     const uint32_t q = iv.key(r0);
     uint32_t lo = iv.inv[q], hi = (uint32_t)iv.inv[q + 1] + 1;               // coarse[lo].r <= r0 < coarse[hi].r, or r0 < coarse[1].r
     while (hi - lo > 1) {
         const uint32_t m = (lo + hi) >> 1;
-        if (coarse[m].x <= r0) lo = m; else hi = m;
+        if (coarse[m] <= r0) lo = m; else hi = m;
     }
     return min(max(lo, cl), ch);
 }
@@ -820,7 +829,7 @@ __device__ __noinline__ Exhaustive draw_exhaustive(Tables T, InvTable iv, Orbit 
     for (; t < HMC_T_MAX; ++t) {
         Trial tr = make_trial(o, seed_lo, seed_hi, step, t);
         double Q0, g;
-        exact_trial(T, o, tr, coarse_locate(T.coarse, iv, cl, ch, tr.r0), Q0, g);
+        exact_trial(T, o, tr, coarse_locate(T.cr, iv, cl, ch, tr.r0), Q0, g);
         if (Q0 > 0.0) {
             x.have_good = true; x.good_r = tr.r0; x.good_Q = Q0; x.good_w3 = tr.w3;
             if (g > o.F) x.st |= HMC_STAR_CLIPPED;
@@ -977,10 +986,35 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (io.step_dev) step += __ldg(io.step_dev);
     Park& pk = reinterpret_cast<Park*>(smem_raw)[threadIdx.x >> 5];
-    double2* coarse = reinterpret_cast<double2*>(smem_raw + ORB_WARPS * sizeof(Park));
-    stage_coarse(coarse, coarse_g, n, shift);
-    Tables T{ nodes, dir, coarse, (FUSED && shift > MID_SHIFT) ? mid_g : nullptr, __ldg(io.r + (n - 1)), n, n >> shift, 1u << shift, shift, l2_keep_policy() };
-    const InvTable iv = build_inv(reinterpret_cast<uint16_t*>(coarse + (n >> shift) + 2), coarse, T.ncoarse, __ldg(io.r), T.r_last);
+    // The coarse table.  Fused kernel: (r, Phi) pairs as in S3 (its search needs Phi exactly).  Sampler proper: the
+    // radii as binary64 (they decide the coarse interval, hence the directory row, exactly) and Phi as binary32 beside
+    // them: Phi is only used by the squeeze, whose bracket of Phi(r0) is a coarse interval wide (1e-4 relative) and is
+    // simply widened by the binary32 rounding.  12 instead of 16 bytes per entry leave 39 KB more of the SM's 256 KB
+    // to the L1 at N = 1e7, which this kernel's spills and streamed loads need: with a full table next to the
+    // parking area nothing was left (sampling, ns per star: 0.0715 at N = 8e6, 0.0785 at 1.04e7, 0.0694 at 1.06e7).
+    const uint32_t nc2 = (n >> shift) + 2;
+    double2* coarse = nullptr;
+    double* coarse_r = nullptr;
+    float* coarse_phi = nullptr;
+    unsigned char* after;
+    if (FUSED) {
+        coarse = reinterpret_cast<double2*>(smem_raw + ORB_WARPS * sizeof(Park));
+        stage_coarse(coarse, coarse_g, n, shift);
+        after = reinterpret_cast<unsigned char*>(coarse + nc2);
+    } else {
+        coarse_r = reinterpret_cast<double*>(smem_raw + ORB_WARPS * sizeof(Park));
+        coarse_phi = reinterpret_cast<float*>(coarse_r + nc2);
+        for (uint32_t c = threadIdx.x; c + 1 < nc2; c += ORB_THREADS) {
+            const double2 e = __ldg(coarse_g + c);
+            coarse_r[c] = e.x; coarse_phi[c] = (float)e.y;
+        }
+        if (threadIdx.x == 0) { coarse_r[nc2 - 1] = pos_inf(); coarse_phi[nc2 - 1] = 0.0f; }
+        __syncthreads();
+        after = reinterpret_cast<unsigned char*>(coarse_phi + ((nc2 + 1u) & ~1u));
+    }
+    const CoarseR cr = FUSED ? CoarseR{ reinterpret_cast<const double*>(coarse), 1 } : CoarseR{ coarse_r, 0 };
+    Tables T{ nodes, dir, coarse, (FUSED && shift > MID_SHIFT) ? mid_g : nullptr, __ldg(io.r + (n - 1)), n, n >> shift, 1u << shift, shift, l2_keep_policy(), cr };
+    const InvTable iv = build_inv(reinterpret_cast<uint16_t*>(after), cr, T.ncoarse, __ldg(io.r), T.r_last);
     unsigned long long my_trials = 0;
     const unsigned lane_lt = lanemask_lt();
     const uint32_t lane = threadIdx.x & 31;
@@ -1042,17 +1076,24 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
         for (int round = 0; round < FRONT_ROUNDS; ++round) {
             if (have && !candidate && t < HMC_T_MAX) {
                 tr = make_trial(o, seed_lo, seed_hi, step, t);
-                c = coarse_locate(coarse, iv, cl, ch, tr.r0);
+                c = coarse_locate(cr, iv, cl, ch, tr.r0);
                 ++t;
                 // squeeze: Phi(r0) lies in [coarse[c].Phi, coarse[c+1].Phi]; everything widened by ~1e-11.
                 // Written multiplied through by r0^2 > 0, so there is no division on this path.
                 const double r2 = tr.r0 * tr.r0;
-                const double top = 2.0 * (o.E - coarse[c].y) * r2;
+                double phi_lo, phi_hi;                                      // Phi_c <= Phi(r0) <= Phi_{c+1}, bounded from outside
+                if (FUSED) { phi_lo = coarse[c].y; phi_hi = coarse[c + 1].y; }
+                else {      // binary32 copies: off by at most 2^-24 relative (or 2^-150 absolute); widened by twice that
+                    const double a = (double)coarse_phi[c], b = (double)coarse_phi[c + 1];
+                    phi_lo = a - (1.25e-7 * fabs(a) + 3e-45);
+                    phi_hi = b + (1.25e-7 * fabs(b) + 3e-45);
+                }
+                const double top = 2.0 * (o.E - phi_lo) * r2;
                 const double tol = 1e-11 * (fabs(top) + o.J2);
                 const double Qh = (top - o.J2) + tol;                       // upper bound of r0^2 Q0
-                candidate = Qh > 0.0;
+                candidate = !(Qh <= 0.0);                                   // (a NaN from overflowing bounds keeps the trial)
                 if (candidate) {
-                    const double Ql = (2.0 * (o.E - coarse[c + 1].y) * r2 - o.J2) - tol;   // lower bound of r0^2 Q0
+                    const double Ql = (2.0 * (o.E - phi_hi) * r2 - o.J2) - tol;   // lower bound of r0^2 Q0
                     const double fx = o.F * tr.Xp, cc = o.three_q * (1.0 - tr.s * tr.s);
                     if (Ql > 0.0 && (fx * fx) * Ql > ((cc * cc) * r2) * (1.0 + 1e-10)) candidate = false;   // F X' > g for certain
                 }
@@ -1119,14 +1160,14 @@ energy_correction_kernel(uint32_t n, const Node* __restrict__ nodes, const doubl
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* coarse = reinterpret_cast<double2*>(smem_raw);
     stage_coarse(coarse, coarse_g, n, shift);
-    Tables T{ nodes, dir, coarse, nullptr, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift, l2_keep_policy() };
+    Tables T{ nodes, dir, coarse, nullptr, __ldg(r + (n - 1)), n, n >> shift, 1u << shift, shift, l2_keep_policy(), CoarseR{ reinterpret_cast<const double*>(coarse), 1 } };
     const uint32_t stride = gridDim.x * ORB_THREADS;
     for (uint32_t a = blockIdx.x * ORB_THREADS + threadIdx.x; a < n; a += stride) {
         const double x = __ldcs(r_old + a);
         double vr = __ldcs(v_r + a), vt = __ldcs(v_t + a);
         const double E = __ldcs(E_old + a), po = __ldcs(p_old + a), ph = __ldcs(phi + a);
         // shell of r_old in the new table: j = #{ i : r_i <= x }, 0 .. n
-        const uint32_t c = coarse_locate(coarse, 0u, T.ncoarse, x);
+        const uint32_t c = coarse_locate(T.cr, 0u, T.ncoarse, x);
         uint32_t lo, hi;
         if (shift == 0) { lo = c; hi = c + 1; }
         else T.dir_range(c, x, lo, hi);
@@ -1221,7 +1262,9 @@ static hmc_status launch_sampler(bool fused, uint64_t n, double G, uint64_t seed
 {
     const int sms = sm_count();
     static constexpr size_t INV_BYTES = (INV_CELLS + 2) * sizeof(uint16_t);
-    const size_t smem = ORB_WARPS * sizeof(Park) + ((n >> shift) + 2) * sizeof(double2) + INV_BYTES;
+    // fused: (r, Phi) pairs; sampler proper: radii as binary64 + Phi as binary32 (an even number of them)
+    const size_t nc2 = (n >> shift) + 2;
+    const size_t smem = ORB_WARPS * sizeof(Park) + (fused ? nc2 * sizeof(double2) : nc2 * sizeof(double) + ((nc2 + 1) & ~(size_t)1) * sizeof(float)) + INV_BYTES;
     static std::atomic<uint64_t> opted[2];
     const size_t cap = ORB_WARPS * sizeof(Park) + COARSE_CAP * sizeof(double2) + INV_BYTES;
     hmc_status so = fused ? smem_opt_in(opted[1], sample_new_radius_kernel<true>, cap)
