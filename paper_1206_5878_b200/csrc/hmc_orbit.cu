@@ -734,27 +734,33 @@ __device__ __forceinline__ uint32_t coarse_locate(const CoarseR coarse, uint32_t
 // mantissa bits: monotone in r), INV_CELLS + 1 keys from that of r_1 on; inv[q] = largest coarse index whose
 // radius is <= the smallest radius of key q.  The interval of r0 then lies in [inv[q], inv[q + 1]]: a handful of
 // coarse entries instead of the orbit's few thousand.
-static constexpr uint32_t INV_CELLS = 2048;
+#ifndef HMC_INV_CELLS_S4
+#define HMC_INV_CELLS_S4 4096        // 2048: 0.705 ms, 4096: 0.699, 8192: 0.694 (and 2 us more set-up per launch), 16384: 0.750 at N = 1e7
+#endif
+static constexpr uint32_t INV_CELLS = 2048;            // fused kernel
+static constexpr uint32_t INV_CELLS_S4 = HMC_INV_CELLS_S4;   // sampler proper
 
 struct InvTable {
     const uint16_t* inv;     // shared memory, [INV_CELLS + 2]
     int base, sh;
+    uint32_t cells;
     __device__ __forceinline__ uint32_t key(double x) const
     {
         const int q = (__double2hiint(x) >> sh) - base;
-        return (uint32_t)min(max(q, 0), (int)INV_CELLS - 1);
+        return (uint32_t)min(max(q, 0), (int)cells - 1);
     }
 };
 
 // built by the whole CTA after stage_coarse; r_first, r_last: the radii of nodes 1 and N
-__device__ __forceinline__ InvTable build_inv(uint16_t* inv, const CoarseR coarse, uint32_t ncoarse, double r_first, double r_last)
+__device__ __forceinline__ InvTable build_inv(uint16_t* inv, uint32_t cells, const CoarseR coarse, uint32_t ncoarse, double r_first, double r_last)
 {
     InvTable t;
+    t.cells = cells;
     const int h1 = __double2hiint(r_first), hn = __double2hiint(r_last);
     int sh = 0;
-    while ((hn >> sh) - (h1 >> sh) > (int)INV_CELLS - 1) ++sh;
+    while ((hn >> sh) - (h1 >> sh) > (int)cells - 1) ++sh;
     t.sh = sh; t.base = h1 >> sh; t.inv = inv;
-    for (uint32_t q = threadIdx.x; q <= INV_CELLS; q += ORB_THREADS) {
+    for (uint32_t q = threadIdx.x; q <= cells; q += ORB_THREADS) {
         const long long hw = ((long long)q + t.base) << sh;                   // leading word of the smallest radius of key q
         uint32_t lo = ncoarse;
         if (hw < 0x7ff00000ll) {
@@ -1014,7 +1020,7 @@ sample_new_radius_kernel(uint32_t n, double G, uint32_t seed_lo, uint32_t seed_h
     }
     const CoarseR cr = FUSED ? CoarseR{ reinterpret_cast<const double*>(coarse), 1 } : CoarseR{ coarse_r, 0 };
     Tables T{ nodes, dir, coarse, (FUSED && shift > MID_SHIFT) ? mid_g : nullptr, __ldg(io.r + (n - 1)), n, n >> shift, 1u << shift, shift, l2_keep_policy(), cr };
-    const InvTable iv = build_inv(reinterpret_cast<uint16_t*>(after), cr, T.ncoarse, __ldg(io.r), T.r_last);
+    const InvTable iv = build_inv(reinterpret_cast<uint16_t*>(after), FUSED ? INV_CELLS : INV_CELLS_S4, cr, T.ncoarse, __ldg(io.r), T.r_last);
     unsigned long long my_trials = 0;
     const unsigned lane_lt = lanemask_lt();
     const uint32_t lane = threadIdx.x & 31;
@@ -1261,12 +1267,12 @@ static hmc_status launch_sampler(bool fused, uint64_t n, double G, uint64_t seed
                                  const Workspace& ws, cudaStream_t st)
 {
     const int sms = sm_count();
-    static constexpr size_t INV_BYTES = (INV_CELLS + 2) * sizeof(uint16_t);
+    const size_t inv_bytes = ((fused ? INV_CELLS : INV_CELLS_S4) + 2) * sizeof(uint16_t);
     // fused: (r, Phi) pairs; sampler proper: radii as binary64 + Phi as binary32 (an even number of them)
     const size_t nc2 = (n >> shift) + 2;
-    const size_t smem = ORB_WARPS * sizeof(Park) + (fused ? nc2 * sizeof(double2) : nc2 * sizeof(double) + ((nc2 + 1) & ~(size_t)1) * sizeof(float)) + INV_BYTES;
+    const size_t smem = ORB_WARPS * sizeof(Park) + (fused ? nc2 * sizeof(double2) : nc2 * sizeof(double) + ((nc2 + 1) & ~(size_t)1) * sizeof(float)) + inv_bytes;
     static std::atomic<uint64_t> opted[2];
-    const size_t cap = ORB_WARPS * sizeof(Park) + COARSE_CAP * sizeof(double2) + INV_BYTES;
+    const size_t cap = ORB_WARPS * sizeof(Park) + COARSE_CAP * (fused ? sizeof(double2) : sizeof(double) + sizeof(float)) + inv_bytes;
     hmc_status so = fused ? smem_opt_in(opted[1], sample_new_radius_kernel<true>, cap)
                           : smem_opt_in(opted[0], sample_new_radius_kernel<false>, cap);
     if (so != HMC_OK) return so;
