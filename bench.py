@@ -336,13 +336,18 @@ def run_gpu(args, cfg):
         hmc.hmc_potential(so["r"], so["m"], stepper.G, phi=stepper.phi, m_cum=stepper.m_cum, workspace=stepper.workspace)
         ev[2].record(stream)
         if args.fused:
+            ev[5].record(stream)
             ev[3].record(stream)      # "turning_points" reads 0; "sampling" is the fused S3 + S4 call
             hmc.hmc_orbit_step(so["r"], so["v_r"], so["v_t"], stepper.phi, stepper.m_cum, so["id"], stepper.seed,
                                stepper.step_index, stepper.G, tp=stepper.tp, out=stepper.sample,
                                counters=stepper.counters, workspace=stepper.workspace)
         else:
+            # S3 as its two launches, with an event between them: hmc_orbit_build_tables + hmc_orbit_turning_points_prebuilt
+            # are exactly what hmc_orbit_turning_points does; the event lets turning_points_kernel be timed by itself
+            hmc.hmc_orbit_build_tables(so["r"], stepper.phi, stepper.m_cum, stepper.G, workspace=stepper.workspace)
+            ev[5].record(stream)
             hmc.hmc_orbit_turning_points(so["r"], so["v_r"], so["v_t"], stepper.phi, stepper.m_cum, stepper.G,
-                                         out=stepper.tp, counters=stepper.counters, workspace=stepper.workspace)
+                                         out=stepper.tp, counters=stepper.counters, workspace=stepper.workspace, prebuilt=True)
             ev[3].record(stream)
             hmc.hmc_sample_new_radius(so["r"], stepper.phi, stepper.m_cum, so["v_r"], so["v_t"], stepper.tp, so["id"],
                                       stepper.seed, stepper.step_index, stepper.G, out=stepper.sample,
@@ -356,7 +361,7 @@ def run_gpu(args, cfg):
         s["id"], so["id"] = so["id"], s["id"]
         stepper.step_index += 1
 
-    mk = lambda: [torch.cuda.Event(enable_timing=True) for _ in range(5)]
+    mk = lambda: [torch.cuda.Event(enable_timing=True) for _ in range(6)]      # 0-4: stage boundaries, 5: after the table build
     for _ in range(args.warmup):
         staged_step(mk())
     torch.cuda.synchronize()
@@ -399,6 +404,7 @@ def run_gpu(args, cfg):
     ms_total = t_start.elapsed_time(t_end)
     value, ms_max = aggregate_throughput(float(n) * args.steps, ms_total, devs)
     stage_ms = {name: sum(e[i].elapsed_time(e[i + 1]) for e in evs) / args.steps for i, name in enumerate(STAGES)}
+    s3_kernel_ms = sum(e[5].elapsed_time(e[3]) for e in evs) / args.steps      # turning_points_kernel alone
     counters = {k: int(v) for k, v in zip(hmc.COUNTER_NAMES, stepper.counters.cpu().tolist())}
 
     # ---- end to end through the host-buffer C-ABI call: pinned host inputs in, results out, every step
@@ -445,24 +451,32 @@ def run_gpu(args, cfg):
     # around that call, recorded on the launching stream, time exactly that kernel, once per step.
     model = algorithmic_bytes_per_star(n)
     peak, peak_src = measured_peak_gbs()
-    dom, dom_kernel = "sampling", "sample_new_radius_kernel"
-    achieved = model[dom] * n / (stage_ms[dom] * 1e-3) / 1e9
+    # The two long launches of a step, each timed exactly by the events around its call; the longer one is reported.
+    cand = {"sampling": ("sample_new_radius_kernel", stage_ms["sampling"])}
+    if not args.fused:
+        cand["turning_points"] = ("turning_points_kernel", s3_kernel_ms)
+    dom = max(cand, key=lambda k: cand[k][1])
+    dom_kernel, dom_ms = cand[dom]
+    achieved = model[dom] * n / (dom_ms * 1e-3) / 1e9
     traffic, capture = ncu_traffic_bytes(dom_kernel, n)
     roofline = dict(bound="hbm", kernel=dom_kernel, stage=dom, achieved=achieved, peak=peak, unit="GB/s",
                     frac=achieved / peak, traffic=traffic, peak_source=peak_src,
-                    algorithmic_bytes_per_star=model[dom], stars_per_launch=n, launch_ms=stage_ms[dom],
+                    algorithmic_bytes_per_star=model[dom], stars_per_launch=n, launch_ms=dom_ms,
                     launches_timed=args.steps,
                     # `achieved` / `frac` are SURVEY.md 8(d)'s ALGORITHMIC bytes over the measured launch time: a model
                     # fraction (one table entry per probe of the paper's bisection; this kernel serves most probes from
                     # shared memory).  What the launch physically moved, by ncu, over the same measured time:
                     model_frac=achieved / peak,
-                    physical=(dict(dram_bytes_per_launch=traffic, achieved=traffic / (stage_ms[dom] * 1e-3) / 1e9,
-                                   frac=traffic / (stage_ms[dom] * 1e-3) / 1e9 / peak, capture=capture,
+                    physical=(dict(dram_bytes_per_launch=traffic, achieved=traffic / (dom_ms * 1e-3) / 1e9,
+                                   frac=traffic / (dom_ms * 1e-3) / 1e9 / peak, capture=capture,
                                    limiter="not streamed bytes: 8 warps per scheduler of dependent fp64 chains and loads "
-                                           "(ncu: issue slots 50 % used, DRAM 34 % busy; profiles/r2b.md, DESIGN.md 5 and 5a)")
+                                           "(ncu: issue slots 50-54 % used), for turning_points_kernel together with the "
+                                           "rate of random 128-byte DRAM lines (profiles/r2b.md, DESIGN.md 5 and 5a)")
                               if traffic else None),
                     # what ncu shows the kernel waits for, as opposed to the roofline the metric is quoted against
-                    bound_observed="issue / dependent-instruction latency at 32 warps per SM")
+                    bound_observed="issue / dependent-instruction latency at 32 warps per SM",
+                    other_long_launch={k: dict(kernel=v[0], launch_ms=v[1], model_frac=model[k] * n / (v[1] * 1e-3) / 1e9 / peak)
+                                       for k, v in cand.items() if k != dom})
     orbit_ms = stage_ms["potential"] + stage_ms["turning_points"] + stage_ms["sampling"]
     orbit_bytes = model["potential"] + model["turning_points"] + model["sampling"]
     stages = {s: dict(ms=stage_ms[s], stars_per_s=n / (stage_ms[s] * 1e-3), algorithmic_bytes_per_star=model[s],

@@ -359,6 +359,26 @@ HMC_API hmc_status hmc_orbit_turning_points_range(uint64_t n, uint64_t first, ui
         uint64_t* counters,
         void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/*
+ * The table build of S3 / S4 as a call of its own, and S3 on tables already built.  Every hmc_orbit_turning_points
+ * call starts by deriving its search tables (node table, coarse table, radius directory: DESIGN.md section 4) from
+ * (r_sorted, phi, m_cum) into the workspace; hmc_orbit_build_tables does just that, and
+ * hmc_orbit_turning_points_prebuilt is hmc_orbit_turning_points_range without it (the tables in the workspace must be
+ * those of the same r_sorted, phi, m_cum, G).  The pair computes exactly what the one call computes, with the same two
+ * launches; it exists so that the ranges of a table can be searched without rebuilding it, and so that bench.py can
+ * put a CUDA event between the two launches and time turning_points_kernel by itself.
+ */
+HMC_API hmc_status hmc_orbit_build_tables(uint64_t n, double G, const double* r_sorted, const double* phi, const double* m_cum,
+        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+HMC_API hmc_status hmc_orbit_turning_points_prebuilt(uint64_t n, uint64_t first, uint64_t count, double G,
+        const double* r_sorted, const double* v_r, const double* v_t,
+        const double* phi, const double* m_cum,
+        double* E, double* J, double* r_min, double* r_max,
+        uint32_t* k_min, uint32_t* k_max, uint8_t* star_status,
+        uint64_t* counters,
+        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 HMC_API hmc_status hmc_sample_new_radius_range(uint64_t n, uint64_t first, uint64_t count, double G, uint64_t seed, uint32_t step,
         const double* r_sorted, const double* phi, const double* m_cum,
         const double* v_r, const double* v_t,

@@ -383,6 +383,39 @@ hmc_status hmc_orbit_turning_points_range(uint64_t n, uint64_t first, uint64_t c
                           counters, carve(workspace, n), static_cast<cudaStream_t>(cuda_stream));
 }
 
+hmc_status hmc_orbit_build_tables(uint64_t n, double G, const double* r_sorted, const double* phi, const double* m_cum,
+                                  void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (n > HMC_MAX_N) return HMC_ERR_SIZE;
+    if (n == 0) return HMC_OK;
+    REQUIRE_PTR(r_sorted); REQUIRE_PTR(phi); REQUIRE_PTR(m_cum);
+    REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(phi, 8); REQUIRE_ALIGN(m_cum, 8);
+    hmc_status s = check_ws(workspace, workspace_bytes, n);
+    if (s != HMC_OK) return s;
+    return orbit_build_tables(n, G, r_sorted, phi, m_cum, carve(workspace, n), static_cast<cudaStream_t>(cuda_stream));
+}
+
+hmc_status hmc_orbit_turning_points_prebuilt(uint64_t n, uint64_t first, uint64_t count, double G, const double* r_sorted,
+                                          const double* v_r, const double* v_t, const double* phi, const double* m_cum,
+                                          double* E, double* J, double* r_min, double* r_max, uint32_t* k_min,
+                                          uint32_t* k_max, uint8_t* star_status, uint64_t* counters, void* workspace,
+                                          size_t workspace_bytes, void* cuda_stream)
+{
+    if (n > HMC_MAX_N || first > n || count > n - first) return HMC_ERR_SIZE;
+    if (n == 0 || count == 0) return HMC_OK;
+    REQUIRE_PTR(r_sorted); REQUIRE_PTR(v_r); REQUIRE_PTR(v_t); REQUIRE_PTR(phi); REQUIRE_PTR(m_cum);
+    REQUIRE_PTR(E); REQUIRE_PTR(J); REQUIRE_PTR(r_min); REQUIRE_PTR(r_max); REQUIRE_PTR(k_min); REQUIRE_PTR(k_max);
+    REQUIRE_PTR(star_status);
+    REQUIRE_ALIGN(r_sorted, 8); REQUIRE_ALIGN(v_r, 8); REQUIRE_ALIGN(v_t, 8); REQUIRE_ALIGN(phi, 8);
+    REQUIRE_ALIGN(m_cum, 8); REQUIRE_ALIGN(E, 8); REQUIRE_ALIGN(J, 8); REQUIRE_ALIGN(r_min, 8);
+    REQUIRE_ALIGN(r_max, 8); REQUIRE_ALIGN(k_min, 4); REQUIRE_ALIGN(k_max, 4);
+    if (counters) REQUIRE_ALIGN(counters, 8);
+    hmc_status s = check_ws(workspace, workspace_bytes, n);
+    if (s != HMC_OK) return s;
+    return turning_points(n, first, count, G, r_sorted, v_r, v_t, phi, m_cum, E, J, r_min, r_max, k_min, k_max, star_status,
+                          counters, carve(workspace, n), static_cast<cudaStream_t>(cuda_stream), true);
+}
+
 hmc_status hmc_sample_new_radius_range(uint64_t n, uint64_t first, uint64_t count, double G, uint64_t seed, uint32_t step,
                                        const double* r_sorted, const double* phi, const double* m_cum, const double* v_r,
                                        const double* v_t, const double* E, const double* J, const double* r_min,

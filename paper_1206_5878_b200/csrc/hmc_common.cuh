@@ -250,7 +250,9 @@ hmc_status partition_points(uint64_t n, const double* r_sorted, uint32_t nsplit,
 hmc_status turning_points(uint64_t n, uint64_t first, uint64_t count, double G, const double* r, const double* v_r, const double* v_t,
                           const double* phi, const double* m_cum, double* E, double* J, double* r_min,
                           double* r_max, uint32_t* k_min, uint32_t* k_max, uint8_t* status, uint64_t* counters,
-                          const Workspace& ws, cudaStream_t st);
+                          const Workspace& ws, cudaStream_t st, bool reuse_tables = false);
+hmc_status orbit_build_tables(uint64_t n, double G, const double* r, const double* phi, const double* m_cum, const Workspace& ws,
+                              cudaStream_t st);
 hmc_status sample_new_radius(uint64_t n, uint64_t first, uint64_t count, double G, uint64_t seed, uint32_t step, const double* r,
                              const double* phi, const double* m_cum, const double* v_r, const double* v_t,
                              const double* E, const double* J, const double* r_min, const double* r_max,

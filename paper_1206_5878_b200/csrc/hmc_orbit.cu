@@ -1237,7 +1237,7 @@ static hmc_status build_tables(uint64_t n, double G, const double* r, const doub
 hmc_status turning_points(uint64_t n, uint64_t first, uint64_t count, double G, const double* r, const double* v_r, const double* v_t,
                           const double* phi, const double* m_cum, double* E, double* J, double* r_min,
                           double* r_max, uint32_t* k_min, uint32_t* k_max, uint8_t* status, uint64_t* counters,
-                          const Workspace& ws, cudaStream_t st)
+                          const Workspace& ws, cudaStream_t st, bool reuse_tables)
 {
     const int sms = sm_count();
     const int shift = coarse_shift(n);
@@ -1247,7 +1247,7 @@ hmc_status turning_points(uint64_t n, uint64_t first, uint64_t count, double G, 
     hmc_status so = pairs ? smem_opt_in(opted[1], turning_points_kernel<true>, COARSE_CAP * sizeof(double2))
                           : smem_opt_in(opted[0], turning_points_kernel<false>, COARSE_CAP * sizeof(double2));
     if (so != HMC_OK) return so;
-    hmc_status s = build_tables(n, G, r, phi, m_cum, ws, shift, st);
+    hmc_status s = reuse_tables ? HMC_OK : build_tables(n, G, r, phi, m_cum, ws, shift, st);
     if (s != HMC_OK) return s;
     if (count == 0) return HMC_OK;
     const int blocks = (int)umin64((count + ORB_THREADS - 1) / ORB_THREADS, (uint64_t)sms);
@@ -1342,6 +1342,13 @@ hmc_status add_u32(uint32_t* p, uint32_t inc, cudaStream_t st)
     add_u32_kernel<<<1, 1, 0, st>>>(p, inc);
     HMC_LAUNCH_CHECK();
     return HMC_OK;
+}
+
+// the tables alone (what every S3 call and an S4 call without reuse_tables start with)
+hmc_status orbit_build_tables(uint64_t n, double G, const double* r, const double* phi, const double* m_cum, const Workspace& ws,
+                              cudaStream_t st)
+{
+    return build_tables(n, G, r, phi, m_cum, ws, coarse_shift(n), st);
 }
 
 // S3 + S4 in one launch: same outputs as the two calls.

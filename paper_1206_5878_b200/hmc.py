@@ -50,7 +50,8 @@ def load(path: str) -> ctypes.CDLL:
                  "hmc_orbit_step", "hmc_diagnostics", "hmc_energy_correction", "hmc_step_host", "hmc_potential_totals",
                  "hmc_potential_shard", "hmc_partition_points", "hmc_orbit_turning_points_range",
                  "hmc_sample_new_radius_range", "hmc_relaxation_timestep", "hmc_two_body_relaxation",
-                 "hmc_sample_new_radius_dstep", "hmc_add_u32", "hmc_potential_shard_push"):
+                 "hmc_sample_new_radius_dstep", "hmc_add_u32", "hmc_potential_shard_push", "hmc_orbit_build_tables",
+                 "hmc_orbit_turning_points_prebuilt"):
         getattr(L, name).restype = ctypes.c_int32
     return L
 
@@ -139,8 +140,18 @@ def hmc_potential(r_sorted: torch.Tensor, m_sorted: torch.Tensor, G: float = 1.0
     return phi, m_cum
 
 
+def hmc_orbit_build_tables(r_sorted, phi, m_cum, G: float = 1.0, *, workspace):
+    """The search tables of S3 / S4 into the workspace (what hmc_orbit_turning_points starts with)."""
+    n = r_sorted.numel()
+    workspace, wp, wb = _ws(workspace, n, r_sorted.device)
+    f = torch.float64
+    _check(lib().hmc_orbit_build_tables(ctypes.c_uint64(n), ctypes.c_double(G), _dev(r_sorted, f, n, "r_sorted"),
+                                        _dev(phi, f, n, "phi"), _dev(m_cum, f, n, "m_cum"), wp, wb, _stream()),
+           "hmc_orbit_build_tables")
+
+
 def hmc_orbit_turning_points(r_sorted, v_r, v_t, phi, m_cum, G: float = 1.0, *, out=None, counters=None,
-                             workspace=None, first: Optional[int] = None):
+                             workspace=None, first: Optional[int] = None, prebuilt: bool = False):
     """S3 (PAPER.md:117-124).  -> dict(E, J, r_min, r_max, k_min, k_max, status)
     ``first`` given (sharded step): hmc_orbit_turning_points_range -- r_sorted, phi, m_cum are the table [n], v_r and
     v_t the stars at positions first .. first + len(v_r) - 1 of it; outputs have that length."""
@@ -153,6 +164,9 @@ def hmc_orbit_turning_points(r_sorted, v_r, v_t, phi, m_cum, G: float = 1.0, *, 
     f = torch.float64
     head = (ctypes.c_uint64(n),) if first is None else (ctypes.c_uint64(n), ctypes.c_uint64(first), ctypes.c_uint64(c))
     fn = lib().hmc_orbit_turning_points if first is None else lib().hmc_orbit_turning_points_range
+    if prebuilt:       # the workspace holds the tables of (r_sorted, phi, m_cum): hmc_orbit_build_tables was called
+        head = (ctypes.c_uint64(n), ctypes.c_uint64(first or 0), ctypes.c_uint64(c))
+        fn = lib().hmc_orbit_turning_points_prebuilt
     rc = fn(*head, ctypes.c_double(G), _dev(r_sorted, f, n, "r_sorted"), _dev(v_r, f, c, "v_r"),
             _dev(v_t, f, c, "v_t"), _dev(phi, f, n, "phi"), _dev(m_cum, f, n, "m_cum"), _dev(out["E"], f, c, "E"),
             _dev(out["J"], f, c, "J"), _dev(out["r_min"], f, c, "r_min"), _dev(out["r_max"], f, c, "r_max"),

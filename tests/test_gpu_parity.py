@@ -583,3 +583,30 @@ def test_graph_replay_equals_eager_steps(oracle, n):
     o = oracle.orbit_step(before["r"], before["v_r"], before["v_t"], before["m"], before["id"], seed, 7)
     assert np.array_equal(host(eager.state["r"]), o["sample"]["r_new"])
     assert np.array_equal(host(eager.sample["n_try"], np.uint16), o["sample"]["n_try"])
+
+
+@pytest.mark.parametrize("n", [1, 40, 100_003, 1_200_000])
+def test_prebuilt_tables_equal_the_one_call(oracle, n):
+    """hmc_orbit_build_tables + hmc_orbit_turning_points_prebuilt (whole table, and a range of it) against
+    hmc_orbit_turning_points: the same two launches, the same bits; one case against the oracle as well."""
+    seed = 31
+    c = inputs.plummer(n, seed)
+    rs, perm, (vrs, vts, ms), ids = oracle.sort_by_radius(c["r"], (c["v_r"], c["v_t"], c["m"]), c["id"])
+    phi, mc = oracle.potential(rs, ms)
+    d = [dev(x) for x in (rs, vrs, vts, phi, mc)]
+    ws = hmc.alloc_workspace(n)
+    one = hmc.hmc_orbit_turning_points(*d, 1.0, workspace=ws)
+    one = {k: v.clone() for k, v in one.items()}
+    ws2 = hmc.alloc_workspace(n)
+    hmc.hmc_orbit_build_tables(d[0], d[3], d[4], 1.0, workspace=ws2)
+    two = hmc.hmc_orbit_turning_points(*d, 1.0, workspace=ws2, prebuilt=True)
+    for k in one:
+        assert torch.equal(one[k], two[k]), k
+    first, count = n // 3, max(1, n // 5)
+    part = hmc.hmc_orbit_turning_points(d[0], d[1][first:first + count].contiguous(), d[2][first:first + count].contiguous(),
+                                        d[3], d[4], 1.0, workspace=ws2, first=first, prebuilt=True)
+    for k in one:
+        assert torch.equal(one[k][first:first + count], part[k]), k
+    if n <= 100_003:
+        otp = oracle.orbit_turning_points(rs, vrs, vts, phi, mc)
+        assert np.array_equal(host(two["k_min"], np.uint32), otp["k_min"]) and np.array_equal(host(two["r_max"]), otp["r_max"])
