@@ -470,7 +470,7 @@ def run_gpu(args, cfg):
                     physical=(dict(dram_bytes_per_launch=traffic, achieved=traffic / (dom_ms * 1e-3) / 1e9,
                                    frac=traffic / (dom_ms * 1e-3) / 1e9 / peak, capture=capture,
                                    limiter="not streamed bytes: 8 warps per scheduler of dependent fp64 chains and loads "
-                                           "(ncu: issue slots 50-54 % used), for turning_points_kernel together with the "
+                                           "(ncu: issue slots 54-56 % used), for turning_points_kernel together with the "
                                            "rate of random 128-byte DRAM lines (profiles/r2b.md, DESIGN.md 5 and 5a)")
                               if traffic else None),
                     # what ncu shows the kernel waits for, as opposed to the roofline the metric is quoted against
