@@ -35,7 +35,7 @@ if ROOT not in sys.path:
 METRIC = "stars/sec per orbit step (sort+potential+turning points+sampling), fp64, N=1e7"
 UNIT = "stars/s"
 STAGES = ("sort", "potential", "turning_points", "sampling")
-GRAPH_AUTO_MAX_N = 2_000_000      # below this a step is bound by launching its kernels (0.147 -> 0.122 ms at N = 1e5)
+GRAPH_AUTO_MAX_N = 20_000_000     # replaying the step from a graph saves 25 us of launch gaps per step (N = 1e5: 0.169 -> 0.126 ms, 1e7: 2.57 -> 2.54)
 
 
 # --------------------------------------------------------------------------- roofline model
