@@ -213,7 +213,7 @@ HMC_API hmc_status hmc_add_u32(uint32_t* word, uint32_t increment, void* cuda_st
  * output of both (E .. star_status are S3's, r_new .. star_status_out S4's): each warp solves 32 stars,
  * keeps their orbits on chip and draws their new radii, so S3's outputs are never read back and
  * searching and drawing warps share an SM.  Arguments as in the two calls.  Measured on B200 at N = 1e7 it is
- * SLOWER than the two calls (about 3 ms against 0.90 + 0.78 ms): it is kept for API completeness
+ * SLOWER than the two calls (about 3 ms against 0.90 + 0.69 ms): it is kept for API completeness
  * and compared with the oracle in the tests; nothing else here uses it.
  */
 HMC_API hmc_status hmc_orbit_step(uint64_t n, double G, uint64_t seed, uint32_t step,
