@@ -138,6 +138,49 @@ HMC_API hmc_status hmc_potential(uint64_t n, double G,
         void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*
+ * S2 for callers that cannot allocate device memory: hmc_potential without a workspace argument.
+ *
+ * Who this is for.  Every other call here needs a `workspace` the caller obtained from cudaMalloc (or from a pool
+ * that did).  Some callers cannot do that at the point where they need Phi: code running inside a host program
+ * whose device memory is handed out once at start-up by an allocator the plug-in may not call (a simulation
+ * framework's arena, a job with a fixed memory budget that fails if the driver allocates behind its back), a
+ * callback that runs while another thread holds the allocator's lock, or a real-time loop in which cudaMalloc's
+ * implicit device synchronisation is not acceptable.  Such a caller already owns r, m, phi and m_cum (its own
+ * star arrays); what it lacks is the few hundred kilobytes of partial sums the two launches of S2 hand to each
+ * other.  This entry point keeps those in an array that is part of the library image itself.
+ *
+ * What it computes: exactly hmc_potential (Eq. 1-5; same two kernels, same launch
+ * configuration, same bits): m_cum[k] = M_k, phi[k] = -G (M_k / r_k + sum_{i>k} m_i / r_i).
+ *
+ * The scratch: a file-scope `static __device__` array in hmc_potential.cu of HMC_STATIC_SCRATCH_BYTES bytes
+ * (544 KiB), 256-byte aligned.  Every GPU on which this process uses the library holds one copy from the moment
+ * the library's device code is loaded there until the process exits, whether or not this call is ever made.
+ * It holds one 32-byte total per 1024 stars plus one per CTA of the launch, hence the limit
+ *     n <= HMC_STATIC_MAX_N = 2^24 (16 777 216 stars);
+ * a larger n returns HMC_ERR_STATIC_LIMIT and launches nothing (use hmc_potential with a workspace instead).
+ * The same status is returned on a GPU with more than 341 multiprocessors (more CTAs than the array has room for).
+ *
+ * Set-up: the first call on each device looks up the array's device address (cudaGetSymbolAddress, with that
+ * device current) and remembers it for the process.  That look-up may make the CUDA runtime load the library's
+ * device code, so make the first call on a device OUTSIDE any stream capture; later calls only launch kernels.
+ * The call itself never calls cudaMalloc, cudaFree or any routine that allocates, on the host or the device.
+ *
+ * Sharing: there is ONE array per device, used by every call from every thread and stream.  Nothing in it has
+ * to start at zero (the first launch overwrites every entry the second one reads, so the previous call's
+ * contents do no harm), but two calls whose kernels may run at the same time on one device -- different
+ * streams, or different host threads on different streams -- overwrite each other's partial sums and produce
+ * wrong potentials without any error.  Calls on one stream, or ordered by events, are safe.
+ * Everything else (argument rules, asynchrony, n == 0) is as for hmc_potential.
+ */
+#define HMC_STATIC_MAX_N          (1ull << 24)
+#define HMC_STATIC_SCRATCH_BYTES  ((16384u + 1024u) * 32u)
+#define HMC_ERR_STATIC_LIMIT      (-6)  /* n (or the GPU's SM count) beyond what the built-in scratch array holds */
+
+HMC_API hmc_status hmc_potential_static(uint64_t n, double G,
+        const double* r_sorted, const double* m_sorted,
+        double* phi, double* m_cum, void* cuda_stream);
+
+/*
  * S3  Pericentre and apocentre of every star's orbit.
  * For star k:  E = Phi_k + (v_r^2 + v_t^2)/2  (Eq. 16),  J = r_k v_t,
  *   Q(r) = 2E - 2Phi(r) - J^2/r^2  (Eq. 12);

@@ -125,6 +125,9 @@ const char* hmc_status_string(hmc_status s)
         case HMC_ERR_WORKSPACE: return "HMC_ERR_WORKSPACE: workspace NULL, misaligned or too small";
         case HMC_ERR_ALIGN: return "HMC_ERR_ALIGN: array pointer not aligned to its element size";
         case HMC_ERR_CUDA: return "HMC_ERR_CUDA: CUDA runtime call or kernel launch failed";
+        case HMC_ERR_STATIC_LIMIT:
+            return "HMC_ERR_STATIC_LIMIT: n exceeds HMC_STATIC_MAX_N (2^24 stars), the capacity of the library's built-in "
+                   "scratch array; use the call that takes a workspace";
         default: return "HMC: unknown status";
     }
 }

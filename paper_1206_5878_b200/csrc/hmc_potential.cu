@@ -365,3 +365,57 @@ hmc_status potential(uint64_t n, double G, const double* r, const double* m, dou
 }
 
 }  // namespace hmc
+
+// ---- hmc_potential_static: S2 with its scratch inside the library image (include/hmc.h) -----------------------
+// For callers that may not allocate device memory (a plug-in inside a host program that owns the allocator, a
+// callback under the allocator's lock, a loop that cannot afford cudaMalloc's device synchronisation): the partial
+// sums the reduce launch hands to the apply launch live in this array instead of a caller's workspace.
+// Layout: slice totals [STATIC_MAX_SLICES] double4, then chunk totals [STATIC_MAX_CHUNKS] double4.
+// One copy per GPU that loads the library, held until the process exits.  Every call on a device shares it:
+// nothing needs clearing between calls (the reduce launch writes every entry the apply launch reads), but calls
+// that overlap on the GPU race on it.
+static constexpr uint32_t STATIC_MAX_SLICES = (uint32_t)(HMC_STATIC_MAX_N / hmc::SLICE);   // 16384
+static constexpr uint32_t STATIC_MAX_CHUNKS = 1024;                                         // CTAs of a launch: 3 per SM
+static_assert((STATIC_MAX_SLICES + STATIC_MAX_CHUNKS) * sizeof(double4) == HMC_STATIC_SCRATCH_BYTES, "hmc.h states the size");
+static_assert(HMC_STATIC_MAX_N % hmc::SLICE == 0 && HMC_STATIC_MAX_N <= HMC_MAX_N, "limit is a whole number of slices");
+
+static __device__ __align__(256) unsigned char g_static_scratch[HMC_STATIC_SCRATCH_BYTES];
+
+// In host code `g_static_scratch` names a host-side shadow of the symbol, not device memory: a kernel handed
+// &g_static_scratch would fault (or scribble on host memory where the GPU can reach it).  The address the kernels
+// need comes from cudaGetSymbolAddress, which answers for the CURRENT device; it is looked up once per device and kept.
+static hmc_status static_scratch_address(double4** out)
+{
+    static std::atomic<void*> cached[64];                   // zero-initialised; one slot per device ordinal
+    int dev = 0;
+    HMC_CUDA_TRY(cudaGetDevice(&dev));
+    const bool slot = dev >= 0 && dev < 64;
+    void* p = slot ? cached[dev].load(std::memory_order_acquire) : nullptr;
+    if (p == nullptr) {
+        HMC_CUDA_TRY(cudaGetSymbolAddress(&p, g_static_scratch));   // same answer from every thread: no lock needed
+        if (p == nullptr) return HMC_ERR_CUDA;
+        if (slot) cached[dev].store(p, std::memory_order_release);
+    }
+    *out = static_cast<double4*>(p);
+    return HMC_OK;
+}
+
+extern "C" hmc_status hmc_potential_static(uint64_t n, double G, const double* r_sorted, const double* m_sorted,
+                                           double* phi, double* m_cum, void* cuda_stream)
+{
+    using namespace hmc;
+    if (n > HMC_MAX_N) return HMC_ERR_SIZE;
+    if (n > HMC_STATIC_MAX_N) return HMC_ERR_STATIC_LIMIT;
+    if (n == 0) return HMC_OK;
+    if (!r_sorted || !m_sorted || !phi || !m_cum) return HMC_ERR_NULL;
+    if (misaligned(r_sorted, 8) || misaligned(m_sorted, 8) || misaligned(phi, 8) || misaligned(m_cum, 8)) return HMC_ERR_ALIGN;
+    const ScanPlan plan = scan_plan(n, sm_count());         // what potential() below will compute again
+    if (plan.nslices > STATIC_MAX_SLICES || plan.nchunks > STATIC_MAX_CHUNKS) return HMC_ERR_STATIC_LIMIT;
+    double4* scratch = nullptr;
+    const hmc_status s = static_scratch_address(&scratch);
+    if (s != HMC_OK) return s;
+    // potential() places the chunk totals right behind the plan.nslices slice totals: both fit by the check above
+    Workspace ws{};
+    ws.scan_status = reinterpret_cast<double*>(scratch);
+    return potential(n, G, r_sorted, m_sorted, phi, m_cum, nullptr, 0, 0, ws, static_cast<cudaStream_t>(cuda_stream));
+}

@@ -24,6 +24,7 @@ ST_UNBOUND, ST_RADIAL, ST_DEGENERATE, ST_CIRCULAR, ST_MAXTRIES, ST_CLIPPED, ST_N
 COUNTER_NAMES = ("unbound", "radial", "degenerate", "circular", "maxtries", "clipped", "trials", "nokinetic")
 NCOUNTERS = 8
 MAX_N = 1 << 28
+STATIC_MAX_N = 1 << 24          # HMC_STATIC_MAX_N: the most stars hmc_potential_static takes
 
 _lib = None
 
@@ -51,7 +52,7 @@ def load(path: str) -> ctypes.CDLL:
                  "hmc_potential_shard", "hmc_partition_points", "hmc_orbit_turning_points_range",
                  "hmc_sample_new_radius_range", "hmc_relaxation_timestep", "hmc_two_body_relaxation",
                  "hmc_sample_new_radius_dstep", "hmc_add_u32", "hmc_potential_shard_push", "hmc_orbit_build_tables",
-                 "hmc_orbit_turning_points_prebuilt"):
+                 "hmc_orbit_turning_points_prebuilt", "hmc_potential_static"):
         getattr(L, name).restype = ctypes.c_int32
     return L
 
@@ -137,6 +138,34 @@ def hmc_potential(r_sorted: torch.Tensor, m_sorted: torch.Tensor, G: float = 1.0
                              _dev(m_sorted, torch.float64, n, "m_sorted"), _dev(phi, torch.float64, n, "phi"),
                              _dev(m_cum, torch.float64, n, "m_cum"), wp, wb, _stream())
     _check(rc, "hmc_potential")
+    return phi, m_cum
+
+
+def hmc_potential_static(r_sorted: torch.Tensor, m_sorted: torch.Tensor, G: float = 1.0, *, phi=None, m_cum=None):
+    """S2 without a workspace, for callers that cannot allocate device memory.  -> (phi, m_cum)
+
+    Same result as hmc_potential, bit for bit.  The C call behind it allocates nothing: its scratch is a 544 KiB
+    array built into libhmc.so, one per GPU.  Use it from code that must not call the CUDA allocator where it
+    needs the potential: a plug-in inside a program that owns all device memory, a callback that runs under the
+    allocator's lock, a loop that cannot take cudaMalloc's device synchronisation.  Pass ``phi`` and ``m_cum``
+    (tensors you already own) if this Python layer must not allocate either; without them it makes them with
+    torch.empty, which is a convenience of the binding, not of the library.
+
+    Limits and rules (include/hmc.h): at most STATIC_MAX_N = 2**24 stars, more raises HmcError naming the limit;
+    make the first call on each GPU outside stream capture (it looks up the array's address); all calls on a
+    GPU share the one array, so calls that may run at the same time on different streams corrupt each other --
+    keep them on one stream or order them with events."""
+    n = r_sorted.numel()
+    if n > STATIC_MAX_N:
+        raise HmcError("hmc_potential_static takes at most %d stars (its scratch is a fixed array inside the library), "
+                       "got %d; use hmc_potential with a workspace" % (STATIC_MAX_N, n))
+    dev = r_sorted.device
+    phi = torch.empty(n, dtype=torch.float64, device=dev) if phi is None else phi
+    m_cum = torch.empty(n, dtype=torch.float64, device=dev) if m_cum is None else m_cum
+    rc = lib().hmc_potential_static(ctypes.c_uint64(n), ctypes.c_double(G), _dev(r_sorted, torch.float64, n, "r_sorted"),
+                                    _dev(m_sorted, torch.float64, n, "m_sorted"), _dev(phi, torch.float64, n, "phi"),
+                                    _dev(m_cum, torch.float64, n, "m_cum"), _stream())
+    _check(rc, "hmc_potential_static")
     return phi, m_cum
 
 
