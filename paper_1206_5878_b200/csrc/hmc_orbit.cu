@@ -769,7 +769,11 @@ __device__ __forceinline__ InvTable build_inv(uint16_t* inv, uint32_t cells, con
             uint32_t hi = ncoarse + 1;
             while (hi - lo > 1) { const uint32_t m = (lo + hi) >> 1; if (coarse[m] <= x) lo = m; else hi = m; }
         }
-        inv[q] = (uint16_t)lo;
+        // Key 0 also receives every radius BELOW r_1 (key() clamps from below), so its lower end must be coarse index 0
+        // (r = 0), not the largest index <= r_1: where coarse[1] == r_1 and r_1 has zero low bits (a round innermost
+        // radius with shift == 0, or 2^shift tied ones) that would be 1 and a trial inside the innermost star would be
+        // given interval 1 instead of 0.
+        inv[q] = (uint16_t)(q == 0 ? 0u : lo);
     }
     __syncthreads();
     return t;

@@ -245,3 +245,51 @@ def test_pair_search_flagged_stars_and_ranges(pairs_build, oracle):
         assert np.array_equal(host(tpr[k]), otp[k][first:first + count]), k
     for k in ("k_min", "k_max"):
         assert np.array_equal(host(tpr[k], np.uint32), otp[k][first:first + count]), k
+
+
+# ----------------------------------------------------------------------------- trials inside the innermost star
+def _draw_both(oracle, rs, vrs, vts, ms, ids, seed, step):
+    phi, mc = oracle.potential(rs, ms)
+    otp = oracle.orbit_turning_points(rs, vrs, vts, phi, mc)
+    osm = oracle.sample_new_radius(rs, phi, mc, rs, vrs, vts, otp["E"], otp["J"], otp["r_min"], otp["r_max"],
+                                   otp["k_min"], otp["k_max"], ids, otp["status"], seed, step)
+    tp, sm = gpu_s3_s4(rs, vrs, vts, phi, mc, ids, seed, step)
+    assert_bitwise(tp, sm, otp, osm)
+    return otp, osm
+
+
+def test_round_innermost_radius_trials_below_it(oracle):
+    """Radii 1, 2, 3, 4: r_1 has zero low mantissa bits and, the coarse table being the whole table (shift 0),
+    coarse[1] = r_1 -- the case in which S4's inverse table used to send a trial radius below r_1 to interval 1
+    instead of interval 0 (round-2 advisor).  Star 0's orbit reaches inside r_1 (k_min = 0); over 64 (seed, step)
+    pairs some ACCEPTED radius lies there, so Phi(r0), Q0, g and the accept decision are all exercised."""
+    r = np.array([1.0, 2.0, 3.0, 4.0])
+    m = np.array([0.25, 0.25, 0.25, 0.25])
+    vr = np.array([0.1, 5.0, 0.1, 0.0])
+    vt = np.array([0.3, 0.1, 0.0, 0.3])
+    ids = np.arange(4, dtype=np.uint32)
+    below = 0
+    for seed in (1, 2, 3, 4):
+        for step in range(16):
+            otp, osm = _draw_both(oracle, r, vr, vt, m, ids, seed, step)
+            assert otp["k_min"][0] == 0 and otp["r_min"][0] < 1.0
+            below += int(osm["r_new"][0] < 1.0)
+    print("accepted radii below r_1: %d of 64" % below)
+    assert below >= 4
+
+
+def test_tied_round_innermost_radii_with_a_directory(oracle):
+    """The same with a directory (N = 20 000: shift 1, coarse[1] is node 2): the two innermost stars share the round
+    radius 1.0, every other radius is larger.  Trials of the inner stars' orbits fall below r_1."""
+    n = 20_000
+    rs, vrs, vts, ms, ids, _, _ = sorted_tables(oracle, n, 77)
+    s = 1.0009765625 / rs[0]                  # lengths by s, velocities by s^-1/2: the cluster stays bound
+    rs, vrs, vts = rs * s, vrs / np.sqrt(s), vts / np.sqrt(s)     # everything above 1 ...
+    rs[0] = rs[1] = 1.0                       # ... except a tied, round innermost pair
+    assert np.all(np.diff(rs) >= 0)
+    below = 0
+    for step in range(6):
+        otp, osm = _draw_both(oracle, rs, vrs, vts, ms, ids, 5, step)
+        below += int((osm["r_new"] < 1.0).sum())
+    print("accepted radii below r_1: %d" % below)
+    assert below >= 3
