@@ -66,6 +66,12 @@ struct ScanPlan {
     uint32_t ntiles, nslices, tpc, nchunks;
 };
 
+// Tiles per chunk whose offsets fit the apply launch's shared arrays.  One chunk per resident CTA would need 296 at
+// n = HMC_MAX_N on 148 SMs (and more on a smaller GPU): scan_plan caps tpc here and lets the grid grow beyond one
+// wave instead -- no CTA of either launch waits for another, so any number of chunks is correct, and the workspace
+// has room for one chunk total per tile.
+static constexpr int MAX_TPC_SMEM = 256;
+
 static inline ScanPlan scan_plan(uint64_t n, int sms)
 {
     ScanPlan p;
@@ -74,6 +80,7 @@ static inline ScanPlan scan_plan(uint64_t n, int sms)
     const uint32_t want = (uint32_t)sms * CHUNK_CTAS_PER_SM;
     p.tpc = (p.ntiles + want - 1) / want;
     if (p.tpc == 0) p.tpc = 1;
+    if (p.tpc > (uint32_t)MAX_TPC_SMEM) p.tpc = MAX_TPC_SMEM;
     p.nchunks = (p.ntiles + p.tpc - 1) / p.tpc;
     return p;
 }
@@ -132,8 +139,6 @@ potential_reduce_kernel(const double* __restrict__ r, const double* __restrict__
 }
 
 // ---- 2. per-tile scans and Phi -----------------------------------------------------------------
-static constexpr int MAX_TPC_SMEM = 256;      // tiles per chunk whose offsets fit the shared array (n <= HMC_MAX_N: 222)
-
 // Sharded step: further destinations of the shard's slice of the replicated table, e.g. the other
 // GPUs' copies at this shard's offset, reached by peer access over NVLink.  The launch that produces Phi and M stores
 // them (and the radii it has in registers) there tile by tile, so the table's all-gather is done when the scan is.
@@ -353,7 +358,7 @@ hmc_status potential(uint64_t n, double G, const double* r, const double* m, dou
     push.npeers = npeers;
     for (int g = 0; g < npeers; ++g) { push.r[g] = peer_r[g]; push.phi[g] = peer_phi[g]; push.m_cum[g] = peer_m_cum[g]; }
     const ScanPlan plan = scan_plan(n, sm_count());
-    if (plan.tpc > MAX_TPC_SMEM) return HMC_ERR_SIZE;             // cannot happen for n <= HMC_MAX_N on >= 4 SMs
+    if (plan.tpc > (uint32_t)MAX_TPC_SMEM) return HMC_ERR_SIZE;   // cannot happen: scan_plan caps it
     double4* slice_tot = reinterpret_cast<double4*>(ws.scan_status);
     double4* chunk_tot = slice_tot + plan.nslices;
     potential_reduce_kernel<<<plan.nchunks, SCAN_THREADS, 0, st>>>(r, m, n, plan, slice_tot, chunk_tot);

@@ -214,3 +214,51 @@ def test_config5_1e8_five_steps(oracle):
     cnt = dict(zip(hmc.COUNTER_NAMES, host(st.counters).tolist()))
     print("counters:", cnt)
     assert cnt["unbound"] == cnt["radial"] == cnt["degenerate"] == cnt["circular"] == cnt["maxtries"] == 0
+
+
+def test_potential_at_the_largest_n_the_header_allows():
+    """hmc_potential at n = HMC_MAX_N = 2^28 (round-2 advisor: the launch plan wanted 296 tiles per chunk there and
+    the call returned HMC_ERR_SIZE; the largest n any other test reaches is 1e8).  No oracle run at this size: the
+    input is chosen so that Eq. 1 has an exact value that Python's rational arithmetic gives at any star --
+    m_i = 2^-28, r_i = 2^(i >> 22) (64 blocks of tied radii 1, 2, 4, ... 2^63).  Then M_k = (k + 1) 2^-28 exactly,
+    S_k = sum_{i > k} m_i / r_i is a dyadic rational, and the call must return both rounded once (R1p),
+    so Phi_k = -(G (M_k / r_k + S_k)) is compared bit for bit on 20 000 sampled stars, the first, the last, and
+    the stars on either side of every block edge."""
+    from fractions import Fraction
+    n = hmc.MAX_N
+    free, _ = torch.cuda.mem_get_info()
+    if free < 4 * 8 * n + hmc.workspace_bytes(n) + (1 << 30):
+        pytest.skip("needs %.0f GB of device memory" % ((32 * n + hmc.workspace_bytes(n)) / 1e9))
+    blk = 22
+    i = torch.arange(n, dtype=torch.int64, device="cuda")
+    r = (((i >> blk) + 1023) << 52).view(torch.float64)          # bit pattern of 2^(i >> 22)
+    del i
+    m = torch.full((n,), 2.0 ** -28, dtype=torch.float64, device="cuda")
+    G = 3.0
+    phi, mc = hmc.hmc_potential(r, m, G)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(28)
+    edges = np.arange(1, 64, dtype=np.int64) << blk
+    ks = np.unique(np.concatenate([rng.integers(0, n, 20_000), [0, 1, n - 2, n - 1], edges - 1, edges, edges + 2047, edges + 2048]))
+    ks = ks[(ks >= 0) & (ks < n)]
+    sel = torch.from_numpy(ks).cuda()
+    g_phi, g_mc, g_r = phi[sel].cpu().numpy(), mc[sel].cpu().numpy(), r[sel].cpu().numpy()
+    tail = [Fraction(0)] * 65                                     # tail[j] = sum over blocks j' >= j of 2^22 * 2^-j'
+    for j in range(63, -1, -1):
+        tail[j] = tail[j + 1] + Fraction(1 << blk, 1 << j)
+    want_phi, want_mc = np.empty(ks.size), np.empty(ks.size)
+    for a, k in enumerate(ks.tolist()):
+        j = k >> blk
+        rest = ((j + 1) << blk) - 1 - k                           # stars after k inside its own block
+        S = float((Fraction(rest, 1 << j) + tail[j + 1]) / (1 << 28))      # exact sum, rounded once
+        M = (k + 1) * 2.0 ** -28                                  # exact
+        assert g_r[a] == 2.0 ** j
+        want_mc[a] = M
+        want_phi[a] = -(G * (M / 2.0 ** j + S))
+    assert np.array_equal(g_mc, want_mc)
+    assert np.array_equal(g_phi, want_phi)
+    # every star: M is the exact ramp; Phi is constant inside a block of tied radii (what M_k / r gains, S_k loses)
+    assert bool((mc == torch.arange(1, n + 1, dtype=torch.float64, device="cuda") * 2.0 ** -28).all())
+    const = [-(G * float((Fraction((j + 1) << blk, 1 << j) + tail[j + 1]) / (1 << 28))) for j in range(64)]
+    want_all = torch.tensor(const, dtype=torch.float64, device="cuda").repeat_interleave(1 << blk)
+    assert bool(((phi - want_all).abs() <= 4e-16 * want_all.abs()).all())
