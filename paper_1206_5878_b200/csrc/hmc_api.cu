@@ -499,6 +499,10 @@ hmc_status hmc_step_host(uint64_t n, double G, uint64_t seed, uint32_t step, con
     hmc_status s = host_step_streams(&hs);
     if (s != HMC_OK) return s;
     cudaStream_t K = hs->kern, D = hs->copy;
+    // Everything is enqueued by `enqueue`; a failure part-way returns from it at once, and the code behind it then
+    // still orders the caller's stream after whatever had been put on K and D by then (work that reads and writes
+    // the arena and the host buffers), so a caller that reuses them after an error does not race with it.
+    auto enqueue = [&]() -> hmc_status {
     // copy in, on the caller's stream, in the order the stages need the columns: r (the sort), m and id (they go
     // back to the host sorted, and S2 needs m), then the velocities (S3)
     HMC_CUDA_TRY(cudaMemcpyAsync(a.r, r, n * 8, cudaMemcpyHostToDevice, st));
@@ -561,6 +565,13 @@ hmc_status hmc_step_host(uint64_t n, double G, uint64_t seed, uint32_t step, con
     HMC_CUDA_TRY(cudaEventRecord(hs->done, D));
     HMC_CUDA_TRY(cudaStreamWaitEvent(st, hs->done, 0));          // the caller's stream completes when everything is back
     return HMC_OK;
+    };
+    s = enqueue();
+    if (s != HMC_OK) {                                           // error path only: K -> D -> the caller's stream
+        if (cudaEventRecord(hs->drawn[0], K) == cudaSuccess) (void)cudaStreamWaitEvent(D, hs->drawn[0], 0);
+        if (cudaEventRecord(hs->done, D) == cudaSuccess) (void)cudaStreamWaitEvent(st, hs->done, 0);
+    }
+    return s;
 }
 
 }  // extern "C"
