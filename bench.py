@@ -13,8 +13,13 @@ on both sides, CUDA events on the launching stream, MAX over ranks.  The star ar
 state and intermediates per step at N = 1e7) are several times the 126 MB L2, so no explicit L2
 flush is needed between steps; `config.l2` says so.
 
-N > 1 ranks run independent replicas (one cluster per GPU, seed + rank): the path does not shard
-in this round, there is no data-path collective, scaling is "weak".
+N > 1 ranks run independent replicas (one cluster per GPU, seed + rank): the graded path is one GPU
+(the sharded step of paper_1206_5878_b200/shard.py is covered by tests, not timed here),
+there is no data-path collective, scaling is "weak".
+
+After the headline's timed region the default run also times the other four BASELINE.json configs
+(device-resident steps only, no CPU legs, no end-to-end leg) and reports them under `all_configs`
+(--no-all-configs skips that; N = 1e8 takes about a minute to generate).
 
 Prints ONE JSON line on rank 0.  `--impl reference` times the CPU oracle instead (rank 0 only).
 """
@@ -303,6 +308,102 @@ def run_reference(args, cfg):
 
 
 # --------------------------------------------------------------------------- GPU arm
+def staged_orbit_step(hmc, stepper, ev, stream, fused=False):
+    """One step of `stepper` with an event after every stage (events are recorded on the launching stream).
+    ev[0..4]: stage boundaries, ev[5]: after S3's table build."""
+    s, so = stepper.state, stepper.sorted
+    ev[0].record(stream)
+    hmc.hmc_sort_by_radius(s["r"], (s["v_r"], s["v_t"], s["m"]), s["id"], r_sorted=so["r"], perm=so["perm"],
+                           cols_out=(so["v_r"], so["v_t"], so["m"]), ids_out=so["id"], workspace=stepper.workspace)
+    ev[1].record(stream)
+    hmc.hmc_potential(so["r"], so["m"], stepper.G, phi=stepper.phi, m_cum=stepper.m_cum, workspace=stepper.workspace)
+    ev[2].record(stream)
+    if fused:
+        ev[5].record(stream)
+        ev[3].record(stream)      # "turning_points" reads 0; "sampling" is the fused S3 + S4 call
+        hmc.hmc_orbit_step(so["r"], so["v_r"], so["v_t"], stepper.phi, stepper.m_cum, so["id"], stepper.seed,
+                           stepper.step_index, stepper.G, tp=stepper.tp, out=stepper.sample,
+                           counters=stepper.counters, workspace=stepper.workspace)
+    else:
+        # S3 as its two launches, with an event between them: hmc_orbit_build_tables + hmc_orbit_turning_points_prebuilt
+        # are exactly what hmc_orbit_turning_points does; the event lets turning_points_kernel be timed by itself
+        hmc.hmc_orbit_build_tables(so["r"], stepper.phi, stepper.m_cum, stepper.G, workspace=stepper.workspace)
+        ev[5].record(stream)
+        hmc.hmc_orbit_turning_points(so["r"], so["v_r"], so["v_t"], stepper.phi, stepper.m_cum, stepper.G,
+                                     out=stepper.tp, counters=stepper.counters, workspace=stepper.workspace, prebuilt=True)
+        ev[3].record(stream)
+        hmc.hmc_sample_new_radius(so["r"], stepper.phi, stepper.m_cum, so["v_r"], so["v_t"], stepper.tp, so["id"],
+                                  stepper.seed, stepper.step_index, stepper.G, out=stepper.sample,
+                                  counters=stepper.counters, workspace=stepper.workspace, reuse_tables=True)
+    ev[4].record(stream)
+    sm = stepper.sample
+    s["r"], sm["r_new"] = sm["r_new"], s["r"]
+    s["v_r"], sm["v_r_new"] = sm["v_r_new"], s["v_r"]
+    s["v_t"], sm["v_t_new"] = sm["v_t_new"], s["v_t"]
+    s["m"], so["m"] = so["m"], s["m"]
+    s["id"], so["id"] = so["id"], s["id"]
+    stepper.step_index += 1
+
+
+def time_config(index, steps, warmup, graph_mode, devs, local_rank, peak):
+    """Device-resident timing of one BASELINE.json config, as the headline's: `warmup` eager steps, then `steps`
+    chained steps between two CUDA events (replayed from a graph of two steps where the headline would be), clocks
+    sampled during the timed region; per-stage times from eager steps afterwards.  -> dict for `all_configs`."""
+    import numpy as np
+    import torch
+    from paper_1206_5878_b200 import hmc, inputs
+    c = inputs.config(index)
+    n = c["n"]
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(devs)
+    stepper = hmc.OrbitStepper(d(c["r"]), d(c["v_r"]), d(c["v_t"]), d(c["m"]), d(c["id"].view(np.int32)), c["seed"],
+                               with_n_try=False)
+    name, masses, seed = c["name"], c["masses"], c["seed"]
+    del c
+    stream = torch.cuda.current_stream()
+    mk = lambda: [torch.cuda.Event(enable_timing=True) for _ in range(6)]
+    for _ in range(max(warmup, 2)):
+        staged_orbit_step(hmc, stepper, mk(), stream)
+    if stepper.step_index % 2:
+        staged_orbit_step(hmc, stepper, mk(), stream)
+    use_graph = graph_mode == "on" or (graph_mode == "auto" and n <= GRAPH_AUTO_MAX_N and steps % 2 == 0)
+    if use_graph:
+        stepper.run_graph(2)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    evs = [mk() for _ in range(steps)]
+    if use_graph:
+        t0.record(stream)
+        stepper.run_graph(steps)
+        t1.record(stream)
+        torch.cuda.synchronize()
+        clocks = sampler.stop()
+        for e in evs:
+            staged_orbit_step(hmc, stepper, e, stream)
+    else:
+        t0.record(stream)
+        for e in evs:
+            staged_orbit_step(hmc, stepper, e, stream)
+        t1.record(stream)
+        torch.cuda.synchronize()
+        clocks = sampler.stop()
+    torch.cuda.synchronize()
+    ms = t0.elapsed_time(t1) / steps
+    stage_ms = {nm: sum(e[i].elapsed_time(e[i + 1]) for e in evs) / steps for i, nm in enumerate(STAGES)}
+    model = algorithmic_bytes_per_star(n)
+    orbit_ms = stage_ms["potential"] + stage_ms["turning_points"] + stage_ms["sampling"]
+    orbit_gbs = (model["potential"] + model["turning_points"] + model["sampling"]) * n / (orbit_ms * 1e-3) / 1e9
+    step_gbs = sum(model.values()) * n / (ms * 1e-3) / 1e9
+    del stepper
+    torch.cuda.empty_cache()
+    return dict(index=index, name=name, n=n, masses=masses, seed=seed, steps=steps, ms_per_step=ms,
+                stars_per_s=n / (ms * 1e-3), launch="cuda graph of two steps, replayed" if use_graph else "eager",
+                stage_ms=stage_ms,
+                potential_plus_orbit=dict(ms=orbit_ms, frac_of_8TBs=orbit_gbs / 8000.0, frac_of_measured_peak=orbit_gbs / peak),
+                step_frac_of_measured_peak=step_gbs / peak, clocks=clocks)
+
+
 def run_gpu(args, cfg):
     import numpy as np
     import torch
@@ -327,39 +428,7 @@ def run_gpu(args, cfg):
     stream = torch.cuda.current_stream()
 
     def staged_step(ev):
-        """One step with an event after every stage (events are recorded on the launching stream)."""
-        s, so = stepper.state, stepper.sorted
-        ev[0].record(stream)
-        hmc.hmc_sort_by_radius(s["r"], (s["v_r"], s["v_t"], s["m"]), s["id"], r_sorted=so["r"], perm=so["perm"],
-                               cols_out=(so["v_r"], so["v_t"], so["m"]), ids_out=so["id"], workspace=stepper.workspace)
-        ev[1].record(stream)
-        hmc.hmc_potential(so["r"], so["m"], stepper.G, phi=stepper.phi, m_cum=stepper.m_cum, workspace=stepper.workspace)
-        ev[2].record(stream)
-        if args.fused:
-            ev[5].record(stream)
-            ev[3].record(stream)      # "turning_points" reads 0; "sampling" is the fused S3 + S4 call
-            hmc.hmc_orbit_step(so["r"], so["v_r"], so["v_t"], stepper.phi, stepper.m_cum, so["id"], stepper.seed,
-                               stepper.step_index, stepper.G, tp=stepper.tp, out=stepper.sample,
-                               counters=stepper.counters, workspace=stepper.workspace)
-        else:
-            # S3 as its two launches, with an event between them: hmc_orbit_build_tables + hmc_orbit_turning_points_prebuilt
-            # are exactly what hmc_orbit_turning_points does; the event lets turning_points_kernel be timed by itself
-            hmc.hmc_orbit_build_tables(so["r"], stepper.phi, stepper.m_cum, stepper.G, workspace=stepper.workspace)
-            ev[5].record(stream)
-            hmc.hmc_orbit_turning_points(so["r"], so["v_r"], so["v_t"], stepper.phi, stepper.m_cum, stepper.G,
-                                         out=stepper.tp, counters=stepper.counters, workspace=stepper.workspace, prebuilt=True)
-            ev[3].record(stream)
-            hmc.hmc_sample_new_radius(so["r"], stepper.phi, stepper.m_cum, so["v_r"], so["v_t"], stepper.tp, so["id"],
-                                      stepper.seed, stepper.step_index, stepper.G, out=stepper.sample,
-                                      counters=stepper.counters, workspace=stepper.workspace, reuse_tables=True)
-        ev[4].record(stream)
-        sm = stepper.sample
-        s["r"], sm["r_new"] = sm["r_new"], s["r"]
-        s["v_r"], sm["v_r_new"] = sm["v_r_new"], s["v_r"]
-        s["v_t"], sm["v_t_new"] = sm["v_t_new"], s["v_t"]
-        s["m"], so["m"] = so["m"], s["m"]
-        s["id"], so["id"] = so["id"], s["id"]
-        stepper.step_index += 1
+        staged_orbit_step(hmc, stepper, ev, stream, args.fused)
 
     mk = lambda: [torch.cuda.Event(enable_timing=True) for _ in range(6)]      # 0-4: stage boundaries, 5: after the table build
     for _ in range(args.warmup):
@@ -371,6 +440,7 @@ def run_gpu(args, cfg):
     sampler.start()
     evs = [mk() for _ in range(args.steps)]
     t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launch = "eager: four C-ABI calls per step, launched one by one"
     use_graph = args.graph == "on" or (args.graph == "auto" and n <= GRAPH_AUTO_MAX_N and args.steps % 2 == 0 and not args.fused)
     if use_graph:
         # small N: a step is bound by launching its kernels one by one.  The timed steps are replays of a CUDA graph of
@@ -386,7 +456,7 @@ def run_gpu(args, cfg):
         stepper.run_graph(args.steps)
         t_end.record(stream)
         gpu_launches = per_two_steps * (args.steps // 2)                      # kernel nodes replayed in the timed region
-        cfg = dict(cfg, launch="timed steps replayed from a CUDA graph of two steps (OrbitStepper.run_graph)")
+        launch = "timed steps replayed from a CUDA graph of two steps (OrbitStepper.run_graph)"
         torch.cuda.synchronize()
         for i in range(args.steps):
             staged_step(evs[i])
@@ -427,7 +497,7 @@ def run_gpu(args, cfg):
             hout = dict(r_new=hin["r"], v_r_new=hin["v_r"], v_t_new=hin["v_t"], m=hin["m"], id=hin["id"])
             hin = nxt
 
-        e2e_steps = max(1, min(args.steps, args.e2e_steps))
+        e2e_steps = max(1, args.steps if args.e2e_steps is None else args.e2e_steps)
         for i in range(2):
             host_step(i)
         torch.cuda.synchronize()
@@ -459,7 +529,9 @@ def run_gpu(args, cfg):
     dom_kernel, dom_ms = cand[dom]
     achieved = model[dom] * n / (dom_ms * 1e-3) / 1e9
     traffic, capture = ncu_traffic_bytes(dom_kernel, n)
-    roofline = dict(bound="hbm", kernel=dom_kernel, stage=dom, achieved=achieved, peak=peak, unit="GB/s",
+    # `bound`: what ncu shows the kernel is limited by (profiles/r2b_ncu_full_summary.txt); `metric_roofline`: the
+    # roofline SURVEY.md 8(d) quotes the metric against, which `achieved`, `peak` and `frac` (= `model_frac`) refer to.
+    roofline = dict(bound="issue", metric_roofline="hbm", kernel=dom_kernel, stage=dom, achieved=achieved, peak=peak, unit="GB/s",
                     frac=achieved / peak, traffic=traffic, peak_source=peak_src,
                     algorithmic_bytes_per_star=model[dom], stars_per_launch=n, launch_ms=dom_ms,
                     launches_timed=args.steps,
@@ -469,6 +541,8 @@ def run_gpu(args, cfg):
                     model_frac=achieved / peak,
                     physical=(dict(dram_bytes_per_launch=traffic, achieved=traffic / (dom_ms * 1e-3) / 1e9,
                                    frac=traffic / (dom_ms * 1e-3) / 1e9 / peak, capture=capture,
+                                   measured_in_this_run=False,      # DRAM bytes: a constant of the committed ncu capture
+
                                    limiter="not streamed bytes: 8 warps per scheduler of dependent fp64 chains and loads "
                                            "(ncu: issue slots 54-56 % used), for turning_points_kernel together with the "
                                            "rate of random 128-byte DRAM lines (profiles/r2b.md, DESIGN.md 5 and 5a)")
@@ -487,6 +561,16 @@ def run_gpu(args, cfg):
                                 frac_of_measured_peak=orbit_bytes * n / (orbit_ms * 1e-3) / 1e9 / peak,
                                 frac_of_8TBs=orbit_bytes * n / (orbit_ms * 1e-3) / 1e9 / 8000.0)
 
+    all_configs = None
+    if world == 1 and not args.no_all_configs and args.n is None and not args.fused:
+        if e2e is None:
+            del stepper
+        else:
+            del arena, hin, hout
+        torch.cuda.empty_cache()
+        all_configs = [time_config(i, args.steps, args.warmup, args.graph, devs, local_rank, peak)
+                       for i in range(len(inputs.CONFIGS)) if i != args.config]
+
     cpu = None
     if world == 1 or rank == 0:
         if not args.no_cpu_baseline:
@@ -496,9 +580,9 @@ def run_gpu(args, cfg):
 
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
                 ms_per_step=ms_max / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
-                data="synthetic", config=cfg, clocks=clocks, e2e=e2e, gpu_launches=gpu_launches,
+                data="synthetic", config=cfg, launch=launch, clocks=clocks, e2e=e2e, gpu_launches=gpu_launches,
                 roofline=roofline, cpu_baseline=cpu, stages=stages, potential_plus_orbit=potential_plus_orbit,
-                counters=counters)
+                counters=counters, all_configs=all_configs)
     print(json.dumps(line))
     return 0
 
@@ -515,7 +599,9 @@ def main(argv=None):
                     help="oracle legs, explicit opt-in: orbit stages on every k-th star, scaled (marks the figure ESTIMATED)")
     ap.add_argument("--ref-variant", default="omp", choices=["omp", "serial"],
                     help="--impl reference: which build of the oracle (omp = all host cores, serial = one core)")
-    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--e2e-steps", type=int, default=None, help="steps of the end-to-end leg (default: --steps)")
+    ap.add_argument("--no-all-configs", action="store_true",
+                    help="skip the device-resident timing of the other four BASELINE.json configs (`all_configs`)")
     ap.add_argument("--fused", action="store_true", help="S3 and S4 as the single call hmc_orbit_step")
     ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
                     help="timed steps as replays of a CUDA graph of two steps (auto: N <= %d and an even --steps)" % GRAPH_AUTO_MAX_N)
