@@ -15,7 +15,8 @@
  *  - Unless a parameter says "host", every array pointer is a DEVICE pointer owned by the
  *    caller.  The library never allocates, frees or keeps device memory between calls; scratch
  *    space is the caller's `workspace` of at least hmc_workspace_bytes(n) bytes, 256-byte aligned.
- *    (The one thing it keeps: hmc_step_host's two streams and their events, see there; and a launch counter.)
+ *    (The one thing it keeps: hmc_step_host's two streams and their events, see there; and a launch counter.
+ *    hmc_potential_static takes no workspace: its scratch is a fixed array inside the library image, see there.)
  *  - Every call is asynchronous on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
  *    legacy default stream) and never synchronises the host.
  *  - Inputs are never modified; outputs must not alias inputs or each other.
@@ -333,7 +334,8 @@ HMC_API hmc_status hmc_diagnostics(uint64_t n, double G,
  * stars" (the expression is in Joshi et al. 2000, not in the paper: DESIGN.md R20 is Henon's scheme).
  * Each pair (2j, 2j+1) undergoes one elastic encounter in its centre-of-mass frame by the deflection angle beta with
  * sin^2(beta/2) = 2 pi G^2 (m_1+m_2)^2 n_b ln(gamma n) dt / w^3 (capped at 1), about a uniformly random axis; the
- * pair's momentum and kinetic energy are conserved.  The angles are Philox4x32-10(counter = (id of the pair's first
+ * pair's momentum and kinetic energy are conserved.  Where that expression has no value -- infinite n_b (a bin of
+ * zero volume) times dt = 0, or a dt that is not finite -- the pair has no encounter (R20a).  The angles are Philox4x32-10(counter = (id of the pair's first
  * star, 1, step, t), key = seed), turned into unit vectors without trigonometric functions.  v_r_out / v_t_out [n]
  * receive the new velocities (an odd last star is copied).  Needs no workspace.  The step is dt, or, when dt_device
  * (DEVICE [1], e.g. t_rel_min of hmc_relaxation_timestep) is not NULL, dt * (*dt_device): no host round trip.

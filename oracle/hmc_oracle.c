@@ -631,6 +631,10 @@ int hmc_ref_two_body_relaxation(uint64_t n, double G, double ln_gamma_n, double 
             continue;
         }
         double S = (((((TWO_PI * (G * G)) * (M * M)) * dens) * ln_gamma_n) * dt) / (w2 * wn);
+        /* DESIGN.md R20a: no encounter where the expression has no value -- S is NaN (a zero-volume bin, density  */
+        /* infinite, with dt = 0: what T_rel's minimum gives when such a bin exists) or dt is not finite (no bin   */
+        /* holds a pair, T_rel = +inf).  Otherwise a step of zero length would turn every such pair head-on.       */
+        if (S != S || !(dt < INFINITY)) S = 0.0;
         if (!(S < 1.0)) S = 1.0;
         if (!(S > 0.0)) S = 0.0;
         double cb = 1.0 - 2.0 * S, sb = 2.0 * sqrt(S * (1.0 - S));

@@ -118,6 +118,8 @@ two_body_relaxation_kernel(uint32_t n, double G, double ln_gamma_n, double dt_in
     double2 out_r = rr, out_t = tt;
     if ((wn > 0.0) && (M > 0.0)) {
         double S = (((((HMC_TWO_PI * (G * G)) * (M * M)) * dens) * ln_gamma_n) * dt) / (w2 * wn);
+        // R20a: no encounter where the expression has no value (S NaN: infinite density times dt = 0; or dt not finite)
+        if (!(S == S) || !(dt < __longlong_as_double(0x7ff0000000000000ll))) S = 0.0;
         if (!(S < 1.0)) S = 1.0;
         if (!(S > 0.0)) S = 0.0;
         const double cb = 1.0 - 2.0 * S, sb = 2.0 * sqrt(S * (1.0 - S));

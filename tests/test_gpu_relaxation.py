@@ -88,6 +88,23 @@ def test_two_body_relaxation_degenerate_pairs(oracle):
     assert o_vr[2] == 0.25 and o_vr[0] == vr[0]
 
 
+def test_zero_length_step_with_a_zero_volume_bin(oracle):
+    """DESIGN.md R20a on the device, driven the way OrbitStepper(relaxation=True) drives it: the step is T_rel's minimum,
+    read from device memory; with a zero-volume bin that minimum is 0 and nothing may move.  Also dt = +inf."""
+    c = sorted_cluster(400, 42)
+    r = c["r"].copy()
+    r[19:40] = r[19]
+    d = [dev(x) for x in (r, c["v_r"], c["v_t"], c["m"])]
+    _, t_min = hmc.hmc_relaxation_timestep(*d)
+    assert float(t_min.cpu()[0]) == 0.0
+    vr, vt = hmc.hmc_two_body_relaxation(d[0], d[1], d[2], d[3], dev(c["id"]), 1.0, 1, 0, dt_device=t_min)
+    assert np.max(np.abs(vr.cpu().numpy() - c["v_r"])) < 1e-15 and np.max(np.abs(vt.cpu().numpy() - c["v_t"])) < 1e-15
+    for dt in (0.0, math.inf, 1e-300):
+        o_vr, o_vt = oracle.two_body_relaxation(r, c["v_r"], c["v_t"], c["m"], c["id"], dt, seed=1, step=0)
+        vr, vt = hmc.hmc_two_body_relaxation(d[0], d[1], d[2], d[3], dev(c["id"]), dt, 1, 0)
+        assert np.array_equal(vr.cpu().numpy(), o_vr) and np.array_equal(vt.cpu().numpy(), o_vt), dt
+
+
 def test_relaxation_inside_the_step_loop(oracle):
     """Potential -> timestep -> relaxation -> new orbits -> sort, three times, GPU chain against oracle chain
     (the paper's order of steps 1-6)."""

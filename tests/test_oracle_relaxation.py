@@ -222,3 +222,22 @@ def test_openmp_build_of_the_relaxation_is_bit_identical(oracle):
     with oracle.use("omp"):
         b = oracle.two_body_relaxation(*args, seed=3, step=1)
     assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+def test_zero_length_step_with_a_zero_volume_bin_moves_nothing(oracle):
+    """DESIGN.md R20a.  Twenty-one tied radii give bin 1 zero volume: its T_rel is 0, so the global step is 0, and a
+    step of zero length must leave every velocity as it was -- also in the tied bin, where sin^2(beta/2) is
+    infinity times zero.  Likewise an infinite step (what T_rel's minimum is when no bin holds a pair) moves nothing,
+    while a finite positive step still turns the pairs of the infinitely dense bin head-on (equal masses swap)."""
+    c = sorted_cluster(400, 42)
+    r, vr, vt, m, ids = c["r"].copy(), c["v_r"], c["v_t"], c["m"], c["id"]
+    r[19:40] = r[19]
+    t_bin, t_min = oracle.relaxation_timestep(r, vr, vt, m)
+    assert t_bin[1] == 0.0 and t_min == 0.0
+    for dt in (t_min, math.inf):
+        a, b = oracle.two_body_relaxation(r, vr, vt, m, ids, dt, seed=1, step=0)
+        assert np.max(np.abs(a - vr)) < 1e-15 and np.max(np.abs(b - vt)) < 1e-15, dt     # up to the rounding of V +- f w
+    a, b = oracle.two_body_relaxation(r, vr, vt, m, ids, 1e-300, seed=1, step=0)
+    sw = lambda x: x.reshape(-1, 2)[:, ::-1].reshape(-1)
+    assert np.max(np.abs(a[20:40] - sw(vr)[20:40])) < 1e-15 and np.max(np.abs(b[20:40] - sw(vt)[20:40])) < 1e-15
+    assert np.max(np.abs(a[40:] - vr[40:])) < 1e-12           # everywhere else 1e-300 is no step at all
