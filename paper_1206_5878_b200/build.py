@@ -1,7 +1,6 @@
 """Build libhmc.so (the C-ABI CUDA library, include/hmc.h) in-tree with nvcc for sm_100a.
 
     python -m paper_1206_5878_b200.build [--force]
-    python -m paper_1206_5878_b200.build --probe     (the stand-alone random-access probe, see build_probe)
 
 nvcc cross-compiles without a GPU.  Flags that matter:
   -gencode arch=compute_100a,code=sm_100a   B200 only, no other target
@@ -85,22 +84,6 @@ def build_all(force: bool = False, verbose: bool = False):
     return [build(force, verbose, v) for v in VARIANTS]
 
 
-PROBE = os.path.join(HERE, "probe_random_access")
-
-
-def build_probe() -> str:
-    """csrc/probe_random_access.cu -> paper_1206_5878_b200/probe_random_access: a stand-alone executable that measures
-    what a random table look-up costs on the GPU it runs on (TLB reach, requests per ns, lanes sharing a line); the
-    numbers behind HMC_S3_PAIRS_MIN_N (profiles/r2_random_access.md).  Not part of libhmc."""
-    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
-                    os.path.join(CSRC, "probe_random_access.cu"), "-o", PROBE], check=True)
-    return PROBE
-
-
 if __name__ == "__main__":
-    if "--probe" in sys.argv:
-        print(build_probe())
-        sys.exit(0)
     for path in build_all(force="--force" in sys.argv, verbose="-v" in sys.argv):
         print(path)

@@ -65,7 +65,7 @@ struct Workspace {
     uint32_t* digit_hist;    // [8][256] global digit counts -> exclusive bin offsets
     uint32_t* lookback;      // [8][sort_tiles][256] tile status words
     uint32_t* tickets;       // [32]: sort tile tickets 0..7, sort pass_live 8..15, scan tickets 16..17
-    // sort, fast path (packed words, hmc_sort.cu)
+    // sort, fast path (packed words, hmc_sort_fast.cu)
     uint64_t* pk_alt;        // [n] second packed-word buffer (the first is keys_alt)
     unsigned char* rec;      // [n] 64-byte star records (r, columns, id)
     uint64_t* sortctl;       // [8]: key minimum, key maximum, long-run flag

@@ -484,7 +484,7 @@ __device__ __forceinline__ Located locate_star(const Tables& T, uint32_t a, doub
 // Tier 3 by lane pairs (warp-collective: all 32 lanes call it together; a lane without a search passes closed
 // sides).  What a random access to a table of gigabytes costs is the REQUEST -- one per load instruction and
 // 128-byte line, about 37 per ns on the whole chip once the table is far beyond the reach of the TLB -- not the
-// bytes (profiles/r2_tlb.md).  A lane that loads nodes p and p+1 itself issues two instructions, hence two requests,
+// bytes (profiles/r2_random_access.md).  A lane that loads nodes p and p+1 itself issues two instructions, hence two requests,
 // and a third to fetch the bracketing node again for the roots.  Here lanes 2i and 2i+1 serve their two stars one
 // after the other: for the star whose turn it is, the even lane loads node p and the odd lane node p+1 in the SAME
 // instruction (one request when both lie in one line, 3 times in 4), each evaluates the sign of Q at its node for
@@ -550,6 +550,34 @@ __device__ __forceinline__ void probe_pairs(const Node* __restrict__ nodes, Side
     }
 }
 
+// Closed-form roots of Q(u) = 2C + 2Bu - J^2 u^2 in the bracketing shells (R3), from their nodes ea (shell k_min) and
+// eb (shell k_max); sets DEGENERATE when the outer quadratic has C >= 0.  Shared by the one-lane and the lane-pair search.
+__device__ __forceinline__ void roots_and_bound(const Node ea, const Node eb, double E, double J2, double& rmin, double& rmax,
+                                                double& Fv, unsigned& st)
+{
+    const double Ca = (E - ea.phi) - ea.B * ea.u;
+    const double Cb = (E - eb.phi) - eb.B * eb.u;
+    double D = ea.B * ea.B + 2.0 * (J2 * Ca);
+    if (D < 0.0) D = 0.0;
+    rmin = J2 / (ea.B + sqrt(D));
+    D = eb.B * eb.B + 2.0 * (J2 * Cb);
+    if (D < 0.0) D = 0.0;
+    if (Cb < 0.0) rmax = (eb.B + sqrt(D)) / (-2.0 * Cb);
+    else { rmax = pos_inf(); st |= HMC_STAR_DEGENERATE; }
+    // S4's bound F (R7) needs G M at both bracketing shells, which are in registers here and
+    // would cost S4 two random node reads per star: computed here and left in the workspace for a
+    // following S4 call with reuse_tables (0 = no draw).  S4 writes F = 1.2 max(sqrt(3 D / q1), sqrt(3 D / -q2));
+    // division and square root are correctly rounded, hence monotone, so the larger square root is the
+    // square root of the larger quotient, which is the quotient by the smaller divisor: the same bits
+    // from one division and one square root instead of two each.
+    const double delta = rmax - rmin;
+    if (!(st & HMC_STAR_DEGENERATE) && delta > 0.0) {
+        const double q1 = (2.0 * (J2 / rmin - ea.B)) / (rmin * rmin);      // Q'(r_min) in shell k_min
+        const double q2 = (2.0 * (J2 / rmax - eb.B)) / (rmax * rmax);      // Q'(r_max) in shell k_max
+        if ((q1 > 0.0) && (q2 < 0.0)) Fv = 1.2 * sqrt((3.0 * delta) / fmin(q1, -q2));
+    }
+}
+
 __device__ __forceinline__ Solved finish_star_s3(const Tables& T, uint32_t a, const Located& L)
 {
     const Node* __restrict__ nodes = T.nodes;
@@ -576,29 +604,7 @@ __device__ __forceinline__ Solved finish_star_s3(const Tables& T, uint32_t a, co
             if (a2) s2.update(p2, !q_negative(e20.r, e20.phi, E, J2), !q_negative(e21.r, e21.phi, E, J2));
         }
         kmin = s1.lo; kmax = s2.lo;
-        // closed-form roots of Q(u) = 2C + 2Bu - J^2 u^2 in the bracketing shells (R3)
-        const Node ea = ld_node(nodes + kmin), eb = ld_node(nodes + kmax);
-        const double Ca = (E - ea.phi) - ea.B * ea.u;
-        const double Cb = (E - eb.phi) - eb.B * eb.u;
-        double D = ea.B * ea.B + 2.0 * (J2 * Ca);
-        if (D < 0.0) D = 0.0;
-        rmin = J2 / (ea.B + sqrt(D));
-        D = eb.B * eb.B + 2.0 * (J2 * Cb);
-        if (D < 0.0) D = 0.0;
-        if (Cb < 0.0) rmax = (eb.B + sqrt(D)) / (-2.0 * Cb);
-        else { rmax = pos_inf(); st |= HMC_STAR_DEGENERATE; }
-        // S4's bound F (R7) needs G M at both bracketing shells, which are in registers here and
-        // would cost S4 two random node reads per star: computed here and left in the workspace for a
-        // following S4 call with reuse_tables (0 = no draw).  S4 writes F = 1.2 max(sqrt(3 D / q1), sqrt(3 D / -q2));
-        // division and square root are correctly rounded, hence monotone, so the larger square root is the
-        // square root of the larger quotient, which is the quotient by the smaller divisor: the same bits
-        // from one division and one square root instead of two each.
-        const double delta = rmax - rmin;
-        if (!(st & HMC_STAR_DEGENERATE) && delta > 0.0) {
-            const double q1 = (2.0 * (J2 / rmin - ea.B)) / (rmin * rmin);      // Q'(r_min) in shell k_min
-            const double q2 = (2.0 * (J2 / rmax - eb.B)) / (rmax * rmax);      // Q'(r_max) in shell k_max
-            if ((q1 > 0.0) && (q2 < 0.0)) Fv = 1.2 * sqrt((3.0 * delta) / fmin(q1, -q2));
-        }
+        roots_and_bound(ld_node(nodes + kmin), ld_node(nodes + kmax), E, J2, rmin, rmax, Fv, st);
     }
     return Solved{ E, J, rmin, rmax, Fv, kmin, kmax, st };
 }
@@ -623,29 +629,7 @@ __device__ __forceinline__ Solved finish_star_s3_pairs(const Tables& T, uint32_t
         rmax = (st & HMC_STAR_UNBOUND) ? pos_inf() : rk;
     } else if (valid) {
         kmin = s1.lo; kmax = s2.lo;
-        // closed-form roots of Q(u) = 2C + 2Bu - J^2 u^2 in the bracketing shells (R3)
-        const Node ea = have_a ? ka : ld_node(nodes + kmin), eb = have_b ? kb : ld_node(nodes + kmax);
-        const double Ca = (E - ea.phi) - ea.B * ea.u;
-        const double Cb = (E - eb.phi) - eb.B * eb.u;
-        double D = ea.B * ea.B + 2.0 * (J2 * Ca);
-        if (D < 0.0) D = 0.0;
-        rmin = J2 / (ea.B + sqrt(D));
-        D = eb.B * eb.B + 2.0 * (J2 * Cb);
-        if (D < 0.0) D = 0.0;
-        if (Cb < 0.0) rmax = (eb.B + sqrt(D)) / (-2.0 * Cb);
-        else { rmax = pos_inf(); st |= HMC_STAR_DEGENERATE; }
-        // S4's bound F (R7) needs G M at both bracketing shells, which are in registers here and
-        // would cost S4 two random node reads per star: computed here and left in the workspace for a
-        // following S4 call with reuse_tables (0 = no draw).  S4 writes F = 1.2 max(sqrt(3 D / q1), sqrt(3 D / -q2));
-        // division and square root are correctly rounded, hence monotone, so the larger square root is the
-        // square root of the larger quotient, which is the quotient by the smaller divisor: the same bits
-        // from one division and one square root instead of two each.
-        const double delta = rmax - rmin;
-        if (!(st & HMC_STAR_DEGENERATE) && delta > 0.0) {
-            const double q1 = (2.0 * (J2 / rmin - ea.B)) / (rmin * rmin);      // Q'(r_min) in shell k_min
-            const double q2 = (2.0 * (J2 / rmax - eb.B)) / (rmax * rmax);      // Q'(r_max) in shell k_max
-            if ((q1 > 0.0) && (q2 < 0.0)) Fv = 1.2 * sqrt((3.0 * delta) / fmin(q1, -q2));
-        }
+        roots_and_bound(have_a ? ka : ld_node(nodes + kmin), have_b ? kb : ld_node(nodes + kmax), E, J2, rmin, rmax, Fv, st);
     }
     return Solved{ E, J, rmin, rmax, Fv, kmin, kmax, st };
 }

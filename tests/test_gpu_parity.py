@@ -261,7 +261,8 @@ def test_config1_whole_step_chained(oracle):
 
 
 def test_config2_eleven_chained_steps(oracle):
-    """BASELINE.json configs[1] at reduced N (same recipe, seed 2): 1 + 10 steps re-sorting each step.
+    """A quick version of BASELINE.json configs[1] at N = 60 000 (same recipe, seed 2): 1 + 10 steps re-sorting each
+    step; tests/test_gpu_fullsize.py::test_config2_1e6_eleven_steps runs the config itself at its full N = 1e6.
     The oracle is fed its own previous output; the GPU its own.  Any divergence would compound."""
     cfg = inputs.config(1, n_override=60_000)
     c = {k: cfg[k] for k in ("r", "v_r", "v_t", "m", "id")}
@@ -528,7 +529,7 @@ def test_repeated_steps_are_bit_reproducible():
     """The same step run ten times from the same state writes the same bits every time, every array.  The sort's
     decoupled look-back, the sampler's dynamic batches and the shared-memory parking all order their work
     differently from run to run; a data race would show as a difference (compute-sanitizer is closed on this pool:
-    profiles/r2.md).  Covers the fast sort path, the fallback sort (runs of 200 near-equal keys) and the fused call."""
+    profiles/r2b.md).  Covers the fast sort path, the fallback sort (runs of 200 near-equal keys) and the fused call."""
     n, seed = 400_003, 61
     c = inputs.plummer(n, seed, "salpeter")
     r = c["r"].copy()

@@ -83,7 +83,20 @@ def test_roots_satisfy_eq12_with_brute_force_potential(oracle):
             assert R[j] * (1 - 1e-12) <= x <= R[j + 1] * (1 + 1e-12)              # root inside its shell
         assert tp["r_min"][a] <= r[a] * (1 + 1e-12) and r[a] <= tp["r_max"][a] * (1 + 1e-12)
     assert worst < 1e-13
-    assert (tp["k_min"] == 0).sum() + (tp["k_max"] == n).sum() >= 0
+
+
+def test_both_sentinel_shells_occur_in_a_plummer_cluster(oracle):
+    """at N = 2e5 about 0.03 % of the stars have their pericentre inside the innermost star
+    (k_min = 0) and a few in 1e5 their apocentre beyond the outermost (k_max = N), so natural inputs reach both
+    sentinel nodes of the table; their roots still bracket the star."""
+    n = 200_000
+    c = sorted_cluster(n, 23)
+    phi, mc = oracle.potential(c["r"], c["m"])
+    tp = oracle.orbit_turning_points(c["r"], c["v_r"], c["v_t"], phi, mc)
+    inner, outer = tp["k_min"] == 0, tp["k_max"] == n
+    assert 20 <= inner.sum() <= 200 and 1 <= outer.sum() <= 20
+    assert np.all(tp["r_min"][inner] <= c["r"][0]) and np.all(tp["r_min"][inner] > 0)
+    assert np.all(tp["r_max"][outer] >= c["r"][-1]) and np.all(np.isfinite(tp["r_max"][outer]))
 
 
 def test_sentinel_shells_are_exercised(oracle):
