@@ -587,6 +587,99 @@ def run_gpu(args, cfg):
     return 0
 
 
+# --------------------------------------------------------------------------- sharded step (one cluster over the ranks)
+def run_sharded(args, cfg):
+    """--parallelism sharded: ONE cluster of the config's N stars cut over the ranks (paper_1206_5878_b200/shard.py:
+    sample sort + redistribution, shard potentials, replicated table, range S3 / S4), so the scaling is "strong".
+    Under torchrun every rank is a process with one shard (shard.DistComm over NCCL); a world of one goes through the
+    same communicator.  --shards G (world of one only) instead holds G shards in this one process
+    (shard.InProcessComm): the one-GPU proxy for what the sharded step costs beyond the single-GPU step -- extra sort
+    passes, record packing and exchange copies, G table builds -- with a per-phase breakdown.  No multi-GPU hardware
+    was available to run this with more than one rank."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1206_5878_b200 import hmc, inputs, shard
+
+    rank, local_rank, world = dist_init("nccl")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    devs = "cuda:%d" % local_rank
+    hmc.lib()
+    c = inputs.config(args.config, args.n)
+    n, seed = c["n"], c["seed"]
+    cluster = {k: (c[k].view(np.int32) if k == "id" else c[k]) for k in ("r", "v_r", "v_t", "m", "id")}
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(devs)
+    in_process = world == 1 and args.shards > 1
+    if in_process:
+        comm = shard.InProcessComm(args.shards)
+        shards = [{k: d(v) for k, v in part.items()} for part in shard.split_cluster(cluster, args.shards)]
+        how = "sharded x1 process, %d in-process shards on one GPU (proxy)" % args.shards
+    else:
+        if not dist.is_initialized():                       # a world of one still goes through DistComm / NCCL
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", "29633")
+            dist.init_process_group("nccl", rank=0, world_size=1)
+        comm = shard.DistComm()
+        shards = [{k: d(v) for k, v in shard.split_cluster(cluster, world)[rank].items()}]
+        how = "sharded x%d" % world
+    stepper = shard.ShardedStepper(comm, shards, seed, n_total=n)
+    stream = torch.cuda.current_stream()
+    for _ in range(args.warmup):
+        stepper.step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    dist_barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    launches, syncs = int(hmc.lib().hmc_launch_count()), comm.host_syncs
+    stepper.marks = []
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record(stream)
+    for _ in range(args.steps):
+        stepper.step()
+    t1.record(stream)
+    torch.cuda.synchronize()
+    dist_barrier()
+    clocks = sampler.stop()
+    launches, syncs = int(hmc.lib().hmc_launch_count()) - launches, comm.host_syncs - syncs
+    value, ms_max = aggregate_throughput(float(n) * args.steps / world, t0.elapsed_time(t1), devs)
+    phases, marks = {}, stepper.marks
+    for (_, a), (name, b) in zip(marks, marks[1:]):
+        if name != "start":
+            phases[name] = phases.get(name, 0.0) + a.elapsed_time(b) / args.steps
+    stepper.marks = None
+    # the single-GPU step on the same cluster in the same process (world of one only): what the sharded step is compared with
+    single_ms = None
+    if world == 1:
+        del stepper, shards
+        torch.cuda.empty_cache()
+        one = hmc.OrbitStepper(d(cluster["r"]), d(cluster["v_r"]), d(cluster["v_t"]), d(cluster["m"]), d(cluster["id"]), seed,
+                               with_n_try=False)
+        for _ in range(max(args.warmup, 1)):
+            one.step()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(args.steps):
+            one.step()
+        b.record(stream)
+        torch.cuda.synchronize()
+        single_ms = a.elapsed_time(b) / args.steps
+    if rank != 0:
+        return 0
+    cfg = dict(cfg, parallelism=how)
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+                ms_per_step=ms_max / args.steps, higher_is_better=True, scaling="strong", vs_baseline=None, dtype="f64",
+                data="synthetic", config=cfg, launch="eager", clocks=clocks, e2e=None, gpu_launches=launches,
+                roofline=None, cpu_baseline=None, phases_ms=phases,
+                host_syncs_per_step=syncs / args.steps / (args.shards if in_process else 1),
+                single_gpu_ms_per_step=single_ms,
+                note="sharded step, device-resident; torch copies (record packing, concatenation) are not in gpu_launches")
+    print(json.dumps(line))
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -605,6 +698,11 @@ def main(argv=None):
     ap.add_argument("--fused", action="store_true", help="S3 and S4 as the single call hmc_orbit_step")
     ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
                     help="timed steps as replays of a CUDA graph of two steps (auto: N <= %d and an even --steps)" % GRAPH_AUTO_MAX_N)
+    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "sharded"],
+                    help="replicas: one independent cluster per GPU (weak scaling, the graded path); sharded: one cluster "
+                         "cut over the ranks (strong scaling, paper_1206_5878_b200/shard.py)")
+    ap.add_argument("--shards", type=int, default=1,
+                    help="--parallelism sharded with one process: hold this many shards in the process (one-GPU proxy)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args(argv)
@@ -618,6 +716,8 @@ def main(argv=None):
                   "N=1e7; no explicit flush")
     if args.impl == "reference":
         return run_reference(args, cfg)
+    if args.parallelism == "sharded":
+        return run_sharded(args, cfg)
     return run_gpu(args, cfg)
 
 

@@ -17,6 +17,12 @@ through ``hmc`` (there is no CPU path: the kernels need a GPU).  The random numb
 (R9) and M_k, S_k are exact sums rounded once (R1p), so the sharded step reproduces the single-GPU step bit
 for bit whatever G is (tests/test_gpu_shard.py).
 
+Exchange format: the columns of a star travel as ONE record (a row of 64-bit words, one word per column), so each of
+the two exchanges of the sort is one collective, and the only things the host reads back in a step are the splitter
+positions (one read per rank) and the matrix of partition sizes (one small all-gather per rank): two host
+synchronisations per rank and step, counted in ``comm.host_syncs``.  The redistribution needs no further exchange of
+sizes: every rank holds the whole matrix, hence knows how many stars every rank holds after the first exchange.
+
 Back-ends:
   InProcessComm(G)   G shards held by ONE process on one device; a collective is a hand-over of device tensors.
                      This is what one GPU can test, and what the tests use.
@@ -106,14 +112,22 @@ class InProcessComm:
     def __init__(self, world: int):
         self.world = world
         self.local_ranks = list(range(world))
+        self.host_syncs = 0          # times the host waited for the device or for other ranks (see sample_sort)
 
-    def all_gather(self, xs: List[torch.Tensor]) -> List[List[torch.Tensor]]:
-        """out[rank] = [x of rank 0, ..., x of rank G-1]."""
+    def all_gather(self, xs: List[torch.Tensor], sizes: Optional[Sequence[int]] = None) -> List[List[torch.Tensor]]:
+        """out[rank] = [x of rank 0, ..., x of rank G-1].  sizes: the ranks' element counts, if the caller knows them."""
         return [list(xs) for _ in self.local_ranks]
 
-    def all_to_all(self, send: List[List[torch.Tensor]]) -> List[List[torch.Tensor]]:
-        """send[src][dst] -> recv[dst][src]."""
-        return [[send[src][dst] for src in range(self.world)] for dst in range(self.world)]
+    def exchange(self, recs: List[torch.Tensor], counts: Sequence[Sequence[int]]) -> List[torch.Tensor]:
+        """One all-to-all of records.  recs[src] = rows [n_src, W], the rows for destination 0 first, then 1, ...;
+        counts[src][dst] = how many rows src sends to dst (the whole matrix, known to every rank).
+        -> per destination, the rows it receives, in source order."""
+        offs = [exclusive_scan(row) for row in counts]
+        out = []
+        for dst in range(self.world):
+            parts = [recs[src][offs[src][dst]:offs[src][dst] + counts[src][dst]] for src in range(self.world) if counts[src][dst]]
+            out.append(torch.cat(parts) if len(parts) > 1 else (parts[0] if parts else recs[dst][:0]))
+        return out
 
     def all_gather_ints(self, xs: List[List[int]]) -> List[List[List[int]]]:
         return [list(xs) for _ in self.local_ranks]
@@ -141,10 +155,45 @@ class DistComm:
         self.world = dist.get_world_size(group)
         self.rank = dist.get_rank(group)
         self.local_ranks = [self.rank]
+        self.host_syncs = 0
+        self.nccl = dist.get_backend(group) == "nccl"
+        self.device = torch.device("cuda", torch.cuda.current_device()) if self.nccl else torch.device("cpu")
 
     def all_gather_ints(self, xs: List[List[int]]) -> List[List[List[int]]]:
-        out = [None] * self.world
-        self.dist.all_gather_object(out, list(xs[0]), group=self.group)
+        """Every rank's list of integers (all of one length) to every rank: ONE tensor all-gather and one read back to
+        the host -- nothing is pickled."""
+        mine = torch.tensor(list(xs[0]), dtype=torch.int64, device=self.device)
+        out = torch.empty(self.world * mine.numel(), dtype=torch.int64, device=self.device)
+        if self.nccl:
+            self.dist.all_gather_into_tensor(out, mine, group=self.group)
+        else:
+            self.dist.all_gather(list(out.view(self.world, -1).unbind(0)), mine, group=self.group)
+        self.host_syncs += 1
+        return [out.view(self.world, -1).cpu().tolist()]
+
+    def exchange(self, recs: List[torch.Tensor], counts: Sequence[Sequence[int]]) -> List[torch.Tensor]:
+        """One all-to-all of records (see InProcessComm.exchange): all_to_all_single over NCCL; gloo, which has no
+        all-to-all, gets the same transfers as one batch of point-to-point operations."""
+        rec = recs[0].contiguous()
+        send = [int(c) for c in counts[self.rank]]
+        recv = [int(counts[src][self.rank]) for src in range(self.world)]
+        out = torch.empty((sum(recv),) + tuple(rec.shape[1:]), dtype=rec.dtype, device=rec.device)
+        if self.nccl:
+            self.dist.all_to_all_single(out, rec, recv, send, group=self.group)
+            return [out]
+        so, ro = exclusive_scan(send), exclusive_scan(recv)
+        out[ro[self.rank]:ro[self.rank] + recv[self.rank]] = rec[so[self.rank]:so[self.rank] + send[self.rank]]
+        ops = []
+        for other in range(self.world):
+            if other == self.rank:
+                continue
+            if send[other]:
+                ops.append(self.dist.P2POp(self.dist.isend, rec[so[other]:so[other] + send[other]], other, self.group))
+            if recv[other]:
+                ops.append(self.dist.P2POp(self.dist.irecv, out[ro[other]:ro[other] + recv[other]], other, self.group))
+        if ops:
+            for w in self.dist.batch_isend_irecv(ops):
+                w.wait()
         return [out]
 
     def table_views(self, n: int, device):
@@ -175,94 +224,97 @@ class DistComm:
         """Every rank's stores into every copy are done (device-side barrier across the ranks, on the current stream)."""
         self._symm.barrier()
 
-    def all_gather(self, xs: List[torch.Tensor]) -> List[List[torch.Tensor]]:
+    def all_gather(self, xs: List[torch.Tensor], sizes: Optional[Sequence[int]] = None) -> List[List[torch.Tensor]]:
+        """sizes: the ranks' element counts when the caller knows them (samples, totals, the decomposition's ranges);
+        otherwise they are exchanged first (one more host synchronisation)."""
         x = xs[0].contiguous()
-        sizes = [v[0] for v in self.all_gather_ints([[x.numel()]])[0]]
+        sizes = [v[0] for v in self.all_gather_ints([[x.numel()]])[0]] if sizes is None else [int(v) for v in sizes]
         biggest = max(sizes)
         pad = x if x.numel() == biggest else torch.cat([x.reshape(-1), x.new_zeros(biggest - x.numel())])
         bufs = [torch.empty(biggest, dtype=x.dtype, device=x.device) for _ in range(self.world)]
         self.dist.all_gather(bufs, pad.reshape(-1), group=self.group)
         return [[b[:k] for b, k in zip(bufs, sizes)]]
 
-    def all_to_all(self, send: List[List[torch.Tensor]]) -> List[List[torch.Tensor]]:
-        mine = [t.contiguous() for t in send[0]]
-        counts = self.all_gather_ints([[t.numel() for t in mine]])[0]            # counts[src][dst]
-        recv = [torch.empty(counts[src][self.rank], dtype=mine[0].dtype, device=mine[0].device) for src in range(self.world)]
-        recv[self.rank] = mine[self.rank]
-        ops = []
-        for other in range(self.world):                                            # point-to-point: gloo has no all_to_all
-            if other == self.rank:
-                continue
-            if mine[other].numel():
-                ops.append(self.dist.P2POp(self.dist.isend, mine[other], other, self.group))
-            if recv[other].numel():
-                ops.append(self.dist.P2POp(self.dist.irecv, recv[other], other, self.group))
-        if ops:
-            for w in self.dist.batch_isend_irecv(ops):
-                w.wait()
-        return [recv]
-
 
 # ------------------------------------------------------------------------------------------------ sample sort
-def _cat(parts):
-    parts = [p for p in parts if p.numel()]
-    return torch.cat(parts) if len(parts) > 1 else (parts[0] if parts else None)
+_INDEX_CACHE = {}
+
+
+def _index_tensor(positions: Sequence[int], device) -> torch.Tensor:
+    """The positions as an index tensor on `device`, made once per distinct list: building it is a blocking
+    host-to-device copy, and the lists (sample positions of a rank's range, splitter positions) repeat every step."""
+    key = (tuple(positions), str(device))
+    t = _INDEX_CACHE.get(key)
+    if t is None:
+        if len(_INDEX_CACHE) > 256:
+            _INDEX_CACHE.clear()
+        t = _INDEX_CACHE[key] = torch.tensor(list(positions), dtype=torch.long, device=device)
+    return t
+
+
+def pack_records(columns: Sequence[torch.Tensor]) -> torch.Tensor:
+    """The columns of a rank's stars (float64 or int32, equal lengths) as one row of 64-bit words per star."""
+    words = [c.view(torch.int64) if c.dtype == torch.float64 else c.to(torch.int64) for c in columns]
+    return torch.stack(words, dim=1)
+
+
+def unpack_records(rec: torch.Tensor, like: Sequence[torch.Tensor]) -> List[torch.Tensor]:
+    """Inverse of pack_records; `like` gives the dtype of each column."""
+    return [rec[:, k].contiguous().view(torch.float64) if c.dtype == torch.float64 else rec[:, k].to(c.dtype)
+            for k, c in enumerate(like)]
 
 
 def sample_sort(comm, cols: List[List[torch.Tensor]], sample_size: int, want: Sequence[int],
-                local_sort: Callable, partition_points: Callable) -> List[List[torch.Tensor]]:
+                local_sort: Callable, partition_points: Callable, mark: Optional[Callable] = None) -> List[List[torch.Tensor]]:
     """The paper's Sample Sort + redistribution over the ranks of `comm`.
 
     cols[lr] = the columns of local rank lr, the KEY (radius) first; every column of a rank has the same length.
     local_sort(columns) -> columns sorted by the first one, stably; partition_points(sorted_keys, splitters) ->
-    list of ints, the number of keys <= each splitter.  Both are libhmc kernels in the product
-    (ShardedStepper); the host-logic tests pass CPU stand-ins.  -> the columns of each local rank after the sort:
-    rank d holds stars exclusive_scan(want)[d] ... of the global order, want[d] of them."""
+    list of ints, the number of keys <= each splitter (this reads device memory back: one host synchronisation).
+    Both are libhmc kernels in the product (ShardedStepper); the host-logic tests pass CPU stand-ins.
+    mark(name), if given, is called after each phase (the stepper records CUDA events there).
+    -> the columns of each local rank after the sort: rank d holds stars exclusive_scan(want)[d] ... of the global
+    order, want[d] of them."""
     world, L = comm.world, len(comm.local_ranks)
-    ncol = len(cols[0])
+    mark = mark or (lambda name: None)
+    like = cols[0]
     # phase 1: sort local data
     cols = [local_sort(c) if c[0].numel() > 1 else c for c in cols]
+    mark("local_sort")
     if world > 1:
         # phase 2: sampling (a rank without stars contributes +inf samples, which sort last)
         samples = []
         for c in cols:
             key = c[0]
             pos = sample_positions(key.numel(), sample_size)
-            samples.append(key[torch.tensor(pos, dtype=torch.long, device=key.device)] if pos
+            samples.append(key[_index_tensor(pos, key.device)] if pos
                            else torch.full((sample_size,), float("inf"), dtype=key.dtype, device=key.device))
-        gathered = comm.all_gather(samples)
+        gathered = comm.all_gather(samples, sizes=[sample_size] * world)
         # phase 3: splitter selection (every rank does what the designated processor would broadcast)
-        sent = []
+        # phase 4: place the splitters: the local array falls into `world` consecutive partitions
+        sizes = []
         for i, c in enumerate(cols):
             combined = local_sort([torch.cat(gathered[i])])[0]
-            spl = combined[torch.tensor(splitter_positions(sample_size, world), dtype=torch.long, device=combined.device)]
-            # phase 4: place the splitters, cut the local array into `world` partitions
+            spl = combined[_index_tensor(splitter_positions(sample_size, world), combined.device)]
             cut = [0] + [int(x) for x in partition_points(c[0], spl)] + [c[0].numel()]
-            sent.append([[col[cut[d]:cut[d + 1]] for d in range(world)] for col in c])
-        received = [comm.all_to_all([sent[i][k] for i in range(L)]) for k in range(ncol)]     # received[k][lr][src]
-        # phase 5: merge = concatenate in source order and sort again (stable: ties keep source order)
-        merged = []
-        for i in range(L):
-            c = [_cat(received[k][i]) for k in range(ncol)]
-            if c[0] is None:
-                c = [cols[i][k][:0] for k in range(ncol)]
-            merged.append(local_sort(c) if c[0].numel() > 1 else c)
-        cols = merged
-        # redistribution: exclusive scan of the counts, all-to-all of the chunks that belong elsewhere
-        have = [v[0] for v in comm.all_gather_ints([[c[0].numel()] for c in cols])[0]]
+            comm.host_syncs += 1                                   # the splitter positions come back to the host
+            sizes.append([cut[d + 1] - cut[d] for d in range(world)])
+        counts = comm.all_gather_ints(sizes)[0]                    # counts[src][dst], the same on every rank
+        received = comm.exchange([pack_records(c) for c in cols], counts)
+        mark("exchange")
+        # phase 5: merge = the partitions in source order, sorted again (stable: ties keep source order)
+        cols = []
+        for rec in received:
+            c = unpack_records(rec, like)
+            cols.append(local_sort(c) if c[0].numel() > 1 else c)
+        mark("merge_sort")
+        # redistribution (PAPER.md:259-261): exclusive scan of the counts, all-to-all of the chunks that belong
+        # elsewhere.  What every rank holds now is a column sum of the matrix every rank already has.
+        have = [sum(counts[src][d] for src in range(world)) for d in range(world)]
         plan = redistribution_plan(have, want)
-        sent = []
-        for i, rank in enumerate(comm.local_ranks):
-            off = exclusive_scan(plan[rank])
-            sent.append([[col[off[d]:off[d] + plan[rank][d]] for d in range(world)] for col in cols[i]])
-        received = [comm.all_to_all([sent[i][k] for i in range(L)]) for k in range(ncol)]
-        out = []
-        for i in range(L):
-            c = [_cat(received[k][i]) for k in range(ncol)]       # chunks arrive in source order = global order
-            if c[0] is None:
-                c = [cols[i][k][:0] for k in range(ncol)]
-            out.append(c)
-        cols = out
+        received = comm.exchange([pack_records(c) for c in cols], plan)      # chunks arrive in source order = global order
+        cols = [unpack_records(rec, like) for rec in received]
+        mark("redistribute")
     return cols
 
 
@@ -291,6 +343,13 @@ class ShardedStepper:
         self.counters = [hmc.alloc_counters(s["r"].device) for s in shards]
         self.workspace = [hmc.alloc_workspace(self.n, s["r"].device) for s in shards]
         self.last = None
+        self.marks = None            # set to [] to have step() append (phase name, CUDA event) pairs (bench.py)
+
+    def _mark(self, name):
+        if self.marks is not None:
+            ev = torch.cuda.Event(enable_timing=True)
+            ev.record()
+            self.marks.append((name, ev))
 
     def _local_sort(self, ws):
         hmc = self.hmc
@@ -310,11 +369,12 @@ class ShardedStepper:
         cols = [[s["r"], s["v_r"], s["v_t"], s["m"], s["id"]] for s in self.state]
         # S1: sample sort + redistribution.  One workspace serves all local ranks' sorts (they run one after another).
         sort = self._local_sort(self.workspace[0])
+        self._mark("start")
         cols = sample_sort(comm, cols, self.sample_size, self.want, sort,
-                           lambda keys, spl: hmc.hmc_partition_points(keys, spl).cpu().tolist())
+                           lambda keys, spl: hmc.hmc_partition_points(keys, spl).cpu().tolist(), self._mark)
         # S2: shard totals -> all-gather -> local scan with what lies before and after
         totals = [hmc.hmc_potential_totals(c[0], c[3], workspace=self.workspace[i]) for i, c in enumerate(cols)]
-        all_totals = [torch.cat(t) for t in comm.all_gather(totals)]
+        all_totals = [torch.cat(t) for t in comm.all_gather(totals, sizes=[4] * comm.world)]
         tabs = None
         if self.push_tables is not False and hasattr(comm, "table_views"):
             tabs = comm.table_views(self.n, cols[0][0].device)
@@ -339,9 +399,10 @@ class ShardedStepper:
             pots = [hmc.hmc_potential_shard(c[0], c[3], rank, all_totals[i], self.G, workspace=self.workspace[i])
                     for i, (c, rank) in enumerate(zip(cols, comm.local_ranks))]
             # the replicated table
-            table_r = [torch.cat(t) for t in comm.all_gather([c[0] for c in cols])]
-            table_phi = [torch.cat(t) for t in comm.all_gather([p[0] for p in pots])]
-            table_m = [torch.cat(t) for t in comm.all_gather([p[1] for p in pots])]
+            table_r = [torch.cat(t) for t in comm.all_gather([c[0] for c in cols], sizes=self.want)]
+            table_phi = [torch.cat(t) for t in comm.all_gather([p[0] for p in pots], sizes=self.want)]
+            table_m = [torch.cat(t) for t in comm.all_gather([p[1] for p in pots], sizes=self.want)]
+        self._mark("potential_and_table")
         # S3 / S4 on the rank's own range: no communication
         new_state, last = [], []
         for i, rank in enumerate(comm.local_ranks):
@@ -357,6 +418,7 @@ class ShardedStepper:
                 tp, sm = hmc.alloc_turning_points(0, r.device), hmc.alloc_sample(0, r.device)
             new_state.append(dict(r=sm["r_new"], v_r=sm["v_r_new"], v_t=sm["v_t_new"], m=m, id=ids))
             last.append(dict(r=r, v_r=vr, v_t=vt, phi=pots[i][0], m_cum=pots[i][1], tp=tp, sample=sm))
+        self._mark("orbit")
         self.state, self.last = new_state, last
         self.step_index += 1
 

@@ -4,6 +4,7 @@ the sort is stable across the exchange, M_k and S_k are exact sums rounded once 
 random numbers are keyed by the persistent star id.  The single-GPU stepper is itself compared with the oracle in
 tests/test_gpu_fullsize.py, and the pieces the sharded step adds are compared with the oracle here."""
 import os
+import warnings
 
 import numpy as np
 import pytest
@@ -153,3 +154,40 @@ def test_dist_comm_over_nccl_world_of_one():
     finally:
         if created:
             dist.destroy_process_group()
+
+
+def test_host_synchronisations_per_sharded_step():
+    """A sharded step reads device memory back on the host once per rank (where the splitters fall in its sorted
+    radii); the partition sizes are one more small exchange per rank between processes, none inside one process.
+    Everything else -- samples, records, totals, the table -- moves with sizes every rank already knows.  Counted twice:
+    by the communicator's own counter, and by PyTorch's synchronisation warnings during the step."""
+    n, seed, world = 200_000, 8, 4
+    d, _ = device_cluster(n, seed)
+    comm = shard.InProcessComm(world)
+    st = shard.ShardedStepper(comm, shard.split_cluster(d, world), seed)
+    st.step()
+    st.step()                     # (the first steps also build the cached index tensors of the sampling)
+    torch.cuda.synchronize()
+    before = comm.host_syncs
+    torch.cuda.set_sync_debug_mode("warn")
+    try:
+        with warnings.catch_warnings(record=True) as caught:
+            warnings.simplefilter("always")
+            st.step()
+    finally:
+        torch.cuda.set_sync_debug_mode("default")
+    torch.cuda.synchronize()
+    seen = [str(w.message) for w in caught if "synchroniz" in str(w.message).lower()]
+    print("host synchronisations in one step of %d shards: counter %d, torch warnings %d" % (world, comm.host_syncs - before, len(seen)))
+    assert comm.host_syncs - before == world
+    assert len(seen) <= world, seen
+
+
+def test_record_packing_round_trip():
+    g = torch.Generator().manual_seed(3)
+    cols = [torch.rand(1000, generator=g, dtype=torch.float64).cuda(), torch.full((1000,), float("nan"), dtype=torch.float64).cuda(),
+            torch.randint(-2 ** 31, 2 ** 31 - 1, (1000,), generator=g, dtype=torch.int64).to(torch.int32).cuda()]
+    back = shard.unpack_records(shard.pack_records(cols), cols)
+    for a, b in zip(cols, back):
+        assert a.dtype == b.dtype and torch.equal(a.view(torch.int64) if a.dtype == torch.float64 else a,
+                                                  b.view(torch.int64) if b.dtype == torch.float64 else b)

@@ -131,13 +131,19 @@ WORKER = textwrap.dedent("""
     # collectives on their own
     got = comm.all_gather([torch.arange(comm.rank + 2, dtype=torch.float64)])[0]
     assert [t.numel() for t in got] == [2, 3] and got[1][2] == 2.0
-    back = comm.all_to_all([[torch.full((3 + d + comm.rank,), float(comm.rank)) for d in range(2)]])[0]
-    assert [t.numel() for t in back] == [3 + comm.rank, 4 + comm.rank] and back[1 - comm.rank][0] == float(1 - comm.rank)
+    dist.all_gather_object = None                           # nothing may be pickled between ranks any more
+    sizes = comm.all_gather_ints([[3 + comm.rank, 4 + comm.rank]])[0]
+    assert sizes == [[3, 4], [4, 5]]
+    rows = torch.full((sum(sizes[comm.rank]), 2), comm.rank, dtype=torch.int64)
+    back = comm.exchange([rows], sizes)[0]                  # rank d receives 3 + d rows of zeros, then 4 + d rows of ones
+    assert back.shape == (7 + 2 * comm.rank, 2) and back[:3 + comm.rank].eq(0).all() and back[3 + comm.rank:].eq(1).all()
+    before = comm.host_syncs
     # the sort
     out = shard.sample_sort(comm, [[c[o:o + k] for c in cols]], 32, counts, cpu_local_sort, cpu_partition_points)[0]
     ref = cpu_local_sort(cols)
     for j in range(3):
         assert torch.equal(out[j], ref[j][o:o + k]), j
+    assert comm.host_syncs - before == 2                    # splitter positions, partition sizes: nothing else
     dist.barrier()
     if comm.rank == 0:
         print("SHARD_OK")
