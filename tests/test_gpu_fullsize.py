@@ -181,6 +181,14 @@ def test_second_search_table_with_the_pair_search(oracle, monkeypatch):
     run_self_chained(oracle, 2, n_override=12_000_000, steps=1)
 
 
+def test_product_large_n_path_on_every_star_at_2_to_the_25(oracle):
+    """N = 2^25 = 33 554 432 (recipe of configs[2]) is where the PRODUCT build switches to its large-N path: S3's exact
+    search by lane pairs, the second search table doing several bisection steps (coarse spacing 2^12), the four-pass
+    sort.  One step, every star, against the oracle's -fopenmp build (about half a minute): the paper's own bar,
+    "matching ... to the last significant digit", on the path that N = 1e8 is only sampled on."""
+    run_self_chained(oracle, 2, n_override=1 << 25, steps=1)
+
+
 STRIDE_1E8 = 16
 
 
