@@ -478,9 +478,10 @@ class OrbitStepper:
         call (the carried arrays alternate between two sets of buffers with period two).  What changes from step to
         step, the Philox step number, is kept on the device: hmc_sample_new_radius_dstep reads it, hmc_add_u32
         advances it inside the graph.  For small N, where a step is bound by launching its 13 kernels one
-        by one rather than by the GPU.  Plain steps only (no energy correction, no relaxation stage)."""
-        if self.energy_correction or self.relaxation:
-            raise HmcError("run_graph supports the plain step only")
+        by one rather than by the GPU.  With or without the energy correction; not with the relaxation stage (its
+        Philox step number is a host argument)."""
+        if self.relaxation:
+            raise HmcError("run_graph does not support the relaxation stage")
         if steps % 2:
             raise HmcError("run_graph takes an even number of steps (the buffers alternate with period two)")
         if self._graph is None:
@@ -514,6 +515,15 @@ class OrbitStepper:
     def _step_body(self, fused: bool, step_dev):
         s, so = self.state, self.sorted
         correct = self.energy_correction and self.step_index > 0
+        if correct:
+            # What the correction needs from the previous step -- each star's E in that potential (S3's output), its
+            # radius then and the potential there -- becomes three record columns of this step's sort by exchanging
+            # buffers, not by copying: the previous outputs are read as columns, and the previous columns' buffers
+            # receive this step's E, sorted radii and potential.  (Until the next step begins, tp["E"], sorted["r"]
+            # and phi still hold this step's values.)  The arrangement repeats with period two, like the state's.
+            s["E"], self.tp["E"] = self.tp["E"], s["E"]
+            s["r_old"], so["r"] = so["r"], s["r_old"]
+            s["p_old"], self.phi = self.phi, s["p_old"]
         extra = ("E", "r_old", "p_old") if correct else ()
         hmc_sort_by_radius(s["r"], (s["v_r"], s["v_t"], s["m"]) + tuple(s[k] for k in extra), s["id"], r_sorted=so["r"],
                            perm=so["perm"], cols_out=(so["v_r"], so["v_t"], so["m"]) + tuple(so[k] for k in extra),
@@ -553,10 +563,6 @@ class OrbitStepper:
         s["v_t"], sm["v_t_new"] = sm["v_t_new"], s["v_t"]
         s["m"], so["m"] = so["m"], s["m"]
         s["id"], so["id"] = so["id"], s["id"]
-        if self.energy_correction:      # what the next step's correction needs: E in this potential, r and Phi here
-            s["E"].copy_(self.tp["E"])
-            s["r_old"].copy_(so["r"])
-            s["p_old"].copy_(self.phi)
         self.step_index += 1
 
     def diagnostics(self, fractions=()):

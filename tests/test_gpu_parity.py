@@ -445,6 +445,29 @@ def test_stepper_with_energy_correction_conserves_total_energy(oracle):
     assert abs(e[2] - e[0]) <= 2e-5 * abs(e[0])            # uncorrected: about 1e-4 per step at this N
 
 
+def test_energy_correction_steps_replayed_from_a_graph_equal_eager_steps():
+    """The correction's three extra columns are handed from step to step by exchanging buffers (no copies), so this
+    mode can be captured too: six steps through run_graph (two eager, two captured, replayed twice) leave the same
+    bits as six eager steps, in the state and in what the last step's S1-S3 produced."""
+    n, seed = 100_000, 31
+    c = inputs.plummer(n, seed)
+    mk = lambda: hmc.OrbitStepper(dev(c["r"]), dev(c["v_r"]), dev(c["v_t"]), dev(c["m"]), dev(c["id"].view(np.int32)), seed,
+                                  energy_correction=True)
+    eager, graph = mk(), mk()
+    for _ in range(6):
+        eager.step()
+    graph.run_graph(6)
+    torch.cuda.synchronize()
+    assert graph.step_index == eager.step_index == 6
+    for k in ("r", "v_r", "v_t", "m", "id"):
+        assert torch.equal(graph.state[k], eager.state[k]), k
+    assert torch.equal(graph.sorted["r"], eager.sorted["r"]) and torch.equal(graph.phi, eager.phi)
+    assert torch.equal(graph.tp["E"], eager.tp["E"])
+    assert torch.equal(graph.counters, eager.counters)
+    eager.step(); graph.step()                      # and an eager step after the replays picks up where they left
+    assert torch.equal(graph.state["r"], eager.state["r"])
+
+
 def test_twenty_step_soak_properties():
     """Twenty chained steps of a 10^6-star cluster with the energy correction on: properties that hold at any size
     and step (no oracle): sorted radii, the ids stay a permutation, no star flagged by S3/S4, the cluster stays in
